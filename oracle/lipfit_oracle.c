@@ -1,0 +1,213 @@
+/*
+ * lipfit_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see lipfit_oracle.h).
+ *
+ * Plain double-precision CPU code following PAPER.md equation by equation.
+ * No blocking, fusion or reordering beyond what the formulas state; the only
+ * parallelism is an OpenMP `parallel for` over independent queries / rows.
+ * Build: gcc -O2 -fopenmp -shared -fPIC (oracle/build.py).
+ */
+#include "lipfit_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+static int check_common(const void* X, int64_t N, int32_t d, const int32_t* mask,
+                        int32_t norm, const float* w) {
+    if (!X) return -1;
+    if (d < 1) return -2;
+    if (N < 1) return -3;
+    if (norm < 1 || norm > 3) return -4;
+    for (int i = 0; i < d; ++i) {
+        if (mask && (mask[i] < -1 || mask[i] > 1)) return -4;
+        if (w && !(w[i] >= 0.0f && isfinite(w[i]))) return -4;
+    }
+    return 0;
+}
+
+/* The two one-sided distances between a point x ("query" role) and a datum
+ * xk.  Eq.(4): dist = ||(x - x^k)_+|| on the monotone-increasing
+ * coordinates; PAPER.md:140 fixes which side serves which bound (R1):
+ *   *Du = d_s(x^k, x) uses (x - x^k)_+   -> goes into H^upper,
+ *   *Dl = d_s(x, x^k) uses (x^k - x)_+   -> goes into H^lower.
+ * s_i = -1 is the mirrored coordinate (R2); s_i = 0 contributes |delta| to
+ * both (R4).  The norm is ||w (.) v||_p, p in {1,2,inf} (R3). */
+static void one_sided_distances(const float* x, const float* xk, int32_t d,
+                                const int32_t* mask, int32_t norm, const float* w,
+                                double* Du, double* Dl) {
+    double au = 0.0, al = 0.0;
+    for (int i = 0; i < d; ++i) {
+        double delta = (double)x[i] - (double)xk[i];
+        int s = mask ? mask[i] : 0;
+        double cu, cl;
+        if (s == 0) {
+            cu = fabs(delta);
+            cl = fabs(delta);
+        } else {
+            cu = fmax((double)s * delta, 0.0);
+            cl = fmax(-(double)s * delta, 0.0);
+        }
+        double wi = w ? (double)w[i] : 1.0;
+        cu *= wi;
+        cl *= wi;
+        if (norm == 1) {
+            au += cu;
+            al += cl;
+        } else if (norm == 2) {
+            au += cu * cu;
+            al += cl * cl;
+        } else {
+            au = fmax(au, cu);
+            al = fmax(al, cl);
+        }
+    }
+    if (norm == 2) {
+        au = sqrt(au);
+        al = sqrt(al);
+    }
+    *Du = au;
+    *Dl = al;
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* Eq.(2): H^upper(x) = min_k (y^k + M dist), H^lower(x) = max_k (y^k - M dist);
+ * Eq.(3): g = (H^lower + H^upper)/2.  PAPER.md:103-116. */
+int oracle_bounds(const float* X, const float* y, int64_t N, int32_t d,
+                  const float* Xq, int64_t Q, double M,
+                  const int32_t* mono_mask, int32_t norm, const float* weights,
+                  double* upper, double* lower, double* g) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || (Q > 0 && !Xq)) return -1;
+    if (Q < 0) return -3;
+    if (!(M >= 0.0) || !isfinite(M)) return -4;
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < Q; ++q) {
+        double U = INFINITY, L = -INFINITY;
+        for (int64_t k = 0; k < N; ++k) {
+            double Du, Dl;
+            one_sided_distances(Xq + q * d, X + k * d, d, mono_mask, norm, weights, &Du, &Dl);
+            double hi = (double)y[k] + M * Du;
+            double lo = (double)y[k] - M * Dl;
+            if (hi < U) U = hi;
+            if (lo > L) L = lo;
+        }
+        if (upper) upper[q] = U;
+        if (lower) lower[q] = L;
+        if (g) g[q] = 0.5 * (U + L);
+    }
+    return 0;
+}
+
+/* k nearest by distance; keep the k smallest (dist, index) seen so far in
+ * ascending order by straight insertion.  PAPER.md:179 (d_(1) <= d_(2) ...). */
+int oracle_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+               const int32_t* mono_mask, int32_t side, int32_t norm,
+               const float* weights, int32_t k, int32_t* idx, double* dist) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if ((Q > 0 && !Xq) || !idx || !dist) return -1;
+    if (Q < 0 || k < 1 || k > N) return -3;
+    if (side < -1 || side > 1) return -4;
+    const int32_t* m = (side == 0) ? NULL : mono_mask; /* side 0: symmetric, mask ignored (R6) */
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < Q; ++q) {
+        int32_t* bi = idx + q * k;
+        double* bd = dist + q * k;
+        int32_t have = 0;
+        for (int64_t j = 0; j < N; ++j) {
+            double Du, Dl;
+            one_sided_distances(Xq + q * d, X + j * d, d, m, norm, weights, &Du, &Dl);
+            double dj = (side < 0) ? Dl : Du;
+            /* position: after every kept (dist,idx) that is <= (dj,j); j grows, so
+             * equal distances keep the earlier (lower) index first (R7). */
+            int32_t pos = have;
+            while (pos > 0 && bd[pos - 1] > dj) --pos;
+            if (pos >= k) continue;
+            int32_t last = (have < k) ? have : k - 1;
+            for (int32_t t = last; t > pos; --t) {
+                bd[t] = bd[t - 1];
+                bi[t] = bi[t - 1];
+            }
+            bd[pos] = dj;
+            bi[pos] = (int32_t)j;
+            if (have < k) ++have;
+        }
+    }
+    return 0;
+}
+
+/* Eq.(7) PAPER.md:197:
+ *   F = (1/p)||eps||^2
+ *     + sum_{i!=k} ((y_i - y_k - M d_ik - (eps_k - eps_i))_+)^2      [from (5)]
+ *     + sum_{i!=k} ((y_k - y_i - M d'_ik + eps_k - eps_i)_+)^2       [from (6)]
+ * with d_ik = d_s(x^k,x^i) (upper-bound distance of datum k seen from x^i) and
+ * d'_ik = d_s(x^i,x^k) (lower-bound distance), reading R12.  Gradient by the
+ * chain rule, term by term:  d/deps_i of the (5)-term (i,k) is +2A_ik, of the
+ * (5)-term (k,i) is -2A_ki, of the (6)-term (i,k) is -2B_ik, of (k,i) +2B_ki. */
+int oracle_smooth_objective(const float* X, const float* y, int64_t N, int32_t d,
+                            double M, const int32_t* mono_mask, int32_t norm,
+                            const float* weights, double p, const double* eps,
+                            double* F, double* grad) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || !eps || !F) return -1;
+    if (!(M >= 0.0) || !isfinite(M) || !(p > 0.0)) return -4;
+    double total = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : total)
+    for (int64_t i = 0; i < N; ++i) {
+        double zi = (double)y[i] + eps[i];
+        double gi = 2.0 * eps[i] / p;
+        double fi = eps[i] * eps[i] / p;
+        for (int64_t k = 0; k < N; ++k) {
+            if (k == i) continue;
+            double zk = (double)y[k] + eps[k];
+            double d_ik, dp_ik; /* point x^i against datum x^k */
+            one_sided_distances(X + i * d, X + k * d, d, mono_mask, norm, weights, &d_ik, &dp_ik);
+            double d_ki, dp_ki; /* point x^k against datum x^i */
+            one_sided_distances(X + k * d, X + i * d, d, mono_mask, norm, weights, &d_ki, &dp_ki);
+            double A_ik = fmax(zi - zk - M * d_ik, 0.0);  /* (5) at (i,k) */
+            double B_ik = fmax(zk - zi - M * dp_ik, 0.0); /* (6) at (i,k) */
+            double A_ki = fmax(zk - zi - M * d_ki, 0.0);  /* (5) at (k,i) */
+            double B_ki = fmax(zi - zk - M * dp_ki, 0.0); /* (6) at (k,i) */
+            fi += A_ik * A_ik + B_ik * B_ik; /* the two (i,k) terms of the sums */
+            gi += 2.0 * A_ik - 2.0 * A_ki - 2.0 * B_ik + 2.0 * B_ki;
+        }
+        total += fi;
+        if (grad) grad[i] = gi;
+    }
+    *F = total;
+    return 0;
+}
+
+int oracle_max_violation(const float* X, const float* y, int64_t N, int32_t d,
+                         double M, const int32_t* mono_mask, int32_t norm,
+                         const float* weights, const double* eps, double* out) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || !out) return -1;
+    double worst = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : worst)
+    for (int64_t i = 0; i < N; ++i) {
+        double zi = (double)y[i] + (eps ? eps[i] : 0.0);
+        for (int64_t k = 0; k < N; ++k) {
+            if (k == i) continue;
+            double zk = (double)y[k] + (eps ? eps[k] : 0.0);
+            double Du, Dl;
+            one_sided_distances(X + i * d, X + k * d, d, mono_mask, norm, weights, &Du, &Dl);
+            double v = zi - zk - M * Du;
+            if (v > worst) worst = v;
+        }
+    }
+    *out = worst;
+    return 0;
+}
