@@ -1,0 +1,439 @@
+#!/usr/bin/env python
+"""bench.py -- measures the LipFit hot path on B200 (contract: task prompt, "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--configs 2[,1,3,4,5]]
+
+One "step" = one pass of the hot path over one batch of synthetic input of the bench workload:
+BASELINE.json configs[1] (d=4, N=1e5 data, Q=1e6 queries, weighted L1, mask [+1,+1,0,0], M=8) through
+`lipfit_bounds` = a1 prepack + a2 fused bounds (+ finalize).  `value` = query x datum pair
+evaluations per second (Gpairs/s) with inputs resident in HBM; `e2e` = the same through
+`lipfit_bounds_host` (host buffers; H2D and D2H inside the timed region).  The other configs are
+reported under "configs" when asked for with --configs.
+
+Multi-GPU (N > 1, launched by torchrun): queries are independent, so every rank runs the same-size
+batch of its own (seeded by rank) with NO data-path collective ("weak" scaling); time = max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/, fp64, OpenMP) on a bounded sample of the same
+workload on the host cores; only rank 0 works.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from inputs import make_workload, oracle_subset  # noqa: E402
+
+METRIC = "query x datum pair evaluations per second (bounds, config 2)"
+UNIT = "Gpairs/s"
+# Algorithmic lane-ops per pair: 1 lane-op = one fp32
+# add/sub/mul/fma, one min/max/relu/compare, or one sqrt.
+LANE_OPS = {1: 9, 2: 18, 3: 21, 4: 33, "5s": 26, "5b": 31}
+FP32_LANES_PER_SM = 128
+
+
+# ------------------------------------------------------------------------------------------------
+# helpers shared with the gloo test (tests/test_host_abi.py)
+# ------------------------------------------------------------------------------------------------
+def shard_range(Q: int, rank: int, world: int):
+    """Contiguous slice [lo, hi) of Q units owned by `rank` (strong-scaling helper, §8(e))."""
+    base, rem = divmod(Q, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+def max_over_ranks(t: float, device="cuda") -> float:
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return t
+    x = torch.tensor([t], dtype=torch.float64, device=device)
+    dist.all_reduce(x, op=dist.ReduceOp.MAX)
+    return float(x.item())
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except OSError:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(2)
+            except Exception:
+                self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                mx.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def flush_l2(buf):
+    buf.add_(1.0)          # read+write of a buffer larger than the 126 MB L2
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on a bounded sample
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_rate(wl, budget_s: float = 12.0):
+    """Times oracle.bounds on a bounded query sample of `wl`; returns (Gpairs/s, sample text,
+    cores, sample indices, oracle outputs)."""
+    import oracle
+    cores = oracle.num_threads()
+    probe = min(wl.Q, max(64, 4 * cores))
+    t0 = time.perf_counter()
+    oracle.bounds(wl.X, wl.y, wl.Xq[:probe], wl.M, wl.mask, wl.norm, wl.weights)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    qo = int(min(wl.Q, max(probe, budget_s * probe / dt)))
+    sel = oracle_subset(wl.Q, qo)
+    xs = np.ascontiguousarray(wl.Xq[sel])
+    t0 = time.perf_counter()
+    out = oracle.bounds(wl.X, wl.y, xs, wl.M, wl.mask, wl.norm, wl.weights)
+    dt = time.perf_counter() - t0
+    rate = len(sel) * wl.N / dt / 1e9
+    return rate, f"{len(sel)} of {wl.Q} queries (first half + evenly strided) x all {wl.N} data", cores, sel, out
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    wl = make_workload(2)
+    cores = oracle.num_threads()
+    # one "step" = a bounded sample sized for ~6 s of CPU work
+    probe = 8 * cores
+    t0 = time.perf_counter()
+    oracle.bounds(wl.X, wl.y, wl.Xq[:probe], wl.M, wl.mask, wl.norm, wl.weights)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    per_step = max(1.0, min(6.0, 120.0 / max(1, args.steps + args.warmup)))
+    qo = int(min(wl.Q, max(probe, per_step * probe / dt)))
+    sel = oracle_subset(wl.Q, qo)
+    xs = np.ascontiguousarray(wl.Xq[sel])
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.bounds(wl.X, wl.y, xs, wl.M, wl.mask, wl.norm, wl.weights)
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.mean(times))
+    value = len(sel) * wl.N / (ms * 1e-3) / 1e9
+    sample = f"{len(sel)} of {wl.Q} queries x all {wl.N} data per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: bounds d=4 N=100000 Q=1000000 L1 mask[+1,+1,0,0] M=8",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def _time_steps(torch, fn, steps, warmup, l2buf):
+    """W untimed steps, then K steps each bracketed by CUDA events on the launching (current)
+    stream, L2 flushed between steps.  Returns per-step milliseconds."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    out = []
+    for _ in range(steps):
+        flush_l2(l2buf)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        out.append(e0.elapsed_time(e1))
+    return out
+
+
+def _kernel_ms(L, which, fn, reps):
+    """Average device time of dominant kernel `which` alone (library-side CUDA events)."""
+    L.set_timing(True)
+    try:
+        for _ in range(reps):
+            fn()
+        ms, n = L.get_timing(which)
+    finally:
+        L.set_timing(False)
+    return (ms / n if n else None), n
+
+
+def _roofline(pairs, lane_ops, kernel_ms, sms, peaks):
+    peak = sms * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12    # T lane-ops/s
+    ach = pairs * lane_ops / (kernel_ms * 1e-3) / 1e12 if kernel_ms else None
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlane-op/s",
+            "frac": (ach / peak) if ach else None, "traffic": None,
+            "lane_ops_per_pair": lane_ops, "kernel_ms": kernel_ms,
+            "peak_how": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {peaks['sm_max_mhz']:.0f} MHz (clocks.max.sm)"}
+
+
+def bench_bounds(torch, L, wl, steps, warmup, l2buf, dev, lane_ops, do_e2e=True):
+    t = lambda a: torch.from_numpy(a).to(dev)
+    X, y, Xq = t(wl.X), t(wl.y), t(wl.Xq)
+    fn = lambda: L.lipfit_bounds(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
+    n0 = L.launch_count()
+    ms = _time_steps(torch, fn, steps, warmup, l2buf)
+    launches = (L.launch_count() - n0) * steps // (steps + warmup)
+    kms, _ = _kernel_ms(L, 0, fn, max(1, min(3, steps)))
+    pairs = wl.N * wl.Q
+    res = {"ms_per_step": float(np.mean(ms)), "ms_min": float(np.min(ms)), "pairs": pairs,
+           "value": pairs / (np.mean(ms) * 1e-3) / 1e9, "gpu_launches": int(launches),
+           "kernel": L.bounds_variant(wl.d, wl.mask, wl.norm), "kernel_ms": kms,
+           "lane_ops": lane_ops, "outputs": fn()}
+    if do_e2e:
+        pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+        Xh, yh, Xqh = pin(wl.X), pin(wl.y), pin(wl.Xq)
+        outs = tuple(torch.empty(wl.Q, dtype=torch.float32).pin_memory().numpy() for _ in range(3))
+        sp = torch.cuda.current_stream().cuda_stream
+        hfn = lambda: L.lipfit_bounds_host(Xh, yh, Xqh, wl.M, wl.mask, wl.norm, wl.weights, outs, sp)
+        hms = _time_steps(torch, hfn, max(1, steps), min(warmup, 2), l2buf)
+        res["e2e"] = {"value": pairs / (np.mean(hms) * 1e-3) / 1e9, "unit": UNIT,
+                      "ms_per_step": float(np.mean(hms)),
+                      "h2d_bytes_per_step": int(Xh.nbytes + yh.nbytes + Xqh.nbytes),
+                      "d2h_bytes_per_step": int(sum(o.nbytes for o in outs))}
+    return res
+
+
+def bench_knn(torch, L, wl, steps, warmup, l2buf, dev):
+    t = lambda a: torch.from_numpy(a).to(dev)
+    X, Xq = t(wl.X), t(wl.Xq)
+    fn = lambda: L.lipfit_knn(X, Xq, wl.k, None, 0, wl.norm, wl.weights)
+    ms = _time_steps(torch, fn, steps, warmup, l2buf)
+    kms, _ = _kernel_ms(L, 1, fn, 1)
+    pairs = wl.N * wl.Q
+    return {"ms_per_step": float(np.mean(ms)), "pairs": pairs, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+            "kernel_ms": kms, "lane_ops": LANE_OPS[4], "outputs": fn()}
+
+
+def bench_smooth(torch, L, wl, l2buf, dev):
+    """Config 5: host LBFGS (<= 200 iterations) over the device all-pairs pass, then bounds."""
+    t = lambda a: torch.from_numpy(a).to(dev)
+    X, y = t(wl.X), t(wl.y.copy())
+    L.set_timing(True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    eps, info = L.lipfit_smooth(X, y, wl.M, wl.mask, wl.norm, wl.weights, wl.p, wl.max_iter, 1e-6)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    kms, n = L.get_timing(2)
+    L.set_timing(False)
+    pairs_eval = wl.N * (wl.N - 1)
+    return {"wall_s": wall, "info": info, "evals": n, "kernel_ms_per_eval": kms / max(n, 1),
+            "pairs_per_eval": pairs_eval, "value": pairs_eval / (kms / max(n, 1) * 1e-3) / 1e9,
+            "lane_ops": LANE_OPS["5s"], "z": y, "X": X}
+
+
+def parity_bounds(wl, outs, sel, ref):
+    """max |gpu - oracle| / (1e-5 * range) on the oracle's query sample (<= 1 passes)."""
+    tol = 1e-5 * wl.y_range
+    worst = 0.0
+    for o, r in zip(outs, ref):
+        worst = max(worst, float(np.abs(o.cpu().numpy()[sel].astype(np.float64) - r).max()))
+    return {"max_abs_err": worst, "tol": tol, "ok": bool(worst <= tol), "queries": int(len(sel))}
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_04670_b200 as L
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    L.load()
+    peaks, peaks_how = measured_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    l2buf = torch.empty(64 * 1024 * 1024, dtype=torch.float32, device=dev)   # 256 MB > 126 MB L2
+    cfgs = [int(c) for c in args.configs.split(",")]
+
+    # ---- the bench line: config 2 ----
+    wl = make_workload(2, query_seed=1 + 1000 * rank)   # weak scaling: each rank its own batch
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    r2 = bench_bounds(torch, L, wl, args.steps, args.warmup, l2buf, dev, LANE_OPS[2])
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms = max_over_ranks(r2["ms_per_step"])
+    e2e_ms = max_over_ranks(r2["e2e"]["ms_per_step"])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+    line = {
+        "metric": METRIC, "value": world * r2["pairs"] / (ms * 1e-3) / 1e9, "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE.json configs[1]: bounds d=4 N=100000 Q=1000000 L1 mask[+1,+1,0,0] M=8",
+                   "kernel": r2["kernel"], "l2": "flushed between timed steps (256 MB write)",
+                   "step": "lipfit_bounds = a1 prepack + a2 fused bounds + finalize",
+                   "parallelism": f"query-sharded replicas x{world}, no collective"},
+        "clocks": clocks,
+        "e2e": {"value": world * r2["pairs"] / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": r2["e2e"]["h2d_bytes_per_step"],
+                "d2h_bytes_per_step": r2["e2e"]["d2h_bytes_per_step"], "ms_per_step": e2e_ms},
+        "gpu_launches": r2["gpu_launches"] * args.steps,
+        "roofline": _roofline(r2["pairs"], LANE_OPS[2], r2["kernel_ms"], sms, peaks),
+        "peaks": peaks_how,
+    }
+    if clocks and clocks.get("sm_mhz"):
+        rf = line["roofline"]
+        rf["frac_at_observed_clock"] = rf["achieved"] / (sms * FP32_LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)
+    # ---- CPU baseline: the oracle on a bounded sample, with parity on exactly that sample ----
+    if not args.no_cpu:
+        rate, sample, cores, sel, ref = oracle_sample_rate(wl)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        line["parity"] = parity_bounds(wl, r2["outputs"], sel, ref)
+    # ---- the other configs on request ----
+    extra = {}
+    for c in cfgs:
+        if c == 2:
+            continue
+        try:
+            extra[f"config{c}"] = run_other_config(torch, L, c, args, l2buf, dev, sms, peaks)
+        except Exception as e:  # report, do not hide
+            extra[f"config{c}"] = {"error": repr(e)}
+    if extra:
+        line["configs"] = extra
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
+    import oracle
+    wl = make_workload(c)
+    steps = max(1, min(args.steps, 3)) if c in (3, 4) else args.steps
+    out = {}
+    if c in (1, 3):
+        r = bench_bounds(torch, L, wl, steps, 3, l2buf, dev, LANE_OPS[c], do_e2e=False)
+        out.update({k: r[k] for k in ("ms_per_step", "ms_min", "value", "kernel", "kernel_ms")})
+        out["unit"] = UNIT
+        out["roofline"] = _roofline(r["pairs"], LANE_OPS[c], r["kernel_ms"], sms, peaks)
+        if not args.no_cpu:
+            rate, sample, cores, sel, ref = oracle_sample_rate(wl, 8.0)
+            out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "sample": sample}
+            out["parity"] = parity_bounds(wl, r["outputs"], sel, ref)
+    elif c == 4:
+        r = bench_knn(torch, L, wl, steps, 1, l2buf, dev)
+        out.update({k: r[k] for k in ("ms_per_step", "value", "kernel_ms")})
+        out["unit"] = UNIT
+        out["roofline"] = _roofline(r["pairs"], LANE_OPS[4], r["kernel_ms"], sms, peaks)
+        if not args.no_cpu:
+            sel = oracle_subset(wl.Q, 64)
+            t0 = time.perf_counter()
+            oi, od = oracle.knn(wl.X, wl.Xq[sel], wl.k, None, 0, wl.norm)
+            dt = time.perf_counter() - t0
+            gi = r["outputs"][0].cpu().numpy()[sel]
+            gd = r["outputs"][1].cpu().numpy()[sel]
+            out["cpu_baseline"] = {"value": len(sel) * wl.N / dt / 1e9, "unit": UNIT,
+                                   "cores": oracle.num_threads(), "sample": f"{len(sel)} queries x all data"}
+            out["parity"] = {"index_sets_equal": bool(all(set(a) == set(b) for a, b in zip(gi, oi))),
+                             "max_dist_err_ulps": float(np.max(np.abs(gd - od.astype(np.float32))
+                                                               / np.spacing(od.astype(np.float32)))),
+                             "queries": int(len(sel))}
+    elif c == 5:
+        r = bench_smooth(torch, L, wl, l2buf, dev)
+        out.update({"smooth_wall_s": r["wall_s"], "info": r["info"], "evals": r["evals"],
+                    "kernel_ms_per_eval": r["kernel_ms_per_eval"], "value": r["value"], "unit": UNIT,
+                    "roofline": _roofline(r["pairs_per_eval"], LANE_OPS["5s"], r["kernel_ms_per_eval"], sms, peaks)})
+        Xq = torch.from_numpy(wl.Xq).to(dev)
+        fn = lambda: L.lipfit_bounds(r["X"], r["z"], Xq, wl.M, wl.mask, wl.norm, wl.weights)
+        ms = _time_steps(torch, fn, max(1, min(args.steps, 3)), 2, l2buf)
+        kms, _ = _kernel_ms(L, 0, fn, 1)
+        pairs = wl.N * wl.Q
+        out["bounds_after"] = {"ms_per_step": float(np.mean(ms)), "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+                               "roofline": _roofline(pairs, LANE_OPS["5b"], kms, sms, peaks)}
+        if not args.no_cpu:
+            z = r["z"].cpu().numpy()
+            sel = oracle_subset(wl.Q, 2000)
+            ref = oracle.bounds(wl.X, z, wl.Xq[sel], wl.M, wl.mask, wl.norm, wl.weights)
+            wl.y = z
+            out["bounds_after"]["parity"] = parity_bounds(wl, fn(), sel, ref)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--configs", default="2", help="comma list of BASELINE.json configs to report (2 always)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,160 @@
+/*
+ * lipfit.h -- C ABI of the B200-native (sm_100a) LipFit hot path.
+ *
+ * Implements the data-parallel hot path of "Fitting scattered data with
+ * optional monotonicity constraints on GPU: LipFit package" (PAPER.md =
+ * arxiv/paper_2606_04670): evaluation of the optimal Lipschitz interpolant
+ * (Eq.(2),(3) with the monotone distance Eq.(4)), neighbour selection by the
+ * same fused distance-then-reduce pass, and penalty smoothing (Eq.(5)-(7)).
+ *
+ * Conventions common to every entry point
+ *   - Plain C types only.  Unless a parameter says "host", array pointers are
+ *     DEVICE pointers to row-major fp32 (int32 for indices), 4-byte aligned,
+ *     caller-owned.  The library never frees or retains caller memory.
+ *     `mono_mask` and `weights` are HOST arrays of length d (read during the
+ *     call; NULL = all 0 / all 1).  The `*_host` variants take HOST pointers for
+ *     everything and do the host<->device copies themselves.
+ *   - `cuda_stream` is a cudaStream_t (NULL = default stream).  Internal
+ *     workspace comes from cudaMallocAsync on that stream and is released
+ *     (stream-ordered) before the call returns.
+ *   - Every function returns LIPFIT_OK (0) or a negative lipfit_status; no
+ *     exception crosses the boundary; apart from an atomic launch counter there is
+ *     no global mutable state, so calls on distinct streams are thread-safe.
+ *   - lipfit_bounds / lipfit_knn / lipfit_smooth_objective(F==NULL) are
+ *     asynchronous on `cuda_stream`; lipfit_smooth and the *_host variants
+ *     synchronise the stream before returning.
+ *   - Inputs must be finite; NaN/Inf are not scanned for (results undefined,
+ *     never a crash).  There is no CPU fallback: without a CUDA device every
+ *     compute call returns LIPFIT_E_CUDA.
+ *
+ * Distance (Eq.(4), sign convention PAPER.md:140):
+ *   delta_i = xq_i - x^k_i, mask s_i in {-1,0,+1}, weight w_i >= 0,
+ *   u_i = w_i |delta_i| if s_i = 0 else w_i max( s_i delta_i, 0)
+ *   l_i = w_i |delta_i| if s_i = 0 else w_i max(-s_i delta_i, 0)
+ *   D^u = ||u||_p = d_s(x^k, x)   (used by H^upper)
+ *   D^l = ||l||_p = d_s(x, x^k)   (used by H^lower),  p = norm in {1,2,inf}.
+ */
+#ifndef LIPFIT_H
+#define LIPFIT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LIPFIT_MAX_DIM 32
+#define LIPFIT_MAX_K 128
+
+enum lipfit_norm { LIPFIT_L1 = 1, LIPFIT_L2 = 2, LIPFIT_LINF = 3 };
+
+enum lipfit_status {
+    LIPFIT_OK = 0,
+    LIPFIT_E_NULL = -1,  /* a required pointer is NULL */
+    LIPFIT_E_DIM = -2,   /* d < 1 or d > LIPFIT_MAX_DIM */
+    LIPFIT_E_SIZE = -3,  /* N < 1, Q < 0, k < 1, k > N, k > LIPFIT_MAX_K, N or Q > 2^31-1 */
+    LIPFIT_E_PARAM = -4, /* M < 0 or non-finite, mask not in {-1,0,1}, w < 0 or non-finite, bad norm/side, p <= 0 */
+    LIPFIT_E_CUDA = -5,  /* a CUDA runtime call failed (no device, launch error, ...) */
+    LIPFIT_E_NOMEM = -6  /* workspace allocation failed */
+};
+
+/* ---- Eq.(2),(3) PAPER.md:103-116 with the distance of Eq.(4) PAPER.md:142 ------------------
+ *   upper[q] = min_k (y[k] + M D^u(q,k)),  lower[q] = max_k (y[k] - M D^l(q,k)),
+ *   g[q]     = (upper[q] + lower[q]) / 2.
+ * X [N*d], y [N], Xq [Q*d]; upper/lower/g [Q], each may be NULL (at least one non-NULL unless Q=0).
+ * Q = 0 returns LIPFIT_OK and writes nothing.  M = 0 is allowed.  Inconsistent data
+ * (lower > upper somewhere) are not an error.
+ * Steps on the device: a1 prepack (permute / mirror / weight the coordinates, build records)
+ * then a2 fused distance + running min/max; the Q x N distance matrix is never formed. */
+int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d,
+                  const float* Xq, int64_t Q, float M,
+                  const int32_t* mono_mask /* host[d] or NULL */, int32_t norm,
+                  const float* weights /* host[d] or NULL */,
+                  float* upper, float* lower, float* g, void* cuda_stream);
+
+/* Same, every array pointer a HOST pointer (pageable or pinned); copies X, y, Xq to the
+ * device, runs lipfit_bounds, copies the non-NULL outputs back and synchronises. */
+int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d,
+                       const float* Xq, int64_t Q, float M,
+                       const int32_t* mono_mask, int32_t norm, const float* weights,
+                       float* upper, float* lower, float* g, void* cuda_stream);
+
+/* ---- k nearest data per query by distance (d_(1) <= d_(2) <= ...) -------------
+ * side 0: symmetric weighted norm, mask ignored; +1: D^u; -1: D^l.
+ * idx [Q*k] int32 and dist [Q*k] fp32, row-major, ascending distance per query.
+ * Selection runs in fp32 on a pool of k + margin candidates; the pool is then re-ranked
+ * in fp64 from the original fp32 inputs, sorted by (distance, index), so the returned set
+ * equals the exact one except among candidates whose fp32-rounded distances tie. */
+int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+               const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
+               int32_t k, int32_t* idx, float* dist, void* cuda_stream);
+
+int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                    const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
+                    int32_t k, int32_t* idx, float* dist, void* cuda_stream);
+
+/* ---- Penalty smoothing, Eq.(5)-(7) PAPER.md:189-198 ---------------------------------------
+ * F(eps) = ||eps||^2/p + sum_{i!=k} (z_i - z_k - M d_s(x^k,x^i))_+^2
+ *                      + sum_{i!=k} (z_k - z_i - M d_s(x^i,x^k))_+^2,   z = y + eps,
+ * all N(N-1) ordered pairs recomputed on the fly (no N x N matrix).
+ * lipfit_smooth_objective: eps [N] device (NULL = 0); *F host double (may be NULL: then the call
+ * is asynchronous and only grad is produced); grad [N] device fp32 (may be NULL). */
+int lipfit_smooth_objective(const float* X, const float* y, int64_t N, int32_t d, float M,
+                            const int32_t* mono_mask, int32_t norm, const float* weights, float p,
+                            const float* eps, double* F /* host */, float* grad, void* cuda_stream);
+
+typedef struct lipfit_smooth_info {
+    int32_t iters;          /* LBFGS iterations taken */
+    int32_t evals;          /* objective/gradient evaluations (device passes) */
+    int32_t status;         /* 0 converged (gnorm_inf <= tol_grad), 1 max_iter, 2 no further progress */
+    int32_t reserved;
+    double F0, F;           /* objective at eps = 0 and at the returned eps */
+    double gnorm_inf;       /* ||grad F||_inf at the returned eps */
+    double max_violation0;  /* max_{i!=k} (z_i - z_k - M d_s(x^k,x^i))_+ at eps = 0 ... */
+    double max_violation;   /* ... and at the returned eps */
+} lipfit_smooth_info;
+
+/* Minimises F from eps = 0 by LBFGS on the host, each evaluation one
+ * device pass; then y_inout <- y + eps on the device.  eps_out [N] device or
+ * NULL; info host or NULL.  Synchronises the stream. */
+int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
+                  const int32_t* mono_mask, int32_t norm, const float* weights, float p,
+                  int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,
+                  void* cuda_stream);
+
+int lipfit_smooth_host(const float* X, float* y_inout, int64_t N, int32_t d, float M,
+                       const int32_t* mono_mask, int32_t norm, const float* weights, float p,
+                       int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,
+                       void* cuda_stream);
+
+/* ---- Host optimiser on its own (step a5), exposed so that it can be tested without a GPU ----
+ * Minimises a caller-supplied function by the same LBFGS lipfit_smooth uses (history `history`,
+ * strong-Wolfe line search).  x: host double[n], start point on entry and
+ * result on exit.  fn returns 0 on success; a non-zero value aborts and is returned (negated if
+ * positive).  info may be NULL; only iters, evals, status, F0, F, gnorm_inf are filled. */
+typedef int (*lipfit_eval_fn)(void* user, const double* x, double* f, double* grad);
+int lipfit_lbfgs(int64_t n, double* x, lipfit_eval_fn fn, void* user, int32_t max_iter,
+                 double tol_grad, int32_t history, lipfit_smooth_info* info);
+
+/* ---- Introspection ----------------------------------------------------------------------- */
+const char* lipfit_status_string(int code);
+/* "major.minor.patch" of this library. */
+const char* lipfit_version(void);
+/* Number of kernel launches this library has issued since load (all threads); used by
+ * bench.py's gpu_launches.  Monotone counter, not reset. */
+int64_t lipfit_launch_count(void);
+/* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
+ * resets the accumulators and makes every later launch of the three dominant kernels
+ * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs) bracketed by CUDA events on
+ * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
+ * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
+void lipfit_set_timing(int32_t on);
+int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches);
+/* Name of the kernel variant lipfit_bounds would dispatch to for (d, mask, norm), e.g.
+ * "bounds<L1,U2,C2,R8>" or "bounds_generic<L2,DP8>"; writes at most `cap` bytes incl. NUL. */
+int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, char* out, int32_t cap);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LIPFIT_H */

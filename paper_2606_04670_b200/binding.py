@@ -1,0 +1,295 @@
+"""ctypes binding of include/lipfit.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of liblipfit.so; nothing here computes a distance,
+a bound, a neighbour or a penalty.  torch is used for device memory and streams only.  There is no
+CPU fallback: if the library cannot be built/loaded, or no CUDA device is visible, the calls raise.
+Nothing under oracle/ is imported from here.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+LIPFIT_L1, LIPFIT_L2, LIPFIT_LINF = 1, 2, 3
+LIPFIT_MAX_DIM, LIPFIT_MAX_K = 32, 128
+
+EXPORTS = [
+    "lipfit_bounds", "lipfit_bounds_host", "lipfit_knn", "lipfit_knn_host",
+    "lipfit_smooth_objective", "lipfit_smooth", "lipfit_smooth_host", "lipfit_lbfgs",
+    "lipfit_status_string", "lipfit_version", "lipfit_launch_count", "lipfit_bounds_variant",
+    "lipfit_set_timing", "lipfit_get_timing",
+]
+
+
+class LipfitError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {status_string(code)} ({code})")
+
+
+class SmoothInfo(C.Structure):
+    _fields_ = [("iters", C.c_int32), ("evals", C.c_int32), ("status", C.c_int32),
+                ("reserved", C.c_int32), ("F0", C.c_double), ("F", C.c_double),
+                ("gnorm_inf", C.c_double), ("max_violation0", C.c_double),
+                ("max_violation", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+EVAL_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                      C.POINTER(C.c_double))
+
+_lib = None
+
+
+def load():
+    """Builds (if stale) and loads liblipfit.so; raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = C.CDLL(_build.build())
+    P, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
+    lib.lipfit_bounds.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, P, P, P, P]
+    lib.lipfit_bounds_host.argtypes = lib.lipfit_bounds.argtypes
+    lib.lipfit_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, P]
+    lib.lipfit_knn_host.argtypes = lib.lipfit_knn.argtypes
+    lib.lipfit_smooth_objective.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, P, P, P, P]
+    lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
+    lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
+    lib.lipfit_lbfgs.argtypes = [i64, P, EVAL_FN, P, i32, f64, i32, P]
+    lib.lipfit_bounds_variant.argtypes = [i32, P, i32, C.c_char_p, i32]
+    for name in EXPORTS:
+        getattr(lib, name).restype = C.c_int
+    lib.lipfit_status_string.restype = C.c_char_p
+    lib.lipfit_status_string.argtypes = [C.c_int]
+    lib.lipfit_version.restype = C.c_char_p
+    lib.lipfit_launch_count.restype = C.c_int64
+    lib.lipfit_set_timing.restype = None
+    lib.lipfit_set_timing.argtypes = [i32]
+    lib.lipfit_get_timing.argtypes = [i32, P, P]
+    _lib = lib
+    return lib
+
+
+def status_string(code: int) -> str:
+    return load().lipfit_status_string(int(code)).decode()
+
+
+def version() -> str:
+    return load().lipfit_version().decode()
+
+
+def launch_count() -> int:
+    return int(load().lipfit_launch_count())
+
+
+def set_timing(on: bool) -> None:
+    load().lipfit_set_timing(1 if on else 0)
+
+
+def get_timing(which: int):
+    """(total device ms, launches) of dominant kernel `which` (0 bounds, 1 kNN select, 2 smooth)."""
+    ms, n = C.c_double(0.0), C.c_int64(0)
+    _check(load().lipfit_get_timing(int(which), C.cast(C.byref(ms), C.c_void_p),
+                                    C.cast(C.byref(n), C.c_void_p)), "lipfit_get_timing")
+    return float(ms.value), int(n.value)
+
+
+def _check(rc: int, where: str):
+    if rc != 0:
+        raise LipfitError(rc, where)
+
+
+def _host_params(d: int, mono_mask, weights):
+    m = None if mono_mask is None else np.ascontiguousarray(mono_mask, dtype=np.int32).reshape(d)
+    w = None if weights is None else np.ascontiguousarray(weights, dtype=np.float32).reshape(d)
+    return m, w
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def bounds_variant(d: int, mono_mask=None, norm: int = LIPFIT_L2) -> str:
+    m, _ = _host_params(d, mono_mask, None)
+    buf = C.create_string_buffer(96)
+    _check(load().lipfit_bounds_variant(d, _np_ptr(m), norm, buf, 96), "lipfit_bounds_variant")
+    return buf.value.decode()
+
+
+# ---------------------------------------------------------------------------------------------
+# Device-pointer entry points (torch CUDA tensors in, torch CUDA tensors out)
+# ---------------------------------------------------------------------------------------------
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_04670_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _dev_f32(t, ndim, name):
+    torch = _torch()
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32
+            and t.dim() == ndim and t.is_contiguous()):
+        raise TypeError(f"{name}: need a contiguous float32 CUDA tensor with {ndim} dims")
+    return t
+
+
+def _stream(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def lipfit_bounds(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                  want: Sequence[str] = ("upper", "lower", "g"), stream=None):
+    """(upper, lower, g) float32 CUDA tensors of length Q (None for those not in `want`)."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    if Xq.shape[1] != d or y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    m, w = _host_params(d, mono_mask, weights)
+    outs = {k: (torch.empty(Q, dtype=torch.float32, device=X.device) if k in want else None)
+            for k in ("upper", "lower", "g")}
+    ptr = {k: (None if v is None else C.c_void_p(v.data_ptr())) for k, v in outs.items()}
+    rc = load().lipfit_bounds(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M),
+                              _np_ptr(m), int(norm), _np_ptr(w), ptr["upper"], ptr["lower"],
+                              ptr["g"], _stream(stream))
+    _check(rc, "lipfit_bounds")
+    return outs["upper"], outs["lower"], outs["g"]
+
+
+def lipfit_knn(X, Xq, k: int, mono_mask=None, side: int = 0, norm: int = LIPFIT_L2, weights=None,
+               stream=None):
+    """(idx int32 [Q,k], dist float32 [Q,k]) CUDA tensors, ascending distance."""
+    torch = _torch()
+    X, Xq = _dev_f32(X, 2, "X"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _host_params(d, mono_mask, weights)
+    idx = torch.empty((Q, k), dtype=torch.int32, device=X.device)
+    dist = torch.empty((Q, k), dtype=torch.float32, device=X.device)
+    rc = load().lipfit_knn(X.data_ptr(), N, d, Xq.data_ptr(), Q, _np_ptr(m), int(side), int(norm),
+                           _np_ptr(w), int(k), idx.data_ptr(), dist.data_ptr(), _stream(stream))
+    _check(rc, "lipfit_knn")
+    return idx, dist
+
+
+def lipfit_smooth_objective(X, y, M: float, eps=None, mono_mask=None, norm: int = LIPFIT_L2,
+                            weights=None, p: float = 1.0, want_grad: bool = True, stream=None):
+    """(F python float, grad float32 CUDA tensor or None)."""
+    torch = _torch()
+    X, y = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y")
+    N, d = X.shape
+    m, w = _host_params(d, mono_mask, weights)
+    if eps is not None:
+        eps = _dev_f32(eps, 1, "eps")
+    grad = torch.empty(N, dtype=torch.float32, device=X.device) if want_grad else None
+    F = C.c_double(0.0)
+    rc = load().lipfit_smooth_objective(
+        X.data_ptr(), y.data_ptr(), N, d, float(M), _np_ptr(m), int(norm), _np_ptr(w), float(p),
+        None if eps is None else C.c_void_p(eps.data_ptr()), C.cast(C.byref(F), C.c_void_p),
+        None if grad is None else C.c_void_p(grad.data_ptr()), _stream(stream))
+    _check(rc, "lipfit_smooth_objective")
+    return float(F.value), grad
+
+
+def lipfit_smooth(X, y_inout, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                  p: float = 1.0, max_iter: int = 200, tol_grad: float = 1e-7, stream=None):
+    """Smooths y in place (y <- y + eps); returns (eps CUDA tensor, info dict)."""
+    torch = _torch()
+    X, y_inout = _dev_f32(X, 2, "X"), _dev_f32(y_inout, 1, "y_inout")
+    N, d = X.shape
+    m, w = _host_params(d, mono_mask, weights)
+    eps = torch.empty(N, dtype=torch.float32, device=X.device)
+    info = SmoothInfo()
+    rc = load().lipfit_smooth(X.data_ptr(), y_inout.data_ptr(), N, d, float(M), _np_ptr(m),
+                              int(norm), _np_ptr(w), float(p), int(max_iter), float(tol_grad),
+                              eps.data_ptr(), C.cast(C.byref(info), C.c_void_p), _stream(stream))
+    _check(rc, "lipfit_smooth")
+    return eps, info.as_dict()
+
+
+# ---------------------------------------------------------------------------------------------
+# Host-pointer entry points (numpy in, numpy out; copies happen inside the library)
+# ---------------------------------------------------------------------------------------------
+def _host_f32(a, ndim):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if a.ndim != ndim:
+        raise ValueError("bad rank")
+    return a
+
+
+def lipfit_bounds_host(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                       out=None, stream_ptr: Optional[int] = None):
+    """numpy in / numpy out through lipfit_bounds_host.  `out` may be a preallocated (e.g. pinned)
+    tuple of three float32 arrays of length Q."""
+    X, y, Xq = _host_f32(X, 2), _host_f32(y, 1), _host_f32(Xq, 2)
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _host_params(d, mono_mask, weights)
+    up, lo, g = out if out is not None else (np.empty(Q, np.float32) for _ in range(3))
+    rc = load().lipfit_bounds_host(_np_ptr(X), _np_ptr(y), N, d, _np_ptr(Xq), Q, float(M), _np_ptr(m),
+                                   int(norm), _np_ptr(w), _np_ptr(up), _np_ptr(lo), _np_ptr(g),
+                                   C.c_void_p(stream_ptr or 0))
+    _check(rc, "lipfit_bounds_host")
+    return up, lo, g
+
+
+def lipfit_knn_host(X, Xq, k: int, mono_mask=None, side: int = 0, norm: int = LIPFIT_L2,
+                    weights=None, stream_ptr: Optional[int] = None):
+    X, Xq = _host_f32(X, 2), _host_f32(Xq, 2)
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _host_params(d, mono_mask, weights)
+    idx = np.empty((Q, k), np.int32)
+    dist = np.empty((Q, k), np.float32)
+    rc = load().lipfit_knn_host(_np_ptr(X), N, d, _np_ptr(Xq), Q, _np_ptr(m), int(side), int(norm),
+                                _np_ptr(w), int(k), _np_ptr(idx), _np_ptr(dist),
+                                C.c_void_p(stream_ptr or 0))
+    _check(rc, "lipfit_knn_host")
+    return idx, dist
+
+
+def lipfit_smooth_host(X, y, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                       p: float = 1.0, max_iter: int = 200, tol_grad: float = 1e-7,
+                       stream_ptr: Optional[int] = None):
+    """Returns (y_smoothed, eps, info dict); the input y is not modified."""
+    X = _host_f32(X, 2)
+    y = np.array(y, dtype=np.float32, copy=True)
+    N, d = X.shape
+    m, w = _host_params(d, mono_mask, weights)
+    eps = np.empty(N, np.float32)
+    info = SmoothInfo()
+    rc = load().lipfit_smooth_host(_np_ptr(X), _np_ptr(y), N, d, float(M), _np_ptr(m), int(norm),
+                                   _np_ptr(w), float(p), int(max_iter), float(tol_grad), _np_ptr(eps),
+                                   C.cast(C.byref(info), C.c_void_p), C.c_void_p(stream_ptr or 0))
+    _check(rc, "lipfit_smooth_host")
+    return y, eps, info.as_dict()
+
+
+def lipfit_lbfgs(fun, x0, max_iter: int = 200, tol_grad: float = 1e-8, history: int = 20):
+    """Host LBFGS of the library on a Python callable fun(x) -> (f, grad).  No GPU involved."""
+    x = np.array(x0, dtype=np.float64, copy=True)
+    n = x.size
+
+    def _cb(_user, xp, fp, gp):
+        xv = np.ctypeslib.as_array(xp, shape=(n,))
+        f, g = fun(xv.copy())
+        fp[0] = float(f)
+        np.ctypeslib.as_array(gp, shape=(n,))[:] = g
+        return 0
+
+    cb = EVAL_FN(_cb)
+    info = SmoothInfo()
+    rc = load().lipfit_lbfgs(n, _np_ptr(x), cb, None, int(max_iter), float(tol_grad), int(history),
+                             C.cast(C.byref(info), C.c_void_p))
+    _check(rc, "lipfit_lbfgs")
+    return x, info.as_dict()

@@ -1,0 +1,183 @@
+// api.cu -- the extern "C" boundary declared in include/lipfit.h: argument validation, workspace,
+// and the order of device steps.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "kernels.h"
+#include "lbfgs.h"
+
+using namespace lipfit;
+
+namespace {
+
+int check_sizes(int64_t N, int32_t d, int64_t Q) {
+    if (d < 1 || d > LIPFIT_MAX_DIM) return LIPFIT_E_DIM;
+    if (N < 1 || Q < 0 || N > 0x7fffffffLL || Q > 0x7fffffffLL) return LIPFIT_E_SIZE;
+    return LIPFIT_OK;
+}
+int check_norm(int32_t norm) { return (norm >= 1 && norm <= 3) ? LIPFIT_OK : LIPFIT_E_PARAM; }
+int check_M(float M) { return (M >= 0.f && std::isfinite(M)) ? LIPFIT_OK : LIPFIT_E_PARAM; }
+
+// device copy of a host array (stream-ordered)
+template <class T>
+int to_device(Workspace& w, const T* host, size_t n, cudaStream_t s) {
+    int rc = w.alloc(n * sizeof(T), s);
+    if (rc) return rc;
+    if (n) LIPFIT_CUDA(cudaMemcpyAsync(w.p, host, n * sizeof(T), cudaMemcpyHostToDevice, s));
+    return LIPFIT_OK;
+}
+
+}  // namespace
+
+#define LIPFIT_API __attribute__((visibility("default")))
+extern "C" {
+
+const char* lipfit_status_string(int code) {
+    switch (code) {
+        case LIPFIT_OK: return "ok";
+        case LIPFIT_E_NULL: return "null pointer";
+        case LIPFIT_E_DIM: return "bad dimension (need 1 <= d <= 32)";
+        case LIPFIT_E_SIZE: return "bad size";
+        case LIPFIT_E_PARAM: return "bad parameter";
+        case LIPFIT_E_CUDA: return "CUDA error (no device or launch failure)";
+        case LIPFIT_E_NOMEM: return "out of device memory";
+        default: return "unknown status";
+    }
+}
+
+const char* lipfit_version(void) { return "0.1.0"; }
+
+int64_t lipfit_launch_count(void) { return g_launches.load(); }
+
+void lipfit_set_timing(int32_t on) { timing_set(on); }
+
+int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches) {
+    long long n = 0;
+    int rc = timing_get(which, total_ms, &n);
+    if (launches) *launches = n;
+    return rc;
+}
+
+int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, char* out, int32_t cap) {
+    if (!out || cap < 1) return LIPFIT_E_NULL;
+    if (check_norm(norm)) return LIPFIT_E_PARAM;
+    Xform xf;
+    int rc = make_xform(d, mono_mask, nullptr, false, false, &xf);
+    if (rc) return rc;
+    std::strncpy(out, bounds_variant_name(xf, norm), static_cast<size_t>(cap) - 1);
+    out[cap - 1] = '\0';
+    return LIPFIT_OK;
+}
+
+int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                  float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
+                  float* lower, float* g, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    if (!X || !y) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    RecLayout lay = bounds_layout(xf, norm);
+    if (lay.rf == 0) return LIPFIT_E_PARAM;
+    Workspace rec;
+    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
+    if (rc) return rc;
+    rc = launch_prepack(c, X, y, nullptr, N, xf, lay, rec.as<float>());
+    if (rc) return rc;
+    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xf, norm, M, upper, lower, g);
+}
+
+int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
+                       int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
+                       const float* weights, float* upper, float* lower, float* g,
+                       void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    Xform xf;
+    if ((rc = make_xform(d, mono_mask, weights, false, false, &xf))) return rc;
+    if (!X || !y || (Q > 0 && !Xq)) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    Workspace dX, dy, dXq, dout;
+    if ((rc = to_device(dX, X, static_cast<size_t>(N) * d, s))) return rc;
+    if ((rc = to_device(dy, y, static_cast<size_t>(N), s))) return rc;
+    if ((rc = to_device(dXq, Xq, static_cast<size_t>(Q) * d, s))) return rc;
+    if ((rc = dout.alloc(sizeof(float) * 3 * static_cast<size_t>(Q), s))) return rc;
+    float* du = upper ? dout.as<float>() : nullptr;
+    float* dl = lower ? dout.as<float>() + Q : nullptr;
+    float* dg = g ? dout.as<float>() + 2 * Q : nullptr;
+    rc = lipfit_bounds(dX.as<float>(), dy.as<float>(), N, d, dXq.as<float>(), Q, M, mono_mask, norm,
+                       weights, du, dl, dg, cuda_stream);
+    if (rc) return rc;
+    const size_t ob = sizeof(float) * static_cast<size_t>(Q);
+    if (upper && Q) LIPFIT_CUDA(cudaMemcpyAsync(upper, du, ob, cudaMemcpyDeviceToHost, s));
+    if (lower && Q) LIPFIT_CUDA(cudaMemcpyAsync(lower, dl, ob, cudaMemcpyDeviceToHost, s));
+    if (g && Q) LIPFIT_CUDA(cudaMemcpyAsync(g, dg, ob, cudaMemcpyDeviceToHost, s));
+    LIPFIT_CUDA(cudaStreamSynchronize(s));
+    return LIPFIT_OK;
+}
+
+int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+               const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights, int32_t k,
+               int32_t* idx, float* dist, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (k < 1 || k > N || k > LIPFIT_MAX_K) return LIPFIT_E_SIZE;
+    if (check_norm(norm) || side < -1 || side > 1) return LIPFIT_E_PARAM;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, side == 0, side < 0, &xf);
+    if (rc) return rc;
+    if (!X) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || !idx || !dist) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    RecLayout lay = knn_layout(xf, norm);
+    Workspace rec;
+    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
+    if (rc) return rc;
+    rc = launch_prepack(c, X, nullptr, nullptr, N, xf, lay, rec.as<float>());
+    if (rc) return rc;
+    return launch_knn(c, X, rec.as<float>(), N, Xq, Q, xf, norm, k, idx, dist);
+}
+
+int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                    const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
+                    int32_t k, int32_t* idx, float* dist, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (k < 1 || k > N || k > LIPFIT_MAX_K) return LIPFIT_E_SIZE;
+    if (check_norm(norm) || side < -1 || side > 1) return LIPFIT_E_PARAM;
+    Xform xf;
+    if ((rc = make_xform(d, mono_mask, weights, side == 0, side < 0, &xf))) return rc;
+    if (!X || (Q > 0 && (!Xq || !idx || !dist))) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    Workspace dX, dXq, di, dd;
+    if ((rc = to_device(dX, X, static_cast<size_t>(N) * d, s))) return rc;
+    if ((rc = to_device(dXq, Xq, static_cast<size_t>(Q) * d, s))) return rc;
+    const size_t n = static_cast<size_t>(Q) * k;
+    if ((rc = di.alloc(n * sizeof(int32_t), s))) return rc;
+    if ((rc = dd.alloc(n * sizeof(float), s))) return rc;
+    rc = lipfit_knn(dX.as<float>(), N, d, dXq.as<float>(), Q, mono_mask, side, norm, weights, k,
+                    di.as<int32_t>(), dd.as<float>(), cuda_stream);
+    if (rc) return rc;
+    if (n) {
+        LIPFIT_CUDA(cudaMemcpyAsync(idx, di.p, n * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
+        LIPFIT_CUDA(cudaMemcpyAsync(dist, dd.p, n * sizeof(float), cudaMemcpyDeviceToHost, s));
+    }
+    LIPFIT_CUDA(cudaStreamSynchronize(s));
+    return LIPFIT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,349 @@
+// bounds.cu -- step a2: fused distance + running min/max.
+//   upper[q] = min_k (y^k + M D^u),  lower[q] = max_k (y^k - M D^l),  g = (upper+lower)/2
+// Eq.(2),(3) PAPER.md:103-116 with the distance of Eq.(4) PAPER.md:142.  The Q x N distance matrix
+// of the paper's cdist+topk composition is never formed.
+//
+// Shape of the kernel: every thread keeps R queries (R x D coordinates) and their 2R running
+// extrema in registers; packed data records stream through shared memory in double-buffered tiles
+// filled by the TMA engine (cp.async.bulk + mbarrier) and are read with broadcast LDS.128, so one
+// 16-byte shared load feeds R pairs.  Work is cut into (query block, data chunk) tiles spread over a
+// persistent grid; with more than one chunk the partial extrema meet through atomicMin/atomicMax on
+// order-preserving integer keys (min/max are order independent, so the result is deterministic).
+#include "kernels.h"
+
+namespace lipfit {
+
+struct BoundsArgs {
+    const float* rec;
+    const float* Xq;
+    float* upper;
+    float* lower;
+    float* g;
+    uint32_t* keyU;
+    uint32_t* keyL;
+    int N, Q, d, rf, vslot;
+    int nqb, nch, chunk;
+    float M;
+    Xform xf;
+};
+
+template <int THREADS, int R>
+__device__ __forceinline__ int query_index(int qb, int r, int Q) {
+    int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+    return qi;
+}
+
+// Core = compile-time description of the pair arithmetic:
+//   Core::D      packed coordinates held per query
+//   Core::RF     floats per record (0 = runtime a.rf), Core::VSLOT value slot (-1 = runtime)
+//   Core::pair(q, rec_regs, ff, M, hi, lo)
+template <int NORM, int DU, int DC>
+struct SpecCore {
+    static constexpr int D = DU + DC;
+    static constexpr int RF = record_floats(D);
+    static constexpr int VSLOT = D;
+    static constexpr bool kGeneric = false;
+    static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags&,
+                                                float M, float& hi, float& lo) {
+        float au, al;
+        PairAcc<NORM, DU, DC>::run(q, x, au, al);
+        float y = x[VSLOT];
+        if (NORM == 2 && DC == 0) {
+            float dist = fast_sqrt(au);
+            hi = fmaf(M, dist, y);
+            lo = fmaf(-M, dist, y);
+        } else {
+            hi = fmaf(M, PairAcc<NORM, DU, DC>::finish(au), y);
+            lo = fmaf(-M, PairAcc<NORM, DU, DC>::finish(al), y);
+        }
+    }
+};
+
+template <int NORM, int DP>
+struct GenCore {
+    static constexpr int D = DP;
+    static constexpr int RF = DP + 4;
+    static constexpr int VSLOT = DP;
+    static constexpr bool kGeneric = true;
+    static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags& ff,
+                                                float M, float& hi, float& lo) {
+        float au, al;
+        PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+        float y = x[VSLOT];
+        hi = fmaf(M, PairAccGeneric<NORM, DP>::finish(au), y);
+        lo = fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), y);
+    }
+};
+
+template <int RF>
+__device__ __forceinline__ void load_record(const float* s, float* x) {
+#pragma unroll
+    for (int c = 0; c < RF / 4; ++c) {
+        float4 v = reinterpret_cast<const float4*>(s)[c];
+        x[4 * c + 0] = v.x;
+        x[4 * c + 1] = v.y;
+        x[4 * c + 2] = v.z;
+        x[4 * c + 3] = v.w;
+    }
+}
+
+template <int RF>
+__host__ __device__ constexpr int tile_records() {
+    return RF <= 8 ? 512 : (RF <= 16 ? 256 : (RF <= 24 ? 128 : 96));
+}
+
+template <class Core, int R, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+bounds_kernel(const BoundsArgs a, const FreeFlags ff) {
+    constexpr int D = Core::D;
+    constexpr int RF = Core::RF;
+    constexpr int TILE = tile_records<RF>();
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+
+    const int ntiles = a.nqb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int qb = tile / a.nch;
+        const int ch = tile - qb * a.nch;
+
+        // ---- queries of this block -> registers, transformed on the fly (Xform) ----
+        float q[R][D];
+        float U[R], L[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+            qi = qi < a.Q ? qi : a.Q - 1;
+            const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                if (Core::kGeneric)
+                    q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+                else
+                    q[r][j] = a.xf.sw[j] * __ldg(src + a.xf.perm[j]);
+            }
+            U[r] = __int_as_float(0x7f800000);
+            L[r] = __int_as_float(0xff800000);
+        }
+
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            int j = 0;
+            for (; j + 2 <= n; j += 2) {
+                float xa[RF], xb[RF];
+                load_record<RF>(s + j * RF, xa);
+                load_record<RF>(s + (j + 1) * RF, xb);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    float hia, loa, hib, lob;
+                    Core::pair(q[r], xa, ff, a.M, hia, loa);
+                    Core::pair(q[r], xb, ff, a.M, hib, lob);
+                    U[r] = fminf(fminf(U[r], hia), hib);  // FMNMX3
+                    L[r] = fmaxf(fmaxf(L[r], loa), lob);
+                }
+            }
+            if (j < n) {
+                float xa[RF];
+                load_record<RF>(s + j * RF, xa);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    float hia, loa;
+                    Core::pair(q[r], xa, ff, a.M, hia, loa);
+                    U[r] = fminf(U[r], hia);
+                    L[r] = fmaxf(L[r], loa);
+                }
+            }
+            rs.release(t);
+        }
+
+        // ---- results ----
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+            if (qi < a.Q) {
+                if (a.nch == 1) {
+                    if (a.upper) a.upper[qi] = U[r];
+                    if (a.lower) a.lower[qi] = L[r];
+                    if (a.g) a.g[qi] = 0.5f * (U[r] + L[r]);
+                } else {
+                    atomicMin(a.keyU + qi, f2key(U[r]));
+                    atomicMax(a.keyL + qi, f2key(L[r]));
+                }
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+bounds_finalize_kernel(const uint32_t* __restrict__ keyU, const uint32_t* __restrict__ keyL, int Q,
+                       float* __restrict__ upper, float* __restrict__ lower, float* __restrict__ g) {
+    int qi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (qi >= Q) return;
+    float U = key2f(keyU[qi]);
+    float L = key2f(keyL[qi]);
+    if (upper) upper[qi] = U;
+    if (lower) lower[qi] = L;
+    if (g) g[qi] = 0.5f * (U + L);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Host dispatch
+// ---------------------------------------------------------------------------------------------
+namespace {
+
+struct Variant {
+    int norm, dU, dC;  // generic: dU = DP, dC = -1
+    const char* name;
+    RecLayout lay;
+    // launches with the given R flavour (0 = big-R throughput kernel, 1 = small-R latency kernel)
+    int (*launch)(const Ctx&, BoundsArgs&, const FreeFlags&, int flavour);
+};
+
+template <class Core, int R, int THREADS, int MINB>
+int launch_one(const Ctx& c, BoundsArgs& a, const FreeFlags& ff) {
+    auto kern = bounds_kernel<Core, R, THREADS, MINB>;
+    int occ = 0;
+    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
+    if (occ < 1) occ = 1;
+    const int slots = c.num_sms * occ;
+    constexpr int TILE = tile_records<Core::RF>();
+    a.nqb = (a.Q + THREADS * R - 1) / (THREADS * R);
+    // Cut the data into chunks until there are >= 16 tiles per resident CTA (tail effect <= ~6 %),
+    // but keep a chunk at least 4 smem tiles long.
+    int want = (16 * slots + a.nqb - 1) / a.nqb;
+    int max_ch = (a.N + 4 * TILE - 1) / (4 * TILE);
+    int nch = want < 1 ? 1 : want;
+    if (nch > max_ch) nch = max_ch;
+    if (nch < 1) nch = 1;
+    int chunk = (a.N + nch - 1) / nch;
+    chunk = ((chunk + TILE - 1) / TILE) * TILE;
+    nch = (a.N + chunk - 1) / chunk;
+    a.nch = nch;
+    a.chunk = chunk;
+
+    Workspace keys;
+    if (nch > 1) {
+        int rc = keys.alloc(sizeof(uint32_t) * 2 * static_cast<size_t>(a.Q), c.stream);
+        if (rc) return rc;
+        a.keyU = keys.as<uint32_t>();
+        a.keyL = a.keyU + a.Q;
+        LIPFIT_CUDA(cudaMemsetAsync(a.keyU, 0xFF, sizeof(uint32_t) * a.Q, c.stream));
+        LIPFIT_CUDA(cudaMemsetAsync(a.keyL, 0x00, sizeof(uint32_t) * a.Q, c.stream));
+    }
+    long long ntiles = static_cast<long long>(a.nqb) * nch;
+    int grid = static_cast<int>(ntiles < slots ? ntiles : slots);
+    KernelTimer kt(TK_BOUNDS, c.stream);
+    kern<<<grid, THREADS, 0, c.stream>>>(a, ff);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    if (nch > 1) {
+        bounds_finalize_kernel<<<(a.Q + 255) / 256, 256, 0, c.stream>>>(a.keyU, a.keyL, a.Q, a.upper,
+                                                                      a.lower, a.g);
+        ++g_launches;
+        LIPFIT_CUDA(cudaGetLastError());
+    }
+    return LIPFIT_OK;
+}
+
+template <int NORM, int DU, int DC>
+int launch_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    using Core = SpecCore<NORM, DU, DC>;
+    constexpr int D = DU + DC;
+    constexpr int RBIG = (D <= 5) ? 8 : 4;
+    if (flavour == 0) return launch_one<Core, RBIG, 128, 2>(c, a, ff);
+    return launch_one<Core, 1, 128, 4>(c, a, ff);
+}
+
+template <int NORM, int DP>
+int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    using Core = GenCore<NORM, DP>;
+    constexpr int RBIG = (DP <= 8) ? 4 : (DP <= 16 ? 2 : 1);
+    if (flavour == 0 || RBIG == 1) return launch_one<Core, RBIG, 128, 2>(c, a, ff);
+    return launch_one<Core, 1, 128, 2>(c, a, ff);
+}
+
+#define SPEC(NORM, DU, DC, NAME) \
+    { NORM, DU, DC, NAME, {record_floats(DU + DC), DU + DC}, &launch_spec<NORM, DU, DC> }
+#define GEN(NORM, DP, NAME) \
+    { NORM, DP, -1, NAME, {DP + 4, DP}, &launch_gen<NORM, DP> }
+
+const Variant kVariants[] = {
+    // shapes of BASELINE.json configs 1, 2, 3, 5 (+ the symmetric versions of the same dims)
+    SPEC(2, 2, 0, "bounds<L2,U2,C0>"),
+    SPEC(1, 2, 2, "bounds<L1,U2,C2>"),
+    SPEC(3, 7, 1, "bounds<Linf,U7,C1>"),
+    SPEC(2, 0, 5, "bounds<L2,U0,C5>"),
+    SPEC(2, 3, 0, "bounds<L2,U3,C0>"),
+    SPEC(2, 0, 3, "bounds<L2,U0,C3>"),
+    SPEC(1, 4, 0, "bounds<L1,U4,C0>"),
+    SPEC(2, 4, 0, "bounds<L2,U4,C0>"),
+    SPEC(3, 8, 0, "bounds<Linf,U8,C0>"),
+    SPEC(2, 5, 0, "bounds<L2,U5,C0>"),
+    // generic fall-back (any mask / d up to 32): still a GPU kernel, never a CPU path
+    GEN(1, 4, "bounds_generic<L1,DP4>"), GEN(2, 4, "bounds_generic<L2,DP4>"),
+    GEN(3, 4, "bounds_generic<Linf,DP4>"),
+    GEN(1, 8, "bounds_generic<L1,DP8>"), GEN(2, 8, "bounds_generic<L2,DP8>"),
+    GEN(3, 8, "bounds_generic<Linf,DP8>"),
+    GEN(1, 16, "bounds_generic<L1,DP16>"), GEN(2, 16, "bounds_generic<L2,DP16>"),
+    GEN(3, 16, "bounds_generic<Linf,DP16>"),
+    GEN(1, 32, "bounds_generic<L1,DP32>"), GEN(2, 32, "bounds_generic<L2,DP32>"),
+    GEN(3, 32, "bounds_generic<Linf,DP32>"),
+};
+
+const Variant* pick(const Xform& xf, int norm) {
+    for (const Variant& v : kVariants)
+        if (v.dC >= 0 && v.norm == norm && v.dU == xf.dU && v.dC == xf.dC) return &v;
+    for (const Variant& v : kVariants)
+        if (v.dC < 0 && v.norm == norm && v.dU >= xf.d) return &v;
+    return nullptr;
+}
+
+}  // namespace
+
+RecLayout bounds_layout(const Xform& xf, int norm) {
+    const Variant* v = pick(xf, norm);
+    return v ? v->lay : RecLayout{0, 0};
+}
+
+const char* bounds_variant_name(const Xform& xf, int norm) {
+    const Variant* v = pick(xf, norm);
+    return v ? v->name : "none";
+}
+
+int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q,
+                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g) {
+    const Variant* v = pick(xf, norm);
+    if (!v) return LIPFIT_E_PARAM;
+    BoundsArgs a{};
+    a.rec = rec;
+    a.Xq = Xq;
+    a.upper = upper;
+    a.lower = lower;
+    a.g = g;
+    a.N = static_cast<int>(N);
+    a.Q = static_cast<int>(Q);
+    a.d = xf.d;
+    a.rf = v->lay.rf;
+    a.vslot = v->lay.vslot;
+    a.M = M;
+    a.xf = xf;
+    FreeFlags ff = make_free_flags(xf);
+    // Small problems (cannot fill the chip with R-query threads): one query per thread.
+    long long big_threads = (Q + 7) / 8;
+    int flavour = (big_threads < 2LL * c.num_sms * 128) ? 1 : 0;
+    return v->launch(c, a, ff, flavour);
+}
+
+}  // namespace lipfit

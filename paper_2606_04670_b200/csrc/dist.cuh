@@ -1,0 +1,165 @@
+// dist.cuh -- per-pair arithmetic of the monotone weighted distance, in registers.
+//
+// Packed coordinates (common.cuh, Xform): j < DU unconstrained, DU <= j < DU+DC constrained and
+// already mirrored/weighted, so with delta_j = q_j - x_j   (query minus datum)
+//   u_j = l_j = |delta_j|                       (unconstrained)
+//   u_j = max(delta_j, 0),  l_j = max(-delta_j, 0)   (constrained)       Eq.(4)
+//   D^u = ||u||_p,  D^l = ||l||_p.
+// NORM: 1 = L1, 2 = L2, 3 = Linf.
+#pragma once
+#include "common.cuh"
+
+namespace lipfit {
+
+// Accumulated "pre-norm" quantities: L1 -> sums, L2 -> sums of squares, Linf -> maxima.
+// S is the part shared by both sides (unconstrained coordinates); PU / PL the one-sided parts.
+template <int NORM, int DU, int DC>
+struct PairAcc {
+    // q, x: D = DU + DC packed coordinates in registers.
+    static __device__ __forceinline__ void run(const float* __restrict__ q,
+                                               const float* __restrict__ x, float& au, float& al) {
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < DU; ++j) {
+            float dlt = q[j] - x[j];
+            if (NORM == 1) s += fabsf(dlt);
+            if (NORM == 2) s = fmaf(dlt, dlt, s);
+            if (NORM == 3) s = fmaxf(s, fabsf(dlt));
+        }
+        float pu = s, pl = s;
+#pragma unroll
+        for (int j = DU; j < DU + DC; ++j) {
+            float dlt = q[j] - x[j];
+            if (NORM == 1) {
+                float r = fmaxf(dlt, 0.f);
+                pu += r;
+                pl += r - dlt;  // max(-dlt,0) == max(dlt,0) - dlt exactly (one of the two is 0)
+            }
+            if (NORM == 2) {
+                float r = fmaxf(dlt, 0.f);
+                float m = fminf(dlt, 0.f);
+                pu = fmaf(r, r, pu);
+                pl = fmaf(m, m, pl);
+            }
+            if (NORM == 3) {
+                pu = fmaxf(pu, dlt);  // pu >= 0 already, so max(pu, relu(dlt)) == max(pu, dlt)
+                pl = fmaxf(pl, -dlt);
+            }
+        }
+        au = pu;
+        al = pl;
+    }
+    // distance from the accumulated quantity
+    static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
+};
+
+// One-sided distance only (kNN): D^u accumulated quantity (squared for L2).
+template <int NORM, int DU, int DC>
+struct PairAccU {
+    static __device__ __forceinline__ float run(const float* __restrict__ q,
+                                                const float* __restrict__ x) {
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < DU; ++j) {
+            float dlt = q[j] - x[j];
+            if (NORM == 1) s += fabsf(dlt);
+            if (NORM == 2) s = fmaf(dlt, dlt, s);
+            if (NORM == 3) s = fmaxf(s, fabsf(dlt));
+        }
+#pragma unroll
+        for (int j = DU; j < DU + DC; ++j) {
+            float dlt = q[j] - x[j];
+            if (NORM == 1) s += fmaxf(dlt, 0.f);
+            if (NORM == 2) {
+                float r = fmaxf(dlt, 0.f);
+                s = fmaf(r, r, s);
+            }
+            if (NORM == 3) s = fmaxf(s, dlt);
+        }
+        return s;
+    }
+};
+
+// Generic (runtime mask) version over DP zero-padded coordinates: `fr[j]` is 1 for an
+// unconstrained coordinate and 0 for a constrained (or padding) one, so that
+//   u_j = max(delta, -fr*delta)  -> |delta| or relu(delta)
+//   l_j = max(-delta, fr*delta)  -> |delta| or relu(-delta)
+// without a branch.  Padding coordinates have x = q = 0, hence contribute 0 to every norm.
+struct FreeFlags {
+    float fr[kMaxDim];
+};
+
+template <int NORM, int DP>
+struct PairAccGeneric {
+    static __device__ __forceinline__ void run(const float* __restrict__ q,
+                                               const float* __restrict__ x, const FreeFlags& ff,
+                                               float& au, float& al) {
+        float pu = 0.f, pl = 0.f;
+#pragma unroll
+        for (int j = 0; j < DP; ++j) {
+            float dlt = q[j] - x[j];
+            float t = ff.fr[j] * dlt;
+            float u = fmaxf(dlt, -t);
+            float l = fmaxf(-dlt, t);
+            if (NORM == 1) {
+                pu += u;
+                pl += l;
+            }
+            if (NORM == 2) {
+                pu = fmaf(u, u, pu);
+                pl = fmaf(l, l, pl);
+            }
+            if (NORM == 3) {
+                pu = fmaxf(pu, u);
+                pl = fmaxf(pl, l);
+            }
+        }
+        au = pu;
+        al = pl;
+    }
+    static __device__ __forceinline__ float run_u(const float* __restrict__ q,
+                                                  const float* __restrict__ x,
+                                                  const FreeFlags& ff) {
+        float pu = 0.f;
+#pragma unroll
+        for (int j = 0; j < DP; ++j) {
+            float dlt = q[j] - x[j];
+            float u = fmaxf(dlt, -(ff.fr[j] * dlt));
+            if (NORM == 1) pu += u;
+            if (NORM == 2) pu = fmaf(u, u, pu);
+            if (NORM == 3) pu = fmaxf(pu, u);
+        }
+        return pu;
+    }
+    static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
+};
+
+// Uniform policy wrappers (used by the smoothing kernel): D coordinates per point, RF floats per
+// record, value slot VSLOT, run() -> accumulated (au, al), finish() -> distance.
+template <int NORM, int DU, int DC>
+struct SpecAcc {
+    static constexpr int D = DU + DC;
+    static constexpr int RF = record_floats(D);
+    static constexpr int VSLOT = D;
+    static constexpr bool kGeneric = false;
+    static __device__ __forceinline__ void run(const float* q, const float* x, const FreeFlags&,
+                                               float& au, float& al) {
+        PairAcc<NORM, DU, DC>::run(q, x, au, al);
+    }
+    static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
+};
+
+template <int NORM, int DP>
+struct GenAcc {
+    static constexpr int D = DP;
+    static constexpr int RF = DP + 4;
+    static constexpr int VSLOT = DP;
+    static constexpr bool kGeneric = true;
+    static __device__ __forceinline__ void run(const float* q, const float* x, const FreeFlags& ff,
+                                               float& au, float& al) {
+        PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+    }
+    static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
+};
+
+}  // namespace lipfit

@@ -1,0 +1,52 @@
+// kernels.h -- host-side launchers implemented in the .cu translation units.
+#pragma once
+#include "common.cuh"
+#include "dist.cuh"
+
+namespace lipfit {
+
+// Builds the Xform for (mask, weights); flip = true negates the mask first (used by kNN side=-1,
+// where D^l under mask s equals D^u under mask -s).  symmetric = true ignores the mask (R6).
+int make_xform(int32_t d, const int32_t* mono_mask, const float* weights, bool symmetric, bool flip,
+               Xform* xf);
+FreeFlags make_free_flags(const Xform& xf);
+
+// Record layout chosen by the kernel family that will consume the records: `rf` floats per
+// record (multiple of 4), packed coordinates in slots [0, d), the value (y or z) in slot `vslot`,
+// zeros elsewhere.
+struct RecLayout {
+    int rf, vslot;
+};
+RecLayout bounds_layout(const Xform& xf, int norm);
+RecLayout knn_layout(const Xform& xf, int norm);
+RecLayout smooth_layout(const Xform& xf, int norm);
+
+// a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].
+int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
+                   const Xform& xf, RecLayout lay, float* rec);
+
+// a2: fused bounds.  rec: packed records; Xq: ORIGINAL row-major queries (transformed on load).
+int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q,
+                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g);
+const char* bounds_variant_name(const Xform& xf, int norm);
+
+// a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
+int launch_knn(const Ctx& c, const float* X, const float* rec, int64_t N, const float* Xq, int64_t Q,
+               const Xform& xf, int norm, int k, int32_t* idx, float* dist);
+
+// a4: all-pairs objective/gradient.  rec holds z = y + eps in the value slot.
+// F_dev: device double (may be NULL); grad: device float (may be NULL); eps may be NULL (= 0).
+int launch_smooth_objective(const Ctx& c, const float* rec, int64_t N, const Xform& xf, int norm,
+                            float M, float p, const float* eps, double* F_dev, float* grad,
+                            double* maxviol_dev);
+
+// value-slot refresh: rec[k][vslot] = y[k] + eps[k]
+int launch_set_values(const Ctx& c, float* rec, RecLayout lay, const float* y, const float* eps,
+                      int64_t N);
+// y[k] += eps[k]
+int launch_axpy(const Ctx& c, float* y, const float* eps, int64_t N);
+
+void timing_set(int on);
+int timing_get(int which, double* ms, long long* n);
+
+}  // namespace lipfit

@@ -1,0 +1,173 @@
+// prepack.cu -- step a1: build the packed data records once per call so that
+// the mask, the weights and the coordinate order never reach the hot loops
+// ("a suitable modification to distance calculation, which avoids branching").
+// Pure streaming kernels (HBM-bound, microseconds).
+#include <cmath>
+#include <mutex>
+
+#include "kernels.h"
+
+namespace lipfit {
+
+std::atomic<int64_t> g_launches{0};
+
+std::atomic<int> g_timing_on{0};
+static std::mutex g_timing_mu;
+static double g_timing_ms[TK_COUNT] = {0, 0, 0};
+static long long g_timing_n[TK_COUNT] = {0, 0, 0};
+
+KernelTimer::KernelTimer(int which_, cudaStream_t s_) : which(which_), s(s_) {
+    if (!g_timing_on.load()) return;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return;
+    }
+    on = true;
+    cudaEventRecord(e0, s);
+}
+void KernelTimer::stop() {
+    if (!on) return;
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) == cudaSuccess) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess) {
+            std::lock_guard<std::mutex> lk(g_timing_mu);
+            g_timing_ms[which] += ms;
+            g_timing_n[which] += 1;
+        }
+    }
+    (void)cudaGetLastError();
+}
+KernelTimer::~KernelTimer() {
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+}
+void timing_set(int on) {
+    g_timing_on.store(on ? 1 : 0);
+    std::lock_guard<std::mutex> lk(g_timing_mu);
+    for (int i = 0; i < TK_COUNT; ++i) {
+        g_timing_ms[i] = 0;
+        g_timing_n[i] = 0;
+    }
+}
+int timing_get(int which, double* ms, long long* n) {
+    if (which < 0 || which >= TK_COUNT) return LIPFIT_E_PARAM;
+    std::lock_guard<std::mutex> lk(g_timing_mu);
+    if (ms) *ms = g_timing_ms[which];
+    if (n) *n = g_timing_n[which];
+    return LIPFIT_OK;
+}
+
+int make_ctx(void* cuda_stream, Ctx* ctx) {
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int dev = 0;
+    LIPFIT_CUDA(cudaGetDevice(&dev));
+    int sms = 0;
+    LIPFIT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    ctx->device = dev;
+    ctx->num_sms = sms;
+    return LIPFIT_OK;
+}
+
+int make_xform(int32_t d, const int32_t* mono_mask, const float* weights, bool symmetric, bool flip,
+               Xform* xf) {
+    if (d < 1 || d > kMaxDim) return LIPFIT_E_DIM;
+    int32_t s[kMaxDim];
+    for (int i = 0; i < d; ++i) {
+        int32_t m = mono_mask ? mono_mask[i] : 0;
+        if (m < -1 || m > 1) return LIPFIT_E_PARAM;
+        if (weights && !(weights[i] >= 0.f && std::isfinite(weights[i]))) return LIPFIT_E_PARAM;
+        s[i] = symmetric ? 0 : (flip ? -m : m);
+    }
+    int n = 0;
+    for (int i = 0; i < d; ++i)
+        if (s[i] == 0) {
+            xf->perm[n] = i;
+            xf->sw[n] = weights ? weights[i] : 1.f;
+            ++n;
+        }
+    xf->dU = n;
+    for (int i = 0; i < d; ++i)
+        if (s[i] != 0) {
+            xf->perm[n] = i;
+            xf->sw[n] = (weights ? weights[i] : 1.f) * (s[i] < 0 ? -1.f : 1.f);
+            ++n;
+        }
+    xf->dC = n - xf->dU;
+    xf->d = d;
+    for (int i = d; i < kMaxDim; ++i) {
+        xf->perm[i] = 0;
+        xf->sw[i] = 0.f;
+    }
+    return LIPFIT_OK;
+}
+
+FreeFlags make_free_flags(const Xform& xf) {
+    FreeFlags ff;
+    for (int j = 0; j < kMaxDim; ++j) ff.fr[j] = (j < xf.dU) ? 1.f : 0.f;
+    return ff;
+}
+
+// One thread per record; the record is assembled in registers and written as float4s.
+__global__ void __launch_bounds__(256)
+prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
+               const float* __restrict__ eps, int N, Xform xf, int rf, int vslot,
+               float* __restrict__ rec) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const float* src = X + static_cast<size_t>(k) * xf.d;
+    float* dst = rec + static_cast<size_t>(k) * rf;
+    float v = y ? y[k] : 0.f;
+    if (eps) v += eps[k];
+    for (int j0 = 0; j0 < rf; j0 += 4) {
+        float t[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            int j = j0 + c;
+            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : 0.f);
+        }
+        *reinterpret_cast<float4*>(dst + j0) = make_float4(t[0], t[1], t[2], t[3]);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+set_values_kernel(float* __restrict__ rec, int rf, int vslot, const float* __restrict__ y,
+                  const float* __restrict__ eps, int N) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    rec[static_cast<size_t>(k) * rf + vslot] = y[k] + (eps ? eps[k] : 0.f);
+}
+
+__global__ void __launch_bounds__(256)
+axpy_kernel(float* __restrict__ y, const float* __restrict__ eps, int N) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < N) y[k] += eps[k];
+}
+
+int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
+                   const Xform& xf, RecLayout lay, float* rec) {
+    int n = static_cast<int>(N);
+    prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, rec);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+int launch_set_values(const Ctx& c, float* rec, RecLayout lay, const float* y, const float* eps,
+                      int64_t N) {
+    int n = static_cast<int>(N);
+    set_values_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(rec, lay.rf, lay.vslot, y, eps, n);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+int launch_axpy(const Ctx& c, float* y, const float* eps, int64_t N) {
+    int n = static_cast<int>(N);
+    axpy_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(y, eps, n);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+}  // namespace lipfit

@@ -1,0 +1,130 @@
+"""GPU parity: lipfit_bounds (C-ABI, CUDA) vs the fp64 CPU oracle, element by element.
+
+Tolerance (BASELINE.json north_star): |gpu - oracle| <= 1e-5 * (max y - min y) for fp32 values.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from inputs import L1, L2, LINF, make_workload, random_problem
+
+pytestmark = pytest.mark.gpu
+
+NORMS = [L1, L2, LINF]
+
+
+def _gpu_bounds(X, y, Xq, M, mask, norm, w=None, want=("upper", "lower", "g")):
+    import torch
+    import paper_2606_04670_b200 as L
+    dev = torch.device("cuda:0")
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+    up, lo, g = L.lipfit_bounds(t(X), t(y), t(Xq), M, mask, norm, w, want)
+    torch.cuda.synchronize()
+    f = lambda v: None if v is None else v.cpu().numpy()
+    return f(up), f(lo), f(g)
+
+
+def _check(X, y, Xq, M, mask, norm, w=None, tol_scale=1.0):
+    U, L_, g = oracle.bounds(X, y, Xq, M, mask, norm, w)
+    up, lo, gg = _gpu_bounds(X, y, Xq, M, mask, norm, w)
+    rng = float(np.max(y) - np.min(y)) if len(y) > 1 else 1.0
+    rng = max(rng, 1e-30)
+    # 1e-5 * range is the stated bar; for M*D far above the data range the fp32 rounding of the
+    # candidate y + M*D itself (2^-24 relative) is added.
+    mag = np.maximum(np.abs(U), np.abs(L_)).max() if len(U) else 0.0
+    tol = tol_scale * (1e-5 * rng + (np.shape(X)[1] + 4) * 2.0 ** -24 * mag)
+    assert np.abs(up - U).max(initial=0) <= tol, (np.abs(up - U).max(), tol)
+    assert np.abs(lo - L_).max(initial=0) <= tol, (np.abs(lo - L_).max(), tol)
+    assert np.abs(gg - g).max(initial=0) <= tol
+    return up, lo, gg
+
+
+def test_config1_full():
+    wl = make_workload(1)
+    up, lo, g = _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm)
+    assert np.all(lo <= up + 1e-5 * wl.y_range)            # consistent data: sandwich (P2)
+    # interpolation (P1) within the fp32 tolerance
+    up, lo, g = _gpu_bounds(wl.X, wl.y, wl.X, wl.M, wl.mask, wl.norm)
+    assert np.abs(g - wl.y).max() <= 1e-5 * wl.y_range
+
+
+@pytest.mark.parametrize("cfg,N,Q", [(2, 3000, 5003), (3, 2500, 4099), (5, 3001, 4097),
+                                     (2, 40000, 700), (3, 70000, 300)])
+def test_configs_scaled(cfg, N, Q):
+    # sizes span several shared-memory tiles, a ragged tail, the direct and the chunked (atomic) paths
+    wl = make_workload(cfg, N=N, Q=Q)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights)
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("d,mask", [(1, [1]), (2, [0, 0]), (3, [1, -1, 0]), (4, [0, 0, 0, 0]),
+                                    (5, [1, 1, 1, 1, 1]), (5, [0, 0, 0, 0, 0]), (7, [0, 1, 0, -1, 0, 0, 1]),
+                                    (8, [0] * 8), (12, [1, 0] * 6), (17, [-1] * 17), (32, [0, 1, -1, 0] * 8)])
+def test_generic_and_specialised_shapes(norm, d, mask):
+    X, y, Xq = random_problem(100 + d, 1500, 777, d)
+    w = (0.25 + np.arange(d) % 3).astype(np.float32)
+    _check(X, y, Xq, 1.25, mask, norm, w)
+    _check(X, y, Xq, 0.5, mask, norm, None)
+
+
+@pytest.mark.parametrize("Q", [1, 31, 127, 128, 129, 1025])
+def test_ragged_query_counts(Q):
+    X, y, Xq = random_problem(7, 1000, Q, 4)
+    _check(X, y, Xq, 2.0, [1, 1, 0, 0], L1)
+
+
+@pytest.mark.parametrize("N", [1, 2, 511, 512, 513, 1027])
+def test_ragged_data_counts(N):
+    X, y, Xq = random_problem(8, N, 300, 2)
+    _check(X, y, Xq, 4.0, [0, 0], L2)
+
+
+def test_degenerate_cases():
+    import paper_2606_04670_b200 as L
+    import torch
+    X, y, Xq = random_problem(9, 100, 50, 3)
+    # M = 0: upper = min y, lower = max y (R9)
+    up, lo, g = _gpu_bounds(X, y, Xq, 0.0, None, L2)
+    assert np.all(up == y.min()) and np.all(lo == y.max())
+    # duplicates with different y, zero weights
+    X2 = np.concatenate([X, X[:10]])
+    y2 = np.concatenate([y, y[:10] + 1])
+    _check(X2, y2, Xq, 1.0, [1, 0, -1], LINF, np.array([0.0, 1.0, 2.0], np.float32))
+    # only some outputs requested
+    up, lo, g = _gpu_bounds(X, y, Xq, 1.0, None, L2, want=("g",))
+    assert up is None and lo is None and g is not None
+    # Q = 0 is OK and writes nothing
+    dev = torch.device("cuda:0")
+    t = lambda a: torch.from_numpy(a).to(dev)
+    up, lo, g = L.lipfit_bounds(t(X), t(y), t(Xq[:0]), 1.0)
+    assert up.numel() == 0
+    # bad arguments are reported, not crashed on
+    with pytest.raises(L.LipfitError):
+        L.lipfit_bounds(t(X), t(y), t(Xq), -1.0)
+    with pytest.raises(L.LipfitError):
+        L.lipfit_bounds(t(X), t(y), t(Xq), 1.0, [2, 0, 0])
+    with pytest.raises(L.LipfitError):
+        L.lipfit_bounds(t(X), t(y), t(Xq), 1.0, None, 9)
+
+
+def test_host_entry_point_matches_device_entry_point():
+    import paper_2606_04670_b200 as L
+    wl = make_workload(2, N=5000, Q=3000)
+    a = L.lipfit_bounds_host(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights)
+    b = _gpu_bounds(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights)
+    for u, v in zip(a, b):
+        np.testing.assert_array_equal(u, v)
+
+
+def test_properties_at_any_size():
+    """Monotone (P5) and sandwich-free properties that hold for any data, on the GPU output."""
+    wl = make_workload(2, N=20000, Q=4000)
+    base = wl.Xq.copy()
+    hi = base.copy()
+    hi[:, 0] += 0.05
+    hi[:, 1] += 0.02
+    a = _gpu_bounds(wl.X, wl.y, base, wl.M, wl.mask, wl.norm)
+    b = _gpu_bounds(wl.X, wl.y, hi, wl.M, wl.mask, wl.norm)
+    tol = 1e-5 * wl.y_range
+    for Ha, Hb in zip(a, b):
+        assert np.all(Hb >= Ha - tol)

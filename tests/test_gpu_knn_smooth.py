@@ -1,0 +1,194 @@
+"""GPU parity: lipfit_knn and the smoothing path vs the fp64 CPU oracle."""
+import numpy as np
+import pytest
+
+import oracle
+from inputs import L1, L2, LINF, make_workload, random_problem
+
+pytestmark = pytest.mark.gpu
+
+NORMS = [L1, L2, LINF]
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to("cuda:0")
+
+
+def _gpu_knn(X, Xq, k, mask=None, side=0, norm=L2, w=None):
+    import torch
+    import paper_2606_04670_b200 as L
+    idx, dist = L.lipfit_knn(_dev(X), _dev(Xq), k, mask, side, norm, w)
+    torch.cuda.synchronize()
+    return idx.cpu().numpy(), dist.cpu().numpy()
+
+
+def check_knn(X, Xq, k, mask=None, side=0, norm=L2, w=None):
+    """Acceptance rule (DESIGN.md §6 / SURVEY §8(c)): index sets equal the oracle's except among
+    candidates whose fp32-rounded oracle distance is within 1 ulp of the fp32-rounded k-th distance;
+    the sorted fp32 distance lists agree within 1 ulp."""
+    oi, od = oracle.knn(X, Xq, k, mask, side, norm, w)
+    gi, gd = _gpu_knn(X, Xq, k, mask, side, norm, w)
+    od32 = od.astype(np.float32)
+    assert np.all(np.diff(gd, axis=1) >= 0)
+    ulp = np.spacing(np.maximum(np.abs(od32), np.float32(1e-30)))
+    assert np.all(np.abs(gd - od32) <= ulp), np.abs(gd - od32).max()
+    bad = 0
+    for q in range(len(Xq)):
+        if np.array_equal(gi[q], oi[q]):
+            continue
+        so, sg = set(oi[q].tolist()), set(gi[q].tolist())
+        assert len(sg) == k and min(sg) >= 0 and max(sg) < len(X)
+        tau = od32[q, -1]
+        tie_lo = np.nextafter(tau, np.float32(-np.inf))
+        tie_hi = np.nextafter(tau, np.float32(np.inf))
+        # members that differ must be boundary ties (either set), identical elsewhere
+        for i in so ^ sg:
+            di = oracle.knn(X[i:i + 1], Xq[q:q + 1], 1, mask, side, norm, w)[1][0, 0]
+            assert tie_lo <= np.float32(di) <= tie_hi, (q, i, di, tau)
+        # equal sets in a different order are only allowed among equal fp32 distances
+        if so == sg:
+            pos = np.nonzero(gi[q] != oi[q])[0]
+            assert np.all(np.abs(gd[q, pos] - od32[q, pos]) <= ulp[q, pos])
+        bad += 1
+    return bad
+
+
+def test_config4_scaled():
+    wl = make_workload(4, N=30011, Q=1500)
+    check_knn(wl.X, wl.Xq, wl.k, None, 0, wl.norm)
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("d", [1, 3, 4, 7, 8, 16, 21, 32])
+def test_symmetric_dims(norm, d):
+    X, _, Xq = random_problem(200 + d, 5000, 300, d)
+    w = (0.5 + np.arange(d) % 2).astype(np.float32)
+    check_knn(X, Xq, 10, None, 0, norm, w)
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("side", [-1, 1])
+def test_one_sided(norm, side):
+    X, _, Xq = random_problem(31, 4000, 200, 5)
+    check_knn(X, Xq, 7, [1, -1, 0, 1, 0], side, norm)
+
+
+def test_many_exact_ties_on_a_grid():
+    rng = np.random.default_rng(3)
+    X = rng.integers(0, 6, (3000, 3)).astype(np.float32)
+    Xq = rng.integers(0, 6, (100, 3)).astype(np.float32)
+    check_knn(X, Xq, 20, None, 0, L2)
+    check_knn(X, Xq, 20, [1, 1, 0], 1, L1)
+
+
+@pytest.mark.parametrize("N,k", [(1, 1), (5, 5), (40, 33), (200, 128), (3000, 1), (3000, 128)])
+def test_k_extremes(N, k):
+    X, _, Xq = random_problem(5, N, 130, 4)
+    check_knn(X, Xq, k)
+
+
+def test_small_q_large_n_uses_chunks():
+    X, _, Xq = random_problem(6, 120000, 64, 8)
+    check_knn(X, Xq, 32)
+
+
+def test_knn_host_and_errors():
+    import paper_2606_04670_b200 as L
+    X, _, Xq = random_problem(7, 2000, 100, 4)
+    hi, hd = L.lipfit_knn_host(X, Xq, 5)
+    gi, gd = _gpu_knn(X, Xq, 5)
+    np.testing.assert_array_equal(hi, gi)
+    np.testing.assert_array_equal(hd, gd)
+    with pytest.raises(L.LipfitError):
+        L.lipfit_knn_host(X, Xq, 2001)
+    with pytest.raises(L.LipfitError):
+        L.lipfit_knn_host(X, Xq, 129)
+
+
+# --------------------------------------------------------------------------------------------
+# smoothing
+# --------------------------------------------------------------------------------------------
+def _gpu_obj(X, y, M, eps, mask, norm, w, p):
+    import torch
+    import paper_2606_04670_b200 as L
+    F, g = L.lipfit_smooth_objective(_dev(X), _dev(y), M, None if eps is None else _dev(eps), mask,
+                                     norm, w, p)
+    torch.cuda.synchronize()
+    return F, g.cpu().numpy()
+
+
+def check_objective(X, y, M, mask, norm, w, p, sigma=0.05, seed=0):
+    rng = np.random.default_rng(seed)
+    N = len(y)
+    for eps in (None, (sigma * rng.standard_normal(N)).astype(np.float32),
+                (sigma * rng.standard_normal(N)).astype(np.float32)):
+        e64 = np.zeros(N) if eps is None else eps.astype(np.float64)
+        F, grad = oracle.smooth_objective(X, y, M, e64, mask, norm, w, p)
+        Fg, gg = _gpu_obj(X, y, M, eps, mask, norm, w, p)
+        assert abs(Fg - F) <= 1e-5 * max(abs(F), 1e-30), (Fg, F)
+        gscale = max(np.abs(grad).max(), 1e-30)
+        assert np.abs(gg - grad).max() <= 1e-5 * gscale, (np.abs(gg - grad).max(), gscale)
+
+
+def test_objective_config5_scaled():
+    wl = make_workload(5, N=6007)
+    check_objective(wl.X, wl.y, wl.M, wl.mask, wl.norm, wl.weights, wl.p)
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("d,mask", [(2, None), (3, [1, 0, -1]), (5, [1] * 5), (8, [0, 1] * 4),
+                                    (13, [1] * 13), (32, [0] * 32)])
+def test_objective_shapes(norm, d, mask):
+    X, y, _ = random_problem(300 + d, 1300, 1, d, spread=0.3)
+    w = (0.5 + np.arange(d) % 2).astype(np.float32)
+    check_objective(X, y, 0.7, mask, norm, w, 0.5, sigma=0.2, seed=d)
+
+
+def test_objective_consistent_data_is_zero():
+    wl = make_workload(1, N=900)
+    F, g = _gpu_obj(wl.X, wl.y, wl.M, None, wl.mask, wl.norm, None, 1.0)
+    assert F == 0.0 and np.all(g == 0.0)
+
+
+@pytest.mark.parametrize("N", [2, 3, 50, 2000])
+def test_minimiser_parity(N):
+    """Unique minimiser (strong convexity, R14): GPU LBFGS result vs the oracle's minimiser."""
+    import torch
+    import paper_2606_04670_b200 as L
+    wl = make_workload(5, N=N)
+    if N <= 3:   # make the tiny cases inconsistent for sure
+        wl.y[:] = np.array([1.0, -1.0, 0.5][:N], np.float32)
+    eps_o, info_o = oracle.smooth(wl.X, wl.y, wl.M, wl.mask, wl.norm, None, wl.p)
+    yd = _dev(wl.y)
+    eps, info = L.lipfit_smooth(_dev(wl.X), yd, wl.M, wl.mask, wl.norm, None, wl.p, max_iter=500,
+                                tol_grad=1e-7)
+    torch.cuda.synchronize()
+    z_gpu = yd.cpu().numpy().astype(np.float64)
+    z_or = wl.y.astype(np.float64) + eps_o
+    rng = max(wl.y_range, 1e-30)
+    assert np.abs(z_gpu - z_or).max() <= 1e-5 * rng + 2e-6, (np.abs(z_gpu - z_or).max(), info, info_o)
+    np.testing.assert_allclose(eps.cpu().numpy() + wl.y, z_gpu, atol=1e-6)
+    assert info["F"] <= info["F0"]
+    assert info["max_violation"] <= info["max_violation0"] + 1e-7
+    assert abs(float(eps.sum().cpu())) <= 1e-3 * max(1.0, float(eps.abs().sum().cpu()))
+
+
+def test_smooth_then_bounds_config5_scaled():
+    """S(3): the GPU bounds on the GPU's smoothed z match the oracle bounds on the same z."""
+    import torch
+    import paper_2606_04670_b200 as L
+    wl = make_workload(5, N=4000, Q=3000)
+    yd = _dev(wl.y)
+    eps, info = L.lipfit_smooth(_dev(wl.X), yd, wl.M, wl.mask, wl.norm, None, wl.p, max_iter=200)
+    z = yd.cpu().numpy()
+    assert info["F"] < info["F0"] and info["max_violation"] < info["max_violation0"]
+    U, Lo, g = oracle.bounds(wl.X, z, wl.Xq, wl.M, wl.mask, wl.norm)
+    up, lo, gg = L.lipfit_bounds(_dev(wl.X), yd, _dev(wl.Xq), wl.M, wl.mask, wl.norm)
+    torch.cuda.synchronize()
+    tol = 1e-5 * wl.y_range
+    assert np.abs(up.cpu().numpy() - U).max() <= tol
+    assert np.abs(lo.cpu().numpy() - Lo).max() <= tol
+    assert np.abs(gg.cpu().numpy() - g).max() <= tol
+    ys, e2, info2 = L.lipfit_smooth_host(wl.X, wl.y, wl.M, wl.mask, wl.norm, None, wl.p, 200)
+    np.testing.assert_array_equal(ys, z)          # an evaluation is bit-reproducible
