@@ -1,46 +1,59 @@
 // knn.cu -- step a3: fused distance + per-query top-k.
 // Neighbours by distance d_(1) <= d_(2) <= ... without the cdist matrix + topk of
 // PAPER.md:206.  Two device passes:
-//   (1) selection in fp32: every thread keeps R queries in registers, streams packed records through
-//       shared memory (TMA bulk copies) and compares each pair's accumulated distance (squared for
-//       L2) with the query's current threshold tau = worst distance of its candidate list; only the
-//       rare pair that passes (k ln(N/k) of N) touches the list, a sorted array of ksel = k + margin
-//       entries kept in an L2-resident workspace laid out [slot][query] so that a warp's accesses
-//       coalesce;
+//   (1) selection in fp32.  Every thread keeps R queries in registers and streams packed records
+//       through shared memory (TMA bulk copies), exactly like the bounds kernel.  Per query it holds a
+//       threshold tau and a fill count in registers; a pair whose accumulated distance (squared for
+//       L2) is below tau is APPENDED (one 8-byte fire-and-forget store) to the query's candidate pool
+//       of P = 2*ksel entries, ksel = k + margin, in an L2-resident workspace.  When a pool is full
+//       the whole warp compacts it (rank by counting in shared memory), keeps the ksel best in sorted
+//       order and lowers tau to the ksel-th best.  tau only decreases, so the pool always contains
+//       the ksel best of the data seen so far, for ANY data order; a pool is compacted about
+//       log2(N/ksel) times, so the hot loop is the distance arithmetic plus one compare.
 //   (2) re-rank in fp64: the candidates' distances are recomputed in double from the ORIGINAL fp32
-//       inputs, ordered by (distance, index), and the first k are emitted (this makes
-//       the result independent of the fp32 selection arithmetic as long as the pool is a superset).
-#include <cfloat>
-
+//       inputs, ordered by (distance, index), and the first k are emitted (the result
+//       does not depend on the fp32 selection arithmetic as long as the pool is a superset).
 #include "kernels.h"
 
 namespace lipfit {
 
 constexpr int kKnnMargin = 8;
+constexpr int kSelThreads = 128;
+constexpr int kSelWarps = kSelThreads / 32;
+constexpr int kMaxP = 2 * (LIPFIT_MAX_K + kKnnMargin);  // 272 pool entries per (chunk, query)
 
 struct KnnArgs {
     const float* rec;
     const float* Xq;
-    float* Ld;   // [nch][ksel][Qp]
-    int32_t* Li; // [nch][ksel][Qp]
-    int N, Q, Qp, d, ksel;
+    int2* pool;     // [nch][Qp][P]  (x = distance bits, y = datum index)
+    int32_t* fill;  // [nch][Qp]     valid entries of each pool at kernel end
+    int N, Q, Qp, d, ksel, P;
     int nqb, nch, chunk;
     Xform xf;
 };
 
-__device__ __noinline__ float knn_insert(float* Ld, int32_t* Li, size_t stride, int ksel, float dv,
-                                         int32_t iv) {
-    int p = ksel - 1;
-    while (p > 0) {
-        float prev = Ld[(p - 1) * stride];
-        if (!(prev > dv)) break;
-        Ld[p * stride] = prev;
-        Li[p * stride] = Li[(p - 1) * stride];
-        --p;
+// Warp-cooperative compaction of one pool of n entries: keeps the ksel smallest (distance, index)
+// in slots [0, ksel) in ascending order and returns the ksel-th smallest distance (the new tau).
+// All 32 lanes must call it; `scr` is this warp's shared scratch of >= n + 1 entries.
+__device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2* scr, int lane) {
+    for (int c = lane; c < n; c += 32) scr[c] = pool[c];
+    __syncwarp();
+    for (int c = lane; c < n; c += 32) {
+        const int2 e = scr[c];
+        const float de = __int_as_float(e.x);
+        int rank = 0;
+        for (int o = 0; o < n; ++o) {
+            const int2 f = scr[o];
+            const float df = __int_as_float(f.x);
+            rank += (df < de) || (df == de && f.y < e.y);
+        }
+        if (rank < ksel) pool[rank] = e;
+        if (rank == ksel - 1) scr[kMaxP] = e;
     }
-    Ld[p * stride] = dv;
-    Li[p * stride] = iv;
-    return Ld[(ksel - 1) * stride];
+    __syncwarp();
+    const float tau = __int_as_float(scr[kMaxP].x);
+    __syncwarp();
+    return tau;
 }
 
 template <int DP>
@@ -48,12 +61,14 @@ __host__ __device__ constexpr int knn_tile_records() {
     return DP <= 8 ? 512 : (DP <= 16 ? 256 : 128);
 }
 
-template <int NORM, int DP, bool ONESIDED, int R, int THREADS>
-__global__ void __launch_bounds__(THREADS, 2)
+template <int NORM, int DP, bool ONESIDED, int R>
+__global__ void __launch_bounds__(kSelThreads, 3)
 knn_select_kernel(const KnnArgs a, const FreeFlags ff) {
+    constexpr int THREADS = kSelThreads;
     constexpr int TILE = knn_tile_records<DP>();
     __shared__ __align__(128) float sbuf[2 * TILE * DP];
     __shared__ __align__(8) uint64_t bars[2];
+    __shared__ int2 scratch[kSelWarps][kMaxP + 1];
     if (threadIdx.x == 0) {
         mbar_init(&bars[0], 1);
         mbar_init(&bars[1], 1);
@@ -61,6 +76,9 @@ knn_select_kernel(const KnnArgs a, const FreeFlags ff) {
     }
     __syncthreads();
     uint32_t phase = 0;
+    const int lane = threadIdx.x & 31;
+    int2* scr = scratch[threadIdx.x >> 5];
+    const int P = a.P, ksel = a.ksel;
 
     const int ntiles = a.nqb * a.nch;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -68,21 +86,21 @@ knn_select_kernel(const KnnArgs a, const FreeFlags ff) {
         const int ch = tile - qb * a.nch;
         float q[R][DP];
         float tau[R];
-        int qidx[R];
+        int fill[R];
+        const int q0 = qb * R * THREADS + static_cast<int>(threadIdx.x);  // query of r: q0 + r*THREADS
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
-            qidx[r] = qi;
-            int qc = qi < a.Q ? qi : a.Q - 1;
+            const int qi = q0 + r * THREADS;
+            const int qc = qi < a.Q ? qi : a.Q - 1;
             const float* src = a.Xq + static_cast<size_t>(qc) * a.d;
 #pragma unroll
             for (int j = 0; j < DP; ++j)
                 q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
-            tau[r] = __int_as_float(0x7f800000);
+            // padding lanes (qi >= Q) never accept a candidate
+            tau[r] = (qi < a.Q) ? __int_as_float(0x7f800000) : __int_as_float(0xff800000);
+            fill[r] = 0;
         }
-        const size_t stride = static_cast<size_t>(a.Qp);
-        float* Ld = a.Ld + static_cast<size_t>(ch) * a.ksel * stride;
-        int32_t* Li = a.Li + static_cast<size_t>(ch) * a.ksel * stride;
+        int2* pool0 = a.pool + (static_cast<size_t>(ch) * a.Qp + q0) * P;  // pool of r: + r*THREADS*P
 
         const int begin = ch * a.chunk;
         const int end = min(a.N, begin + a.chunk);
@@ -102,87 +120,110 @@ knn_select_kernel(const KnnArgs a, const FreeFlags ff) {
                     x[4 * c + 3] = v.w;
                 }
                 float sv[R];
-                bool any = false;
+                bool hit = false;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     sv[r] = ONESIDED ? PairAccGeneric<NORM, DP>::run_u(q[r], x, ff)
                                      : PairAccU<NORM, DP, 0>::run(q[r], x);
-                    any |= (sv[r] < tau[r]);
+                    hit |= (sv[r] < tau[r]);
                 }
-                if (any) {
+                if (__any_sync(0xffffffffu, hit)) {  // warp-uniform: rare after the first records
+                    bool full = false;
 #pragma unroll
-                    for (int r = 0; r < R; ++r)
-                        if (sv[r] < tau[r] && qidx[r] < a.Q)
-                            tau[r] = knn_insert(Ld + qidx[r], Li + qidx[r], stride, a.ksel, sv[r],
-                                                base + j);
+                    for (int r = 0; r < R; ++r) {
+                        if (sv[r] < tau[r]) {
+                            pool0[static_cast<size_t>(r) * THREADS * P + fill[r]] =
+                                make_int2(__float_as_int(sv[r]), base + j);
+                            ++fill[r];
+                            full |= (fill[r] == P);
+                        }
+                    }
+                    if (__any_sync(0xffffffffu, full)) {
+                        __syncwarp();  // orders the appends above before the cooperative reads below
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            unsigned m = __ballot_sync(0xffffffffu, fill[r] == P);
+                            while (m) {
+                                const int src = __ffs(m) - 1;
+                                m &= m - 1;
+                                int2* pq = a.pool + (static_cast<size_t>(ch) * a.Qp + q0 - lane + src +
+                                                     static_cast<size_t>(r) * THREADS) * P;
+                                const float nt = knn_compact(pq, P, ksel, scr, lane);
+                                if (lane == src) {
+                                    tau[r] = nt;
+                                    fill[r] = ksel;
+                                }
+                            }
+                        }
+                    }
                 }
             }
             rs.release(t);
         }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int qi = q0 + r * THREADS;
+            a.fill[static_cast<size_t>(ch) * a.Qp + qi] = fill[r];
+        }
     }
 }
 
-__global__ void __launch_bounds__(256)
-knn_fill_kernel(float* __restrict__ Ld, int32_t* __restrict__ Li, size_t n) {
-    size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-    if (i < n) {
-        Ld[i] = __int_as_float(0x7f800000);
-        Li[i] = -1;
-    }
-}
-
-// One warp per query.  Pool = nch * ksel candidates (index -1 = empty slot).
+// ---------------------------------------------------------------------------------------------
+// (2) fp64 re-rank.  One warp per query; candidates = the valid entries of its nch pools.
+// ---------------------------------------------------------------------------------------------
 struct RerankArgs {
     const float* X;
     const float* Xq;
-    const int32_t* Li;
+    const int2* pool;
+    const int32_t* fill;
     int32_t* idx;
     float* dist;
-    int N, Q, Qp, d, pool, k, norm;
+    int N, Q, Qp, d, P, nch, k, norm;
     Xform xf;  // perm/sw of the ORIGINAL coordinates; dU tells which packed coords are free
 };
 
 constexpr int kRerankWarps = 4;
-constexpr int kMaxPool = 768;
+constexpr int kMaxCand = 768;
 
 __global__ void __launch_bounds__(kRerankWarps * 32)
 knn_rerank_kernel(const RerankArgs a) {
-    __shared__ double sd[kRerankWarps][kMaxPool];
-    __shared__ int32_t si[kRerankWarps][kMaxPool];
+    __shared__ double sd[kRerankWarps][kMaxCand];
+    __shared__ int32_t si[kRerankWarps][kMaxCand];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int qi = blockIdx.x * kRerankWarps + warp;
     if (qi >= a.Q) return;
     const float* xq = a.Xq + static_cast<size_t>(qi) * a.d;
-    for (int c = lane; c < a.pool; c += 32) {
-        int32_t id = a.Li[static_cast<size_t>(c) * a.Qp + qi];
-        double acc = 0.0;
-        if (id >= 0) {
+    int total = 0;
+    for (int ch = 0; ch < a.nch; ++ch) {
+        const int nf = a.fill[static_cast<size_t>(ch) * a.Qp + qi];
+        const int2* pq = a.pool + (static_cast<size_t>(ch) * a.Qp + qi) * a.P;
+        for (int c = lane; c < nf; c += 32) {
+            const int32_t id = pq[c].y;
             const float* xk = a.X + static_cast<size_t>(id) * a.d;
+            double acc = 0.0;
             for (int j = 0; j < a.d; ++j) {
-                int o = a.xf.perm[j];
-                double sw = static_cast<double>(a.xf.sw[j]);
-                double dlt = sw * (static_cast<double>(xq[o]) - static_cast<double>(xk[o]));
-                double comp = (j < a.xf.dU) ? fabs(dlt) : fmax(dlt, 0.0);
+                const int o = a.xf.perm[j];
+                const double sw = static_cast<double>(a.xf.sw[j]);
+                const double dlt = sw * (static_cast<double>(xq[o]) - static_cast<double>(xk[o]));
+                const double comp = (j < a.xf.dU) ? fabs(dlt) : fmax(dlt, 0.0);
                 if (a.norm == 1) acc += comp;
                 else if (a.norm == 2) acc += comp * comp;
                 else acc = fmax(acc, comp);
             }
             if (a.norm == 2) acc = sqrt(acc);
-        } else {
-            acc = __longlong_as_double(0x7ff0000000000000LL);
-            id = 0x7fffffff;
+            sd[warp][total + c] = acc;
+            si[warp][total + c] = id;
         }
-        sd[warp][c] = acc;
-        si[warp][c] = id;
+        total += nf;
     }
     __syncwarp();
-    for (int c = lane; c < a.pool; c += 32) {
-        double dc = sd[warp][c];
-        int32_t ic = si[warp][c];
+    for (int c = lane; c < total; c += 32) {
+        const double dc = sd[warp][c];
+        const int32_t ic = si[warp][c];
         int rank = 0;
-        for (int o = 0; o < a.pool; ++o) {
-            double d2 = sd[warp][o];
-            int32_t i2 = si[warp][o];
+        for (int o = 0; o < total; ++o) {
+            const double d2 = sd[warp][o];
+            const int32_t i2 = si[warp][o];
             rank += (d2 < dc) || (d2 == dc && i2 < ic);
         }
         if (rank < a.k) {
@@ -194,19 +235,22 @@ knn_rerank_kernel(const RerankArgs a) {
 
 namespace {
 
+int knn_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
+constexpr int knn_r(int dp) { return dp <= 8 ? 8 : (dp <= 16 ? 4 : 2); }
+
 template <int NORM, int DP, bool ONESIDED>
-int launch_select(const Ctx& c, KnnArgs& a, const FreeFlags& ff) {
-    constexpr int R = (DP <= 8) ? 8 : (DP <= 16 ? 4 : 2);
-    constexpr int THREADS = 128;
-    auto kern = knn_select_kernel<NORM, DP, ONESIDED, R, THREADS>;
-    int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
-    if (occ < 1) occ = 1;
-    const int slots = c.num_sms * occ;
+int launch_select(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int slots_hint, bool query_only) {
+    constexpr int R = knn_r(DP);
+    auto kern = knn_select_kernel<NORM, DP, ONESIDED, R>;
+    if (query_only) {  // occupancy query used by the host to size the decomposition
+        int occ = 0;
+        LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSelThreads, 0));
+        return occ < 1 ? 1 : occ;
+    }
     long long ntiles = static_cast<long long>(a.nqb) * a.nch;
-    int grid = static_cast<int>(ntiles < slots ? ntiles : slots);
+    int grid = static_cast<int>(ntiles < slots_hint ? ntiles : slots_hint);
     KernelTimer kt(TK_KNN_SELECT, c.stream);
-    kern<<<grid, THREADS, 0, c.stream>>>(a, ff);
+    kern<<<grid, kSelThreads, 0, c.stream>>>(a, ff);
     kt.stop();
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
@@ -214,17 +258,26 @@ int launch_select(const Ctx& c, KnnArgs& a, const FreeFlags& ff) {
 }
 
 template <int NORM, bool ONESIDED>
-int dispatch_dp(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int dp) {
+int dispatch_dp(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int dp, int slots, bool query_only) {
     switch (dp) {
-        case 4: return launch_select<NORM, 4, ONESIDED>(c, a, ff);
-        case 8: return launch_select<NORM, 8, ONESIDED>(c, a, ff);
-        case 16: return launch_select<NORM, 16, ONESIDED>(c, a, ff);
-        default: return launch_select<NORM, 32, ONESIDED>(c, a, ff);
+        case 4: return launch_select<NORM, 4, ONESIDED>(c, a, ff, slots, query_only);
+        case 8: return launch_select<NORM, 8, ONESIDED>(c, a, ff, slots, query_only);
+        case 16: return launch_select<NORM, 16, ONESIDED>(c, a, ff, slots, query_only);
+        default: return launch_select<NORM, 32, ONESIDED>(c, a, ff, slots, query_only);
     }
 }
 
-int knn_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
-int knn_r(int dp) { return dp <= 8 ? 8 : (dp <= 16 ? 4 : 2); }
+int dispatch(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int norm, bool onesided, int dp, int slots,
+             bool query_only) {
+    if (norm == 1)
+        return onesided ? dispatch_dp<1, true>(c, a, ff, dp, slots, query_only)
+                        : dispatch_dp<1, false>(c, a, ff, dp, slots, query_only);
+    if (norm == 2)
+        return onesided ? dispatch_dp<2, true>(c, a, ff, dp, slots, query_only)
+                        : dispatch_dp<2, false>(c, a, ff, dp, slots, query_only);
+    return onesided ? dispatch_dp<3, true>(c, a, ff, dp, slots, query_only)
+                    : dispatch_dp<3, false>(c, a, ff, dp, slots, query_only);
+}
 
 }  // namespace
 
@@ -241,61 +294,66 @@ int launch_knn(const Ctx& c, const float* X, const float* rec, int64_t N, const 
     a.d = xf.d;
     a.xf = xf;
     a.ksel = static_cast<int>(N < k + kKnnMargin ? N : k + kKnnMargin);
-    const int qper = 128 * knn_r(dp);
+    a.P = 2 * a.ksel;
+    const int qper = kSelThreads * knn_r(dp);
     a.nqb = (a.Q + qper - 1) / qper;
     a.Qp = a.nqb * qper;
-    // Data chunks: only when the query blocks alone cannot fill the chip (small Q, large N).
-    int nch = 1;
-    const int slots = c.num_sms * 2;
-    if (a.nqb < slots) {
-        nch = (slots + a.nqb - 1) / a.nqb;
-        int max_ch = kMaxPool / a.ksel;
-        if (nch > max_ch) nch = max_ch;
-        int by_n = a.N / (4 * a.ksel);
-        if (nch > by_n) nch = by_n;
-        if (nch < 1) nch = 1;
-    }
+    FreeFlags ff = make_free_flags(xf);
+    const bool onesided = xf.dC > 0;
+    const int occ = dispatch(c, a, ff, norm, onesided, dp, 0, true);
+    if (occ < 0) return occ;
+    const int slots = c.num_sms * occ;
+
+    // Data chunks: the fewest (<= 8, pools must fit the re-rank) that keep the last wave of the
+    // persistent grid >= 94 % full; every chunk keeps its own pools, merged by the re-rank.
     const int tile = dp <= 8 ? 512 : (dp <= 16 ? 256 : 128);
+    int max_ch = kMaxCand / a.P;
+    if (max_ch > 8) max_ch = 8;
+    int by_n = a.N / (8 * a.P);
+    if (max_ch > by_n) max_ch = by_n;
+    if (max_ch < 1) max_ch = 1;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int nch = 1; nch <= max_ch; ++nch) {
+        long long tiles = static_cast<long long>(a.nqb) * nch;
+        long long waves = (tiles + slots - 1) / slots;
+        double eff = static_cast<double>(tiles) / static_cast<double>(waves * slots);
+        if (eff > best_eff + 1e-9) {
+            best_eff = eff;
+            best = nch;
+        }
+        if (eff >= 0.94) break;
+    }
+    int nch = best;
     int chunk = (a.N + nch - 1) / nch;
     chunk = ((chunk + tile - 1) / tile) * tile;
     nch = (a.N + chunk - 1) / chunk;
     a.nch = nch;
     a.chunk = chunk;
 
-    const size_t entries = static_cast<size_t>(nch) * a.ksel * a.Qp;
-    Workspace wd, wi;
-    int rc = wd.alloc(entries * sizeof(float), c.stream);
+    Workspace wp, wf;
+    int rc = wp.alloc(sizeof(int2) * static_cast<size_t>(nch) * a.Qp * a.P, c.stream);
     if (rc) return rc;
-    rc = wi.alloc(entries * sizeof(int32_t), c.stream);
+    rc = wf.alloc(sizeof(int32_t) * static_cast<size_t>(nch) * a.Qp, c.stream);
     if (rc) return rc;
-    a.Ld = wd.as<float>();
-    a.Li = wi.as<int32_t>();
-    knn_fill_kernel<<<static_cast<unsigned>((entries + 255) / 256), 256, 0, c.stream>>>(a.Ld, a.Li,
-                                                                                       entries);
-    ++g_launches;
-    LIPFIT_CUDA(cudaGetLastError());
-
-    FreeFlags ff = make_free_flags(xf);
-    const bool onesided = xf.dC > 0;
-    if (norm == 1)
-        rc = onesided ? dispatch_dp<1, true>(c, a, ff, dp) : dispatch_dp<1, false>(c, a, ff, dp);
-    else if (norm == 2)
-        rc = onesided ? dispatch_dp<2, true>(c, a, ff, dp) : dispatch_dp<2, false>(c, a, ff, dp);
-    else
-        rc = onesided ? dispatch_dp<3, true>(c, a, ff, dp) : dispatch_dp<3, false>(c, a, ff, dp);
+    a.pool = wp.as<int2>();
+    a.fill = wf.as<int32_t>();
+    rc = dispatch(c, a, ff, norm, onesided, dp, slots, false);
     if (rc) return rc;
 
     RerankArgs r{};
     r.X = X;
     r.Xq = Xq;
-    r.Li = a.Li;
+    r.pool = a.pool;
+    r.fill = a.fill;
     r.idx = idx;
     r.dist = dist;
     r.N = a.N;
     r.Q = a.Q;
     r.Qp = a.Qp;
     r.d = a.d;
-    r.pool = nch * a.ksel;
+    r.P = a.P;
+    r.nch = nch;
     r.k = k;
     r.norm = norm;
     r.xf = xf;
