@@ -82,9 +82,12 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d,
 /* ---- k nearest data per query by distance (d_(1) <= d_(2) <= ...) -------------
  * side 0: symmetric weighted norm, mask ignored; +1: D^u; -1: D^l.
  * idx [Q*k] int32 and dist [Q*k] fp32, row-major, ascending distance per query.
- * Selection runs in fp32 on a pool of k + margin candidates; the pool is then re-ranked
- * in fp64 from the original fp32 inputs, sorted by (distance, index), so the returned set
- * equals the exact one except among candidates whose fp32-rounded distances tie. */
+ * Selection runs in fp32 (symmetric L2: cross-term key ||x||^2 - 2 q.x) on a pool of k + margin
+ * candidates; the pool is re-ranked in fp64 from the original fp32 inputs, sorted by
+ * (distance, index); a per-query certificate (exact k-th distance below every pool threshold
+ * minus a bound of the fp32 key error) proves the pool contained the answer, and the rare
+ * queries where it fails are redone by an exact fp64 scan.  The returned set is therefore the
+ * exact fp64 one (ties by lower index); dist is the fp64 distance rounded to fp32. */
 int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
                const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
                int32_t k, int32_t* idx, float* dist, void* cuda_stream);
@@ -150,6 +153,10 @@ int64_t lipfit_launch_count(void);
  * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);
 int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches);
+/* Number of queries of the most recent lipfit_knn / lipfit_knn_host call (any thread) whose
+ * superset certificate failed and that were therefore answered by the exact fp64 fallback
+ * scan; valid once that call's stream has been synchronised.  0 on typical data. */
+int64_t lipfit_knn_fallbacks(void);
 /* Name of the kernel variant lipfit_bounds would dispatch to for (d, mask, norm), e.g.
  * "bounds<L1,U2,C2,R8>" or "bounds_generic<L2,DP8>"; writes at most `cap` bytes incl. NUL. */
 int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, char* out, int32_t cap);

@@ -21,7 +21,7 @@ EXPORTS = [
     "lipfit_bounds", "lipfit_bounds_host", "lipfit_knn", "lipfit_knn_host",
     "lipfit_smooth_objective", "lipfit_smooth", "lipfit_smooth_host", "lipfit_lbfgs",
     "lipfit_status_string", "lipfit_version", "lipfit_launch_count", "lipfit_bounds_variant",
-    "lipfit_set_timing", "lipfit_get_timing",
+    "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
 ]
 
 
@@ -70,6 +70,8 @@ def load():
     lib.lipfit_version.restype = C.c_char_p
     lib.lipfit_launch_count.restype = C.c_int64
     lib.lipfit_set_timing.restype = None
+    lib.lipfit_knn_fallbacks.argtypes = []
+    lib.lipfit_knn_fallbacks.restype = i64
     lib.lipfit_set_timing.argtypes = [i32]
     lib.lipfit_get_timing.argtypes = [i32, P, P]
     _lib = lib
@@ -86,6 +88,11 @@ def version() -> str:
 
 def launch_count() -> int:
     return int(load().lipfit_launch_count())
+
+
+def knn_fallbacks() -> int:
+    """Queries of the last lipfit_knn call answered by the exact fp64 fallback (after a sync)."""
+    return int(load().lipfit_knn_fallbacks())
 
 
 def set_timing(on: bool) -> None:

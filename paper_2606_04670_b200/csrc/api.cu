@@ -70,6 +70,8 @@ int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, cha
     return LIPFIT_OK;
 }
 
+int64_t lipfit_knn_fallbacks(void) { return knn_last_fallbacks(); }
+
 int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                   float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
                   float* lower, float* g, void* cuda_stream) {
@@ -142,13 +144,7 @@ int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
-    RecLayout lay = knn_layout(xf, norm);
-    Workspace rec;
-    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
-    if (rc) return rc;
-    rc = launch_prepack(c, X, nullptr, nullptr, N, xf, lay, rec.as<float>());
-    if (rc) return rc;
-    return launch_knn(c, X, rec.as<float>(), N, Xq, Q, xf, norm, k, idx, dist);
+    return launch_knn(c, X, N, Xq, Q, xf, norm, k, idx, dist);
 }
 
 int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,

@@ -191,6 +191,63 @@ struct RecordStream {
     __device__ __forceinline__ void release(int) { __syncthreads(); }
 };
 
+
+// Decoupled multi-stage stream of packed records through shared memory (no CTA-wide barrier per tile).
+//   buf: STAGES * TILE * rf floats (16-byte aligned), full: STAGES mbarriers (count 1),
+//   done: STAGES ints in shared memory (zeroed once), NW = warps of the CTA (all of them consume).
+// A warp that has finished tile t bumps done[t % STAGES]; the LAST warp to do so refills that stage
+// with tile t + STAGES, so warps drift up to STAGES-1 tiles apart instead of meeting at a barrier
+// every tile.  (Every LDS of the tile has completed before the bump: its values were consumed by
+// arithmetic issued earlier in program order.)  Consecutive streams of one CTA are separated by the
+// __syncthreads() in the constructor.
+template <int TILE, int STAGES, int NW>
+struct RecordPipe {
+    const float* rec;
+    float* buf;
+    uint64_t* full;
+    int* done;
+    int rf, begin, end, ntiles;
+    uint32_t* phase;  // per-thread parities of the STAGES full barriers
+
+    __device__ __forceinline__ RecordPipe(const float* rec_, int rf_, int begin_, int end_, float* buf_,
+                                          uint64_t* full_, int* done_, uint32_t* phase_)
+        : rec(rec_), buf(buf_), full(full_), done(done_), rf(rf_), begin(begin_), end(end_),
+          phase(phase_) {
+        ntiles = (end - begin + TILE - 1) / TILE;
+        __syncthreads();  // every warp has left the previous stream of this CTA
+        if (threadIdx.x == 0)
+            for (int t = 0; t < STAGES && t < ntiles; ++t) issue(t);
+    }
+    __device__ __forceinline__ int count(int t) const {
+        int n = end - (begin + t * TILE);
+        return n < TILE ? n : TILE;
+    }
+    __device__ __forceinline__ void issue(int t) {
+        const int b = t % STAGES;
+        const uint32_t bytes = static_cast<uint32_t>(count(t)) * rf * 4u;
+        mbar_arrive_expect_tx(&full[b], bytes);
+        bulk_g2s(buf + static_cast<size_t>(b) * TILE * rf,
+                 rec + static_cast<size_t>(begin + t * TILE) * rf, bytes, &full[b]);
+    }
+    __device__ __forceinline__ const float* acquire(int t) {
+        const int b = t % STAGES;
+        mbar_wait(&full[b], (*phase >> b) & 1u);
+        *phase ^= (1u << b);
+        return buf + static_cast<size_t>(b) * TILE * rf;
+    }
+    __device__ __forceinline__ void release(int t) {
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) {
+            const int b = t % STAGES;
+            const int old = atomicAdd(&done[b], 1);
+            if ((old % NW) == NW - 1 && t + STAGES < ntiles) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                issue(t + STAGES);
+            }
+        }
+    }
+};
+
 #endif  // __CUDACC__
 
 }  // namespace lipfit

@@ -18,7 +18,6 @@ struct RecLayout {
     int rf, vslot;
 };
 RecLayout bounds_layout(const Xform& xf, int norm);
-RecLayout knn_layout(const Xform& xf, int norm);
 RecLayout smooth_layout(const Xform& xf, int norm);
 
 // a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].
@@ -31,8 +30,11 @@ int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, in
 const char* bounds_variant_name(const Xform& xf, int norm);
 
 // a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
-int launch_knn(const Ctx& c, const float* X, const float* rec, int64_t N, const float* Xq, int64_t Q,
-               const Xform& xf, int norm, int k, int32_t* idx, float* dist);
+int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
+               int norm, int k, int32_t* idx, float* dist);
+const char* knn_variant_name(const Xform& xf, int norm);
+// queries of the most recent completed lipfit_knn call that needed the exact fp64 fallback
+int64_t knn_last_fallbacks();
 
 // a4: all-pairs objective/gradient.  rec holds z = y + eps in the value slot.
 // F_dev: device double (may be NULL); grad: device float (may be NULL); eps may be NULL (= 0).

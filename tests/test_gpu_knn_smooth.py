@@ -93,6 +93,35 @@ def test_small_q_large_n_uses_chunks():
     check_knn(X, Xq, 32)
 
 
+def test_certificate_and_exact_fallback():
+    """The selection pool is certified per query; where the certificate fails (ties beyond the
+    margin) the exact fp64 scan answers, so integer-grid data match the oracle EXACTLY, lower
+    index first (R7), through both fallback branches (candidate list / k rounds)."""
+    import paper_2606_04670_b200 as L
+    # general position: nothing needs the fallback
+    wl = make_workload(4, N=20000, Q=700)
+    check_knn(wl.X, wl.Xq, wl.k, None, 0, wl.norm)
+    assert L.knn_fallbacks() == 0
+    # integer grid, one data chunk: dozens of exact ties straddle the k-th place and the pool threshold
+    rng = np.random.default_rng(11)
+    X = rng.integers(0, 5, (1000, 3)).astype(np.float32)
+    Xq = rng.integers(0, 5, (150, 3)).astype(np.float32)
+    for norm, mask, side in ((L2, None, 0), (L1, None, 0), (LINF, [1, 0, -1], 1)):
+        oi, od = oracle.knn(X, Xq, 24, mask, side, norm)
+        gi, gd = _gpu_knn(X, Xq, 24, mask, side, norm)
+        assert L.knn_fallbacks() > 0
+        np.testing.assert_array_equal(gi, oi)
+        np.testing.assert_array_equal(gd, od.astype(np.float32))
+    # all data identical: more than 768 candidates tie -> the k-round branch
+    X = np.ones((2000, 4), np.float32)
+    Xq = rng.standard_normal((40, 4)).astype(np.float32)
+    gi, gd = _gpu_knn(X, Xq, 9)
+    assert L.knn_fallbacks() == 40
+    np.testing.assert_array_equal(gi, np.tile(np.arange(9, dtype=np.int32), (40, 1)))
+    oi, od = oracle.knn(X, Xq, 9)
+    np.testing.assert_array_equal(gd, od.astype(np.float32))
+
+
 def test_knn_host_and_errors():
     import paper_2606_04670_b200 as L
     X, _, Xq = random_problem(7, 2000, 100, 4)
