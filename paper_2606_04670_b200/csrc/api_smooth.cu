@@ -61,9 +61,9 @@ int lipfit_smooth_objective(const float* X, const float* y, int64_t N, int32_t d
     if (rc) return rc;
     rc = fdev.alloc(sizeof(double) * 2, c.stream);
     if (rc) return rc;
-    rc = launch_prepack(c, X, y, eps, N, xf, lay, rec.as<float>());
+    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>());
     if (rc) return rc;
-    rc = launch_smooth_objective(c, rec.as<float>(), N, xf, norm, M, p, eps,
+    rc = launch_smooth_objective(c, rec.as<float>(), y, eps, N, xf, norm, p,
                                  F ? fdev.as<double>() : nullptr, grad, nullptr);
     if (rc) return rc;
     if (F) {
@@ -97,7 +97,7 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
     if ((rc = eps_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = grad_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = fv_h.alloc(sizeof(double) * 2))) return rc;
-    rc = launch_prepack(c, X, y_inout, nullptr, N, xf, lay, rec.as<float>());
+    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>());
     if (rc) return rc;
 
     std::vector<double> viol;  // max violation seen by each evaluation
@@ -105,10 +105,8 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
         float* eh = eps_h.as<float>();
         for (size_t i = 0; i < n; ++i) eh[i] = static_cast<float>(x[i]);
         LIPFIT_CUDA(cudaMemcpyAsync(eps_d.p, eh, sizeof(float) * n, cudaMemcpyHostToDevice, c.stream));
-        int r = launch_set_values(c, rec.as<float>(), lay, y_inout, eps_d.as<float>(), N);
-        if (r) return r;
-        r = launch_smooth_objective(c, rec.as<float>(), N, xf, norm, M, p, eps_d.as<float>(),
-                                    fv_d.as<double>(), grad_d.as<float>(), fv_d.as<double>() + 1);
+        int r = launch_smooth_objective(c, rec.as<float>(), y_inout, eps_d.as<float>(), N, xf, norm, p,
+                                        fv_d.as<double>(), grad_d.as<float>(), fv_d.as<double>() + 1);
         if (r) return r;
         LIPFIT_CUDA(cudaMemcpyAsync(grad_h.p, grad_d.p, sizeof(float) * n, cudaMemcpyDeviceToHost,
                                     c.stream));

@@ -136,28 +136,37 @@ struct PairAccGeneric {
 
 // Uniform policy wrappers (used by the smoothing kernel): D coordinates per point, RF floats per
 // record, value slot VSLOT, run() -> accumulated (au, al), finish() -> distance.
-template <int NORM, int DU, int DC>
+template <int NORM_, int DU, int DC>
 struct SpecAcc {
     static constexpr int D = DU + DC;
     static constexpr int RF = record_floats(D);
     static constexpr int VSLOT = D;
+    static constexpr int NORM = NORM_;
     static constexpr bool kGeneric = false;
     static __device__ __forceinline__ void run(const float* q, const float* x, const FreeFlags&,
                                                float& au, float& al) {
         PairAcc<NORM, DU, DC>::run(q, x, au, al);
     }
+    // one-sided accumulated quantity of D^u only
+    static __device__ __forceinline__ float run_u(const float* q, const float* x, const FreeFlags&) {
+        return PairAccU<NORM, DU, DC>::run(q, x);
+    }
     static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
 };
 
-template <int NORM, int DP>
+template <int NORM_, int DP>
 struct GenAcc {
     static constexpr int D = DP;
     static constexpr int RF = DP + 4;
     static constexpr int VSLOT = DP;
+    static constexpr int NORM = NORM_;
     static constexpr bool kGeneric = true;
     static __device__ __forceinline__ void run(const float* q, const float* x, const FreeFlags& ff,
                                                float& au, float& al) {
         PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+    }
+    static __device__ __forceinline__ float run_u(const float* q, const float* x, const FreeFlags& ff) {
+        return PairAccGeneric<NORM, DP>::run_u(q, x, ff);
     }
     static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
 };

@@ -36,11 +36,14 @@ const char* knn_variant_name(const Xform& xf, int norm);
 // queries of the most recent completed lipfit_knn call that needed the exact fp64 fallback
 int64_t knn_last_fallbacks();
 
-// a4: all-pairs objective/gradient.  rec holds z = y + eps in the value slot.
+// a4: all-pairs objective/gradient.  base: packed records whose coordinates are PRE-MULTIPLIED BY M
+// (prepack with scale_xform(xf, M)); their value slot is ignored, z = y + eps is formed per call.
 // F_dev: device double (may be NULL); grad: device float (may be NULL); eps may be NULL (= 0).
-int launch_smooth_objective(const Ctx& c, const float* rec, int64_t N, const Xform& xf, int norm,
-                            float M, float p, const float* eps, double* F_dev, float* grad,
+int launch_smooth_objective(const Ctx& c, const float* base, const float* y, const float* eps, int64_t N,
+                            const Xform& xf, int norm, float p, double* F_dev, float* grad,
                             double* maxviol_dev);
+// xf with every coordinate factor multiplied by s
+Xform scale_xform(const Xform& xf, float s);
 
 // value-slot refresh: rec[k][vslot] = y[k] + eps[k]
 int launch_set_values(const Ctx& c, float* rec, RecLayout lay, const float* y, const float* eps,

@@ -102,6 +102,12 @@ int make_xform(int32_t d, const int32_t* mono_mask, const float* weights, bool s
     return LIPFIT_OK;
 }
 
+Xform scale_xform(const Xform& xf, float s) {
+    Xform o = xf;
+    for (int j = 0; j < kMaxDim; ++j) o.sw[j] = xf.sw[j] * s;
+    return o;
+}
+
 FreeFlags make_free_flags(const Xform& xf) {
     FreeFlags ff;
     for (int j = 0; j < kMaxDim; ++j) ff.fr[j] = (j < xf.dU) ? 1.f : 0.f;

@@ -3,151 +3,242 @@
 // d_ik / y_k - y_i matrices are its memory wall).
 //
 // With z = y + eps, D_ik = d_s(x^k, x^i) and V_ik = (z_i - z_k - M D_ik)_+ (reading R12):
-//   F = ||eps||^2 / p + 2 sum_{i != k} V_ik^2 = ||eps||^2/p + sum_i sum_k (V_ik^2 + V_ki^2)
-//   dF/deps_i = 2 eps_i / p + 4 sum_k (V_ik - V_ki).
-// Row formulation: a thread owns R rows i (coordinates + z_i in registers) and sweeps the data k
-// through shared memory exactly like the bounds kernel; the pair (i,k) yields both V_ik (from D^u of
-// datum k seen from x^i) and V_ki (from D^l).  The k = i term is 0 by itself (D = 0, z_i - z_i = 0).
-// fp32 pair arithmetic; sums leave the shared-memory tile in fp64; (row block, chunk) partials are
-// combined in a fixed order, so an evaluation is bit-reproducible.
+//   F = ||eps||^2 / p + 2 sum_{i != k} V_ik^2,      dF/deps_i = 2 eps_i / p + 4 sum_k (V_ik - V_ki).
+// V_ik > 0 needs z_i > z_k, so of the two ordered pairs (i,k), (k,i) at most one contributes.  Every
+// evaluation therefore
+//   (1) sorts the data by z (cub radix sort of N keys: microseconds) and gathers the packed records
+//       [M x'_0 .. M x'_{d-1}, z] in that order (coordinates are pre-multiplied by M once per call);
+//   (2) visits every UNORDERED pair once -- row i against the data k < i of the sorted order, where
+//       only V_ik can be non-zero: one one-sided distance per pair, no sign select;
+//   (3) pre-filters on the squared quantity (L2: sum (M u_j)^2 < (z_i - z_k)^2, no square root); the
+//       rare surviving pairs (~1e-5 of all) take a slow path that forms V, adds V^2 to F, +V to row i
+//       and -V to row k.  Gradient sums are kept in 2^-40 fixed point (64-bit integer atomics): exact,
+//       hence independent of the order of the atomics -- an evaluation is bit-reproducible.
+// Kernel shape as in bounds.cu: R rows per thread in registers, data tiles through shared memory via
+// the TMA engine (decoupled 4-stage pipe); work items (row block, data chunk) of the lower triangle
+// are handed out by an atomic counter.
+#include <cub/device/device_radix_sort.cuh>
+
 #include "kernels.h"
 
 namespace lipfit {
 
+constexpr int kSmThreads = 128;
+constexpr int kSmWarps = kSmThreads / 32;
+constexpr int kSmStages = 4;
+constexpr int kSmChunk = 4096;  // data records per work item (multiple of every tile size)
+constexpr double kFix = 1099511627776.0;  // 2^40
+
 struct SmoothArgs {
-    const float* rec;
-    double* gpart;  // [nch][N]   sum_k (V_ik - V_ki) over the chunk
-    double* fpart;  // [ntiles]   sum of (V_ik^2 + V_ki^2) over the tile
-    double* vpart;  // [ntiles]   max violation over the tile
-    int N, nrb, nch, chunk;
-    float M;
+    const float* rec;         // sorted records [N][RF]
+    unsigned long long* gfix; // [N] sum_k (V_ik - V_ki) of sorted position i, 2^-40 fixed point
+    double* fpart;            // [nitems] sum of V^2 over the item
+    float* vpart;             // [nitems] max V over the item
+    int* counter;             // work counter
+    int N, nrb, maxc, nitems;
 };
 
 template <int RF>
 __host__ __device__ constexpr int smooth_tile_records() {
-    return RF <= 8 ? 512 : (RF <= 16 ? 256 : (RF <= 24 ? 128 : 96));
+    return RF <= 8 ? 256 : (RF <= 20 ? 128 : 64);
 }
 
-template <class Acc, int R, int THREADS>
-__global__ void __launch_bounds__(THREADS, 2)
+template <int RF>
+__device__ __forceinline__ void smooth_load_record(const float* s, float* x) {
+#pragma unroll
+    for (int c = 0; c < RF / 4; ++c) {
+        float4 v = reinterpret_cast<const float4*>(s)[c];
+        x[4 * c + 0] = v.x;
+        x[4 * c + 1] = v.y;
+        x[4 * c + 2] = v.z;
+        x[4 * c + 3] = v.w;
+    }
+}
+
+// Slow path for one datum k (sorted position kpos): rows whose pre-filter passed form V.
+template <class Acc, int R>
+__device__ __forceinline__ void smooth_hit(const SmoothArgs& a, const float (&acc)[R], const float (&dz)[R],
+                                           const bool (&pass)[R], int kpos, long long (&grow)[R],
+                                           double& fd, float& vmax) {
+    long long col = 0;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (pass[r]) {
+            const float D = Acc::NORM == 2 ? __fsqrt_rn(acc[r]) : acc[r];  // M * distance
+            const float V = dz[r] - D;
+            if (V > 0.f) {
+                fd += static_cast<double>(V) * static_cast<double>(V);
+                const long long vf = __double2ll_rn(static_cast<double>(V) * kFix);
+                grow[r] += vf;
+                col += vf;
+                vmax = fmaxf(vmax, V);
+            }
+        }
+    }
+    if (col != 0) atomicAdd(a.gfix + kpos, static_cast<unsigned long long>(-col));
+}
+
+template <class Acc, int R>
+__global__ void __launch_bounds__(kSmThreads, 4)
 smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
+    constexpr int THREADS = kSmThreads;
     constexpr int D = Acc::D;
     constexpr int RF = Acc::RF;
     constexpr int TILE = smooth_tile_records<RF>();
-    __shared__ __align__(128) float sbuf[2 * TILE * RF];
-    __shared__ __align__(8) uint64_t bars[2];
-    __shared__ double redf[THREADS / 32];
-    __shared__ float redv[THREADS / 32];
+    constexpr int ST = kSmStages;
+    constexpr int RB = THREADS * R;
+    __shared__ __align__(128) float sbuf[ST * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[ST];
+    __shared__ int done[ST];
+    __shared__ int s_item;
+    __shared__ double redf[kSmWarps];
+    __shared__ float redv[kSmWarps];
     if (threadIdx.x == 0) {
-        mbar_init(&bars[0], 1);
-        mbar_init(&bars[1], 1);
+#pragma unroll
+        for (int b = 0; b < ST; ++b) {
+            mbar_init(&bars[b], 1);
+            done[b] = 0;
+        }
         mbar_fence_init();
     }
-    __syncthreads();
     uint32_t phase = 0;
-    const int ntiles = a.nrb * a.nch;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int rb = tile / a.nch;
-        const int ch = tile - rb * a.nch;
+    for (;;) {
+        __syncthreads();  // s_item and the reduction scratch of the previous item are free
+        if (threadIdx.x == 0) s_item = atomicAdd(a.counter, 1);
+        __syncthreads();
+        const int item = s_item;
+        if (item >= a.nitems) break;
+        const int rb = a.nrb - 1 - item / a.maxc;
+        const int ch = item - (item / a.maxc) * a.maxc;
+        const int row0 = rb * RB;
+        const int rowend = min(a.N, row0 + RB);
+        const int begin = ch * kSmChunk;
+        const int end = min(begin + kSmChunk, rowend - 1);  // k < i <= rowend - 1
+        if (begin >= end) {
+            if (threadIdx.x == 0) {
+                a.fpart[item] = 0.0;
+                a.vpart[item] = 0.f;
+            }
+            continue;
+        }
+        // ---- rows of this block -> registers ----
         float xi[R][D], zi[R];
-        double fd[R], gd[R];
-        float vmax = 0.f;
+        int ipos[R];
+        long long grow[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            int i = (rb * R + r) * THREADS + static_cast<int>(threadIdx.x);
-            int ic = i < a.N ? i : a.N - 1;
-            const float* src = a.rec + static_cast<size_t>(ic) * RF;
+            const int i = row0 + r * THREADS + static_cast<int>(threadIdx.x);
+            ipos[r] = i;
+            grow[r] = 0;
+            if (i < a.N) {
+                const float* src = a.rec + static_cast<size_t>(i) * RF;
 #pragma unroll
-            for (int j = 0; j < D; ++j) xi[r][j] = __ldg(src + j);
-            zi[r] = __ldg(src + Acc::VSLOT);
-            fd[r] = 0.0;
-            gd[r] = 0.0;
+                for (int j = 0; j < D; ++j) xi[r][j] = __ldg(src + j);
+                zi[r] = __ldg(src + Acc::VSLOT);
+            } else {  // padding row: an infinite distance to everything, never passes the filter
+#pragma unroll
+                for (int j = 0; j < D; ++j) xi[r][j] = 1e30f;
+                zi[r] = 0.f;
+            }
         }
-        const int begin = ch * a.chunk;
-        const int end = min(a.N, begin + a.chunk);
-        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        double fd = 0.0;
+        float vmax = 0.f;
+        RecordPipe<TILE, ST, kSmWarps> rs(a.rec, RF, begin, end, sbuf, bars, done, &phase);
         for (int t = 0; t < rs.ntiles; ++t) {
             const float* s = rs.acquire(t);
             const int n = rs.count(t);
-            float ft[R], gt[R];
-#pragma unroll
-            for (int r = 0; r < R; ++r) ft[r] = gt[r] = 0.f;
-#pragma unroll 2
+            const int base = begin + t * TILE;
+            const bool below = (base + n <= row0);  // every k of the tile precedes every row of the block
             for (int j = 0; j < n; ++j) {
                 float x[RF];
-#pragma unroll
-                for (int c = 0; c < RF / 4; ++c) {
-                    float4 v = reinterpret_cast<const float4*>(s + j * RF)[c];
-                    x[4 * c + 0] = v.x;
-                    x[4 * c + 1] = v.y;
-                    x[4 * c + 2] = v.z;
-                    x[4 * c + 3] = v.w;
-                }
+                smooth_load_record<RF>(s + j * RF, x);
                 const float zk = x[Acc::VSLOT];
+                float acc[R], dz[R];
+                bool pass[R];
+                bool hit = false;
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    float au, al;
-                    Acc::run(xi[r], x, ff, au, al);
-                    float dz = zi[r] - zk;
-                    float vik = fmaxf(fmaf(-a.M, Acc::finish(au), dz), 0.f);
-                    float vki = fmaxf(fmaf(-a.M, Acc::finish(al), -dz), 0.f);
-                    ft[r] = fmaf(vik, vik, ft[r]);
-                    ft[r] = fmaf(vki, vki, ft[r]);
-                    gt[r] += vik - vki;
-                    vmax = fmaxf(vmax, fmaxf(vik, vki));
+                    acc[r] = Acc::run_u(xi[r], x, ff);
+                    dz[r] = zi[r] - zk;
+                    pass[r] = Acc::NORM == 2 ? (acc[r] < dz[r] * dz[r]) : (acc[r] < dz[r]);
+                    if (!below) pass[r] = pass[r] && (base + j < ipos[r]) && (dz[r] > 0.f);
+                    hit |= pass[r];
                 }
-            }
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                fd[r] += static_cast<double>(ft[r]);
-                gd[r] += static_cast<double>(gt[r]);
+                if (__any_sync(0xffffffffu, hit))  // warp-uniform, rare
+                    smooth_hit<Acc, R>(a, acc, dz, pass, base + j, grow, fd, vmax);
             }
             rs.release(t);
         }
-        // ---- per-row gradient partials, per-tile objective partial ----
-        double fsum = 0.0;
+        // ---- row sums -> fixed-point atomics; per-item objective partial (fixed order) ----
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            int i = (rb * R + r) * THREADS + static_cast<int>(threadIdx.x);
-            if (i < a.N) {
-                a.gpart[static_cast<size_t>(ch) * a.N + i] = gd[r];
-                fsum += fd[r];
-            }  // rows past N are clamped duplicates of row N-1: not counted (their vmax is harmless)
-        }
+        for (int r = 0; r < R; ++r)
+            if (grow[r] != 0) atomicAdd(a.gfix + ipos[r], static_cast<unsigned long long>(grow[r]));
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            fsum += __shfl_xor_sync(0xffffffffu, fsum, o);
+            fd += __shfl_xor_sync(0xffffffffu, fd, o);
             vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
         }
         if ((threadIdx.x & 31) == 0) {
-            redf[threadIdx.x >> 5] = fsum;
+            redf[threadIdx.x >> 5] = fd;
             redv[threadIdx.x >> 5] = vmax;
         }
         __syncthreads();
         if (threadIdx.x == 0) {
             double f = 0.0;
             float v = 0.f;
-            for (int w = 0; w < THREADS / 32; ++w) {
+            for (int w = 0; w < kSmWarps; ++w) {
                 f += redf[w];
                 v = fmaxf(v, redv[w]);
             }
-            a.fpart[tile] = f;
-            a.vpart[tile] = static_cast<double>(v);
+            a.fpart[item] = f;
+            a.vpart[item] = v;
         }
-        __syncthreads();
     }
 }
 
-// grad[i] = 2 eps_i / p + 4 sum_ch gpart[ch][i]; per-block partial of sum eps^2.
+// z = y + eps and the identity permutation (sort input)
 __global__ void __launch_bounds__(256)
-smooth_grad_kernel(const double* __restrict__ gpart, int nch, int N, const float* __restrict__ eps,
-                   float p, float* __restrict__ grad, double* __restrict__ e2part) {
+smooth_z_kernel(const float* __restrict__ y, const float* __restrict__ eps, int N, float* __restrict__ z,
+                int32_t* __restrict__ idx) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    z[k] = y[k] + (eps ? eps[k] : 0.f);
+    idx[k] = k;
+}
+
+// sorted records: coordinates of datum perm[j] (already M-scaled, from the unsorted base records),
+// value slot = z_sorted[j]; also clears the gradient accumulator of position j.
+__global__ void __launch_bounds__(256)
+smooth_gather_kernel(const float* __restrict__ base, const int32_t* __restrict__ perm,
+                     const float* __restrict__ zs, int N, int rf, int vslot, float* __restrict__ rec,
+                     unsigned long long* __restrict__ gfix) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const float4* src = reinterpret_cast<const float4*>(base + static_cast<size_t>(perm[j]) * rf);
+    float4* dst = reinterpret_cast<float4*>(rec + static_cast<size_t>(j) * rf);
+    for (int c = 0; c < rf / 4; ++c) {
+        float4 v = src[c];
+        const int o = vslot - 4 * c;
+        if (o == 0) v.x = zs[j];
+        if (o == 1) v.y = zs[j];
+        if (o == 2) v.z = zs[j];
+        if (o == 3) v.w = zs[j];
+        dst[c] = v;
+    }
+    gfix[j] = 0ull;
+}
+
+// grad[perm[j]] = 2 eps / p + 4 * gfix[j] * 2^-40; per-block partial of sum eps^2.
+__global__ void __launch_bounds__(256)
+smooth_grad_kernel(const unsigned long long* __restrict__ gfix, const int32_t* __restrict__ perm, int N,
+                   const float* __restrict__ eps, float p, float* __restrict__ grad,
+                   double* __restrict__ e2part) {
     __shared__ double red[8];
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
     double e = 0.0;
-    if (i < N) {
-        double s = 0.0;
-        for (int c = 0; c < nch; ++c) s += gpart[static_cast<size_t>(c) * N + i];
+    if (j < N) {
+        const int i = perm[j];
+        const double s = static_cast<double>(static_cast<long long>(gfix[j])) / kFix;
         e = eps ? static_cast<double>(eps[i]) : 0.0;
         if (grad) grad[i] = static_cast<float>(2.0 * e / static_cast<double>(p) + 4.0 * s);
     }
@@ -163,16 +254,16 @@ smooth_grad_kernel(const double* __restrict__ gpart, int nch, int N, const float
     }
 }
 
-// Single block, fixed order: F = sum(e2part)/p + sum(fpart); maxviol = max(vpart).
+// Single block, fixed order: F = sum(e2part)/p + 2 sum(fpart); maxviol = max(vpart).
 __global__ void __launch_bounds__(256)
-smooth_final_kernel(const double* __restrict__ fpart, const double* __restrict__ vpart, int ntiles,
+smooth_final_kernel(const double* __restrict__ fpart, const float* __restrict__ vpart, int nitems,
                     const double* __restrict__ e2part, int nblk, float p, double* __restrict__ F,
                     double* __restrict__ maxviol) {
     __shared__ double rf_[256], re_[256], rv_[256];
     double f = 0.0, e = 0.0, v = 0.0;
-    for (int t = threadIdx.x; t < ntiles; t += 256) {
+    for (int t = threadIdx.x; t < nitems; t += 256) {
         f += fpart[t];
-        v = fmax(v, vpart[t]);
+        v = fmax(v, static_cast<double>(vpart[t]));
     }
     for (int b = threadIdx.x; b < nblk; b += 256) e += e2part[b];
     rf_[threadIdx.x] = f;
@@ -188,7 +279,7 @@ smooth_final_kernel(const double* __restrict__ fpart, const double* __restrict__
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        if (F) *F = re_[0] / static_cast<double>(p) + rf_[0];
+        if (F) *F = re_[0] / static_cast<double>(p) + 2.0 * rf_[0];
         if (maxviol) *maxviol = rv_[0];
     }
 }
@@ -196,60 +287,29 @@ smooth_final_kernel(const double* __restrict__ fpart, const double* __restrict__
 namespace {
 
 template <class Acc, int R>
-int launch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff, const float* eps, float p,
-                 double* F_dev, float* grad, double* maxviol_dev) {
-    constexpr int THREADS = 128;
-    auto kern = smooth_pairs_kernel<Acc, R, THREADS>;
+int launch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff) {
+    auto kern = smooth_pairs_kernel<Acc, R>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
+    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSmThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
-    constexpr int TILE = smooth_tile_records<Acc::RF>();
-    a.nrb = (a.N + THREADS * R - 1) / (THREADS * R);
-    int want = (16 * slots + a.nrb - 1) / a.nrb;
-    int max_ch = (a.N + 2 * TILE - 1) / (2 * TILE);
-    int nch = want < 1 ? 1 : want;
-    if (nch > max_ch) nch = max_ch;
-    if (nch > 64) nch = 64;
-    if (nch < 1) nch = 1;
-    int chunk = (a.N + nch - 1) / nch;
-    chunk = ((chunk + TILE - 1) / TILE) * TILE;
-    nch = (a.N + chunk - 1) / chunk;
-    a.nch = nch;
-    a.chunk = chunk;
-    const int ntiles = a.nrb * nch;
-    const int nblk = (a.N + 255) / 256;
-
-    Workspace w;
-    size_t bytes = sizeof(double) * (static_cast<size_t>(nch) * a.N + 2 * static_cast<size_t>(ntiles) + nblk);
-    int rc = w.alloc(bytes, c.stream);
-    if (rc) return rc;
-    a.gpart = w.as<double>();
-    a.fpart = a.gpart + static_cast<size_t>(nch) * a.N;
-    a.vpart = a.fpart + ntiles;
-    double* e2part = a.vpart + ntiles;
-
-    int grid = ntiles < slots ? ntiles : slots;
+    const int grid = a.nitems < slots ? a.nitems : slots;
     KernelTimer kt(TK_SMOOTH_PAIRS, c.stream);
-    kern<<<grid, THREADS, 0, c.stream>>>(a, ff);
+    kern<<<grid, kSmThreads, 0, c.stream>>>(a, ff);
     kt.stop();
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
-    smooth_grad_kernel<<<nblk, 256, 0, c.stream>>>(a.gpart, nch, a.N, eps, p, grad, e2part);
-    ++g_launches;
-    LIPFIT_CUDA(cudaGetLastError());
-    if (F_dev || maxviol_dev) {
-        smooth_final_kernel<<<1, 256, 0, c.stream>>>(a.fpart, a.vpart, ntiles, e2part, nblk, p, F_dev,
-                                                     maxviol_dev);
-        ++g_launches;
-        LIPFIT_CUDA(cudaGetLastError());
-    }
     return LIPFIT_OK;
 }
 
 int smooth_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
 bool is_spec(const Xform& xf, int norm) {
     return (norm == 2 && xf.dU == 0 && xf.dC == 5) || (norm == 2 && xf.dU == 2 && xf.dC == 0);
+}
+int smooth_rows(const Xform& xf, int norm) {  // R of the kernel that will run
+    if (is_spec(xf, norm)) return 8;
+    const int dp = smooth_dp(xf.d);
+    return dp <= 8 ? 4 : (dp <= 16 ? 2 : 1);
 }
 
 }  // namespace
@@ -260,15 +320,62 @@ RecLayout smooth_layout(const Xform& xf, int norm) {
     return RecLayout{dp + 4, dp};
 }
 
-int launch_smooth_objective(const Ctx& c, const float* rec, int64_t N, const Xform& xf, int norm,
-                            float M, float p, const float* eps, double* F_dev, float* grad,
+int launch_smooth_objective(const Ctx& c, const float* base, const float* y, const float* eps, int64_t N64,
+                            const Xform& xf, int norm, float p, double* F_dev, float* grad,
                             double* maxviol_dev) {
+    const int N = static_cast<int>(N64);
+    const RecLayout lay = smooth_layout(xf, norm);
+    const int R = smooth_rows(xf, norm);
     SmoothArgs a{};
-    a.rec = rec;
-    a.N = static_cast<int>(N);
-    a.M = M;
+    a.N = N;
+    a.nrb = (N + kSmThreads * R - 1) / (kSmThreads * R);
+    a.maxc = (N + kSmChunk - 1) / kSmChunk;
+    a.nitems = a.nrb * a.maxc;
+    const int nblk = (N + 255) / 256;
+    const size_t n = static_cast<size_t>(N);
+
+    // ---- workspace ----
+    size_t sort_bytes = 0;
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, sort_bytes, static_cast<const float*>(nullptr),
+                                                static_cast<float*>(nullptr),
+                                                static_cast<const int32_t*>(nullptr),
+                                                static_cast<int32_t*>(nullptr), N, 0, 32, c.stream));
+    Workspace wz, wzs, wi, wperm, wsort, wrec, wg, wf, wv, we, wc;
+    int rc;
+    if ((rc = wz.alloc(sizeof(float) * n, c.stream))) return rc;
+    if ((rc = wzs.alloc(sizeof(float) * n, c.stream))) return rc;
+    if ((rc = wi.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    if ((rc = wperm.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    if ((rc = wsort.alloc(sort_bytes, c.stream))) return rc;
+    if ((rc = wrec.alloc(sizeof(float) * n * lay.rf, c.stream))) return rc;
+    if ((rc = wg.alloc(sizeof(unsigned long long) * n, c.stream))) return rc;
+    if ((rc = wf.alloc(sizeof(double) * a.nitems, c.stream))) return rc;
+    if ((rc = wv.alloc(sizeof(float) * a.nitems, c.stream))) return rc;
+    if ((rc = we.alloc(sizeof(double) * nblk, c.stream))) return rc;
+    if ((rc = wc.alloc(sizeof(int), c.stream))) return rc;
+
+    // ---- (1) sort by z, gather ----
+    smooth_z_kernel<<<nblk, 256, 0, c.stream>>>(y, eps, N, wz.as<float>(), wi.as<int32_t>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(wsort.p, sort_bytes, wz.as<float>(), wzs.as<float>(),
+                                                wi.as<int32_t>(), wperm.as<int32_t>(), N, 0, 32,
+                                                c.stream));
+    smooth_gather_kernel<<<nblk, 256, 0, c.stream>>>(base, wperm.as<int32_t>(), wzs.as<float>(), N, lay.rf,
+                                                     lay.vslot, wrec.as<float>(),
+                                                     wg.as<unsigned long long>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    LIPFIT_CUDA(cudaMemsetAsync(wc.p, 0, sizeof(int), c.stream));
+
+    // ---- (2),(3) lower-triangle pairs ----
+    a.rec = wrec.as<float>();
+    a.gfix = wg.as<unsigned long long>();
+    a.fpart = wf.as<double>();
+    a.vpart = wv.as<float>();
+    a.counter = wc.as<int>();
     FreeFlags ff = make_free_flags(xf);
-#define GO(ACC, R) return launch_pairs<ACC, R>(c, a, ff, eps, p, F_dev, grad, maxviol_dev)
+#define GO(ACC, RR) rc = launch_pairs<ACC, RR>(c, a, ff)
     using S205 = SpecAcc<2, 0, 5>;
     using S220 = SpecAcc<2, 2, 0>;
     using G14 = GenAcc<1, 4>;
@@ -283,26 +390,39 @@ int launch_smooth_objective(const Ctx& c, const float* rec, int64_t N, const Xfo
     using G38 = GenAcc<3, 8>;
     using G316 = GenAcc<3, 16>;
     using G332 = GenAcc<3, 32>;
-    if (norm == 2 && xf.dU == 0 && xf.dC == 5) GO(S205, 8);
-    if (norm == 2 && xf.dU == 2 && xf.dC == 0) GO(S220, 8);
     const int dp = smooth_dp(xf.d);
-    if (norm == 1) {
+    if (norm == 2 && xf.dU == 0 && xf.dC == 5) GO(S205, 8);
+    else if (norm == 2 && xf.dU == 2 && xf.dC == 0) GO(S220, 8);
+    else if (norm == 1) {
         if (dp == 4) GO(G14, 4);
-        if (dp == 8) GO(G18, 4);
-        if (dp == 16) GO(G116, 2);
-        GO(G132, 1);
+        else if (dp == 8) GO(G18, 4);
+        else if (dp == 16) GO(G116, 2);
+        else GO(G132, 1);
     } else if (norm == 2) {
         if (dp == 4) GO(G24, 4);
-        if (dp == 8) GO(G28, 4);
-        if (dp == 16) GO(G216, 2);
-        GO(G232, 1);
+        else if (dp == 8) GO(G28, 4);
+        else if (dp == 16) GO(G216, 2);
+        else GO(G232, 1);
     } else {
         if (dp == 4) GO(G34, 4);
-        if (dp == 8) GO(G38, 4);
-        if (dp == 16) GO(G316, 2);
-        GO(G332, 1);
+        else if (dp == 8) GO(G38, 4);
+        else if (dp == 16) GO(G316, 2);
+        else GO(G332, 1);
     }
 #undef GO
+    if (rc) return rc;
+
+    smooth_grad_kernel<<<nblk, 256, 0, c.stream>>>(a.gfix, wperm.as<int32_t>(), N, eps, p, grad,
+                                                   we.as<double>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    if (F_dev || maxviol_dev) {
+        smooth_final_kernel<<<1, 256, 0, c.stream>>>(a.fpart, a.vpart, a.nitems, we.as<double>(), nblk, p,
+                                                     F_dev, maxviol_dev);
+        ++g_launches;
+        LIPFIT_CUDA(cudaGetLastError());
+    }
+    return LIPFIT_OK;
 }
 
 }  // namespace lipfit
