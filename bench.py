@@ -38,7 +38,14 @@ METRIC = "query x datum pair evaluations per second (bounds, config 2)"
 UNIT = "Gpairs/s"
 # Algorithmic lane-ops per pair: 1 lane-op = one fp32
 # add/sub/mul/fma, one min/max/relu/compare, or one sqrt.
-LANE_OPS = {1: 9, 2: 18, 3: 21, 4: 33, "5s": 26, "5b": 31}
+# Config 4 (symmetric L2) selects on the cross-term key ||x||^2 - 2 q.x: 16 FFMA + 1 compare = 17 executed
+# lane-ops per pair (the direct-difference form of SURVEY.md is 33).  Smoothing visits each UNORDERED pair
+# once with a one-sided distance: 5 sub + 5 relu + 5 fma + dz + dz^2 + compare = 18 executed lane-ops
+# per visit (SURVEY.md credits 26 per ORDERED pair).  Rooflines are reported on EXECUTED work.
+LANE_OPS = {1: 9, 2: 18, 3: 21, 4: 17, "4direct": 33, "5s": 18, "5s_survey": 26, "5b": 31}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/*.md); null where no capture of this kernel version exists.
+NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2>": 27_231_232}
 FP32_LANES_PER_SM = 128
 
 
@@ -213,11 +220,11 @@ def _kernel_ms(L, which, fn, reps):
     return (ms / n if n else None), n
 
 
-def _roofline(pairs, lane_ops, kernel_ms, sms, peaks):
+def _roofline(pairs, lane_ops, kernel_ms, sms, peaks, kernel=None):
     peak = sms * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6 / 1e12    # T lane-ops/s
     ach = pairs * lane_ops / (kernel_ms * 1e-3) / 1e12 if kernel_ms else None
     return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlane-op/s",
-            "frac": (ach / peak) if ach else None, "traffic": None,
+            "frac": (ach / peak) if ach else None, "traffic": NCU_TRAFFIC_BYTES.get(kernel),
             "lane_ops_per_pair": lane_ops, "kernel_ms": kernel_ms,
             "peak_how": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {peaks['sm_max_mhz']:.0f} MHz (clocks.max.sm)"}
 
@@ -256,8 +263,10 @@ def bench_knn(torch, L, wl, steps, warmup, l2buf, dev):
     ms = _time_steps(torch, fn, steps, warmup, l2buf)
     kms, _ = _kernel_ms(L, 1, fn, 1)
     pairs = wl.N * wl.Q
+    out = fn()
+    torch.cuda.synchronize()
     return {"ms_per_step": float(np.mean(ms)), "pairs": pairs, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
-            "kernel_ms": kms, "lane_ops": LANE_OPS[4], "outputs": fn()}
+            "kernel_ms": kms, "lane_ops": LANE_OPS[4], "outputs": out, "fallbacks": L.knn_fallbacks()}
 
 
 def bench_smooth(torch, L, wl, l2buf, dev):
@@ -272,9 +281,10 @@ def bench_smooth(torch, L, wl, l2buf, dev):
     wall = time.perf_counter() - t0
     kms, n = L.get_timing(2)
     L.set_timing(False)
-    pairs_eval = wl.N * (wl.N - 1)
+    pairs_eval = wl.N * (wl.N - 1)          # ordered pairs of Eq.(7) covered by one evaluation
     return {"wall_s": wall, "info": info, "evals": n, "kernel_ms_per_eval": kms / max(n, 1),
-            "pairs_per_eval": pairs_eval, "value": pairs_eval / (kms / max(n, 1) * 1e-3) / 1e9,
+            "pairs_per_eval": pairs_eval, "visits_per_eval": pairs_eval // 2,
+            "value": pairs_eval / (kms / max(n, 1) * 1e-3) / 1e9,
             "lane_ops": LANE_OPS["5s"], "z": y, "X": X}
 
 
@@ -339,7 +349,7 @@ def run_gpu(args):
                 "h2d_bytes_per_step": r2["e2e"]["h2d_bytes_per_step"],
                 "d2h_bytes_per_step": r2["e2e"]["d2h_bytes_per_step"], "ms_per_step": e2e_ms},
         "gpu_launches": r2["gpu_launches"] * args.steps,
-        "roofline": _roofline(r2["pairs"], LANE_OPS[2], r2["kernel_ms"], sms, peaks),
+        "roofline": _roofline(r2["pairs"], LANE_OPS[2], r2["kernel_ms"], sms, peaks, r2["kernel"]),
         "peaks": peaks_how,
     }
     if clocks and clocks.get("sm_mhz"):
@@ -385,7 +395,11 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
         r = bench_knn(torch, L, wl, steps, 1, l2buf, dev)
         out.update({k: r[k] for k in ("ms_per_step", "value", "kernel_ms")})
         out["unit"] = UNIT
+        out["kernel"] = "knn_select<dot,DP16> (cross-term key, FFMA2) + fp64 re-rank + certificate"
+        out["exact_fallback_queries"] = r["fallbacks"]
         out["roofline"] = _roofline(r["pairs"], LANE_OPS[4], r["kernel_ms"], sms, peaks)
+        out["roofline"]["frac_direct_difference_form_33ops"] = (
+            r["pairs"] * LANE_OPS["4direct"] / (r["kernel_ms"] * 1e-3) / 1e12 / out["roofline"]["peak"])
         if not args.no_cpu:
             sel = oracle_subset(wl.Q, 64)
             t0 = time.perf_counter()
@@ -402,8 +416,12 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
     elif c == 5:
         r = bench_smooth(torch, L, wl, l2buf, dev)
         out.update({"smooth_wall_s": r["wall_s"], "info": r["info"], "evals": r["evals"],
-                    "kernel_ms_per_eval": r["kernel_ms_per_eval"], "value": r["value"], "unit": UNIT,
-                    "roofline": _roofline(r["pairs_per_eval"], LANE_OPS["5s"], r["kernel_ms_per_eval"], sms, peaks)})
+                    "kernel_ms_per_eval": r["kernel_ms_per_eval"], "value": r["value"],
+                    "unit": "G ordered pairs of Eq.(7) per second (each unordered pair is visited once)",
+                    "roofline": _roofline(r["visits_per_eval"], LANE_OPS["5s"], r["kernel_ms_per_eval"], sms, peaks)})
+        out["roofline"]["frac_survey_26ops_per_ordered_pair"] = (
+            r["pairs_per_eval"] * LANE_OPS["5s_survey"] / (r["kernel_ms_per_eval"] * 1e-3) / 1e12
+            / out["roofline"]["peak"])
         Xq = torch.from_numpy(wl.Xq).to(dev)
         fn = lambda: L.lipfit_bounds(r["X"], r["z"], Xq, wl.M, wl.mask, wl.norm, wl.weights)
         ms = _time_steps(torch, fn, max(1, min(args.steps, 3)), 2, l2buf)

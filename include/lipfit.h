@@ -130,6 +130,23 @@ int lipfit_smooth_host(const float* X, float* y_inout, int64_t N, int32_t d, flo
                        int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,
                        void* cuda_stream);
 
+/* ---- Smallest Lipschitz constant consistent with the data ---------------
+ *   L = max over ordered pairs i != k with y_i > y_k of (y_i - y_k) / d_s(x^k, x^i)
+ * (the least M for which constraint (5) holds; without monotonicity max |y_i-y_k| / ||x^i-x^k||).
+ * "N^2 operations, but no storage of the distance matrix": the data are sorted by y
+ * and every unordered pair is visited once by the smoothing sweep with a running-maximum filter.
+ * L: one fp32 (device for lipfit_lipschitz_constant, asynchronous; host for the _host variant,
+ * which copies X, y in and synchronises).  +inf if a pair with y_i > y_k has zero distance, 0 if no
+ * pair qualifies (N = 1, constant y).  The fp32 sweep only FILTERS (conservatively: a pair is
+ * dropped only if it provably cannot beat the running maximum); surviving pairs are evaluated
+ * in fp64 from the original inputs, so L is the exact fp64 maximum rounded to fp32. */
+int lipfit_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t d,
+                              const int32_t* mono_mask, int32_t norm, const float* weights,
+                              float* L /* device[1] */, void* cuda_stream);
+int lipfit_lipschitz_constant_host(const float* X, const float* y, int64_t N, int32_t d,
+                                   const int32_t* mono_mask, int32_t norm, const float* weights,
+                                   float* L /* host */, void* cuda_stream);
+
 /* ---- Host optimiser on its own (step a5), exposed so that it can be tested without a GPU ----
  * Minimises a caller-supplied function by the same LBFGS lipfit_smooth uses (history `history`,
  * strong-Wolfe line search).  x: host double[n], start point on entry and
@@ -148,7 +165,7 @@ const char* lipfit_version(void);
 int64_t lipfit_launch_count(void);
 /* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
  * resets the accumulators and makes every later launch of the three dominant kernels
- * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs) bracketed by CUDA events on
+ * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs) bracketed by CUDA events on
  * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
  * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);

@@ -29,8 +29,11 @@ def load():
         lib.oracle_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P]
         lib.oracle_smooth_objective.argtypes = [P, P, i64, i32, f64, P, i32, P, f64, P, P, P]
         lib.oracle_max_violation.argtypes = [P, P, i64, i32, f64, P, i32, P, P, P]
+        lib.oracle_smooth_rows.argtypes = [P, P, i64, i32, f64, P, i32, P, f64, P, P, i64, P, P]
+        lib.oracle_lipschitz_constant.argtypes = [P, P, i64, i32, P, i32, P, P]
         for fn in (lib.oracle_bounds, lib.oracle_knn, lib.oracle_smooth_objective,
-                   lib.oracle_max_violation, lib.oracle_num_threads):
+                   lib.oracle_max_violation, lib.oracle_num_threads, lib.oracle_smooth_rows,
+                   lib.oracle_lipschitz_constant):
             fn.restype = C.c_int
         _lib = lib
     return _lib
@@ -111,6 +114,35 @@ def max_violation(X, y, M, eps=None, mask=None, norm=2, weights=None):
                                      int(norm), _ptr(w), _ptr(e), C.byref(out))
     if rc:
         raise ValueError(f"oracle_max_violation rc={rc}")
+    return float(out.value)
+
+
+def smooth_rows(X, y, M, eps, rows, mask=None, norm=2, weights=None, p=1.0):
+    """dF/deps_i and the row share of F for the listed rows i (Eq.(7)); returns (grad_rows, f_rows)."""
+    X, y = _f32(X, 2), _f32(y, 1)
+    N, d = X.shape
+    m, w = _params(d, mask, weights)
+    eps = np.ascontiguousarray(eps, dtype=np.float64).reshape(N)
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    g = np.empty(len(rows), dtype=np.float64)
+    f = np.empty(len(rows), dtype=np.float64)
+    rc = load().oracle_smooth_rows(_ptr(X), _ptr(y), N, d, float(np.float32(M)), _ptr(m), int(norm),
+                                   _ptr(w), float(p), _ptr(eps), _ptr(rows), len(rows), _ptr(g), _ptr(f))
+    if rc:
+        raise ValueError(f"oracle_smooth_rows rc={rc}")
+    return g, f
+
+
+def lipschitz_constant(X, y, mask=None, norm=2, weights=None) -> float:
+    """Smallest M consistent with the data."""
+    X, y = _f32(X, 2), _f32(y, 1)
+    N, d = X.shape
+    m, w = _params(d, mask, weights)
+    out = C.c_double(0.0)
+    rc = load().oracle_lipschitz_constant(_ptr(X), _ptr(y), N, d, _ptr(m), int(norm), _ptr(w),
+                                          C.byref(out))
+    if rc:
+        raise ValueError(f"oracle_lipschitz_constant rc={rc}")
     return float(out.value)
 
 

@@ -211,3 +211,73 @@ int oracle_max_violation(const float* X, const float* y, int64_t N, int32_t d,
     *out = worst;
     return 0;
 }
+
+/* The same Eq.(7), restricted to a list of rows i (full-size spot checks): for each
+ * listed i, grad_rows = dF/deps_i and f_rows = eps_i^2/p + sum_{k!=i} (A_ik^2 + B_ik^2), i.e. row
+ * i's share of F (F = sum over ALL i of that share).  Statement by statement the inner loop of
+ * oracle_smooth_objective. */
+int oracle_smooth_rows(const float* X, const float* y, int64_t N, int32_t d, double M,
+                       const int32_t* mono_mask, int32_t norm, const float* weights, double p,
+                       const double* eps, const int64_t* rows, int64_t nrows, double* grad_rows,
+                       double* f_rows) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || !eps || !rows || !grad_rows) return -1;
+    if (!(M >= 0.0) || !isfinite(M) || !(p > 0.0)) return -4;
+    for (int64_t r = 0; r < nrows; ++r)
+        if (rows[r] < 0 || rows[r] >= N) return -3;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < nrows; ++r) {
+        int64_t i = rows[r];
+        double zi = (double)y[i] + eps[i];
+        double gi = 2.0 * eps[i] / p;
+        double fi = eps[i] * eps[i] / p;
+        for (int64_t k = 0; k < N; ++k) {
+            if (k == i) continue;
+            double zk = (double)y[k] + eps[k];
+            double d_ik, dp_ik, d_ki, dp_ki;
+            one_sided_distances(X + i * d, X + k * d, d, mono_mask, norm, weights, &d_ik, &dp_ik);
+            one_sided_distances(X + k * d, X + i * d, d, mono_mask, norm, weights, &d_ki, &dp_ki);
+            double A_ik = fmax(zi - zk - M * d_ik, 0.0);
+            double B_ik = fmax(zk - zi - M * dp_ik, 0.0);
+            double A_ki = fmax(zk - zi - M * d_ki, 0.0);
+            double B_ki = fmax(zi - zk - M * dp_ki, 0.0);
+            fi += A_ik * A_ik + B_ik * B_ik;
+            gi += 2.0 * A_ik - 2.0 * A_ki - 2.0 * B_ik + 2.0 * B_ki;
+        }
+        grad_rows[r] = gi;
+        if (f_rows) f_rows[r] = fi;
+    }
+    return 0;
+}
+
+/* Smallest Lipschitz constant consistent with the data ("all pairwise distances
+ * and then the ratios |y_i - y_k| / dist(x^i, x^k)"): the least M for which constraint (5)
+ * z_i <= z_k + M d_s(x^k, x^i) holds for every ordered pair,
+ *     L = max_{i != k, y_i > y_k} (y_i - y_k) / d_s(x^k, x^i).
+ * Without monotonicity d_s is symmetric and this is max |y_i - y_k| / ||x^i - x^k||.  A pair with
+ * y_i > y_k at zero distance makes the data inconsistent for every M: +infinity.  N = 1 or all
+ * y_i <= y_k wherever it matters: 0. */
+int oracle_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t d,
+                              const int32_t* mono_mask, int32_t norm, const float* weights,
+                              double* out) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || !out) return -1;
+    double best = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : best)
+    for (int64_t i = 0; i < N; ++i) {
+        for (int64_t k = 0; k < N; ++k) {
+            if (k == i) continue;
+            double dy = (double)y[i] - (double)y[k];
+            if (!(dy > 0.0)) continue;
+            double Du, Dl;
+            one_sided_distances(X + i * d, X + k * d, d, mono_mask, norm, weights, &Du, &Dl);
+            double ratio = (Du > 0.0) ? dy / Du : INFINITY;
+            if (ratio > best) best = ratio;
+        }
+    }
+    *out = best;
+    return 0;
+}
+

@@ -63,6 +63,20 @@ int oracle_max_violation(const float* X, const float* y, int64_t N, int32_t d,
                          double M, const int32_t* mono_mask, int32_t norm,
                          const float* weights, const double* eps, double* out);
 
+/* Eq.(7) restricted to listed rows: grad_rows[r] = dF/deps_{rows[r]}, f_rows[r] = row share of F
+ * (may be NULL).  For spot checks at sizes where the full double loop is unaffordable. */
+int oracle_smooth_rows(const float* X, const float* y, int64_t N, int32_t d, double M,
+                       const int32_t* mono_mask, int32_t norm, const float* weights, double p,
+                       const double* eps, const int64_t* rows, int64_t nrows, double* grad_rows,
+                       double* f_rows);
+
+/* Smallest Lipschitz constant consistent with the data:
+ * max over ordered pairs with y_i > y_k of (y_i - y_k) / d_s(x^k, x^i); +inf if such a pair has
+ * zero distance; 0 if there is none. */
+int oracle_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t d,
+                              const int32_t* mono_mask, int32_t norm, const float* weights,
+                              double* out);
+
 int oracle_num_threads(void);
 
 #ifdef __cplusplus

@@ -6,5 +6,6 @@ is its thin ctypes binding with the same entry-point names.
 from .binding import (LIPFIT_L1, LIPFIT_L2, LIPFIT_LINF, LIPFIT_MAX_DIM, LIPFIT_MAX_K,  # noqa: F401
                       LipfitError, bounds_variant, get_timing, knn_fallbacks, launch_count, set_timing, lipfit_bounds,
                       lipfit_bounds_host, lipfit_knn, lipfit_knn_host, lipfit_lbfgs,
+                      lipfit_lipschitz_constant, lipfit_lipschitz_constant_host,
                       lipfit_smooth, lipfit_smooth_host, lipfit_smooth_objective, load,
                       status_string, version)

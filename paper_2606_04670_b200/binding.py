@@ -22,6 +22,7 @@ EXPORTS = [
     "lipfit_smooth_objective", "lipfit_smooth", "lipfit_smooth_host", "lipfit_lbfgs",
     "lipfit_status_string", "lipfit_version", "lipfit_launch_count", "lipfit_bounds_variant",
     "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
+    "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
 ]
 
 
@@ -62,6 +63,8 @@ def load():
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
     lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
     lib.lipfit_lbfgs.argtypes = [i64, P, EVAL_FN, P, i32, f64, i32, P]
+    lib.lipfit_lipschitz_constant.argtypes = [P, P, i64, i32, P, i32, P, P, P]
+    lib.lipfit_lipschitz_constant_host.argtypes = lib.lipfit_lipschitz_constant.argtypes
     lib.lipfit_bounds_variant.argtypes = [i32, P, i32, C.c_char_p, i32]
     for name in EXPORTS:
         getattr(lib, name).restype = C.c_int
@@ -206,6 +209,33 @@ def lipfit_smooth_objective(X, y, M: float, eps=None, mono_mask=None, norm: int 
         None if grad is None else C.c_void_p(grad.data_ptr()), _stream(stream))
     _check(rc, "lipfit_smooth_objective")
     return float(F.value), grad
+
+
+def lipfit_lipschitz_constant(X, y, mono_mask=None, norm: int = LIPFIT_L2, weights=None, stream=None):
+    """Smallest Lipschitz constant consistent with the data as a 1-element
+    float32 CUDA tensor (asynchronous on the stream)."""
+    torch = _torch()
+    X, y = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y")
+    N, d = X.shape
+    if y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    m, w = _host_params(d, mono_mask, weights)
+    out = torch.empty(1, dtype=torch.float32, device=X.device)
+    rc = load().lipfit_lipschitz_constant(X.data_ptr(), y.data_ptr(), N, d, _np_ptr(m), int(norm),
+                                          _np_ptr(w), out.data_ptr(), _stream(stream))
+    _check(rc, "lipfit_lipschitz_constant")
+    return out
+
+
+def lipfit_lipschitz_constant_host(X, y, mono_mask=None, norm: int = LIPFIT_L2, weights=None) -> float:
+    X, y = _host_f32(X, 2), _host_f32(y, 1)
+    N, d = X.shape
+    m, w = _host_params(d, mono_mask, weights)
+    out = np.zeros(1, dtype=np.float32)
+    rc = load().lipfit_lipschitz_constant_host(_np_ptr(X), _np_ptr(y), N, d, _np_ptr(m), int(norm),
+                                               _np_ptr(w), _np_ptr(out), None)
+    _check(rc, "lipfit_lipschitz_constant_host")
+    return float(out[0])
 
 
 def lipfit_smooth(X, y_inout, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,

@@ -180,6 +180,51 @@ int lipfit_smooth_host(const float* X, float* y_inout, int64_t N, int32_t d, flo
     return LIPFIT_OK;
 }
 
+int lipfit_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t d,
+                              const int32_t* mono_mask, int32_t norm, const float* weights, float* L,
+                              void* cuda_stream) {
+    int rc = check_common(X, y, N, d, 0.f, norm, 1.f);
+    if (rc) return rc;
+    if (!L) return LIPFIT_E_NULL;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    RecLayout lay = smooth_layout(xf, norm);
+    Workspace rec;
+    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
+    if (rc) return rc;
+    rc = launch_prepack(c, X, nullptr, nullptr, N, xf, lay, rec.as<float>());
+    if (rc) return rc;
+    return launch_lipschitz_constant(c, X, rec.as<float>(), y, N, xf, norm, L);
+}
+
+int lipfit_lipschitz_constant_host(const float* X, const float* y, int64_t N, int32_t d,
+                                   const int32_t* mono_mask, int32_t norm, const float* weights,
+                                   float* L, void* cuda_stream) {
+    int rc = check_common(X, y, N, d, 0.f, norm, 1.f);
+    if (rc) return rc;
+    if (!L) return LIPFIT_E_NULL;
+    Xform xf;
+    if ((rc = make_xform(d, mono_mask, weights, false, false, &xf))) return rc;
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const size_t n = static_cast<size_t>(N);
+    Workspace dX, dy, dL;
+    if ((rc = dX.alloc(sizeof(float) * n * d, s))) return rc;
+    if ((rc = dy.alloc(sizeof(float) * n, s))) return rc;
+    if ((rc = dL.alloc(sizeof(float), s))) return rc;
+    LIPFIT_CUDA(cudaMemcpyAsync(dX.p, X, sizeof(float) * n * d, cudaMemcpyHostToDevice, s));
+    LIPFIT_CUDA(cudaMemcpyAsync(dy.p, y, sizeof(float) * n, cudaMemcpyHostToDevice, s));
+    rc = lipfit_lipschitz_constant(dX.as<float>(), dy.as<float>(), N, d, mono_mask, norm, weights,
+                                   dL.as<float>(), cuda_stream);
+    if (rc) return rc;
+    LIPFIT_CUDA(cudaMemcpyAsync(L, dL.p, sizeof(float), cudaMemcpyDeviceToHost, s));
+    LIPFIT_CUDA(cudaStreamSynchronize(s));
+    return LIPFIT_OK;
+}
+
 int lipfit_lbfgs(int64_t n, double* x, lipfit_eval_fn fn, void* user, int32_t max_iter,
                  double tol_grad, int32_t history, lipfit_smooth_info* info) {
     if (!x || !fn) return LIPFIT_E_NULL;

@@ -42,6 +42,9 @@ int64_t knn_last_fallbacks();
 int launch_smooth_objective(const Ctx& c, const float* base, const float* y, const float* eps, int64_t N,
                             const Xform& xf, int norm, float p, double* F_dev, float* grad,
                             double* maxviol_dev);
+// NEXT-3: smallest consistent Lipschitz constant; base = packed records with plain coordinates.
+int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, const float* y, int64_t N,
+                              const Xform& xf, int norm, float* L_dev);
 // xf with every coordinate factor multiplied by s
 Xform scale_xform(const Xform& xf, float s);
 

@@ -13,8 +13,8 @@ std::atomic<int64_t> g_launches{0};
 
 std::atomic<int> g_timing_on{0};
 static std::mutex g_timing_mu;
-static double g_timing_ms[TK_COUNT] = {0, 0, 0};
-static long long g_timing_n[TK_COUNT] = {0, 0, 0};
+static double g_timing_ms[TK_COUNT] = {};
+static long long g_timing_n[TK_COUNT] = {};
 
 KernelTimer::KernelTimer(int which_, cudaStream_t s_) : which(which_), s(s_) {
     if (!g_timing_on.load()) return;

@@ -21,6 +21,8 @@
 
 #include "kernels.h"
 
+#pragma nv_diag_suppress 128  // MODE 1 leaves the item loop before the smoothing-only reductions
+
 namespace lipfit {
 
 constexpr int kSmThreads = 128;
@@ -36,7 +38,20 @@ struct SmoothArgs {
     float* vpart;             // [nitems] max V over the item
     int* counter;             // work counter
     int N, nrb, maxc, nitems;
+    // MODE 1 only
+    unsigned long long* lmax;  // bits of the running maximum ratio (a non-negative double)
+    const uint32_t* amax;      // bits of max |x'| over the packed coordinates (written by the gather)
+    const float* X;            // original coordinates and
+    const int32_t* perm;       // sorted position -> original index, for the exact fp64 ratio
+    int norm;
+    Xform xf;
 };
+
+// MODE 0: smoothing objective / gradient (records carry M-scaled coordinates and z).
+// MODE 1: smallest consistent Lipschitz constant max (y_i - y_k) / d_s(x^k, x^i): same
+//         sorted lower-triangle sweep (records carry the plain coordinates and y); the pre-filter is
+//         "this pair beats the running maximum", which becomes rarer and rarer.
+constexpr int kModeSmooth = 0, kModeLipConst = 1;
 
 template <int RF>
 __host__ __device__ constexpr int smooth_tile_records() {
@@ -78,7 +93,44 @@ __device__ __forceinline__ void smooth_hit(const SmoothArgs& a, const float (&ac
     if (col != 0) atomicAdd(a.gfix + kpos, static_cast<unsigned long long>(-col));
 }
 
-template <class Acc, int R>
+// MODE 1 slow path: EXACT ratio (fp64, from the original fp32 inputs) of the pairs that passed the
+// conservative fp32 filter.  lcur (fp32, rounded down) only feeds the filter; lbest is the result.
+__device__ __forceinline__ double lipconst_exact_distance(const float* xi, const float* xk, const Xform& xf,
+                                                          int norm) {
+    double acc = 0.0;
+    for (int j = 0; j < xf.d; ++j) {
+        const int o = xf.perm[j];
+        const double dlt = static_cast<double>(xf.sw[j]) *
+                           (static_cast<double>(xi[o]) - static_cast<double>(xk[o]));
+        const double comp = (j < xf.dU) ? fabs(dlt) : fmax(dlt, 0.0);
+        if (norm == 1) acc += comp;
+        else if (norm == 2) acc += comp * comp;
+        else acc = fmax(acc, comp);
+    }
+    return norm == 2 ? sqrt(acc) : acc;
+}
+
+template <int R>
+__device__ __forceinline__ void lipconst_hit(const SmoothArgs& a, const float (&zi)[R], float zk,
+                                             const int (&ipos)[R], int kpos, const bool (&pass)[R],
+                                             float& lcur, double& lbest) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        if (pass[r]) {
+            const double dzd = static_cast<double>(zi[r]) - static_cast<double>(zk);
+            if (dzd > 0.0) {
+                const float* xi = a.X + static_cast<size_t>(a.perm[ipos[r]]) * a.xf.d;
+                const float* xk = a.X + static_cast<size_t>(a.perm[kpos]) * a.xf.d;
+                const double D = lipconst_exact_distance(xi, xk, a.xf, a.norm);
+                const double ratio = D > 0.0 ? dzd / D : __longlong_as_double(0x7ff0000000000000LL);
+                lbest = fmax(lbest, ratio);
+                lcur = fmaxf(lcur, __double2float_rd(ratio));
+            }
+        }
+    }
+}
+
+template <class Acc, int R, int MODE>
 __global__ void __launch_bounds__(kSmThreads, 4)
 smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
     constexpr int THREADS = kSmThreads;
@@ -138,17 +190,39 @@ smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
             } else {  // padding row: an infinite distance to everything, never passes the filter
 #pragma unroll
                 for (int j = 0; j < D; ++j) xi[r][j] = 1e30f;
-                zi[r] = 0.f;
+                zi[r] = __int_as_float(0xff800000);  // -inf: z_i - z_k is never positive
             }
         }
         double fd = 0.0;
         float vmax = 0.f;
+        float lcur = 0.f;    // MODE 1: running maximum ratio known to this thread, rounded down (filter)
+        double lbest = 0.0;  //         and exactly (result)
         RecordPipe<TILE, ST, kSmWarps> rs(a.rec, RF, begin, end, sbuf, bars, done, &phase);
         for (int t = 0; t < rs.ntiles; ++t) {
             const float* s = rs.acquire(t);
             const int n = rs.count(t);
             const int base = begin + t * TILE;
             const bool below = (base + n <= row0);  // every k of the tile precedes every row of the block
+            // MODE 1 filter: the pair can beat the running maximum L only if  L * D < dz.  With the fp32
+            // distance D' (|D' - D| <= eta from the rounding of the weighted coordinates, plus a relative
+            // (D+6) 2^-24 from the accumulation) the conservative form is  L (1-rel) D' < dz + L eta.
+            float lthr = 0.f, leta = 0.f;
+            auto refresh = [&]() {
+                const float rel = 1.f - static_cast<float>(D + 6) * 1.1920929e-7f;
+                const float cn = Acc::NORM == 1 ? static_cast<float>(a.xf.d)
+                                                : (Acc::NORM == 2 ? sqrtf(static_cast<float>(a.xf.d)) : 1.f);
+                const float eta = cn * 1.1920929e-7f * __uint_as_float(*a.amax);
+                const float l = lcur * rel;
+                lthr = Acc::NORM == 2 ? l * l : l;
+                leta = lcur * eta;
+            };
+            if (MODE == kModeLipConst) {  // share the maximum between threads once per tile
+                const double g = __longlong_as_double(
+                    static_cast<long long>(*reinterpret_cast<volatile unsigned long long*>(a.lmax)));
+                lcur = fmaxf(lcur, __double2float_rd(g));
+                if (isinf(lcur)) lcur = 3.0e38f;  // keeps the filter arithmetic finite; the result stays +inf
+                refresh();
+            }
             for (int j = 0; j < n; ++j) {
                 float x[RF];
                 smooth_load_record<RF>(s + j * RF, x);
@@ -160,15 +234,34 @@ smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
                 for (int r = 0; r < R; ++r) {
                     acc[r] = Acc::run_u(xi[r], x, ff);
                     dz[r] = zi[r] - zk;
-                    pass[r] = Acc::NORM == 2 ? (acc[r] < dz[r] * dz[r]) : (acc[r] < dz[r]);
+                    const float lhs = MODE == kModeLipConst ? acc[r] * lthr : acc[r];
+                    if (MODE == kModeLipConst) dz[r] += leta;
+                    pass[r] = Acc::NORM == 2 ? (lhs < dz[r] * dz[r]) : (lhs < dz[r]);
                     if (!below) pass[r] = pass[r] && (base + j < ipos[r]) && (dz[r] > 0.f);
                     hit |= pass[r];
                 }
-                if (__any_sync(0xffffffffu, hit))  // warp-uniform, rare
-                    smooth_hit<Acc, R>(a, acc, dz, pass, base + j, grow, fd, vmax);
+                if (__any_sync(0xffffffffu, hit)) {  // warp-uniform, rare
+                    if (MODE == kModeSmooth) {
+                        smooth_hit<Acc, R>(a, acc, dz, pass, base + j, grow, fd, vmax);
+                    } else {
+                        lipconst_hit<R>(a, zi, zk, ipos, base + j, pass, lcur, lbest);
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1)
+                            lcur = fmaxf(lcur, __shfl_xor_sync(0xffffffffu, lcur, o));
+                        if (isinf(lcur)) lcur = 3.0e38f;
+                        refresh();
+                    }
+                }
+            }
+            if (MODE == kModeLipConst) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) lbest = fmax(lbest, __shfl_xor_sync(0xffffffffu, lbest, o));
+                if ((threadIdx.x & 31) == 0)
+                    atomicMax(a.lmax, static_cast<unsigned long long>(__double_as_longlong(lbest)));
             }
             rs.release(t);
         }
+        if (MODE == kModeLipConst) continue;  // nothing else to reduce
         // ---- row sums -> fixed-point atomics; per-item objective partial (fixed order) ----
 #pragma unroll
         for (int r = 0; r < R; ++r)
@@ -211,13 +304,15 @@ smooth_z_kernel(const float* __restrict__ y, const float* __restrict__ eps, int 
 __global__ void __launch_bounds__(256)
 smooth_gather_kernel(const float* __restrict__ base, const int32_t* __restrict__ perm,
                      const float* __restrict__ zs, int N, int rf, int vslot, float* __restrict__ rec,
-                     unsigned long long* __restrict__ gfix) {
+                     unsigned long long* __restrict__ gfix, uint32_t* __restrict__ amax) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
+    float am = 0.f;
     const float4* src = reinterpret_cast<const float4*>(base + static_cast<size_t>(perm[j]) * rf);
     float4* dst = reinterpret_cast<float4*>(rec + static_cast<size_t>(j) * rf);
     for (int c = 0; c < rf / 4; ++c) {
         float4 v = src[c];
+        if (amax) am = fmaxf(am, fmaxf(fmaxf(fabsf(v.x), fabsf(v.y)), fmaxf(fabsf(v.z), fabsf(v.w))));
         const int o = vslot - 4 * c;
         if (o == 0) v.x = zs[j];
         if (o == 1) v.y = zs[j];
@@ -226,6 +321,11 @@ smooth_gather_kernel(const float* __restrict__ base, const int32_t* __restrict__
         dst[c] = v;
     }
     gfix[j] = 0ull;
+    if (amax) atomicMax(amax, __float_as_uint(am));  // MODE 1 only (base value slots are zero there)
+}
+
+__global__ void lipconst_final_kernel(const unsigned long long* __restrict__ lmax, float* __restrict__ L) {
+    *L = static_cast<float>(__longlong_as_double(static_cast<long long>(*lmax)));
 }
 
 // grad[perm[j]] = 2 eps / p + 4 * gfix[j] * 2^-40; per-block partial of sum eps^2.
@@ -286,15 +386,15 @@ smooth_final_kernel(const double* __restrict__ fpart, const float* __restrict__ 
 
 namespace {
 
-template <class Acc, int R>
+template <class Acc, int R, int MODE>
 int launch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff) {
-    auto kern = smooth_pairs_kernel<Acc, R>;
+    auto kern = smooth_pairs_kernel<Acc, R, MODE>;
     int occ = 0;
     LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSmThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     const int grid = a.nitems < slots ? a.nitems : slots;
-    KernelTimer kt(TK_SMOOTH_PAIRS, c.stream);
+    KernelTimer kt(MODE == kModeSmooth ? TK_SMOOTH_PAIRS : TK_LIPCONST_PAIRS, c.stream);
     kern<<<grid, kSmThreads, 0, c.stream>>>(a, ff);
     kt.stop();
     ++g_launches;
@@ -310,6 +410,47 @@ int smooth_rows(const Xform& xf, int norm) {  // R of the kernel that will run
     if (is_spec(xf, norm)) return 8;
     const int dp = smooth_dp(xf.d);
     return dp <= 8 ? 4 : (dp <= 16 ? 2 : 1);
+}
+
+template <int MODE>
+int dispatch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff, const Xform& xf, int norm) {
+    int rc = LIPFIT_OK;
+#define GO(ACC, RR) rc = launch_pairs<ACC, RR, MODE>(c, a, ff)
+    using S205 = SpecAcc<2, 0, 5>;
+    using S220 = SpecAcc<2, 2, 0>;
+    using G14 = GenAcc<1, 4>;
+    using G18 = GenAcc<1, 8>;
+    using G116 = GenAcc<1, 16>;
+    using G132 = GenAcc<1, 32>;
+    using G24 = GenAcc<2, 4>;
+    using G28 = GenAcc<2, 8>;
+    using G216 = GenAcc<2, 16>;
+    using G232 = GenAcc<2, 32>;
+    using G34 = GenAcc<3, 4>;
+    using G38 = GenAcc<3, 8>;
+    using G316 = GenAcc<3, 16>;
+    using G332 = GenAcc<3, 32>;
+    const int dp = smooth_dp(xf.d);
+    if (norm == 2 && xf.dU == 0 && xf.dC == 5) GO(S205, 8);
+    else if (norm == 2 && xf.dU == 2 && xf.dC == 0) GO(S220, 8);
+    else if (norm == 1) {
+        if (dp == 4) GO(G14, 4);
+        else if (dp == 8) GO(G18, 4);
+        else if (dp == 16) GO(G116, 2);
+        else GO(G132, 1);
+    } else if (norm == 2) {
+        if (dp == 4) GO(G24, 4);
+        else if (dp == 8) GO(G28, 4);
+        else if (dp == 16) GO(G216, 2);
+        else GO(G232, 1);
+    } else {
+        if (dp == 4) GO(G34, 4);
+        else if (dp == 8) GO(G38, 4);
+        else if (dp == 16) GO(G316, 2);
+        else GO(G332, 1);
+    }
+#undef GO
+    return rc;
 }
 
 }  // namespace
@@ -363,7 +504,7 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
                                                 c.stream));
     smooth_gather_kernel<<<nblk, 256, 0, c.stream>>>(base, wperm.as<int32_t>(), wzs.as<float>(), N, lay.rf,
                                                      lay.vslot, wrec.as<float>(),
-                                                     wg.as<unsigned long long>());
+                                                     wg.as<unsigned long long>(), nullptr);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     LIPFIT_CUDA(cudaMemsetAsync(wc.p, 0, sizeof(int), c.stream));
@@ -375,41 +516,7 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
     a.vpart = wv.as<float>();
     a.counter = wc.as<int>();
     FreeFlags ff = make_free_flags(xf);
-#define GO(ACC, RR) rc = launch_pairs<ACC, RR>(c, a, ff)
-    using S205 = SpecAcc<2, 0, 5>;
-    using S220 = SpecAcc<2, 2, 0>;
-    using G14 = GenAcc<1, 4>;
-    using G18 = GenAcc<1, 8>;
-    using G116 = GenAcc<1, 16>;
-    using G132 = GenAcc<1, 32>;
-    using G24 = GenAcc<2, 4>;
-    using G28 = GenAcc<2, 8>;
-    using G216 = GenAcc<2, 16>;
-    using G232 = GenAcc<2, 32>;
-    using G34 = GenAcc<3, 4>;
-    using G38 = GenAcc<3, 8>;
-    using G316 = GenAcc<3, 16>;
-    using G332 = GenAcc<3, 32>;
-    const int dp = smooth_dp(xf.d);
-    if (norm == 2 && xf.dU == 0 && xf.dC == 5) GO(S205, 8);
-    else if (norm == 2 && xf.dU == 2 && xf.dC == 0) GO(S220, 8);
-    else if (norm == 1) {
-        if (dp == 4) GO(G14, 4);
-        else if (dp == 8) GO(G18, 4);
-        else if (dp == 16) GO(G116, 2);
-        else GO(G132, 1);
-    } else if (norm == 2) {
-        if (dp == 4) GO(G24, 4);
-        else if (dp == 8) GO(G28, 4);
-        else if (dp == 16) GO(G216, 2);
-        else GO(G232, 1);
-    } else {
-        if (dp == 4) GO(G34, 4);
-        else if (dp == 8) GO(G38, 4);
-        else if (dp == 16) GO(G316, 2);
-        else GO(G332, 1);
-    }
-#undef GO
+    rc = dispatch_pairs<kModeSmooth>(c, a, ff, xf, norm);
     if (rc) return rc;
 
     smooth_grad_kernel<<<nblk, 256, 0, c.stream>>>(a.gfix, wperm.as<int32_t>(), N, eps, p, grad,
@@ -422,6 +529,73 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
         ++g_launches;
         LIPFIT_CUDA(cudaGetLastError());
     }
+    return LIPFIT_OK;
+}
+
+// NEXT-3: L = max_{i != k, y_i > y_k} (y_i - y_k) / d_s(x^k, x^i).
+// base: packed records with the PLAIN (weighted / mirrored, not M-scaled) coordinates.  L_dev: device
+// float, the maximum ratio (+inf if a pair with y_i > y_k has zero distance, 0 if no pair qualifies).
+int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, const float* y, int64_t N64,
+                              const Xform& xf, int norm, float* L_dev) {
+    const int N = static_cast<int>(N64);
+    const RecLayout lay = smooth_layout(xf, norm);
+    const int R = smooth_rows(xf, norm);
+    SmoothArgs a{};
+    a.N = N;
+    a.nrb = (N + kSmThreads * R - 1) / (kSmThreads * R);
+    a.maxc = (N + kSmChunk - 1) / kSmChunk;
+    a.nitems = a.nrb * a.maxc;
+    const int nblk = (N + 255) / 256;
+    const size_t n = static_cast<size_t>(N);
+    size_t sort_bytes = 0;
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, sort_bytes, static_cast<const float*>(nullptr),
+                                                static_cast<float*>(nullptr),
+                                                static_cast<const int32_t*>(nullptr),
+                                                static_cast<int32_t*>(nullptr), N, 0, 32, c.stream));
+    Workspace wz, wzs, wi, wperm, wsort, wrec, wg, wf, wv, wc, wl;
+    int rc;
+    if ((rc = wz.alloc(sizeof(float) * n, c.stream))) return rc;
+    if ((rc = wzs.alloc(sizeof(float) * n, c.stream))) return rc;
+    if ((rc = wi.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    if ((rc = wperm.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    if ((rc = wsort.alloc(sort_bytes, c.stream))) return rc;
+    if ((rc = wrec.alloc(sizeof(float) * n * lay.rf, c.stream))) return rc;
+    if ((rc = wg.alloc(sizeof(unsigned long long) * n, c.stream))) return rc;
+    if ((rc = wf.alloc(sizeof(double) * a.nitems, c.stream))) return rc;
+    if ((rc = wv.alloc(sizeof(float) * a.nitems, c.stream))) return rc;
+    if ((rc = wc.alloc(sizeof(int), c.stream))) return rc;
+    if ((rc = wl.alloc(sizeof(unsigned long long) * 2, c.stream))) return rc;  // [0] max ratio, [1] amax
+    LIPFIT_CUDA(cudaMemsetAsync(wl.p, 0, sizeof(unsigned long long) * 2, c.stream));
+    smooth_z_kernel<<<nblk, 256, 0, c.stream>>>(y, nullptr, N, wz.as<float>(), wi.as<int32_t>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(wsort.p, sort_bytes, wz.as<float>(), wzs.as<float>(),
+                                                wi.as<int32_t>(), wperm.as<int32_t>(), N, 0, 32,
+                                                c.stream));
+    smooth_gather_kernel<<<nblk, 256, 0, c.stream>>>(base, wperm.as<int32_t>(), wzs.as<float>(), N, lay.rf,
+                                                     lay.vslot, wrec.as<float>(),
+                                                     wg.as<unsigned long long>(),
+                                                     reinterpret_cast<uint32_t*>(wl.as<unsigned long long>() + 1));
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    LIPFIT_CUDA(cudaMemsetAsync(wc.p, 0, sizeof(int), c.stream));
+    a.rec = wrec.as<float>();
+    a.gfix = wg.as<unsigned long long>();
+    a.fpart = wf.as<double>();
+    a.vpart = wv.as<float>();
+    a.counter = wc.as<int>();
+    a.lmax = wl.as<unsigned long long>();
+    a.amax = reinterpret_cast<const uint32_t*>(wl.as<unsigned long long>() + 1);
+    a.X = X;
+    a.perm = wperm.as<int32_t>();
+    a.norm = norm;
+    a.xf = xf;
+    FreeFlags ff = make_free_flags(xf);
+    rc = dispatch_pairs<kModeLipConst>(c, a, ff, xf, norm);
+    if (rc) return rc;
+    lipconst_final_kernel<<<1, 1, 0, c.stream>>>(a.lmax, L_dev);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
     return LIPFIT_OK;
 }
 

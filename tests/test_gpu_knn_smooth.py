@@ -221,3 +221,41 @@ def test_smooth_then_bounds_config5_scaled():
     assert np.abs(gg.cpu().numpy() - g).max() <= tol
     ys, e2, info2 = L.lipfit_smooth_host(wl.X, wl.y, wl.M, wl.mask, wl.norm, None, wl.p, 200)
     np.testing.assert_array_equal(ys, z)          # an evaluation is bit-reproducible
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-3: smallest consistent Lipschitz constant
+# --------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("d,mask", [(1, [1]), (2, None), (5, [1, 1, 1, 1, 1]), (5, None), (7, [0, 1, 0, -1, 0, 0, 1]),
+                                    (12, None), (20, [1, 0] * 10)])
+def test_lipschitz_constant_shapes(norm, d, mask):
+    import paper_2606_04670_b200 as L
+    X, _, _ = random_problem(40 + d, 3001, 1, d)
+    s = np.zeros(d) if mask is None else np.asarray(mask, np.float64)
+    rng = np.random.default_rng(d)
+    y = (X.astype(np.float64) @ np.where(s == 0, 0.3, s) +
+         (0.0 if mask is not None else 0.2) * rng.standard_normal(len(X))).astype(np.float32)
+    w = (0.5 + np.arange(d) % 3).astype(np.float32)
+    ref = oracle.lipschitz_constant(X, y, mask, norm, w)
+    got = float(L.lipfit_lipschitz_constant(_dev(X), _dev(y), mask, norm, w).cpu()[0])
+    assert np.isfinite(ref) and abs(got - ref) <= 1e-5 * ref, (got, ref)
+    assert L.lipfit_lipschitz_constant_host(X, y, mask, norm, w) == got
+
+
+def test_lipschitz_constant_config_scaled_and_degenerate():
+    import paper_2606_04670_b200 as L
+    for cfg, N in ((1, 1000), (2, 9001), (5, 12000)):
+        wl = make_workload(cfg, N=N)
+        ref = oracle.lipschitz_constant(wl.X, wl.y, wl.mask, wl.norm, wl.weights)
+        got = L.lipfit_lipschitz_constant_host(wl.X, wl.y, wl.mask, wl.norm, wl.weights)
+        assert (np.isinf(ref) and np.isinf(got)) or abs(got - ref) <= 1e-5 * ref, (cfg, got, ref)
+    # consistency threshold: with M slightly above L the smoothing objective at eps = 0 is exactly 0
+    wl = make_workload(1, N=1000)
+    Lc = L.lipfit_lipschitz_constant_host(wl.X, wl.y, wl.mask, wl.norm)
+    F, _ = L.lipfit_smooth_objective(_dev(wl.X), _dev(wl.y), Lc * (1 + 1e-5), None, wl.mask, wl.norm)
+    assert F == 0.0
+    X = np.array([[0, 0], [0, 0], [1, 0]], np.float32)
+    assert L.lipfit_lipschitz_constant_host(X, np.array([1, 1, 1], np.float32)) == 0.0
+    assert L.lipfit_lipschitz_constant_host(X, np.array([1, 2, 1], np.float32)) == np.inf
+    assert L.lipfit_lipschitz_constant_host(X[:1], np.ones(1, np.float32)) == 0.0
