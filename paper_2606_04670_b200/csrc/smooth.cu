@@ -19,6 +19,8 @@
 // are handed out by an atomic counter.
 #include <cub/device/device_radix_sort.cuh>
 
+#include <type_traits>
+
 #include "kernels.h"
 
 #pragma nv_diag_suppress 128  // MODE 1 leaves the item loop before the smoothing-only reductions
@@ -223,6 +225,10 @@ smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
                 if (isinf(lcur)) lcur = 3.0e38f;  // keeps the filter arithmetic finite; the result stays +inf
                 refresh();
             }
+            // Two copies of the loop: tiles strictly below the diagonal (the vast majority) need neither
+            // the index test nor the sign test -- sorted order guarantees k < i and z_k <= z_i there.
+            auto sweep = [&](auto below_c) {
+            constexpr bool BELOW = decltype(below_c)::value;
             for (int j = 0; j < n; ++j) {
                 float x[RF];
                 smooth_load_record<RF>(s + j * RF, x);
@@ -237,7 +243,7 @@ smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
                     const float lhs = MODE == kModeLipConst ? acc[r] * lthr : acc[r];
                     if (MODE == kModeLipConst) dz[r] += leta;
                     pass[r] = Acc::NORM == 2 ? (lhs < dz[r] * dz[r]) : (lhs < dz[r]);
-                    if (!below) pass[r] = pass[r] && (base + j < ipos[r]) && (dz[r] > 0.f);
+                    if (!BELOW) pass[r] = pass[r] && (base + j < ipos[r]) && (dz[r] > 0.f);
                     hit |= pass[r];
                 }
                 if (__any_sync(0xffffffffu, hit)) {  // warp-uniform, rare
@@ -253,6 +259,9 @@ smooth_pairs_kernel(const SmoothArgs a, const FreeFlags ff) {
                     }
                 }
             }
+            };
+            if (below) sweep(std::true_type{});
+            else sweep(std::false_type{});
             if (MODE == kModeLipConst) {
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) lbest = fmax(lbest, __shfl_xor_sync(0xffffffffu, lbest, o));
