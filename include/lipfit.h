@@ -174,6 +174,16 @@ int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches);
  * superset certificate failed and that were therefore answered by the exact fp64 fallback
  * scan; valid once that call's stream has been synchronised.  0 on typical data. */
 int64_t lipfit_knn_fallbacks(void);
+/* Largest observed |selection key - exact fp64 key| divided by the certificate's error bound E,
+ * over every pool candidate of that call (same validity rule).  The bound is sound iff this
+ * stays <= 1; the tests assert it on every kNN case. */
+double lipfit_knn_key_error_ratio(void);
+/* Selection kernel choice for symmetric L2 with d <= 16: 1 (default) = tensor cores (tcgen05 bf16x3
+ * cross-term GEMM, csrc/knn_tc.cu), 0 = CUDA-core FFMA2 kernel.  Process-wide; results are identical
+ * (both feed the same exact re-rank). */
+void lipfit_knn_set_tensor_cores(int32_t on);
+/* Name of the selection kernel lipfit_knn would use for (d, side, norm). */
+int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, char* out, int32_t cap);
 /* Name of the kernel variant lipfit_bounds would dispatch to for (d, mask, norm), e.g.
  * "bounds<L1,U2,C2,R8>" or "bounds_generic<L2,DP8>"; writes at most `cap` bytes incl. NUL. */
 int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, char* out, int32_t cap);

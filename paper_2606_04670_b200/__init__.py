@@ -4,7 +4,7 @@ The product is the C-ABI library `liblipfit.so` (include/lipfit.h, sources in cs
 is its thin ctypes binding with the same entry-point names.
 """
 from .binding import (LIPFIT_L1, LIPFIT_L2, LIPFIT_LINF, LIPFIT_MAX_DIM, LIPFIT_MAX_K,  # noqa: F401
-                      LipfitError, bounds_variant, get_timing, knn_fallbacks, launch_count, set_timing, lipfit_bounds,
+                      LipfitError, bounds_variant, get_timing, knn_fallbacks, knn_key_error_ratio, knn_set_tensor_cores, knn_variant, launch_count, set_timing, lipfit_bounds,
                       lipfit_bounds_host, lipfit_knn, lipfit_knn_host, lipfit_lbfgs,
                       lipfit_lipschitz_constant, lipfit_lipschitz_constant_host,
                       lipfit_smooth, lipfit_smooth_host, lipfit_smooth_objective, load,

@@ -23,6 +23,7 @@ EXPORTS = [
     "lipfit_status_string", "lipfit_version", "lipfit_launch_count", "lipfit_bounds_variant",
     "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
+    "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
 ]
 
 
@@ -73,6 +74,11 @@ def load():
     lib.lipfit_version.restype = C.c_char_p
     lib.lipfit_launch_count.restype = C.c_int64
     lib.lipfit_set_timing.restype = None
+    lib.lipfit_knn_key_error_ratio.argtypes = []
+    lib.lipfit_knn_key_error_ratio.restype = C.c_double
+    lib.lipfit_knn_set_tensor_cores.argtypes = [i32]
+    lib.lipfit_knn_set_tensor_cores.restype = None
+    lib.lipfit_knn_variant.argtypes = [i32, i32, i32, C.c_char_p, i32]
     lib.lipfit_knn_fallbacks.argtypes = []
     lib.lipfit_knn_fallbacks.restype = i64
     lib.lipfit_set_timing.argtypes = [i32]
@@ -96,6 +102,21 @@ def launch_count() -> int:
 def knn_fallbacks() -> int:
     """Queries of the last lipfit_knn call answered by the exact fp64 fallback (after a sync)."""
     return int(load().lipfit_knn_fallbacks())
+
+
+def knn_key_error_ratio() -> float:
+    """Largest observed selection-key error / certificate bound of the last lipfit_knn call (<= 1)."""
+    return float(load().lipfit_knn_key_error_ratio())
+
+
+def knn_set_tensor_cores(on: bool) -> None:
+    load().lipfit_knn_set_tensor_cores(1 if on else 0)
+
+
+def knn_variant(d: int, side: int = 0, norm: int = LIPFIT_L2) -> str:
+    buf = C.create_string_buffer(96)
+    _check(load().lipfit_knn_variant(d, side, norm, buf, 96), "lipfit_knn_variant")
+    return buf.value.decode()
 
 
 def set_timing(on: bool) -> None:

@@ -71,6 +71,20 @@ int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, cha
 }
 
 int64_t lipfit_knn_fallbacks(void) { return knn_last_fallbacks(); }
+double lipfit_knn_key_error_ratio(void) { return knn_last_key_error_ratio(); }
+void lipfit_knn_set_tensor_cores(int32_t on) { knn_set_tensor_cores(on); }
+int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, char* out, int32_t cap) {
+    if (!out || cap < 1) return LIPFIT_E_NULL;
+    if (check_norm(norm) || side < -1 || side > 1) return LIPFIT_E_PARAM;
+    if (d < 1 || d > LIPFIT_MAX_DIM) return LIPFIT_E_DIM;
+    Xform xf;
+    std::vector<int32_t> mask(static_cast<size_t>(d), side == 0 ? 0 : 1);  // any constrained coordinate => one-sided
+    int rc = make_xform(d, mask.data(), nullptr, side == 0, false, &xf);
+    if (rc) return rc;
+    std::strncpy(out, knn_variant_name(xf, norm), static_cast<size_t>(cap) - 1);
+    out[cap - 1] = '\0';
+    return LIPFIT_OK;
+}
 
 int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                   float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,

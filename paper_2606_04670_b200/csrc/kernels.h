@@ -35,6 +35,11 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
 const char* knn_variant_name(const Xform& xf, int norm);
 // queries of the most recent completed lipfit_knn call that needed the exact fp64 fallback
 int64_t knn_last_fallbacks();
+// largest observed |selection key - exact fp64 key| / certificate bound E over all pool candidates of
+// the most recent completed call (must stay <= 1; the tests assert it)
+double knn_last_key_error_ratio();
+// 1 (default): symmetric L2 with d <= 16 selects on the tensor cores; 0: CUDA-core selection everywhere
+void knn_set_tensor_cores(int on);
 
 // a4: all-pairs objective/gradient.  base: packed records whose coordinates are PRE-MULTIPLIED BY M
 // (prepack with scale_xform(xf, M)); their value slot is ignored, z = y + eps is formed per call.

@@ -22,6 +22,9 @@
 //       adversarial inputs): one CTA per such query scans all data in fp64.
 // The result therefore never depends on the fp32 selection arithmetic.
 #include "kernels.h"
+#include "knn_common.cuh"
+
+#include <cstring>
 
 namespace lipfit {
 
@@ -31,31 +34,6 @@ namespace lipfit {
 #ifndef LIPFIT_KNN_MINB
 #define LIPFIT_KNN_MINB 3  // resident CTAs per SM the selection kernel is compiled for
 #endif
-constexpr int kKnnMargin = 8;
-constexpr int kSelThreads = 128;
-constexpr int kSelWarps = kSelThreads / 32;
-constexpr int kMaxP = 2 * (LIPFIT_MAX_K + kKnnMargin);  // 272 pool entries per (chunk, query)
-
-struct KnnArgs {
-    const float* rec;
-    const float* Xq;
-    int2* pool;     // [nch][Qp][P]  (x = key bits, y = datum index)
-    int32_t* fill;  // [nch][Qp]     valid entries of each pool at kernel end
-    float* tau;     // [nch][Qp]     final threshold: every datum of the chunk outside the pool has key >= tau
-    int N, Q, Qp, d, ksel, P;
-    // Work items: query blocks [0, nfull) sweep all N data as ONE chunk (fewest pool insertions);
-    // the remaining ntail blocks (the last, partial wave of the persistent grid) are cut into T
-    // data chunks of `chunk` records each so that the wave stays full.  Pools: chunk 0 of query slot
-    // q lives at pool slot q; chunk c >= 1 of a tail query at Qp + (c-1)*Qtp + (q - nfullq).
-    int nqb, nfull, ntail, T, chunk, nfullq, Qtp;
-    Xform xf;
-};
-
-__host__ __device__ __forceinline__ size_t knn_pool_slot(int qslot, int c, int Qp, int Qtp, int nfullq) {
-    return c == 0 ? static_cast<size_t>(qslot)
-                  : static_cast<size_t>(Qp) + static_cast<size_t>(c - 1) * Qtp + (qslot - nfullq);
-}
-
 // ---------------------------------------------------------------------------------------------
 // (0) pack
 // ---------------------------------------------------------------------------------------------
@@ -103,30 +81,6 @@ knn_pack_kernel(const float* __restrict__ X, int N, Xform xf, int rf, int x2slot
 // ---------------------------------------------------------------------------------------------
 // (1) selection
 // ---------------------------------------------------------------------------------------------
-// Warp-cooperative compaction of one pool of n entries: keeps the ksel smallest (key, index)
-// in slots [0, ksel) in ascending order and returns the ksel-th smallest key (the new tau).
-// All 32 lanes must call it; `scr` is this warp's shared scratch of >= n + 1 entries.
-__device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2* scr, int lane) {
-    for (int c = lane; c < n; c += 32) scr[c] = pool[c];
-    __syncwarp();
-    for (int c = lane; c < n; c += 32) {
-        const int2 e = scr[c];
-        const float de = __int_as_float(e.x);
-        int rank = 0;
-        for (int o = 0; o < n; ++o) {
-            const int2 f = scr[o];
-            const float df = __int_as_float(f.x);
-            rank += (df < de) || (df == de && f.y < e.y);
-        }
-        if (rank < ksel) pool[rank] = e;
-        if (rank == ksel - 1) scr[kMaxP] = e;
-    }
-    __syncwarp();
-    const float tau = __int_as_float(scr[kMaxP].x);
-    __syncwarp();
-    return tau;
-}
-
 // Slow path of the selection loop, entered warp-uniformly when some lane has a key below its
 // threshold: append (NREC records at once), and compact the pools that are (nearly) full.  A pool
 // is compacted as soon as fewer than NREC free entries are left, so NREC appends always fit.
@@ -338,7 +292,8 @@ struct RerankArgs {
     const int2* pool;
     const int32_t* fill;
     const float* tau;
-    const uint32_t* stats;
+    const uint32_t* stats;  // [0] max |x'|, [1] max ||x'||^2, [2] flagged count, [4] max observed key error / E
+    const float* mu;        // tensor-core path: centre of the coordinates
     int32_t* idx;
     float* dist;
     int32_t* flagged;   // [Q] queries whose certificate failed
@@ -371,11 +326,30 @@ __device__ __forceinline__ double knn_exact_key(const float* xq, const float* xk
 //   dot : E = (d + 8) u (sqrt(max ||x'||^2) + ||q'||)^2
 //   diff: L1  E = u a (4 d + 2 d^2),  Linf  E = 4 u a,  L2 (squared)  E = u a^2 (20 d + 4 d^2)
 // u = 2^-24; every formula is then doubled as slack for the fp32-rounded statistics themselves.
+//   tc  : key from the bf16-split GEMM on coordinates centred at mu (knn_tc.cu); qn = ||q_c||,
+//         xn = sqrt(max ||x_c||^2):  E = 10.5 2^-16 qn xn          (1.5 x the split residue 7 2^-16 qn xn)
+//                                      + 2^-17 (6 qn xn + xn^2)    (fp32 accumulation of <= 64 terms)
+//                                      + 4 (qn + xn) sqrt(d) 2^-23 (amax + qinf + qn + xn)   (centring in fp32)
 __device__ __forceinline__ void knn_error_bound(const float* xq, const Xform& xf, int norm, int dot,
-                                                const uint32_t* stats, double* E, double* shift) {
+                                                const uint32_t* stats, const float* mu, double* E,
+                                                double* shift) {
     const double u = 5.9604644775390625e-08;
     const double amax = static_cast<double>(__uint_as_float(stats[0]));
     const double x2max = static_cast<double>(__uint_as_float(stats[1]));
+    if (dot == 2) {
+        double qinf = 0.0, qc2 = 0.0;
+        for (int j = 0; j < xf.d; ++j) {
+            const double v = static_cast<double>(xf.sw[j]) * static_cast<double>(xq[xf.perm[j]]);
+            const double vc = v - static_cast<double>(mu[j]);
+            qinf = fmax(qinf, fabs(v));
+            qc2 += vc * vc;
+        }
+        const double qn = sqrt(qc2), xn = sqrt(x2max);
+        *E = 10.5 * 1.52587890625e-05 * qn * xn + 7.62939453125e-06 * (6.0 * qn * xn + x2max) +
+             4.0 * (qn + xn) * sqrt(static_cast<double>(xf.d)) * 2.0 * u * (amax + qinf + qn + xn);
+        *shift = qc2;
+        return;
+    }
     double qinf = 0.0, q2 = 0.0;
     for (int j = 0; j < xf.d; ++j) {
         const double v = fabs(static_cast<double>(xf.sw[j]) * static_cast<double>(xq[xf.perm[j]]));
@@ -410,6 +384,9 @@ knn_rerank_kernel(const RerankArgs a) {
     const float* xq = a.Xq + static_cast<size_t>(qi) * a.d;
     int total = 0;
     float tmin = __int_as_float(0x7f800000);
+    // certificate: every datum outside the pools has exact key >= tmin + shift - E
+    double E, shift, worst = 0.0;
+    knn_error_bound(xq, a.xf, a.norm, a.dot, a.stats, a.mu, &E, &shift);
     const int nch = qi >= a.nfullq ? a.T : 1;
     for (int ch = 0; ch < nch; ++ch) {
         const size_t slot = knn_pool_slot(qi, ch, a.Qp, a.Qtp, a.nfullq);
@@ -417,16 +394,22 @@ knn_rerank_kernel(const RerankArgs a) {
         tmin = fminf(tmin, a.tau[slot]);
         const int2* pq = a.pool + slot * a.P;
         for (int c = lane; c < nf; c += 32) {
-            const int32_t id = pq[c].y;
-            sd[warp][total + c] = knn_exact_key(xq, a.X + static_cast<size_t>(id) * a.d, a.xf, a.norm);
-            si[warp][total + c] = id;
+            const int2 e = pq[c];
+            const double ex = knn_exact_key(xq, a.X + static_cast<size_t>(e.y) * a.d, a.xf, a.norm);
+            sd[warp][total + c] = ex;
+            si[warp][total + c] = e.y;
+            worst = fmax(worst, fabs(static_cast<double>(__int_as_float(e.x)) + shift - ex));
         }
         total += nf;
     }
     __syncwarp();
-    // certificate: every datum outside the pools has exact key >= tmin + shift - E
-    double E, shift;
-    knn_error_bound(xq, a.xf, a.norm, a.dot, a.stats, &E, &shift);
+    // diagnostic (lipfit_knn_key_error_ratio): largest observed |selection key - exact key| over E
+    {
+        float ratio = E > 0.0 ? static_cast<float>(worst / E) : 0.f;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ratio = fmaxf(ratio, __shfl_xor_sync(0xffffffffu, ratio, o));
+        if (lane == 0 && ratio > 0.f) atomicMax(const_cast<uint32_t*>(a.stats) + 4, __float_as_uint(ratio));
+    }
     const bool all_in = !(tmin < __int_as_float(0x7f800000));  // no pool was ever compacted
     const double lb = static_cast<double>(tmin) + shift - E;
     int myrank[kMaxCand / 32];
@@ -630,18 +613,24 @@ int dispatch(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int norm, bool onesi
                     : dispatch_dp<3, false>(c, a, ff, dp, slots, query_only);
 }
 
+// pinned host words written stream-ordered at the end of every call: [0] exact-fallback queries,
+// [1] bits of the largest observed key error / bound
 int32_t* fallback_word() {
     static int32_t* h = [] {
         int32_t* p = nullptr;
-        if (cudaMallocHost(&p, sizeof(int32_t)) != cudaSuccess) {
+        if (cudaMallocHost(&p, 2 * sizeof(int32_t)) != cudaSuccess) {
             (void)cudaGetLastError();
             return static_cast<int32_t*>(nullptr);
         }
-        *p = 0;
+        p[0] = p[1] = 0;
         return p;
     }();
     return h;
 }
+
+std::atomic<int> g_knn_tc{1};
+
+bool use_tc(const Xform& xf, int norm) { return norm == 2 && xf.dC == 0 && xf.d <= 16 && g_knn_tc.load() != 0; }
 
 }  // namespace
 
@@ -649,8 +638,18 @@ int64_t knn_last_fallbacks() {
     int32_t* h = fallback_word();
     return h ? static_cast<int64_t>(*reinterpret_cast<volatile int32_t*>(h)) : -1;
 }
+double knn_last_key_error_ratio() {
+    int32_t* h = fallback_word();
+    if (!h) return -1.0;
+    const int32_t bits = *reinterpret_cast<volatile int32_t*>(h + 1);
+    float f;
+    memcpy(&f, &bits, sizeof(f));
+    return static_cast<double>(f);
+}
+void knn_set_tensor_cores(int on) { g_knn_tc.store(on ? 1 : 0); }
 
 const char* knn_variant_name(const Xform& xf, int norm) {
+    if (use_tc(xf, norm)) return "knn_tc_select<bf16x3,K64>";
     return (norm == 2 && xf.dC == 0) ? "knn_select<dot>" : "knn_select<diff>";
 }
 
@@ -668,17 +667,21 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     a.xf = xf;
     a.ksel = static_cast<int>(N < k + kKnnMargin ? N : k + kKnnMargin);
     a.P = 2 * a.ksel;
-    const int qper = kSelThreads * knn_r(dp);
+    const bool tc = use_tc(xf, norm);  // tensor-core selection (knn_tc.cu)
+    const int qper = tc ? kTcQueries : kSelThreads * knn_r(dp);
     a.nqb = (a.Q + qper - 1) / qper;
     a.Qp = a.nqb * qper;
     FreeFlags ff = make_free_flags(xf);
-    const int occ = dispatch(c, a, ff, norm, onesided, dot, dp, 0, true);
-    if (occ < 0) return occ;
-    const int slots = c.num_sms * occ;
+    int slots = knn_tc_slots(c);
+    if (!tc) {
+        const int occ = dispatch(c, a, ff, norm, onesided, dot, dp, 0, true);
+        if (occ < 0) return occ;
+        slots = c.num_sms * occ;
+    }
 
     // Schedule (KnnArgs): whole waves of query blocks sweep the data unsplit; the blocks of the last,
     // partial wave are cut into T <= 8 data chunks (pools must fit the re-rank) to keep it full.
-    const int tile = rf <= 8 ? 256 : (rf <= 20 ? 128 : 64);
+    const int tile = tc ? kTcBN : (rf <= 8 ? 256 : (rf <= 20 ? 128 : 64));
     int maxT = kMaxCand / a.P;
     if (maxT > 8) maxT = 8;
     const int by_n = a.N / (8 * a.P);
@@ -699,25 +702,30 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
 
     // workspace: records | stats + flagged counter | pools | fill | tau | flagged list
     const size_t nq = static_cast<size_t>(a.Qp) + static_cast<size_t>(T - 1) * a.Qtp;
-    Workspace wrec, wp, wf, wt, wfl, wflT, wst;
+    Workspace wrec, wp, wf, wt, wfl, wflT, wst, wmu;
     int rc;
-    if ((rc = wrec.alloc(sizeof(float) * static_cast<size_t>(N) * rf, c.stream))) return rc;
-    if ((rc = wst.alloc(sizeof(uint32_t) * 4, c.stream))) return rc;
+    if ((rc = wrec.alloc(tc ? 16 : sizeof(float) * static_cast<size_t>(N) * rf, c.stream))) return rc;
+    if ((rc = wst.alloc(sizeof(uint32_t) * 8, c.stream))) return rc;
+    if ((rc = wmu.alloc(sizeof(float) * kMaxDim, c.stream))) return rc;
     if ((rc = wp.alloc(sizeof(int2) * nq * a.P, c.stream))) return rc;
     if ((rc = wf.alloc(sizeof(int32_t) * nq, c.stream))) return rc;
     if ((rc = wt.alloc(sizeof(float) * nq, c.stream))) return rc;
     if ((rc = wfl.alloc(sizeof(int32_t) * static_cast<size_t>(a.Q), c.stream))) return rc;
     if ((rc = wflT.alloc(sizeof(double) * static_cast<size_t>(a.Q), c.stream))) return rc;
-    LIPFIT_CUDA(cudaMemsetAsync(wst.p, 0, sizeof(uint32_t) * 4, c.stream));
+    LIPFIT_CUDA(cudaMemsetAsync(wst.p, 0, sizeof(uint32_t) * 8, c.stream));
     uint32_t* stats = wst.as<uint32_t>();
-    knn_pack_kernel<<<(a.N + 255) / 256, 256, 0, c.stream>>>(X, a.N, xf, rf, dp, wrec.as<float>(), stats);
-    ++g_launches;
-    LIPFIT_CUDA(cudaGetLastError());
     a.rec = wrec.as<float>();
     a.pool = wp.as<int2>();
     a.fill = wf.as<int32_t>();
     a.tau = wt.as<float>();
-    rc = dispatch(c, a, ff, norm, onesided, dot, dp, slots, false);
+    if (tc) {
+        rc = launch_knn_tc_select(c, X, Xq, a, wmu.as<float>(), stats);
+    } else {
+        knn_pack_kernel<<<(a.N + 255) / 256, 256, 0, c.stream>>>(X, a.N, xf, rf, dp, wrec.as<float>(), stats);
+        ++g_launches;
+        LIPFIT_CUDA(cudaGetLastError());
+        rc = dispatch(c, a, ff, norm, onesided, dot, dp, slots, false);
+    }
     if (rc) return rc;
 
     RerankArgs r{};
@@ -727,6 +735,7 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     r.fill = a.fill;
     r.tau = a.tau;
     r.stats = stats;
+    r.mu = wmu.as<float>();
     r.idx = idx;
     r.dist = dist;
     r.flagged = wfl.as<int32_t>();
@@ -742,7 +751,7 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     r.P = a.P;
     r.k = k;
     r.norm = norm;
-    r.dot = dot ? 1 : 0;
+    r.dot = tc ? 2 : (dot ? 1 : 0);
     r.xf = xf;
     knn_rerank_kernel<<<(a.Q + kRerankWarps - 1) / kRerankWarps, kRerankWarps * 32, 0, c.stream>>>(r);
     ++g_launches;
@@ -752,8 +761,10 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     // introspection (lipfit_knn_fallbacks): copied to pinned host memory, stream-ordered, no sync
-    if (int32_t* h = fallback_word())
+    if (int32_t* h = fallback_word()) {
         LIPFIT_CUDA(cudaMemcpyAsync(h, stats + 2, sizeof(int32_t), cudaMemcpyDeviceToHost, c.stream));
+        LIPFIT_CUDA(cudaMemcpyAsync(h + 1, stats + 4, sizeof(int32_t), cudaMemcpyDeviceToHost, c.stream));
+    }
     return LIPFIT_OK;
 }
 

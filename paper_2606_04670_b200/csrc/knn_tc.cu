@@ -1,0 +1,460 @@
+// knn_tc.cu -- step a3 on the 5th-generation tensor cores (north_star:
+// "Tensor cores are used only if the L2 cross term is done as a GEMM, and then only with an
+// fp32-accurate correction").  Symmetric L2, d <= 16.
+//
+// Selection key of (query q, datum x), both centred at mu (c = . - mu):
+//     key = ||x_c||^2 - 2 q_c . x_c      ( = ||q - x||^2 - ||q_c||^2 : same order as the distance )
+// as ONE bf16 GEMM with K = 64 and fp32 accumulation in tensor memory.  fp32 values are split
+// v = hi + lo (two bf16, 16 significant bits) and the operand rows are
+//     A (query) = [ hi(-2 q_c) | hi(-2 q_c) | lo(-2 q_c) | 1 1 1 0.. ]      16 + 16 + 16 + 16 = 64 bf16
+//     B (datum) = [ hi(x_c)    | lo(x_c)    | hi(x_c)    | x2_h x2_m x2_l 0.. ]   (||x_c||^2 in 3 bf16)
+// so A.B = hi.hi + hi.lo + lo.hi + ||x_c||^2: the dropped lo.lo terms and the split residue are
+// <= 3 * 2^-16 |q'_j x_j| per coordinate; the fp64 re-rank + certificate of knn.cu
+// turn the selected pools into the exact answer, whatever the key arithmetic was.
+//
+// Kernel (one CTA per SM, 320 threads, warp-specialised):
+//   warp 8   TMA producer : 1-D bulk copies of pre-swizzled operand tiles (the pack kernels write the
+//                           global image in the canonical K-major SWIZZLE_128B shared-memory layout,
+//                           so no tensor map is needed) into a 4-stage ring; A (2 x 128 queries) once
+//                           per work item.
+//   warp 9   MMA issuer   : one thread; per B tile 2 x 4 tcgen05.mma (M=128, N=128, K=16) into
+//                           double-buffered TMEM accumulators (2 query halves x 2 stages x 128 columns).
+//   warps 0-7 epilogue    : tcgen05.ld 32 columns at a time (thread = query row), min-tree + one compare
+//                           against the query's threshold; rare hits append to the candidate pool /
+//                           compact it exactly as in knn.cu.
+#include <cuda_bf16.h>
+
+#include "knn_common.cuh"
+
+namespace lipfit {
+
+namespace {
+
+constexpr int kTcThreads = 320;
+constexpr int kTcStages = 4;
+constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
+constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
+constexpr int kTcValsPerWarp = 32 * 33;           // padded [lane][column] scratch of the slow path
+constexpr size_t kTcSmemBytes = 1024 /*alignment slack*/ + 2 * kTcTileBytes + kTcStages * kTcTileBytes +
+                                8 * kTcValsPerWarp * sizeof(float) + 8 * (kMaxP + 1) * sizeof(int2);
+
+// byte offset of 16-byte chunk c (0..7) of row r inside a K-major SWIZZLE_128B tile of 128-byte rows
+__host__ __device__ __forceinline__ uint32_t sw128_offset(int r, int c) {
+    return static_cast<uint32_t>((r >> 3) * 1024 + (r & 7) * 128 + ((c ^ (r & 7)) << 4));
+}
+
+// ---- PTX wrappers (tcgen05 / mbarrier) -------------------------------------------------------
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_fence_after() {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {  // arrives when all prior MMAs of this thread are done
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(
+                     smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                       uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// K-major, SWIZZLE_128B, 128-byte rows: LBO = 1 (unused), SBO = 1024 B between 8-row groups, version 1
+__device__ __forceinline__ uint64_t tc_smem_desc(uint32_t saddr) {
+    return static_cast<uint64_t>((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | (64ull << 32) | (1ull << 46) |
+           (2ull << 61);
+}
+// kind::f16: D fp32, A/B bf16, both K-major, N = 128, M = 128
+constexpr uint32_t kTcIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((kTcBN >> 3) << 17) | ((128u >> 4) << 24);
+
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]),
+          "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]),
+          "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]),
+          "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr));
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Operand images
+// ---------------------------------------------------------------------------------------------
+// Centre: the mean of the first min(N, 4096) records, one block, fixed summation order (so that the
+// whole call is deterministic).  Any centre is valid; a good one shrinks the error bound.
+__global__ void __launch_bounds__(256)
+knn_tc_centre_kernel(const float* __restrict__ X, int N, Xform xf, float* __restrict__ mu) {
+    __shared__ double red[256];
+    const int n = N < 4096 ? N : 4096;
+    for (int j = 0; j < kMaxDim; ++j) {
+        double s = 0.0;
+        if (j < xf.d)
+            for (int k = threadIdx.x; k < n; k += 256)
+                s += static_cast<double>(xf.sw[j] * X[static_cast<size_t>(k) * xf.d + xf.perm[j]]);
+        red[threadIdx.x] = s;
+        __syncthreads();
+        for (int o = 128; o > 0; o >>= 1) {
+            if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) mu[j] = j < xf.d ? static_cast<float>(red[0] / n) : 0.f;
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ void split2(float v, __nv_bfloat16& hi, __nv_bfloat16& lo) {
+    hi = __float2bfloat16_rn(v);
+    lo = __float2bfloat16_rn(v - __bfloat162float(hi));
+}
+
+__device__ __forceinline__ void store_row(unsigned char* tile, int r, const __nv_bfloat16 (&row)[kTcK]) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        uint4 w;
+        const uint16_t* p = reinterpret_cast<const uint16_t*>(&row[8 * c]);
+        w.x = p[0] | (static_cast<uint32_t>(p[1]) << 16);
+        w.y = p[2] | (static_cast<uint32_t>(p[3]) << 16);
+        w.z = p[4] | (static_cast<uint32_t>(p[5]) << 16);
+        w.w = p[6] | (static_cast<uint32_t>(p[7]) << 16);
+        *reinterpret_cast<uint4*>(tile + sw128_offset(r, c)) = w;
+    }
+}
+
+// B image: record k -> tile k / 128, row k % 128.  Rows past N carry key = +huge.
+__global__ void __launch_bounds__(256)
+knn_tc_pack_b_kernel(const float* __restrict__ X, int N, int Npad, Xform xf, const float* __restrict__ mu,
+                     unsigned char* __restrict__ img, uint32_t* __restrict__ stats) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    float amax = 0.f, x2f = 0.f;
+    if (k < Npad) {
+        __nv_bfloat16 row[kTcK];
+#pragma unroll
+        for (int j = 0; j < kTcK; ++j) row[j] = __float2bfloat16_rn(0.f);
+        if (k < N) {
+            const float* src = X + static_cast<size_t>(k) * xf.d;
+            double s2 = 0.0;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                float xc = 0.f;
+                if (j < xf.d) {
+                    const float xw = xf.sw[j] * src[xf.perm[j]];
+                    amax = fmaxf(amax, fabsf(xw));
+                    xc = xw - mu[j];
+                }
+                s2 += static_cast<double>(xc) * static_cast<double>(xc);
+                __nv_bfloat16 hi, lo;
+                split2(xc, hi, lo);
+                row[j] = hi;
+                row[16 + j] = lo;
+                row[32 + j] = hi;
+            }
+            x2f = static_cast<float>(s2);
+            const __nv_bfloat16 h = __float2bfloat16_rn(x2f);
+            const float r1 = x2f - __bfloat162float(h);
+            const __nv_bfloat16 m = __float2bfloat16_rn(r1);
+            const __nv_bfloat16 l = __float2bfloat16_rn(r1 - __bfloat162float(m));
+            row[48] = h;
+            row[49] = m;
+            row[50] = l;
+        } else {
+            row[48] = __float2bfloat16_rn(3.0e38f);
+        }
+        store_row(img + static_cast<size_t>(k / kTcBN) * kTcTileBytes, k % kTcBN, row);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+        x2f = fmaxf(x2f, __shfl_xor_sync(0xffffffffu, x2f, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(stats + 0, __float_as_uint(amax));
+        atomicMax(stats + 1, __float_as_uint(x2f));
+    }
+}
+
+// A image: query slot q -> tile q / 128, row q % 128.  Slots past Q are all-zero rows.
+__global__ void __launch_bounds__(256)
+knn_tc_pack_a_kernel(const float* __restrict__ Xq, int Q, int Qp, Xform xf, const float* __restrict__ mu,
+                     unsigned char* __restrict__ img) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= Qp) return;
+    __nv_bfloat16 row[kTcK];
+#pragma unroll
+    for (int j = 0; j < kTcK; ++j) row[j] = __float2bfloat16_rn(0.f);
+    if (q < Q) {
+        const float* src = Xq + static_cast<size_t>(q) * xf.d;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            float qc = 0.f;
+            if (j < xf.d) qc = xf.sw[j] * src[xf.perm[j]] - mu[j];
+            __nv_bfloat16 hi, lo;
+            split2(-2.f * qc, hi, lo);
+            row[j] = hi;
+            row[16 + j] = hi;
+            row[32 + j] = lo;
+        }
+        row[48] = row[49] = row[50] = __float2bfloat16_rn(1.f);
+    }
+    store_row(img + static_cast<size_t>(q / 128) * kTcTileBytes, q % 128, row);
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// Selection kernel
+// ---------------------------------------------------------------------------------------------
+struct KnnTcArgs {
+    const unsigned char* Aimg;  // [Qp/128] tiles of 128 query rows
+    const unsigned char* Bimg;  // [ntilesB] tiles of 128 data rows
+    int ntilesB;
+    KnnArgs k;                  // pools, schedule (query blocks of kTcQueries), N, Q, ksel, P
+};
+
+// Epilogue work on 32 keys of one query (this lane's row): v[c] is the key of datum kbase + c.
+__device__ __forceinline__ void tc_process(const KnnArgs& a, const float (&v)[32], int kbase, float& tau,
+                                           int& fill, int2* pool, float* scrv, int2* scr2, int lane) {
+    float m = v[0];
+#pragma unroll
+    for (int c = 1; c < 32; ++c) m = fminf(m, v[c]);
+    if (!__any_sync(0xffffffffu, m < tau)) return;  // the common case
+    unsigned mask = 0;
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+        mask |= (v[c] < tau) ? (1u << c) : 0u;
+        scrv[lane * 33 + c] = v[c];
+    }
+    __syncwarp();
+    const int P = a.P;
+    for (;;) {
+        while (mask != 0 && fill < P) {
+            const int c = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const float val = scrv[lane * 33 + c];
+            const int idx = kbase + c;
+            if (val < tau && idx < a.N) {  // rows past N are padding
+                pool[fill] = make_int2(__float_as_int(val), idx);
+                ++fill;
+            }
+        }
+        unsigned fm = __ballot_sync(0xffffffffu, fill == P);
+        if (fm == 0) break;  // no pool is full => every lane has drained its mask
+        __syncwarp();        // orders the appends above before the cooperative reads below
+        while (fm) {
+            const int src = __ffs(fm) - 1;
+            fm &= fm - 1;
+            int2* pq = pool + static_cast<ptrdiff_t>(src - lane) * P;  // consecutive lanes = consecutive slots
+            const float nt = knn_compact(pq, P, a.ksel, scr2, lane);
+            if (lane == src) {
+                tau = nt;
+                fill = a.ksel;
+            }
+        }
+    }
+    __syncwarp();
+}
+
+__global__ void __launch_bounds__(kTcThreads, 1)
+knn_tc_select_kernel(const KnnTcArgs g) {
+    extern __shared__ unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t a_full, a_empty, b_full[kTcStages], b_empty[kTcStages], acc_full[2][2],
+        acc_empty[2][2];
+    __shared__ uint32_t s_tmem;
+    // 1024-byte aligned carve-up (SWIZZLE_128B atoms are 1024 B)
+    const uint32_t raw = smem_u32(smem_raw);
+    unsigned char* base = smem_raw + ((1024u - (raw & 1023u)) & 1023u);
+    unsigned char* sA = base;                                // 2 tiles
+    unsigned char* sB = sA + 2 * kTcTileBytes;               // kTcStages tiles
+    float* sV = reinterpret_cast<float*>(sB + kTcStages * kTcTileBytes);        // 8 x [32][33]
+    int2* sC = reinterpret_cast<int2*>(sV + 8 * kTcValsPerWarp);                // 8 x [kMaxP + 1]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const KnnArgs& a = g.k;
+    if (threadIdx.x == 0) {
+        mbar_init(&a_full, 1);
+        mbar_init(&a_empty, 1);
+        for (int s = 0; s < kTcStages; ++s) {
+            mbar_init(&b_full[s], 1);
+            mbar_init(&b_empty[s], 1);
+        }
+        for (int h = 0; h < 2; ++h)
+            for (int b = 0; b < 2; ++b) {
+                mbar_init(&acc_full[h][b], 1);
+                mbar_init(&acc_empty[h][b], 4);  // the 4 epilogue warps of the half
+            }
+        mbar_fence_init();
+    }
+    if (warp == 8) {  // the whole warp allocates all 512 TMEM columns of this SM
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         smem_u32(&s_tmem)),
+                     "r"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    const int nitems = a.nfull + a.ntail * a.T;
+    const int chunk_tiles = a.chunk / kTcBN;
+    // item -> (query block, chunk, B tile range)
+    auto decode = [&](int item, int& qb, int& ch, int& tb, int& te) {
+        if (item < a.nfull) {
+            qb = item;
+            ch = 0;
+            tb = 0;
+            te = g.ntilesB;
+        } else {
+            const int t = item - a.nfull;
+            qb = a.nfull + t / a.T;
+            ch = t - (qb - a.nfull) * a.T;
+            tb = ch * chunk_tiles;
+            te = min(g.ntilesB, tb + chunk_tiles);
+        }
+    };
+
+    if (warp == 8) {
+        // ================= TMA producer =================
+        if (lane == 0) {
+            uint32_t gB = 0, it = 0;
+            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
+                int qb, ch, tb, te;
+                decode(item, qb, ch, tb, te);
+                mbar_wait(&a_empty, (it & 1u) ^ 1u);
+                mbar_arrive_expect_tx(&a_full, 2 * kTcTileBytes);
+                bulk_g2s(sA, g.Aimg + static_cast<size_t>(qb) * 2 * kTcTileBytes, 2 * kTcTileBytes, &a_full);
+                for (int t = tb; t < te; ++t, ++gB) {
+                    const uint32_t s = gB % kTcStages, u = gB / kTcStages;
+                    mbar_wait(&b_empty[s], (u & 1u) ^ 1u);
+                    mbar_arrive_expect_tx(&b_full[s], kTcTileBytes);
+                    bulk_g2s(sB + s * kTcTileBytes, g.Bimg + static_cast<size_t>(t) * kTcTileBytes,
+                             kTcTileBytes, &b_full[s]);
+                }
+            }
+        }
+    } else if (warp == 9) {
+        // ================= MMA issuer =================
+        if (lane == 0) {
+            uint32_t gB = 0, it = 0;
+            const uint64_t adesc0 = tc_smem_desc(smem_u32(sA));
+            const uint64_t adesc1 = tc_smem_desc(smem_u32(sA + kTcTileBytes));
+            for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
+                int qb, ch, tb, te;
+                decode(item, qb, ch, tb, te);
+                mbar_wait(&a_full, it & 1u);
+                tc_fence_after();
+                for (int t = tb; t < te; ++t, ++gB) {
+                    const uint32_t s = gB % kTcStages, u = gB / kTcStages;
+                    const uint32_t b = gB & 1u, ua = gB >> 1;
+                    mbar_wait(&b_full[s], u & 1u);
+                    tc_fence_after();
+                    const uint64_t bdesc = tc_smem_desc(smem_u32(sB + s * kTcTileBytes));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        mbar_wait(&acc_empty[h][b], (ua & 1u) ^ 1u);
+                        tc_fence_after();
+                        const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
+                        const uint64_t ad = h ? adesc1 : adesc0;
+#pragma unroll
+                        for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
+                            tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
+                        tc_commit(&acc_full[h][b]);
+                    }
+                    tc_commit(&b_empty[s]);
+                }
+                tc_commit(&a_empty);
+            }
+        }
+    } else {
+        // ================= epilogue warps: h = query half, quad = TMEM lane quadrant =================
+        const int h = warp >> 2, quad = warp & 3;
+        float* scrv = sV + warp * kTcValsPerWarp;
+        int2* scr2 = sC + warp * (kMaxP + 1);
+        uint32_t gB = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            int qb, ch, tb, te;
+            decode(item, qb, ch, tb, te);
+            const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
+            float tau = qslot < a.Q ? __int_as_float(0x7f800000) : __int_as_float(0xff800000);
+            int fill = 0;
+            const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
+            int2* pool = a.pool + slot * a.P;
+            for (int t = tb; t < te; ++t, ++gB) {
+                const uint32_t b = gB & 1u, ua = gB >> 1;
+                mbar_wait(&acc_full[h][b], ua & 1u);
+                tc_fence_after();
+#pragma unroll 1
+                for (int cb = 0; cb < kTcBN / 32; ++cb) {
+                    float v[32];
+                    tc_ld32(tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN + cb * 32, v);
+                    tc_process(a, v, t * kTcBN + cb * 32, tau, fill, pool, scrv, scr2, lane);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+            }
+            a.fill[slot] = fill;
+            a.tau[slot] = tau;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 8)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
+}
+
+int knn_tc_slots(const Ctx& c) { return c.num_sms; }
+
+int launch_knn_tc_select(const Ctx& c, const float* X, const float* Xq, KnnArgs& a, float* mu_dev,
+                         uint32_t* stats) {
+    const int ntilesB = (a.N + kTcBN - 1) / kTcBN;
+    const int Npad = ntilesB * kTcBN;
+    Workspace wa, wb;
+    int rc;
+    if ((rc = wa.alloc(static_cast<size_t>(a.Qp) * kTcK * 2, c.stream))) return rc;
+    if ((rc = wb.alloc(static_cast<size_t>(Npad) * kTcK * 2, c.stream))) return rc;
+    knn_tc_centre_kernel<<<1, 256, 0, c.stream>>>(X, a.N, a.xf, mu_dev);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    knn_tc_pack_b_kernel<<<(Npad + 255) / 256, 256, 0, c.stream>>>(X, a.N, Npad, a.xf, mu_dev,
+                                                                   wb.as<unsigned char>(), stats);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    knn_tc_pack_a_kernel<<<(a.Qp + 255) / 256, 256, 0, c.stream>>>(Xq, a.Q, a.Qp, a.xf, mu_dev,
+                                                                   wa.as<unsigned char>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    KnnTcArgs g{};
+    g.Aimg = wa.as<unsigned char>();
+    g.Bimg = wb.as<unsigned char>();
+    g.ntilesB = ntilesB;
+    g.k = a;
+    LIPFIT_CUDA(cudaFuncSetAttribute(knn_tc_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     static_cast<int>(kTcSmemBytes)));
+    const long long nitems = static_cast<long long>(a.nfull) + static_cast<long long>(a.ntail) * a.T;
+    const int grid = static_cast<int>(nitems < c.num_sms ? nitems : c.num_sms);
+    KernelTimer kt(TK_KNN_SELECT, c.stream);
+    knn_tc_select_kernel<<<grid, kTcThreads, kTcSmemBytes, c.stream>>>(g);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+}  // namespace lipfit

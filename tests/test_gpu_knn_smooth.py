@@ -20,6 +20,8 @@ def _gpu_knn(X, Xq, k, mask=None, side=0, norm=L2, w=None):
     import paper_2606_04670_b200 as L
     idx, dist = L.lipfit_knn(_dev(X), _dev(Xq), k, mask, side, norm, w)
     torch.cuda.synchronize()
+    # the certificate's error bound must dominate every observed selection-key error
+    assert L.knn_key_error_ratio() <= 1.0, L.knn_key_error_ratio()
     return idx.cpu().numpy(), dist.cpu().numpy()
 
 
@@ -120,6 +122,29 @@ def test_certificate_and_exact_fallback():
     np.testing.assert_array_equal(gi, np.tile(np.arange(9, dtype=np.int32), (40, 1)))
     oi, od = oracle.knn(X, Xq, 9)
     np.testing.assert_array_equal(gd, od.astype(np.float32))
+
+
+@pytest.mark.parametrize("d", [1, 2, 5, 8, 13, 16])
+def test_tensor_core_and_cuda_core_selection_agree(d):
+    """Symmetric L2, d <= 16 selects on the tensor cores (bf16x3 cross-term GEMM); switching them off
+    uses the FFMA2 kernel.  Both feed the same exact re-rank: identical outputs, both equal to the oracle."""
+    import paper_2606_04670_b200 as L
+    assert "tc" in L.knn_variant(d, 0, L2) and "tc" not in L.knn_variant(17, 0, L2)
+    assert "tc" not in L.knn_variant(d, 1, L2) and "tc" not in L.knn_variant(d, 0, L1)
+    X, _, Xq = random_problem(300 + d, 20011, 700, d, spread=3.0)
+    X += 5.0                                                   # off-centre data: the centring matters
+    Xq += 5.0
+    w = (0.5 + np.arange(d) % 2).astype(np.float32)
+    try:
+        check_knn(X, Xq, 32, None, 0, L2, w)
+        a = _gpu_knn(X, Xq, 32, None, 0, L2, w)
+        L.knn_set_tensor_cores(False)
+        assert "tc" not in L.knn_variant(d, 0, L2)
+        b = _gpu_knn(X, Xq, 32, None, 0, L2, w)
+    finally:
+        L.knn_set_tensor_cores(True)
+    np.testing.assert_array_equal(a[0], b[0])
+    np.testing.assert_array_equal(a[1], b[1])
 
 
 def test_knn_host_and_errors():
