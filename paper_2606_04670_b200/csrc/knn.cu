@@ -668,6 +668,7 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     a.ksel = static_cast<int>(N < k + kKnnMargin ? N : k + kKnnMargin);
     a.P = 2 * a.ksel;
     const bool tc = use_tc(xf, norm);  // tensor-core selection (knn_tc.cu)
+    if (tc) a.P = a.ksel + kTcPoolExtra;
     const int qper = tc ? kTcQueries : kSelThreads * knn_r(dp);
     a.nqb = (a.Q + qper - 1) / qper;
     a.Qp = a.nqb * qper;

@@ -30,30 +30,57 @@ __host__ __device__ __forceinline__ size_t knn_pool_slot(int qslot, int c, int Q
                   : static_cast<size_t>(Qp) + static_cast<size_t>(c - 1) * Qtp + (qslot - nfullq);
 }
 
-// Warp-cooperative compaction of one pool of n entries: keeps the ksel smallest (key, index)
-// in slots [0, ksel) in ascending order and returns the ksel-th smallest key (the new tau).
-// All 32 lanes must call it; `scr` is this warp's shared scratch of >= n + 1 entries.
-__device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2* scr, int lane) {
-    for (int c = lane; c < n; c += 32) scr[c] = pool[c];
-    __syncwarp();
-    for (int c = lane; c < n; c += 32) {
-        const int2 e = scr[c];
-        const float de = __int_as_float(e.x);
-        int rank = 0;
-        for (int o = 0; o < n; ++o) {
-            const int2 f = scr[o];
-            const float df = __int_as_float(f.x);
-            rank += (df < de) || (df == de && f.y < e.y);
+// Warp-cooperative compaction of one pool of n entries: keeps exactly the ksel entries with the
+// smallest keys in slots [0, ksel) (unordered; the re-rank sorts) and returns the ksel-th smallest key
+// (the new tau).  Register-resident radix select: every lane holds NE entries (n <= 32 NE), the
+// ksel-th smallest order-preserving integer key is found bit by bit with warp votes (no shared
+// memory, no data-dependent loads), then the kept entries are written back at their ballot-prefix
+// positions; ties at the threshold are kept in pool order.  All 32 lanes must call it.
+template <int NE>
+__device__ __forceinline__ float knn_compact_regs(int2* pool, int n, int ksel, int lane) {
+    uint32_t key[NE];
+    int2 e[NE];
+#pragma unroll
+    for (int i = 0; i < NE; ++i) {
+        const int c = lane + 32 * i;
+        e[i] = c < n ? pool[c] : make_int2(0, 0);
+        key[i] = c < n ? f2key(__int_as_float(e[i].x)) : 0xFFFFFFFFu;  // padding sorts last
+    }
+    uint32_t prefix = 0;
+    int need = ksel;  // rank still wanted among the keys that agree with `prefix` on the decided bits
+#pragma unroll 1
+    for (int bit = 31; bit >= 0; --bit) {
+        int cnt0 = 0;  // keys that agree with prefix above `bit` and have a 0 at `bit`
+#pragma unroll
+        for (int i = 0; i < NE; ++i)
+            cnt0 += __popc(__ballot_sync(0xffffffffu, ((key[i] ^ prefix) >> bit) == 0u));
+        if (need > cnt0) {
+            need -= cnt0;
+            prefix |= 1u << bit;
         }
-        if (rank < ksel) pool[rank] = e;
-        if (rank == ksel - 1) scr[kMaxP] = e;
+    }
+    // prefix = the ksel-th smallest key; `need` of the entries equal to it are kept
+    const unsigned below = (1u << lane) - 1u;
+    int base = 0, eqbase = 0;
+#pragma unroll
+    for (int i = 0; i < NE; ++i) {
+        const bool lt = key[i] < prefix;
+        const bool eq = key[i] == prefix;
+        const unsigned be = __ballot_sync(0xffffffffu, eq);
+        const bool keep = lt || (eq && eqbase + __popc(be & below) < need);
+        const unsigned bk = __ballot_sync(0xffffffffu, keep);
+        if (keep) pool[base + __popc(bk & below)] = e[i];
+        base += __popc(bk);
+        eqbase += __popc(be);
     }
     __syncwarp();
-    const float tau = __int_as_float(scr[kMaxP].x);
-    __syncwarp();
-    return tau;
+    return key2f(prefix);
 }
 
+__device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2*, int lane) {
+    if (n <= 128) return knn_compact_regs<4>(pool, n, ksel, lane);
+    return knn_compact_regs<(kMaxP + 31) / 32>(pool, n, ksel, lane);
+}
 
 // knn_tc.cu: tensor-core (tcgen05) selection for symmetric L2, d <= 16.  Packs its own operand images,
 // fills a.pool / a.fill / a.tau with the schedule already set in `a` (query blocks of kTcQueries) and
@@ -61,6 +88,7 @@ __device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2* 
 // certificate.  slots = CTAs of the persistent grid.
 constexpr int kTcQueries = 256;  // queries per work item
 constexpr int kTcBN = 128;       // data records per B tile
+constexpr int kTcPoolExtra = 64; // pools of the tensor-core path hold ksel + 64 entries (see tc_append32)
 int knn_tc_slots(const Ctx& c);
 int launch_knn_tc_select(const Ctx& c, const float* X, const float* Xq, KnnArgs& a, float* mu_dev,
                          uint32_t* stats);

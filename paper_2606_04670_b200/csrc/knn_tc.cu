@@ -26,6 +26,10 @@
 
 #include "knn_common.cuh"
 
+#ifndef LIPFIT_TC_EXPERIMENT
+#define LIPFIT_TC_EXPERIMENT 0  // 1, 2: timing experiments with invalid results (never in a product build)
+#endif
+
 namespace lipfit {
 
 namespace {
@@ -34,9 +38,8 @@ constexpr int kTcThreads = 320;
 constexpr int kTcStages = 4;
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
-constexpr int kTcValsPerWarp = 32 * 33;           // padded [lane][column] scratch of the slow path
 constexpr size_t kTcSmemBytes = 1024 /*alignment slack*/ + 2 * kTcTileBytes + kTcStages * kTcTileBytes +
-                                8 * kTcValsPerWarp * sizeof(float) + 8 * (kMaxP + 1) * sizeof(int2);
+                                8 * (kMaxP + 1) * sizeof(int2);
 
 // byte offset of 16-byte chunk c (0..7) of row r inside a K-major SWIZZLE_128B tile of 128-byte rows
 __host__ __device__ __forceinline__ uint32_t sw128_offset(int r, int c) {
@@ -89,10 +92,10 @@ __device__ __forceinline__ void tc_ld32(uint32_t taddr, float (&v)[32]) {
           "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]),
           "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
         : "r"(taddr));
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
+__device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------------
 // Operand images
@@ -227,47 +230,57 @@ struct KnnTcArgs {
     KnnArgs k;                  // pools, schedule (query blocks of kTcQueries), N, Q, ksel, P
 };
 
-// Epilogue work on 32 keys of one query (this lane's row): v[c] is the key of datum kbase + c.
-__device__ __forceinline__ void tc_process(const KnnArgs& a, const float (&v)[32], int kbase, float& tau,
-                                           int& fill, int2* pool, float* scrv, int2* scr2, int lane) {
-    float m = v[0];
-#pragma unroll
-    for (int c = 1; c < 32; ++c) m = fminf(m, v[c]);
-    if (!__any_sync(0xffffffffu, m < tau)) return;  // the common case
-    unsigned mask = 0;
-#pragma unroll
-    for (int c = 0; c < 32; ++c) {
-        mask |= (v[c] < tau) ? (1u << c) : 0u;
-        scrv[lane * 33 + c] = v[c];
-    }
-    __syncwarp();
+// Epilogue slow path for 32 keys of one query (this lane's row): v[c] is the key of datum kbase + c.
+// Entered warp-uniformly when some lane of the warp has a key below its threshold.  Pools of the
+// tensor-core path have P = ksel + 64 entries and are compacted (warp-cooperatively) as soon as
+// fewer than 32 entries are free, so the 32 predicated appends below always fit: no loop, no
+// shared-memory staging.  Padding rows (index >= N) carry key 3e38 > the initial threshold 1e38.
+__device__ __forceinline__ void tc_append32(const KnnArgs& a, const float (&v)[32], int kbase, float& tau,
+                                            int& fill, int2* pool, int2* scr2, int lane) {
     const int P = a.P;
-    for (;;) {
-        while (mask != 0 && fill < P) {
-            const int c = __ffs(mask) - 1;
-            mask &= mask - 1;
-            const float val = scrv[lane * 33 + c];
-            const int idx = kbase + c;
-            if (val < tau && idx < a.N) {  // rows past N are padding
-                pool[fill] = make_int2(__float_as_int(val), idx);
-                ++fill;
-            }
-        }
-        unsigned fm = __ballot_sync(0xffffffffu, fill == P);
-        if (fm == 0) break;  // no pool is full => every lane has drained its mask
-        __syncwarp();        // orders the appends above before the cooperative reads below
+    unsigned fm = __ballot_sync(0xffffffffu, fill > P - 32);
+    if (fm) {
+        __syncwarp();  // orders earlier appends before the cooperative reads below
         while (fm) {
             const int src = __ffs(fm) - 1;
             fm &= fm - 1;
             int2* pq = pool + static_cast<ptrdiff_t>(src - lane) * P;  // consecutive lanes = consecutive slots
-            const float nt = knn_compact(pq, P, a.ksel, scr2, lane);
+            const int n = __shfl_sync(0xffffffffu, fill, src);
+            const float nt = knn_compact(pq, n, a.ksel, scr2, lane);
             if (lane == src) {
                 tau = nt;
                 fill = a.ksel;
             }
         }
     }
-    __syncwarp();
+#pragma unroll
+    for (int c = 0; c < 32; ++c) {
+        const float val = v[c];
+        // predicated store + predicated increment: 32 divergent branches here cost far more than the work
+        int inc;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "setp.lt.f32 p, %1, %2;\n\t"
+            "@p st.global.v2.b32 [%3], {%4, %5};\n\t"
+            "selp.s32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(inc)
+            : "f"(val), "f"(tau), "l"(pool + fill), "r"(__float_as_int(val)), "r"(kbase + c)
+            : "memory");
+        fill += inc;
+    }
+}
+
+// min of 32 values as a depth-4 tree of 3-input minima (FMNMX3)
+__device__ __forceinline__ float tc_min32(const float (&v)[32]) {
+    float t[11];
+#pragma unroll
+    for (int i = 0; i < 10; ++i) t[i] = fminf(fminf(v[3 * i], v[3 * i + 1]), v[3 * i + 2]);
+    t[10] = fminf(v[30], v[31]);
+    const float u0 = fminf(fminf(t[0], t[1]), t[2]), u1 = fminf(fminf(t[3], t[4]), t[5]);
+    const float u2 = fminf(fminf(t[6], t[7]), t[8]), u3 = fminf(t[9], t[10]);
+    return fminf(fminf(u0, u1), fminf(u2, u3));
 }
 
 __global__ void __launch_bounds__(kTcThreads, 1)
@@ -281,8 +294,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
     unsigned char* base = smem_raw + ((1024u - (raw & 1023u)) & 1023u);
     unsigned char* sA = base;                                // 2 tiles
     unsigned char* sB = sA + 2 * kTcTileBytes;               // kTcStages tiles
-    float* sV = reinterpret_cast<float*>(sB + kTcStages * kTcTileBytes);        // 8 x [32][33]
-    int2* sC = reinterpret_cast<int2*>(sV + 8 * kTcValsPerWarp);                // 8 x [kMaxP + 1]
+    int2* sC = reinterpret_cast<int2*>(sB + kTcStages * kTcTileBytes);  // 8 x [kMaxP + 1] compaction scratch
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const KnnArgs& a = g.k;
@@ -384,14 +396,13 @@ knn_tc_select_kernel(const KnnTcArgs g) {
     } else {
         // ================= epilogue warps: h = query half, quad = TMEM lane quadrant =================
         const int h = warp >> 2, quad = warp & 3;
-        float* scrv = sV + warp * kTcValsPerWarp;
         int2* scr2 = sC + warp * (kMaxP + 1);
         uint32_t gB = 0;
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
             const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
-            float tau = qslot < a.Q ? __int_as_float(0x7f800000) : __int_as_float(0xff800000);
+            float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);  // real keys are far below 1e38
             int fill = 0;
             const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
             int2* pool = a.pool + slot * a.P;
@@ -399,16 +410,33 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 const uint32_t b = gB & 1u, ua = gB >> 1;
                 mbar_wait(&acc_full[h][b], ua & 1u);
                 tc_fence_after();
-#pragma unroll 1
+                const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
+#pragma unroll 1  // ONE copy of the block code: the kernel must stay small enough for the instruction cache
                 for (int cb = 0; cb < kTcBN / 32; ++cb) {
                     float v[32];
-                    tc_ld32(tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN + cb * 32, v);
-                    tc_process(a, v, t * kTcBN + cb * 32, tau, fill, pool, scrv, scr2, lane);
+                    tc_ld32(trow + cb * 32, v);
+                    tc_ld_wait();
+                    if (cb == kTcBN / 32 - 1) {  // last block is in registers: hand the TMEM stage back
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+                    }
+#if LIPFIT_TC_EXPERIMENT == 1  // timing experiment: accumulators are read and dropped
+                    if (v[0] == 12345.f && v[31] == 1.f) tau = 0.f;
+#elif LIPFIT_TC_EXPERIMENT == 2  // timing experiment: fast path only
+                    const float m = tc_min32(v);
+                    if (__any_sync(0xffffffffu, m < -1e30f)) tau = 0.f;
+#else
+                    const float m = tc_min32(v);
+                    if (__any_sync(0xffffffffu, m < tau))  // rare after the first tiles
+                        tc_append32(a, v, t * kTcBN + cb * 32, tau, fill, pool, scr2, lane);
+#endif
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
             }
+#if LIPFIT_TC_EXPERIMENT
+            fill = 0;
+            tau = __int_as_float(0x7f800000);
+#endif
             a.fill[slot] = fill;
             a.tau[slot] = tau;
         }
