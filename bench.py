@@ -45,7 +45,8 @@ UNIT = "Gpairs/s"
 LANE_OPS = {1: 9, 2: 18, 3: 21, 4: 17, "4direct": 33, "5s": 18, "5s_survey": 26, "5b": 31}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md); null where no capture of this kernel version exists.
-NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2>": 27_231_232}
+NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2>": 27_238_400, "knn_select<dot>": 5_975_622_000,
+                     "smooth_pairs<L2,U0,C5>": 8_126_976}
 FP32_LANES_PER_SM = 128
 
 
@@ -256,17 +257,34 @@ def bench_bounds(torch, L, wl, steps, warmup, l2buf, dev, lane_ops, do_e2e=True)
     return res
 
 
-def bench_knn(torch, L, wl, steps, warmup, l2buf, dev):
+def bench_knn(torch, L, wl, steps, warmup, l2buf, dev, tensor_cores=True):
     t = lambda a: torch.from_numpy(a).to(dev)
     X, Xq = t(wl.X), t(wl.Xq)
     fn = lambda: L.lipfit_knn(X, Xq, wl.k, None, 0, wl.norm, wl.weights)
-    ms = _time_steps(torch, fn, steps, warmup, l2buf)
-    kms, _ = _kernel_ms(L, 1, fn, 1)
+    L.knn_set_tensor_cores(tensor_cores)
+    try:
+        variant = L.knn_variant(wl.d, 0, wl.norm)
+        ms = _time_steps(torch, fn, steps, warmup, l2buf)
+        kms, _ = _kernel_ms(L, 1, fn, 1)
+        out = fn()
+        torch.cuda.synchronize()
+        res = {"fallbacks": L.knn_fallbacks(), "key_error_over_bound": L.knn_key_error_ratio()}
+    finally:
+        L.knn_set_tensor_cores(True)
     pairs = wl.N * wl.Q
-    out = fn()
-    torch.cuda.synchronize()
-    return {"ms_per_step": float(np.mean(ms)), "pairs": pairs, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
-            "kernel_ms": kms, "lane_ops": LANE_OPS[4], "outputs": out, "fallbacks": L.knn_fallbacks()}
+    res.update({"ms_per_step": float(np.mean(ms)), "pairs": pairs, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+                "kernel_ms": kms, "kernel": variant, "outputs": out})
+    return res
+
+
+def _roofline_tensor(pairs, k_dim, kernel_ms, peaks):
+    """bf16 GEMM roofline of the tensor-core selection: 2 * K flop per pair (K = 64 operand columns)."""
+    peak = peaks.get("bf16_tflops", 1590.0)
+    ach = pairs * 2.0 * k_dim / (kernel_ms * 1e-3) / 1e12 if kernel_ms else None
+    return {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+            "frac": (ach / peak) if ach else None, "traffic": NCU_TRAFFIC_BYTES.get("knn_tc_select"),
+            "flop_per_pair": 2 * k_dim, "kernel_ms": kernel_ms,
+            "peak_how": "MEASURED_PEAKS.json bf16_tflops (cuBLAS bf16, burst; the kernel is timed alone)"}
 
 
 def bench_smooth(torch, L, wl, l2buf, dev):
@@ -392,14 +410,22 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "sample": sample}
             out["parity"] = parity_bounds(wl, r["outputs"], sel, ref)
     elif c == 4:
-        r = bench_knn(torch, L, wl, steps, 1, l2buf, dev)
-        out.update({k: r[k] for k in ("ms_per_step", "value", "kernel_ms")})
+        r = bench_knn(torch, L, wl, steps, 1, l2buf, dev, tensor_cores=True)
+        out.update({k: r[k] for k in ("ms_per_step", "value", "kernel_ms", "kernel")})
         out["unit"] = UNIT
-        out["kernel"] = "knn_select<dot,DP16> (cross-term key, FFMA2) + fp64 re-rank + certificate"
+        out["step"] = "lipfit_knn = operand images + tensor-core selection + fp64 re-rank / certificate + exact fallback"
         out["exact_fallback_queries"] = r["fallbacks"]
-        out["roofline"] = _roofline(r["pairs"], LANE_OPS[4], r["kernel_ms"], sms, peaks)
-        out["roofline"]["frac_direct_difference_form_33ops"] = (
-            r["pairs"] * LANE_OPS["4direct"] / (r["kernel_ms"] * 1e-3) / 1e12 / out["roofline"]["peak"])
+        out["key_error_over_bound"] = r["key_error_over_bound"]
+        out["roofline"] = _roofline_tensor(r["pairs"], 64, r["kernel_ms"], peaks)
+        # the CUDA-core selection kernel (tensor cores switched off), same outputs
+        rc = bench_knn(torch, L, wl, max(1, min(steps, 2)), 1, l2buf, dev, tensor_cores=False)
+        out["cuda_core_selection"] = {k: rc[k] for k in ("ms_per_step", "value", "kernel_ms", "kernel")}
+        out["cuda_core_selection"]["roofline"] = _roofline(rc["pairs"], LANE_OPS[4], rc["kernel_ms"], sms, peaks)
+        out["cuda_core_selection"]["roofline"]["frac_direct_difference_form_33ops"] = (
+            rc["pairs"] * LANE_OPS["4direct"] / (rc["kernel_ms"] * 1e-3) / 1e12
+            / out["cuda_core_selection"]["roofline"]["peak"])
+        out["cuda_core_selection"]["same_outputs"] = bool(
+            torch.equal(r["outputs"][0], rc["outputs"][0]) and torch.equal(r["outputs"][1], rc["outputs"][1]))
         if not args.no_cpu:
             sel = oracle_subset(wl.Q, 64)
             t0 = time.perf_counter()
