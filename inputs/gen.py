@@ -138,3 +138,13 @@ def random_problem(seed: int, N: int, Q: int, d: int, spread: float = 1.0):
     Xq = (spread * rng.standard_normal((Q, d))).astype(np.float32)
     y = rng.standard_normal(N).astype(np.float32)
     return np.ascontiguousarray(X), np.ascontiguousarray(y), np.ascontiguousarray(Xq)
+
+
+def sample_pairs(seed: int, N: int, S: int):
+    """S random index pairs (i != k) for the inter-point distance sample of local Lipschitz
+    interpolation: the random numbers the method draws, passed in as inputs."""
+    rng = np.random.default_rng(seed)
+    i = rng.integers(0, N, S, dtype=np.int64)
+    k = (i + 1 + rng.integers(0, max(N - 1, 1), S, dtype=np.int64)) % max(N, 1)
+    return i.astype(np.int32), k.astype(np.int32)
+

@@ -31,6 +31,11 @@ def load():
         lib.oracle_max_violation.argtypes = [P, P, i64, i32, f64, P, i32, P, P, P]
         lib.oracle_smooth_rows.argtypes = [P, P, i64, i32, f64, P, i32, P, f64, P, P, i64, P, P]
         lib.oracle_lipschitz_constant.argtypes = [P, P, i64, i32, P, i32, P, P]
+        lib.oracle_distance_quantiles.argtypes = [P, i64, i32, i32, P, P, P, i64, i32, P]
+        lib.oracle_local_lipschitz.argtypes = [P, P, i64, i32, i32, P, P, i32, P]
+        lib.oracle_values_local.argtypes = [P, P, i64, i32, P, i64, i32, P, P, i32, P, P, P, P]
+        for fn in (lib.oracle_distance_quantiles, lib.oracle_local_lipschitz, lib.oracle_values_local):
+            fn.restype = C.c_int
         for fn in (lib.oracle_bounds, lib.oracle_knn, lib.oracle_smooth_objective,
                    lib.oracle_max_violation, lib.oracle_num_threads, lib.oracle_smooth_rows,
                    lib.oracle_lipschitz_constant):
@@ -144,6 +149,51 @@ def lipschitz_constant(X, y, mask=None, norm=2, weights=None) -> float:
     if rc:
         raise ValueError(f"oracle_lipschitz_constant rc={rc}")
     return float(out.value)
+
+
+def distance_quantiles(X, pair_i, pair_k, J, norm=2, weights=None):
+    """J spline knots (float64): nearest-rank quantiles of the sampled inter-point distances."""
+    X = _f32(X, 2)
+    N, d = X.shape
+    _, w = _params(d, None, weights)
+    pi = np.ascontiguousarray(pair_i, dtype=np.int32)
+    pk = np.ascontiguousarray(pair_k, dtype=np.int32)
+    knots = np.empty(J, dtype=np.float64)
+    rc = load().oracle_distance_quantiles(_ptr(X), N, d, int(norm), _ptr(w), _ptr(pi), _ptr(pk), len(pi),
+                                          int(J), _ptr(knots))
+    if rc:
+        raise ValueError(f"oracle_distance_quantiles rc={rc}")
+    return knots
+
+
+def local_lipschitz(X, y, knots, norm=2, weights=None):
+    """table [N, J] (float64) of the per-datum step functions M_k."""
+    X, y = _f32(X, 2), _f32(y, 1)
+    N, d = X.shape
+    _, w = _params(d, None, weights)
+    knots = np.ascontiguousarray(knots, dtype=np.float64)
+    table = np.empty((N, len(knots)), dtype=np.float64)
+    rc = load().oracle_local_lipschitz(_ptr(X), _ptr(y), N, d, int(norm), _ptr(w), _ptr(knots), len(knots),
+                                       _ptr(table))
+    if rc:
+        raise ValueError(f"oracle_local_lipschitz rc={rc}")
+    return table
+
+
+def values_local(X, y, Xq, knots, table, norm=2, weights=None):
+    """(upper, lower, g) with M replaced by M_k(D(x, x^k))."""
+    X, y, Xq = _f32(X, 2), _f32(y, 1), _f32(Xq, 2)
+    N, d = X.shape
+    Q = Xq.shape[0]
+    _, w = _params(d, None, weights)
+    knots = np.ascontiguousarray(knots, dtype=np.float64)
+    table = np.ascontiguousarray(table, dtype=np.float64).reshape(N, len(knots))
+    U, L, G = (np.empty(Q, dtype=np.float64) for _ in range(3))
+    rc = load().oracle_values_local(_ptr(X), _ptr(y), N, d, _ptr(Xq), Q, int(norm), _ptr(w), _ptr(knots),
+                                    len(knots), _ptr(table), _ptr(U), _ptr(L), _ptr(G))
+    if rc:
+        raise ValueError(f"oracle_values_local rc={rc}")
+    return U, L, G
 
 
 def smooth(X, y, M, mask=None, norm=2, weights=None, p=1.0, max_iter=10000, gtol=1e-12):

@@ -281,3 +281,122 @@ int oracle_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t
     return 0;
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * Local Lipschitz interpolation, PAPER.md:169-183 (section 4.3), readings R20-R23 of DESIGN.md.
+ * Radial (symmetric, weighted) distance D(a,b) = ||w (a - b)||_p: "an approximation to M(x) based on
+ * radial distances from data x^k".
+ * ------------------------------------------------------------------------------------------- */
+static double radial_distance(const float* a, const float* b, int32_t d, int32_t norm, const float* w) {
+    double Du, Dl;
+    one_sided_distances(a, b, d, NULL, norm, w, &Du, &Dl);
+    return Du;
+}
+
+static int cmp_double(const void* a, const void* b) {
+    double x = *(const double*)a, y = *(const double*)b;
+    return (x > y) - (x < y);
+}
+
+/* Spline knots: "quantiles of the distribution of distances from a random point x_k, approximated from
+ * a sample of interpoint distances".  The sample is the list of index pairs
+ * (pair_i[s], pair_k[s]); knot j (1-based) is the nearest-rank j/J quantile of the S sampled distances,
+ * i.e. the sorted sample at index ceil(j S / J) - 1 (R20). */
+int oracle_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm, const float* weights,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int32_t J,
+                              double* knots) {
+    int rc = check_common(X, N, d, NULL, norm, weights);
+    if (rc) return rc;
+    if (!pair_i || !pair_k || !knots) return -1;
+    if (S < 1 || J < 1 || J > S) return -3;
+    double* ds = (double*)malloc(sizeof(double) * (size_t)S);
+    if (!ds) return -6;
+    for (int64_t s = 0; s < S; ++s) {
+        if (pair_i[s] < 0 || pair_i[s] >= N || pair_k[s] < 0 || pair_k[s] >= N) {
+            free(ds);
+            return -3;
+        }
+        ds[s] = radial_distance(X + (int64_t)pair_i[s] * d, X + (int64_t)pair_k[s] * d, d, norm, weights);
+    }
+    qsort(ds, (size_t)S, sizeof(double), cmp_double);
+    for (int32_t j = 1; j <= J; ++j) {
+        int64_t idx = ((int64_t)j * S + J - 1) / J - 1; /* ceil(j S / J) - 1 */
+        knots[j - 1] = ds[idx];
+    }
+    free(ds);
+    return 0;
+}
+
+/* Per-datum non-decreasing step function M_k: table[k*J + j] is the value of M_k on
+ * (t_{j-1}, t_j]:
+ *     max( |y_k - y_(1)| / d_(1),  max_{i != k, D(x^k,x^i) <= t_j} |y_k - y_i| / D(x^k,x^i) ),
+ * where d_(1) is the distance from x^k to its closest neighbour ("the first segment ... has the value
+ * |y_k - y_(1)|/d_(1) ... the smallest value consistent with the data"; several closest neighbours at
+ * the same distance: the largest of their ratios) and the LAST knot is treated as +infinity, so the
+ * last column is the maximum over all data (R21).  A different value at zero distance gives +infinity;
+ * an equal value at zero distance (a duplicate) is ignored. */
+int oracle_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                           const float* weights, const double* knots, int32_t J, double* table) {
+    int rc = check_common(X, N, d, NULL, norm, weights);
+    if (rc) return rc;
+    if (!y || !knots || !table) return -1;
+    if (J < 1) return -3;
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < N; ++k) {
+        double* M = table + k * J;
+        for (int32_t j = 0; j < J; ++j) M[j] = 0.0;
+        double dmin = INFINITY, rnn = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            if (i == k) continue;
+            double D = radial_distance(X + k * d, X + i * d, d, norm, weights);
+            double dy = fabs((double)y[k] - (double)y[i]);
+            if (D == 0.0 && dy == 0.0) continue; /* duplicate datum */
+            double ratio = (D > 0.0) ? dy / D : INFINITY;
+            if (D < dmin) {
+                dmin = D;
+                rnn = ratio;
+            } else if (D == dmin && ratio > rnn) {
+                rnn = ratio;
+            }
+            for (int32_t j = 0; j < J; ++j)
+                if ((j == J - 1 || D <= knots[j]) && ratio > M[j]) M[j] = ratio;
+        }
+        for (int32_t j = 0; j < J; ++j)
+            if (rnn > M[j]) M[j] = rnn;
+    }
+    return 0;
+}
+
+/* Eq.(2),(3) "with global constant M replaced with M_k(||x - x^k||)":
+ *   upper = min_k (y_k + M_k(D) D),  lower = max_k (y_k - M_k(D) D),  D = D(x, x^k),
+ * M_k(D) = table[k*J + b], b the first knot index with D <= t_b (the last one if none). */
+int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                        int32_t norm, const float* weights, const double* knots, int32_t J,
+                        const double* table, double* upper, double* lower, double* g) {
+    int rc = check_common(X, N, d, NULL, norm, weights);
+    if (rc) return rc;
+    if (!y || !knots || !table || (Q > 0 && !Xq)) return -1;
+    if (J < 1 || Q < 0) return -3;
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < Q; ++q) {
+        double U = INFINITY, L = -INFINITY;
+        for (int64_t k = 0; k < N; ++k) {
+            double D = radial_distance(Xq + q * d, X + k * d, d, norm, weights);
+            int32_t b = J - 1;
+            for (int32_t j = 0; j < J - 1; ++j)
+                if (D <= knots[j]) {
+                    b = j;
+                    break;
+                }
+            double Mk = table[k * J + b];
+            double MD = (D == 0.0) ? 0.0 : Mk * D; /* M_k may be +inf at a duplicate: inf * 0 := 0 */
+            double hi = (double)y[k] + MD, lo = (double)y[k] - MD;
+            if (hi < U) U = hi;
+            if (lo > L) L = lo;
+        }
+        if (upper) upper[q] = U;
+        if (lower) lower[q] = L;
+        if (g) g[q] = 0.5 * (U + L);
+    }
+    return 0;
+}
+

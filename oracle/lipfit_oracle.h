@@ -77,6 +77,19 @@ int oracle_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t
                               const int32_t* mono_mask, int32_t norm, const float* weights,
                               double* out);
 
+/* ---- Local Lipschitz interpolation, PAPER.md:169-183 (radial symmetric distance) ---------------- */
+/* knots[j-1] = nearest-rank j/J quantile of the S sampled inter-point distances D(x^{pair_i}, x^{pair_k}). */
+int oracle_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm, const float* weights,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int32_t J,
+                              double* knots);
+/* table[k*J+j] = value of the step function M_k on (t_{j-1}, t_j] (last knot = +inf). */
+int oracle_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                           const float* weights, const double* knots, int32_t J, double* table);
+/* Eq.(2),(3) with M -> M_k(D(x, x^k)). */
+int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                        int32_t norm, const float* weights, const double* knots, int32_t J,
+                        const double* table, double* upper, double* lower, double* g);
+
 int oracle_num_threads(void);
 
 #ifdef __cplusplus
