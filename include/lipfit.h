@@ -45,6 +45,7 @@ extern "C" {
 
 #define LIPFIT_MAX_DIM 32
 #define LIPFIT_MAX_K 128
+#define LIPFIT_LOCAL_KNOTS 16 /* knots of the local Lipschitz step functions M_k */
 
 enum lipfit_norm { LIPFIT_L1 = 1, LIPFIT_L2 = 2, LIPFIT_LINF = 3 };
 
@@ -147,6 +148,31 @@ int lipfit_lipschitz_constant_host(const float* X, const float* y, int64_t N, in
                                    const int32_t* mono_mask, int32_t norm, const float* weights,
                                    float* L /* host */, void* cuda_stream);
 
+/* ---- Local Lipschitz interpolation, PAPER.md:169-183 (section 4.3) --------------------------
+ * Radial symmetric weighted distance D(a,b) = ||w (a - b)||_p (no monotonicity: the paper gives no
+ * formula for combining the two, R23).  J = LIPFIT_LOCAL_KNOTS for the last two calls.
+ *
+ * lipfit_distance_quantiles: spline knots = nearest-rank j/J quantiles (j = 1..J) of the S sampled
+ *   inter-point distances D(x^{pair_i[s]}, x^{pair_k[s]}) ("quantiles of the distribution
+ *   of distances ... approximated from a sample of interpoint distances"; the sample is an INPUT).
+ *   pair_i, pair_k: device int32[S]; knots: HOST float[J], 1 <= J <= 1024, J <= S; synchronises.
+ * lipfit_local_lipschitz: per-datum non-decreasing step functions
+ *   table[k*J+j] = max(|y_k - y_(1)|/d_(1), max_{i != k, D(x^k,x^i) <= knots[j]} |y_k - y_i|/D),
+ *   last knot treated as +infinity; +inf where a different value sits at zero distance.
+ *   knots: HOST float[J]; table: device float[N*J]; asynchronous.  An all-pairs pass (N^2 pairs).
+ * lipfit_values_local: Eq.(2),(3) with M replaced by M_k(D(x, x^k)) = table[k][first j with
+ *   D <= knots[j], else J-1]; upper/lower/g as in lipfit_bounds. */
+int lipfit_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm, const float* weights,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int32_t J,
+                              float* knots /* host[J] */, void* cuda_stream);
+int lipfit_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                           const float* weights, const float* knots /* host[J] */, int32_t J,
+                           float* table /* device[N*J] */, void* cuda_stream);
+int lipfit_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                        int32_t norm, const float* weights, const float* knots /* host[J] */, int32_t J,
+                        const float* table /* device[N*J] */, float* upper, float* lower, float* g,
+                        void* cuda_stream);
+
 /* ---- Host optimiser on its own (step a5), exposed so that it can be tested without a GPU ----
  * Minimises a caller-supplied function by the same LBFGS lipfit_smooth uses (history `history`,
  * strong-Wolfe line search).  x: host double[n], start point on entry and
@@ -165,7 +191,7 @@ const char* lipfit_version(void);
 int64_t lipfit_launch_count(void);
 /* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
  * resets the accumulators and makes every later launch of the three dominant kernels
- * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs) bracketed by CUDA events on
+ * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation) bracketed by CUDA events on
  * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
  * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);

@@ -7,5 +7,6 @@ from .binding import (LIPFIT_L1, LIPFIT_L2, LIPFIT_LINF, LIPFIT_MAX_DIM, LIPFIT_
                       LipfitError, bounds_variant, get_timing, knn_fallbacks, knn_key_error_ratio, knn_set_tensor_cores, knn_variant, launch_count, set_timing, lipfit_bounds,
                       lipfit_bounds_host, lipfit_knn, lipfit_knn_host, lipfit_lbfgs,
                       lipfit_lipschitz_constant, lipfit_lipschitz_constant_host,
+                      lipfit_distance_quantiles, lipfit_local_lipschitz, lipfit_values_local, LIPFIT_LOCAL_KNOTS,
                       lipfit_smooth, lipfit_smooth_host, lipfit_smooth_objective, load,
                       status_string, version)

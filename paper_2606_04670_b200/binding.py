@@ -24,7 +24,9 @@ EXPORTS = [
     "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
     "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
+    "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local",
 ]
+LIPFIT_LOCAL_KNOTS = 16
 
 
 class LipfitError(RuntimeError):
@@ -64,6 +66,9 @@ def load():
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
     lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
     lib.lipfit_lbfgs.argtypes = [i64, P, EVAL_FN, P, i32, f64, i32, P]
+    lib.lipfit_distance_quantiles.argtypes = [P, i64, i32, i32, P, P, P, i64, i32, P, P]
+    lib.lipfit_local_lipschitz.argtypes = [P, P, i64, i32, i32, P, P, i32, P, P]
+    lib.lipfit_values_local.argtypes = [P, P, i64, i32, P, i64, i32, P, P, i32, P, P, P, P, P]
     lib.lipfit_lipschitz_constant.argtypes = [P, P, i64, i32, P, i32, P, P, P]
     lib.lipfit_lipschitz_constant_host.argtypes = lib.lipfit_lipschitz_constant.argtypes
     lib.lipfit_bounds_variant.argtypes = [i32, P, i32, C.c_char_p, i32]
@@ -257,6 +262,53 @@ def lipfit_lipschitz_constant_host(X, y, mono_mask=None, norm: int = LIPFIT_L2, 
                                                _np_ptr(w), _np_ptr(out), None)
     _check(rc, "lipfit_lipschitz_constant_host")
     return float(out[0])
+
+
+def lipfit_distance_quantiles(X, pair_i, pair_k, J: int = LIPFIT_LOCAL_KNOTS, norm: int = LIPFIT_L2,
+                              weights=None, stream=None):
+    """Knots (numpy float32 [J]) = nearest-rank quantiles of the sampled inter-point distances."""
+    torch = _torch()
+    X = _dev_f32(X, 2, "X")
+    N, d = X.shape
+    _, w = _host_params(d, None, weights)
+    pi = pair_i.to(device=X.device, dtype=torch.int32).contiguous()
+    pk = pair_k.to(device=X.device, dtype=torch.int32).contiguous()
+    knots = np.zeros(J, dtype=np.float32)
+    rc = load().lipfit_distance_quantiles(X.data_ptr(), N, d, int(norm), _np_ptr(w), pi.data_ptr(),
+                                          pk.data_ptr(), pi.numel(), int(J), _np_ptr(knots), _stream(stream))
+    _check(rc, "lipfit_distance_quantiles")
+    return knots
+
+
+def lipfit_local_lipschitz(X, y, knots, norm: int = LIPFIT_L2, weights=None, stream=None):
+    """Step tables M_k as a float32 CUDA tensor [N, J]."""
+    torch = _torch()
+    X, y = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y")
+    N, d = X.shape
+    _, w = _host_params(d, None, weights)
+    kn = np.ascontiguousarray(knots, dtype=np.float32)
+    table = torch.empty((N, len(kn)), dtype=torch.float32, device=X.device)
+    rc = load().lipfit_local_lipschitz(X.data_ptr(), y.data_ptr(), N, d, int(norm), _np_ptr(w), _np_ptr(kn),
+                                       len(kn), table.data_ptr(), _stream(stream))
+    _check(rc, "lipfit_local_lipschitz")
+    return table
+
+
+def lipfit_values_local(X, y, Xq, knots, table, norm: int = LIPFIT_L2, weights=None, stream=None):
+    """(upper, lower, g) with M replaced by M_k(D(x, x^k))."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    _, w = _host_params(d, None, weights)
+    kn = np.ascontiguousarray(knots, dtype=np.float32)
+    table = _dev_f32(table, 2, "table")
+    outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    rc = load().lipfit_values_local(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, int(norm), _np_ptr(w),
+                                    _np_ptr(kn), len(kn), table.data_ptr(), outs[0].data_ptr(),
+                                    outs[1].data_ptr(), outs[2].data_ptr(), _stream(stream))
+    _check(rc, "lipfit_values_local")
+    return tuple(outs)
 
 
 def lipfit_smooth(X, y_inout, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,

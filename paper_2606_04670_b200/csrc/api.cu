@@ -190,4 +190,71 @@ int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64
     return LIPFIT_OK;
 }
 
+// ---- local Lipschitz interpolation ----
+int lipfit_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm, const float* weights,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int32_t J, float* knots,
+                              void* cuda_stream) {
+    int rc = check_sizes(N, d, 0);
+    if (rc) return rc;
+    if (check_norm(norm)) return LIPFIT_E_PARAM;
+    if (S < 1 || S > 0x7fffffffLL || J < 1 || J > 1024 || J > S) return LIPFIT_E_SIZE;
+    Xform xf;
+    if ((rc = make_xform(d, nullptr, weights, true, false, &xf))) return rc;
+    if (!X || !pair_i || !pair_k || !knots) return LIPFIT_E_NULL;
+    Ctx c;
+    if ((rc = make_ctx(cuda_stream, &c))) return rc;
+    Workspace wk;
+    if ((rc = wk.alloc(sizeof(float) * 1024 + sizeof(int), c.stream))) return rc;
+    int* bad = reinterpret_cast<int*>(wk.as<float>() + 1024);
+    LIPFIT_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), c.stream));
+    if ((rc = launch_distance_quantiles(c, X, N, xf, norm, pair_i, pair_k, S, J, wk.as<float>(), bad))) return rc;
+    int bad_h = 0;
+    LIPFIT_CUDA(cudaMemcpyAsync(knots, wk.p, sizeof(float) * J, cudaMemcpyDeviceToHost, c.stream));
+    LIPFIT_CUDA(cudaMemcpyAsync(&bad_h, bad, sizeof(int), cudaMemcpyDeviceToHost, c.stream));
+    LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+    return bad_h ? LIPFIT_E_SIZE : LIPFIT_OK;  // an index pair outside [0, N)
+}
+
+static int check_knots(const float* knots, int32_t J) {
+    if (!knots) return LIPFIT_E_NULL;
+    if (J != LIPFIT_LOCAL_KNOTS) return LIPFIT_E_SIZE;
+    for (int j = 0; j < J; ++j) {
+        if (!(knots[j] >= 0.f) || (j > 0 && knots[j] < knots[j - 1])) return LIPFIT_E_PARAM;  // also rejects NaN
+    }
+    return LIPFIT_OK;
+}
+
+int lipfit_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                           const float* weights, const float* knots, int32_t J, float* table,
+                           void* cuda_stream) {
+    int rc = check_sizes(N, d, 0);
+    if (rc) return rc;
+    if (check_norm(norm)) return LIPFIT_E_PARAM;
+    if ((rc = check_knots(knots, J))) return rc;
+    Xform xf;
+    if ((rc = make_xform(d, nullptr, weights, true, false, &xf))) return rc;
+    if (!X || !y || !table) return LIPFIT_E_NULL;
+    if (N * static_cast<int64_t>(J) > 0x7fffffffLL) return LIPFIT_E_SIZE;
+    Ctx c;
+    if ((rc = make_ctx(cuda_stream, &c))) return rc;
+    return launch_local_lipschitz(c, X, y, N, xf, norm, knots, table);
+}
+
+int lipfit_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                        int32_t norm, const float* weights, const float* knots, int32_t J, const float* table,
+                        float* upper, float* lower, float* g, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm)) return LIPFIT_E_PARAM;
+    if ((rc = check_knots(knots, J))) return rc;
+    Xform xf;
+    if ((rc = make_xform(d, nullptr, weights, true, false, &xf))) return rc;
+    if (!X || !y || !table) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    if ((rc = make_ctx(cuda_stream, &c))) return rc;
+    return launch_values_local(c, X, y, N, Xq, Q, xf, norm, knots, table, upper, lower, g);
+}
+
 }  // extern "C"

@@ -50,6 +50,15 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
 // NEXT-3: smallest consistent Lipschitz constant; base = packed records with plain coordinates.
 int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, const float* y, int64_t N,
                               const Xform& xf, int norm, float* L_dev);
+// NEXT-1: local Lipschitz interpolation (local.cu).  knots_host: host float[LIPFIT_LOCAL_KNOTS].
+int launch_distance_quantiles(const Ctx& c, const float* X, int64_t N, const Xform& xf, int norm,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int J, float* knots_dev,
+                              int* bad_dev);
+int launch_local_lipschitz(const Ctx& c, const float* X, const float* y, int64_t N, const Xform& xf, int norm,
+                           const float* knots_host, float* table);
+int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
+                        const Xform& xf, int norm, const float* knots_host, const float* table, float* upper,
+                        float* lower, float* g);
 // xf with every coordinate factor multiplied by s
 Xform scale_xform(const Xform& xf, float s);
 

@@ -1,0 +1,445 @@
+// local.cu -- NEXT-1: local Lipschitz interpolation, PAPER.md:169-183 (section 4.3).
+//   (1) knots t_1..t_J: nearest-rank quantiles of a sample of inter-point distances;
+//   (2) per-datum non-decreasing step functions M_k: table[k][j] = max(|y_k - y_(1)|/d_(1),
+//       max_{i != k, D(x^k,x^i) <= t_j} |y_k - y_i| / D), last knot = +inf -- an all-pairs pass, J running
+//       maxima per row in registers, nothing of size N x N stored;
+//   (3) evaluation: Eq.(2),(3) with M replaced by M_k(D(x, x^k)): the fused bounds pass
+//       with the table row riding in the packed record and a compare/select chain for the knot lookup
+//       (the paper's torch.searchsorted).
+// Radial, symmetric weighted distance D(a,b) = ||w (a - b)||_p; J is fixed at LIPFIT_LOCAL_KNOTS = 16.
+#include <cub/device/device_radix_sort.cuh>
+
+#include "kernels.h"
+
+namespace lipfit {
+
+constexpr int kJ = LIPFIT_LOCAL_KNOTS;
+constexpr int kLocThreads = 128;
+
+struct Knots {
+    float t[kJ];
+};
+
+// exact-ish distance from the accumulated quantity: IEEE square root (bin decisions compare D with knots)
+template <int NORM>
+__device__ __forceinline__ float local_finish(float acc) {
+    return NORM == 2 ? __fsqrt_rn(acc) : acc;
+}
+
+template <int RF>
+__device__ __forceinline__ void local_load_record(const float* s, float* x) {
+#pragma unroll
+    for (int c = 0; c < RF / 4; ++c) {
+        float4 v = reinterpret_cast<const float4*>(s)[c];
+        x[4 * c + 0] = v.x;
+        x[4 * c + 1] = v.y;
+        x[4 * c + 2] = v.z;
+        x[4 * c + 3] = v.w;
+    }
+}
+
+template <int RF>
+__host__ __device__ constexpr int local_tile_records() {
+    return RF <= 8 ? 512 : (RF <= 20 ? 256 : (RF <= 40 ? 128 : 64));
+}
+
+// ---------------------------------------------------------------------------------------------
+// (1) knots
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+local_pair_dist_kernel(const float* __restrict__ X, int N, Xform xf, int norm, const int32_t* __restrict__ pi,
+                       const int32_t* __restrict__ pk, int S, float* __restrict__ out, int* __restrict__ bad) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    const int i = pi[s], k = pk[s];
+    if (i < 0 || i >= N || k < 0 || k >= N) {
+        *bad = 1;
+        out[s] = 0.f;
+        return;
+    }
+    const float* a = X + static_cast<size_t>(i) * xf.d;
+    const float* b = X + static_cast<size_t>(k) * xf.d;
+    float acc = 0.f;
+    for (int j = 0; j < xf.d; ++j) {
+        const int o = xf.perm[j];
+        const float c = fabsf(xf.sw[j] * a[o] - xf.sw[j] * b[o]);
+        if (norm == 1) acc += c;
+        else if (norm == 2) acc = fmaf(c, c, acc);
+        else acc = fmaxf(acc, c);
+    }
+    out[s] = norm == 2 ? __fsqrt_rn(acc) : acc;
+}
+
+__global__ void local_pick_kernel(const float* __restrict__ sorted, long long S, int J, float* __restrict__ knots) {
+    int j = threadIdx.x + 1;
+    if (j > J) return;
+    const long long idx = (static_cast<long long>(j) * S + J - 1) / J - 1;  // ceil(j S / J) - 1
+    knots[j - 1] = sorted[idx];
+}
+
+// ---------------------------------------------------------------------------------------------
+// (2) step tables
+// ---------------------------------------------------------------------------------------------
+struct TableArgs {
+    const float* rec;          // [N][RF]: x' (DP), y at slot DP
+    uint32_t* tab;             // [N][kJ] bits of the running maxima (non-negative floats)
+    unsigned long long* nn;    // [N] (bits of d_(1)) << 32 | ~(bits of its ratio): atomicMin = nearest, then largest ratio
+    int N, nrb, nch, chunk;
+};
+
+template <int NORM, int DP, int R>
+__global__ void __launch_bounds__(kLocThreads, 2)
+local_table_kernel(const TableArgs a, const Knots kn) {
+    constexpr int RF = DP + 4;
+    constexpr int TILE = local_tile_records<RF>();
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+    const float inf = __int_as_float(0x7f800000);
+    const int ntiles = a.nrb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int rb = tile / a.nch, ch = tile - rb * a.nch;
+        float xi[R][DP], yi[R], M[R][kJ], dmin[R], rnn[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int i = (rb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
+            i = i < a.N ? i : a.N - 1;
+            const float* src = a.rec + static_cast<size_t>(i) * RF;
+#pragma unroll
+            for (int j = 0; j < DP; ++j) xi[r][j] = __ldg(src + j);
+            yi[r] = __ldg(src + DP);
+#pragma unroll
+            for (int j = 0; j < kJ; ++j) M[r][j] = 0.f;
+            dmin[r] = inf;
+            rnn[r] = 0.f;
+        }
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            for (int jrec = 0; jrec < n; ++jrec) {
+                float x[DP + 4];
+                local_load_record<DP + 4>(s + jrec * RF, x);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float D = local_finish<NORM>(PairAccU<NORM, DP, 0>::run(xi[r], x));
+                    const float dy = fabsf(yi[r] - x[DP]);
+                    // self / duplicate (D = 0, same value): ratio 0 changes nothing; different value at D = 0: +inf
+                    const float ratio = D > 0.f ? __fdiv_rn(dy, D) : (dy > 0.f ? inf : 0.f);
+#pragma unroll
+                    for (int j = 0; j < kJ - 1; ++j)
+                        if (D <= kn.t[j]) M[r][j] = fmaxf(M[r][j], ratio);
+                    M[r][kJ - 1] = fmaxf(M[r][kJ - 1], ratio);
+                    const bool valid = (D > 0.f) || (dy > 0.f);
+                    if (valid && D < dmin[r]) {
+                        dmin[r] = D;
+                        rnn[r] = ratio;
+                    } else if (valid && D == dmin[r]) {
+                        rnn[r] = fmaxf(rnn[r], ratio);
+                    }
+                }
+            }
+            rs.release(t);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int i = (rb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
+            if (i < a.N) {
+#pragma unroll
+                for (int j = 0; j < kJ; ++j)
+                    if (M[r][j] > 0.f) atomicMax(a.tab + static_cast<size_t>(i) * kJ + j, __float_as_uint(M[r][j]));
+                const unsigned long long key = (static_cast<unsigned long long>(__float_as_uint(dmin[r])) << 32) |
+                                               static_cast<unsigned long long>(~__float_as_uint(rnn[r]));
+                atomicMin(a.nn + i, key);
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+local_table_final_kernel(const uint32_t* __restrict__ tab, const unsigned long long* __restrict__ nn, int N,
+                         float* __restrict__ table) {
+    int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= N * kJ) return;
+    const int i = e / kJ;
+    const unsigned long long key = nn[i];
+    const float dmin = __uint_as_float(static_cast<uint32_t>(key >> 32));
+    const float rnn = (dmin < __int_as_float(0x7f800000)) ? __uint_as_float(~static_cast<uint32_t>(key)) : 0.f;
+    table[e] = fmaxf(__uint_as_float(tab[e]), rnn);
+}
+
+// ---------------------------------------------------------------------------------------------
+// (3) evaluation
+// ---------------------------------------------------------------------------------------------
+// records for the evaluation: [x' (DP), y, 0, 0, 0, M_k[0..15]]
+__global__ void __launch_bounds__(256)
+local_eval_pack_kernel(const float* __restrict__ X, const float* __restrict__ y, const float* __restrict__ table,
+                       int N, Xform xf, int dp, float* __restrict__ rec) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int rf = dp + 4 + kJ;
+    float* dst = rec + static_cast<size_t>(k) * rf;
+    const float* src = X + static_cast<size_t>(k) * xf.d;
+    for (int j = 0; j < dp + 4; ++j) dst[j] = j < xf.d ? xf.sw[j] * src[xf.perm[j]] : (j == dp ? y[k] : 0.f);
+    for (int j = 0; j < kJ; ++j) dst[dp + 4 + j] = table[static_cast<size_t>(k) * kJ + j];
+}
+
+struct EvalArgs {
+    const float* rec;
+    const float* Xq;
+    uint32_t* keyU;
+    uint32_t* keyL;
+    int N, Q, d, nqb, nch, chunk;
+    Xform xf;
+};
+
+template <int NORM, int DP, int R>
+__global__ void __launch_bounds__(kLocThreads, 2)
+local_eval_kernel(const EvalArgs a, const Knots kn) {
+    constexpr int RF = DP + 4 + kJ;
+    constexpr int TILE = local_tile_records<RF>();
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+    const int ntiles = a.nqb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int qb = tile / a.nch, ch = tile - qb * a.nch;
+        float q[R][DP], U[R], L[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int qi = (qb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
+            qi = qi < a.Q ? qi : a.Q - 1;
+            const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
+#pragma unroll
+            for (int j = 0; j < DP; ++j) q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+            U[r] = __int_as_float(0x7f800000);
+            L[r] = __int_as_float(0xff800000);
+        }
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            for (int jrec = 0; jrec < n; ++jrec) {
+                float x[RF];
+                local_load_record<RF>(s + jrec * RF, x);
+                const float yk = x[DP];
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float D = local_finish<NORM>(PairAccU<NORM, DP, 0>::run(q[r], x));
+                    float Mk = x[DP + 4 + kJ - 1];  // first knot with D <= t_j, the last one if none
+#pragma unroll
+                    for (int j = kJ - 2; j >= 0; --j) Mk = (D <= kn.t[j]) ? x[DP + 4 + j] : Mk;
+                    const float MD = D > 0.f ? Mk * D : 0.f;  // M_k may be +inf at a duplicate: inf * 0 := 0
+                    U[r] = fminf(U[r], yk + MD);
+                    L[r] = fmaxf(L[r], yk - MD);
+                }
+            }
+            rs.release(t);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int qi = (qb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
+            if (qi < a.Q) {
+                atomicMin(a.keyU + qi, f2key(U[r]));
+                atomicMax(a.keyL + qi, f2key(L[r]));
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+local_eval_final_kernel(const uint32_t* __restrict__ keyU, const uint32_t* __restrict__ keyL, int Q,
+                        float* __restrict__ upper, float* __restrict__ lower, float* __restrict__ g) {
+    int qi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (qi >= Q) return;
+    const float U = key2f(keyU[qi]), L = key2f(keyL[qi]);
+    if (upper) upper[qi] = U;
+    if (lower) lower[qi] = L;
+    if (g) g[qi] = 0.5f * (U + L);
+}
+
+namespace {
+
+int local_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
+constexpr int local_r(int dp) { return dp <= 8 ? 4 : (dp <= 16 ? 2 : 1); }
+
+// (row/query blocks) x (data chunks): enough work items for ~8 per resident CTA
+void local_schedule(int units, int per_block, int N, int tile, int slots, int* nb, int* nch, int* chunk) {
+    *nb = (units + per_block - 1) / per_block;
+    int want = (8 * slots + *nb - 1) / *nb;
+    int max_ch = (N + 2 * tile - 1) / (2 * tile);
+    int c = want < 1 ? 1 : want;
+    if (c > max_ch) c = max_ch;
+    if (c < 1) c = 1;
+    int ck = (N + c - 1) / c;
+    ck = ((ck + tile - 1) / tile) * tile;
+    *nch = (N + ck - 1) / ck;
+    *chunk = ck;
+}
+
+template <int NORM, int DP>
+int launch_table(const Ctx& c, TableArgs& a, const Knots& kn) {
+    constexpr int R = local_r(DP);
+    auto kern = local_table_kernel<NORM, DP, R>;
+    int occ = 0;
+    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLocThreads, 0));
+    if (occ < 1) occ = 1;
+    const int slots = c.num_sms * occ;
+    local_schedule(a.N, kLocThreads * R, a.N, local_tile_records<DP + 4>(), slots, &a.nrb, &a.nch, &a.chunk);
+    const long long nt = static_cast<long long>(a.nrb) * a.nch;
+    KernelTimer kt(TK_LOCAL_TABLE, c.stream);
+    kern<<<static_cast<int>(nt < slots ? nt : slots), kLocThreads, 0, c.stream>>>(a, kn);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+template <int NORM, int DP>
+int launch_eval(const Ctx& c, EvalArgs& a, const Knots& kn) {
+    constexpr int R = local_r(DP);
+    auto kern = local_eval_kernel<NORM, DP, R>;
+    int occ = 0;
+    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLocThreads, 0));
+    if (occ < 1) occ = 1;
+    const int slots = c.num_sms * occ;
+    local_schedule(a.Q, kLocThreads * R, a.N, local_tile_records<DP + 4 + kJ>(), slots, &a.nqb, &a.nch, &a.chunk);
+    const long long nt = static_cast<long long>(a.nqb) * a.nch;
+    KernelTimer kt(TK_LOCAL_EVAL, c.stream);
+    kern<<<static_cast<int>(nt < slots ? nt : slots), kLocThreads, 0, c.stream>>>(a, kn);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+#define LOCAL_DISPATCH(FN, ARGS)                                          \
+    do {                                                                  \
+        if (norm == 1) {                                                  \
+            if (dp == 4) return FN<1, 4> ARGS;                            \
+            if (dp == 8) return FN<1, 8> ARGS;                            \
+            if (dp == 16) return FN<1, 16> ARGS;                          \
+            return FN<1, 32> ARGS;                                        \
+        } else if (norm == 2) {                                           \
+            if (dp == 4) return FN<2, 4> ARGS;                            \
+            if (dp == 8) return FN<2, 8> ARGS;                            \
+            if (dp == 16) return FN<2, 16> ARGS;                          \
+            return FN<2, 32> ARGS;                                        \
+        } else {                                                          \
+            if (dp == 4) return FN<3, 4> ARGS;                            \
+            if (dp == 8) return FN<3, 8> ARGS;                            \
+            if (dp == 16) return FN<3, 16> ARGS;                          \
+            return FN<3, 32> ARGS;                                        \
+        }                                                                 \
+    } while (0)
+
+int dispatch_table(const Ctx& c, TableArgs& a, const Knots& kn, int norm, int dp) {
+    LOCAL_DISPATCH(launch_table, (c, a, kn));
+}
+int dispatch_eval(const Ctx& c, EvalArgs& a, const Knots& kn, int norm, int dp) {
+    LOCAL_DISPATCH(launch_eval, (c, a, kn));
+}
+
+}  // namespace
+
+int launch_distance_quantiles(const Ctx& c, const float* X, int64_t N, const Xform& xf, int norm,
+                              const int32_t* pair_i, const int32_t* pair_k, int64_t S, int J, float* knots,
+                              int* bad_dev) {
+    const int s = static_cast<int>(S);
+    Workspace wd, ws, wt;
+    int rc;
+    if ((rc = wd.alloc(sizeof(float) * static_cast<size_t>(S), c.stream))) return rc;
+    if ((rc = ws.alloc(sizeof(float) * static_cast<size_t>(S), c.stream))) return rc;
+    size_t bytes = 0;
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortKeys(nullptr, bytes, static_cast<const float*>(nullptr),
+                                               static_cast<float*>(nullptr), s, 0, 32, c.stream));
+    if ((rc = wt.alloc(bytes, c.stream))) return rc;
+    local_pair_dist_kernel<<<(s + 255) / 256, 256, 0, c.stream>>>(X, static_cast<int>(N), xf, norm, pair_i, pair_k,
+                                                                 s, wd.as<float>(), bad_dev);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortKeys(wt.p, bytes, wd.as<float>(), ws.as<float>(), s, 0, 32, c.stream));
+    local_pick_kernel<<<1, 32 * ((J + 31) / 32), 0, c.stream>>>(ws.as<float>(), S, J, knots);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+int launch_local_lipschitz(const Ctx& c, const float* X, const float* y, int64_t N64, const Xform& xf, int norm,
+                           const float* knots_host, float* table) {
+    const int N = static_cast<int>(N64);
+    const int dp = local_dp(xf.d);
+    RecLayout lay{dp + 4, dp};
+    Workspace wrec, wtab, wnn;
+    int rc;
+    if ((rc = wrec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream))) return rc;
+    if ((rc = wtab.alloc(sizeof(uint32_t) * static_cast<size_t>(N) * kJ, c.stream))) return rc;
+    if ((rc = wnn.alloc(sizeof(unsigned long long) * static_cast<size_t>(N), c.stream))) return rc;
+    if ((rc = launch_prepack(c, X, y, nullptr, N, xf, lay, wrec.as<float>()))) return rc;
+    LIPFIT_CUDA(cudaMemsetAsync(wtab.p, 0, sizeof(uint32_t) * static_cast<size_t>(N) * kJ, c.stream));
+    LIPFIT_CUDA(cudaMemsetAsync(wnn.p, 0xFF, sizeof(unsigned long long) * static_cast<size_t>(N), c.stream));
+    Knots kn;
+    for (int j = 0; j < kJ; ++j) kn.t[j] = knots_host[j];
+    TableArgs a{};
+    a.rec = wrec.as<float>();
+    a.tab = wtab.as<uint32_t>();
+    a.nn = wnn.as<unsigned long long>();
+    a.N = N;
+    if ((rc = dispatch_table(c, a, kn, norm, dp))) return rc;
+    const int ne = N * kJ;
+    local_table_final_kernel<<<(ne + 255) / 256, 256, 0, c.stream>>>(a.tab, a.nn, N, table);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N64, const float* Xq, int64_t Q64,
+                        const Xform& xf, int norm, const float* knots_host, const float* table, float* upper,
+                        float* lower, float* g) {
+    const int N = static_cast<int>(N64), Q = static_cast<int>(Q64);
+    const int dp = local_dp(xf.d);
+    const int rf = dp + 4 + kJ;
+    Workspace wrec, wkeys;
+    int rc;
+    if ((rc = wrec.alloc(sizeof(float) * static_cast<size_t>(N) * rf, c.stream))) return rc;
+    if ((rc = wkeys.alloc(sizeof(uint32_t) * 2 * static_cast<size_t>(Q), c.stream))) return rc;
+    local_eval_pack_kernel<<<(N + 255) / 256, 256, 0, c.stream>>>(X, y, table, N, xf, dp, wrec.as<float>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    Knots kn;
+    for (int j = 0; j < kJ; ++j) kn.t[j] = knots_host[j];
+    EvalArgs a{};
+    a.rec = wrec.as<float>();
+    a.Xq = Xq;
+    a.keyU = wkeys.as<uint32_t>();
+    a.keyL = a.keyU + Q;
+    a.N = N;
+    a.Q = Q;
+    a.d = xf.d;
+    a.xf = xf;
+    LIPFIT_CUDA(cudaMemsetAsync(a.keyU, 0xFF, sizeof(uint32_t) * Q, c.stream));
+    LIPFIT_CUDA(cudaMemsetAsync(a.keyL, 0x00, sizeof(uint32_t) * Q, c.stream));
+    if ((rc = dispatch_eval(c, a, kn, norm, dp))) return rc;
+    local_eval_final_kernel<<<(Q + 255) / 256, 256, 0, c.stream>>>(a.keyU, a.keyL, Q, upper, lower, g);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+}  // namespace lipfit
