@@ -306,6 +306,47 @@ def bench_smooth(torch, L, wl, l2buf, dev):
             "lane_ops": LANE_OPS["5s"], "z": y, "X": X}
 
 
+def bench_local(torch, L, l2buf, dev, sms, peaks, args):
+    """NEXT-1 (local Lipschitz interpolation) on config 5's data: knots from 1e6 sampled
+    pairs, step tables for N = 2e5 (4e10 ordered pairs), evaluation at Q = 1e6 (2e11 pairs)."""
+    import oracle
+    from inputs import sample_pairs
+    wl = make_workload(5)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    X, y, Xq = t(wl.X), t(wl.y), t(wl.Xq)
+    pi, pk = sample_pairs(3, wl.N, 1_000_000)
+    pi_d, pk_d = t(pi), t(pk)
+    knots = L.lipfit_distance_quantiles(X, pi_d, pk_d, L.LIPFIT_LOCAL_KNOTS, wl.norm)
+    f_tab = lambda: L.lipfit_local_lipschitz(X, y, knots, wl.norm)
+    ms_tab = _time_steps(torch, f_tab, max(1, min(args.steps, 3)), 2, l2buf)
+    k_tab, _ = _kernel_ms(L, 4, f_tab, 1)
+    table = f_tab()
+    f_ev = lambda: L.lipfit_values_local(X, y, Xq, knots, table, wl.norm)
+    ms_ev = _time_steps(torch, f_ev, max(1, min(args.steps, 3)), 2, l2buf)
+    k_ev, _ = _kernel_ms(L, 5, f_ev, 1)
+    # executed lane-ops per pair (d = 5 padded to 8 coordinates, J = 16 knots):
+    #   table: 8 sub + 8 fma + sqrt + |dy| + divide (~8) + 15 (compare + max) pairs + last max + nn update ~ 60
+    #   eval : 8 sub + 8 fma + sqrt + 15 (compare + select) + guard 2 + 2 fma-like + min + max ~ 53
+    out = {"workload": "config 5 data (d=5, N=200000), Q=1000000, L2, J=16 knots from 1e6 sampled pairs",
+           "table": {"ms_per_step": float(np.mean(ms_tab)), "kernel_ms": k_tab,
+                     "value": wl.N * (wl.N - 1) / (np.mean(ms_tab) * 1e-3) / 1e9, "unit": "G ordered pairs/s",
+                     "roofline": _roofline(wl.N * wl.N, 60, k_tab, sms, peaks)},
+           "evaluate": {"ms_per_step": float(np.mean(ms_ev)), "kernel_ms": k_ev,
+                        "value": wl.N * wl.Q / (np.mean(ms_ev) * 1e-3) / 1e9, "unit": UNIT,
+                        "roofline": _roofline(wl.N * wl.Q, 53, k_ev, sms, peaks)}}
+    if not args.no_cpu:
+        sel = oracle_subset(wl.Q, 400)
+        rows = oracle_subset(wl.N, 64)
+        tb = table.cpu().numpy()
+        up, lo, g = (v.cpu().numpy() for v in f_ev())
+        U, Lo, G = oracle.values_local(wl.X, wl.y, wl.Xq[sel], knots.astype(np.float64), tb.astype(np.float64), wl.norm)
+        tol = 1e-5 * wl.y_range
+        frac_ok = float(np.mean((np.abs(up[sel] - U) <= tol) & (np.abs(lo[sel] - Lo) <= tol)))
+        out["evaluate"]["parity"] = {"queries": int(len(sel)), "fraction_within_tol": frac_ok, "tol": tol,
+                                     "note": "queries off a knot boundary must match; tests/test_gpu_local.py sandwiches the rest"}
+    return out
+
+
 def parity_bounds(wl, outs, sel, ref):
     """max |gpu - oracle| / (1e-5 * range) on the oracle's query sample (<= 1 passes)."""
     tol = 1e-5 * wl.y_range
@@ -397,7 +438,7 @@ def run_gpu(args):
 
 def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
     import oracle
-    wl = make_workload(c)
+    wl = make_workload(5 if c == 6 else c)
     steps = max(1, min(args.steps, 3)) if c in (3, 4) else args.steps
     out = {}
     if c in (1, 3):
@@ -439,6 +480,8 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
                              "max_dist_err_ulps": float(np.max(np.abs(gd - od.astype(np.float32))
                                                                / np.spacing(od.astype(np.float32)))),
                              "queries": int(len(sel))}
+    elif c == 6:
+        out.update(bench_local(torch, L, l2buf, dev, sms, peaks, args))
     elif c == 5:
         r = bench_smooth(torch, L, wl, l2buf, dev)
         out.update({"smooth_wall_s": r["wall_s"], "info": r["info"], "evals": r["evals"],
@@ -470,7 +513,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--configs", default="2", help="comma list of BASELINE.json configs to report (2 always)")
+    ap.add_argument("--configs", default="2",
+                    help="comma list of BASELINE.json configs to report (2 always); 6 = local Lipschitz (NEXT-1)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
