@@ -38,14 +38,16 @@ METRIC = "query x datum pair evaluations per second (bounds, config 2)"
 UNIT = "Gpairs/s"
 # Algorithmic lane-ops per pair: 1 lane-op = one fp32
 # add/sub/mul/fma, one min/max/relu/compare, or one sqrt.
+# Config 2 (weighted L1, 2 free + 2 constrained coordinates) runs the FOLDED form (bounds.cu FoldL1Core):
+# 4 sub + 4 add + 2 relu + 1 sub + min + max = 13 executed lane-ops per pair (SURVEY.md's plain form: 18).
 # Config 4 (symmetric L2) selects on the cross-term key ||x||^2 - 2 q.x: 16 FFMA + 1 compare = 17 executed
 # lane-ops per pair (the direct-difference form of SURVEY.md is 33).  Smoothing visits each UNORDERED pair
 # once with a one-sided distance: 5 sub + 5 relu + 5 fma + dz + dz^2 + compare = 18 executed lane-ops
 # per visit (SURVEY.md credits 26 per ORDERED pair).  Rooflines are reported on EXECUTED work.
-LANE_OPS = {1: 9, 2: 18, 3: 21, 4: 17, "4direct": 33, "5s": 18, "5s_survey": 26, "5b": 31}
+LANE_OPS = {1: 9, 2: 13, "2survey": 18, 3: 21, 4: 17, "4direct": 33, "5s": 18, "5s_survey": 26, "5b": 31}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md); null where no capture of this kernel version exists.
-NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2>": 27_238_400, "knn_select<dot>": 5_975_622_000,
+NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2,folded>": None, "knn_select<dot>": 5_975_622_000,
                      "smooth_pairs<L2,U0,C5>": 8_126_976}
 FP32_LANES_PER_SM = 128
 
@@ -411,6 +413,8 @@ def run_gpu(args):
         "roofline": _roofline(r2["pairs"], LANE_OPS[2], r2["kernel_ms"], sms, peaks, r2["kernel"]),
         "peaks": peaks_how,
     }
+    line["roofline"]["frac_survey_18ops"] = (
+        r2["pairs"] * LANE_OPS["2survey"] / (r2["kernel_ms"] * 1e-3) / 1e12 / line["roofline"]["peak"])
     if clocks and clocks.get("sm_mhz"):
         rf = line["roofline"]
         rf["frac_at_observed_clock"] = rf["achieved"] / (sms * FP32_LANES_PER_SM * clocks["sm_mhz"] * 1e6 / 1e12)

@@ -103,12 +103,13 @@ int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const fl
     if (rc) return rc;
     RecLayout lay = bounds_layout(xf, norm);
     if (lay.rf == 0) return LIPFIT_E_PARAM;
+    const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
     Workspace rec;
     rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
     if (rc) return rc;
-    rc = launch_prepack(c, X, y, nullptr, N, xf, lay, rec.as<float>());
+    rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>());
     if (rc) return rc;
-    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xf, norm, M, upper, lower, g);
+    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g);
 }
 
 int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,

@@ -43,6 +43,8 @@ struct SpecCore {
     static constexpr int RF = record_floats(D);
     static constexpr int VSLOT = D;
     static constexpr bool kGeneric = false;
+    static constexpr bool kFold = false;
+    static __device__ __forceinline__ float query_term(const float*) { return 0.f; }
     static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags&,
                                                 float M, float& hi, float& lo) {
         float au, al;
@@ -59,12 +61,48 @@ struct SpecCore {
     }
 };
 
+// Weighted L1 with constrained coordinates, folded (the coordinates arrive PRE-MULTIPLIED BY M):
+//   P  = sum_free |delta_j| + sum_constr (delta_j)_+                    ( = M D^u )
+//   M D^l = P - sum_constr delta_j = P - (sq - sx),  sq / sx = sum of the constrained coordinates of q / x
+//   hi = y + P,      lo = y - M D^l = (2 y - sx) - hi + sq = c' - hi + sq
+// c' = 2y - sx rides in the record, sq is constant per query and is added AFTER the running maximum, and y
+// starts the accumulation chain: 9 FMA-pipe + 2 ALU-pipe operations per pair instead of 14 + 2.
+// (Valid for L1 only: no square root stands between the sums.  Rounding: the terms of lo are of magnitude
+// M |x|, so its error is a few 2^-24 M |x| -- inside the budget of DESIGN.md §6, measured in the tests.)
+template <int DU, int DC>
+struct FoldL1Core {
+    static constexpr int D = DU + DC;
+    static constexpr int RF = record_floats(D + 1);
+    static constexpr int VSLOT = D;
+    static constexpr int CSLOT = D + 1;
+    static constexpr bool kGeneric = false;
+    static constexpr bool kFold = true;
+    static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags&, float,
+                                                float& hi, float& lo) {
+        float a = x[VSLOT];
+#pragma unroll
+        for (int j = 0; j < DU; ++j) a += fabsf(q[j] - x[j]);
+#pragma unroll
+        for (int j = DU; j < D; ++j) a += fmaxf(q[j] - x[j], 0.f);
+        hi = a;
+        lo = x[CSLOT] - a;
+    }
+    static __device__ __forceinline__ float query_term(const float* q) {
+        float sq = 0.f;
+#pragma unroll
+        for (int j = DU; j < D; ++j) sq += q[j];
+        return sq;
+    }
+};
+
 template <int NORM, int DP>
 struct GenCore {
     static constexpr int D = DP;
     static constexpr int RF = DP + 4;
     static constexpr int VSLOT = DP;
     static constexpr bool kGeneric = true;
+    static constexpr bool kFold = false;
+    static __device__ __forceinline__ float query_term(const float*) { return 0.f; }
     static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags& ff,
                                                 float M, float& hi, float& lo) {
         float au, al;
@@ -171,6 +209,7 @@ bounds_kernel(const BoundsArgs a, const FreeFlags ff) {
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+            if (Core::kFold) L[r] += Core::query_term(q[r]);  // the per-query constant of the folded lower bound
             if (qi < a.Q) {
                 if (a.nch == 1) {
                     if (a.upper) a.upper[qi] = U[r];
@@ -266,6 +305,13 @@ int launch_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     return launch_one<Core, 1, 128, 4>(c, a, ff);
 }
 
+template <int DU, int DC>
+int launch_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    using Core = FoldL1Core<DU, DC>;
+    if (flavour == 0) return launch_one<Core, 8, 128, 2>(c, a, ff);
+    return launch_one<Core, 1, 128, 4>(c, a, ff);
+}
+
 template <int NORM, int DP>
 int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     using Core = GenCore<NORM, DP>;
@@ -276,13 +322,15 @@ int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
 
 #define SPEC(NORM, DU, DC, NAME) \
     { NORM, DU, DC, NAME, {record_floats(DU + DC), DU + DC}, &launch_spec<NORM, DU, DC> }
+#define FOLD(DU, DC, NAME) \
+    { 1, DU, DC, NAME, {record_floats(DU + DC + 1), DU + DC, DU + DC + 1, true}, &launch_fold<DU, DC> }
 #define GEN(NORM, DP, NAME) \
     { NORM, DP, -1, NAME, {DP + 4, DP}, &launch_gen<NORM, DP> }
 
 const Variant kVariants[] = {
     // shapes of BASELINE.json configs 1, 2, 3, 5 (+ the symmetric versions of the same dims)
     SPEC(2, 2, 0, "bounds<L2,U2,C0>"),
-    SPEC(1, 2, 2, "bounds<L1,U2,C2>"),
+    FOLD(2, 2, "bounds<L1,U2,C2,folded>"),
     SPEC(3, 7, 1, "bounds<Linf,U7,C1>"),
     SPEC(2, 0, 5, "bounds<L2,U0,C5>"),
     SPEC(2, 3, 0, "bounds<L2,U3,C0>"),

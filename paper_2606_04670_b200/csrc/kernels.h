@@ -16,6 +16,8 @@ FreeFlags make_free_flags(const Xform& xf);
 // zeros elsewhere.
 struct RecLayout {
     int rf, vslot;
+    int cslot = -1;       // >= 0: slot of c' = 2 value - sum of the constrained coordinates (folded L1 bounds)
+    bool mscale = false;  // true: the kernel family wants the coordinates pre-multiplied by M
 };
 RecLayout bounds_layout(const Xform& xf, int norm);
 RecLayout smooth_layout(const Xform& xf, int norm);

@@ -117,7 +117,7 @@ FreeFlags make_free_flags(const Xform& xf) {
 // One thread per record; the record is assembled in registers and written as float4s.
 __global__ void __launch_bounds__(256)
 prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
-               const float* __restrict__ eps, int N, Xform xf, int rf, int vslot,
+               const float* __restrict__ eps, int N, Xform xf, int rf, int vslot, int cslot,
                float* __restrict__ rec) {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
@@ -125,12 +125,18 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
     float* dst = rec + static_cast<size_t>(k) * rf;
     float v = y ? y[k] : 0.f;
     if (eps) v += eps[k];
+    float cval = 0.f;
+    if (cslot >= 0) {  // c' = 2 y - sum of the constrained (packed) coordinates, see bounds.cu FoldL1Core
+        float sc = 0.f;
+        for (int j = xf.dU; j < xf.d; ++j) sc += xf.sw[j] * src[xf.perm[j]];
+        cval = 2.f * v - sc;
+    }
     for (int j0 = 0; j0 < rf; j0 += 4) {
         float t[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             int j = j0 + c;
-            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : 0.f);
+            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : (j == cslot ? cval : 0.f));
         }
         *reinterpret_cast<float4*>(dst + j0) = make_float4(t[0], t[1], t[2], t[3]);
     }
@@ -153,7 +159,7 @@ axpy_kernel(float* __restrict__ y, const float* __restrict__ eps, int N) {
 int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
                    const Xform& xf, RecLayout lay, float* rec) {
     int n = static_cast<int>(N);
-    prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, rec);
+    prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, lay.cslot, rec);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     return LIPFIT_OK;
