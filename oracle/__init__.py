@@ -34,6 +34,8 @@ def load():
         lib.oracle_distance_quantiles.argtypes = [P, i64, i32, i32, P, P, P, i64, i32, P]
         lib.oracle_local_lipschitz.argtypes = [P, P, i64, i32, i32, P, P, i32, P]
         lib.oracle_values_local.argtypes = [P, P, i64, i32, P, i64, i32, P, P, i32, P, P, P, P]
+        lib.oracle_bounds_topk.argtypes = [P, P, i64, i32, P, i64, f64, P, i32, P, i32, P, P, P, P]
+        lib.oracle_bounds_topk.restype = C.c_int
         for fn in (lib.oracle_distance_quantiles, lib.oracle_local_lipschitz, lib.oracle_values_local):
             fn.restype = C.c_int
         for fn in (lib.oracle_bounds, lib.oracle_knn, lib.oracle_smooth_objective,
@@ -76,6 +78,21 @@ def bounds(X, y, Xq, M, mask=None, norm=2, weights=None):
     if rc:
         raise ValueError(f"oracle_bounds rc={rc}")
     return up, lo, g
+
+
+def bounds_topk(X, y, Xq, M, wk, mask=None, norm=2, weights=None):
+    """(upper, lower, g): weighted sums of the k = len(wk) best bound values."""
+    X, y, Xq = _f32(X, 2), _f32(y, 1), _f32(Xq, 2)
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _params(d, mask, weights)
+    wk = np.ascontiguousarray(wk, dtype=np.float32)
+    U, L, G = (np.empty(Q, dtype=np.float64) for _ in range(3))
+    rc = load().oracle_bounds_topk(_ptr(X), _ptr(y), N, d, _ptr(Xq), Q, float(np.float32(M)), _ptr(m),
+                                   int(norm), _ptr(w), len(wk), _ptr(wk), _ptr(U), _ptr(L), _ptr(G))
+    if rc:
+        raise ValueError(f"oracle_bounds_topk rc={rc}")
+    return U, L, G
 
 
 def knn(X, Xq, k, mask=None, side=0, norm=2, weights=None):

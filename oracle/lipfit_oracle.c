@@ -400,3 +400,55 @@ int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, co
     return 0;
 }
 
+/* Approximation with k > 1 ("Extra features" 2; PAPER.md:226 `values(query, LC, model, k)`):
+ * "a weighting vector w in R^k_+ ... the weights of the 'nearest' neighbour, second nearest and so on, so
+ * that both upper and lower bound are calculated using k neighbours", evaluated with torch.topk
+ * (PAPER.md:206).  Reading R24: with u_(1) <= u_(2) <= ... the sorted values y^k + M D^u and
+ * l_(1) >= l_(2) >= ... the sorted values y^k - M D^l,
+ *     upper = sum_j w_j u_(j),   lower = sum_j w_j l_(j),   g = (upper + lower) / 2,   j = 1..k.
+ * k = 1, w = (1) is Eq.(2),(3). */
+static int cmp_double_desc(const void* a, const void* b) { return -cmp_double(a, b); }
+
+int oracle_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                       double M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
+                       const float* wk, double* upper, double* lower, double* g) {
+    int rc = check_common(X, N, d, mono_mask, norm, weights);
+    if (rc) return rc;
+    if (!y || !wk || (Q > 0 && !Xq)) return -1;
+    if (Q < 0 || k < 1 || k > N) return -3;
+    if (!(M >= 0.0) || !isfinite(M)) return -4;
+    int bad = 0;
+#pragma omp parallel
+    {
+        double* hi = (double*)malloc(sizeof(double) * (size_t)N);
+        double* lo = (double*)malloc(sizeof(double) * (size_t)N);
+        if (!hi || !lo) {
+#pragma omp atomic write
+            bad = 1;
+        } else {
+#pragma omp for schedule(static)
+            for (int64_t q = 0; q < Q; ++q) {
+                for (int64_t j = 0; j < N; ++j) {
+                    double Du, Dl;
+                    one_sided_distances(Xq + q * d, X + j * d, d, mono_mask, norm, weights, &Du, &Dl);
+                    hi[j] = (double)y[j] + M * Du;
+                    lo[j] = (double)y[j] - M * Dl;
+                }
+                qsort(hi, (size_t)N, sizeof(double), cmp_double);
+                qsort(lo, (size_t)N, sizeof(double), cmp_double_desc);
+                double U = 0.0, L = 0.0;
+                for (int32_t j = 0; j < k; ++j) {
+                    U += (double)wk[j] * hi[j];
+                    L += (double)wk[j] * lo[j];
+                }
+                if (upper) upper[q] = U;
+                if (lower) lower[q] = L;
+                if (g) g[q] = 0.5 * (U + L);
+            }
+        }
+        free(hi);
+        free(lo);
+    }
+    return bad ? -6 : 0;
+}
+

@@ -90,6 +90,12 @@ int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, co
                         int32_t norm, const float* weights, const double* knots, int32_t J,
                         const double* table, double* upper, double* lower, double* g);
 
+/* k > 1 approximation: upper = sum_j wk[j] * (j-th smallest of y^k + M D^u),
+ * lower = sum_j wk[j] * (j-th largest of y^k - M D^l), j = 1..k; wk: float[k]. */
+int oracle_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                       double M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
+                       const float* wk, double* upper, double* lower, double* g);
+
 int oracle_num_threads(void);
 
 #ifdef __cplusplus
