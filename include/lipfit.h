@@ -45,6 +45,7 @@ extern "C" {
 
 #define LIPFIT_MAX_DIM 32
 #define LIPFIT_MAX_K 128
+#define LIPFIT_MAX_TOPK 8    /* neighbours of the k > 1 approximation (lipfit_bounds_topk) */
 #define LIPFIT_LOCAL_KNOTS 16 /* knots of the local Lipschitz step functions M_k */
 
 enum lipfit_norm { LIPFIT_L1 = 1, LIPFIT_L2 = 2, LIPFIT_LINF = 3 };
@@ -79,6 +80,18 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d,
                        const float* Xq, int64_t Q, float M,
                        const int32_t* mono_mask, int32_t norm, const float* weights,
                        float* upper, float* lower, float* g, void* cuda_stream);
+
+/* ---- Approximation with k > 1 neighbours ("Extra features" 2) -------
+ *   upper[q] = sum_j wk[j] * (j-th smallest of y[k] + M D^u(q,k)),
+ *   lower[q] = sum_j wk[j] * (j-th largest  of y[k] - M D^l(q,k)),   j = 1..k,   g = (upper+lower)/2
+ * "the weights of the 'nearest' neighbour, second nearest and so on ... The data set will not be
+ * interpolated".  wk: HOST float[k], wk[j] >= 0 finite (assumed to add to 1; not enforced);
+ * 1 <= k <= min(N, LIPFIT_MAX_TOPK); k = 1, wk = {1} is lipfit_bounds.  Other arguments, layout and
+ * error behaviour as lipfit_bounds; asynchronous on the stream. */
+int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                       float M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
+                       const float* wk /* host[k] */, float* upper, float* lower, float* g,
+                       void* cuda_stream);
 
 /* ---- k nearest data per query by distance (d_(1) <= d_(2) <= ...) -------------
  * side 0: symmetric weighted norm, mask ignored; +1: D^u; -1: D^l.

@@ -24,8 +24,9 @@ EXPORTS = [
     "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
     "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
-    "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local",
+    "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
 ]
+LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
 
 
@@ -66,6 +67,7 @@ def load():
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
     lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
     lib.lipfit_lbfgs.argtypes = [i64, P, EVAL_FN, P, i32, f64, i32, P]
+    lib.lipfit_bounds_topk.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, i32, P, P, P, P, P]
     lib.lipfit_distance_quantiles.argtypes = [P, i64, i32, i32, P, P, P, i64, i32, P, P]
     lib.lipfit_local_lipschitz.argtypes = [P, P, i64, i32, i32, P, P, i32, P, P]
     lib.lipfit_values_local.argtypes = [P, P, i64, i32, P, i64, i32, P, P, i32, P, P, P, P, P]
@@ -200,6 +202,23 @@ def lipfit_bounds(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, wei
                               ptr["g"], _stream(stream))
     _check(rc, "lipfit_bounds")
     return outs["upper"], outs["lower"], outs["g"]
+
+
+def lipfit_bounds_topk(X, y, Xq, M: float, wk, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                       stream=None):
+    """(upper, lower, g): weighted sums of the k = len(wk) best bound values."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _host_params(d, mono_mask, weights)
+    wk = np.ascontiguousarray(wk, dtype=np.float32)
+    outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    rc = load().lipfit_bounds_topk(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(m),
+                                   int(norm), _np_ptr(w), len(wk), _np_ptr(wk), outs[0].data_ptr(),
+                                   outs[1].data_ptr(), outs[2].data_ptr(), _stream(stream))
+    _check(rc, "lipfit_bounds_topk")
+    return tuple(outs)
 
 
 def lipfit_knn(X, Xq, k: int, mono_mask=None, side: int = 0, norm: int = LIPFIT_L2, weights=None,

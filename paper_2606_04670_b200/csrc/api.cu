@@ -112,6 +112,34 @@ int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const fl
     return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g);
 }
 
+int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                       float M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
+                       const float* wk, float* upper, float* lower, float* g, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (k < 1 || k > LIPFIT_MAX_TOPK || k > N) return LIPFIT_E_SIZE;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    if (!wk) return LIPFIT_E_NULL;
+    for (int j = 0; j < k; ++j)
+        if (!(wk[j] >= 0.f) || !std::isfinite(wk[j])) return LIPFIT_E_PARAM;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    if (!X || !y) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    RecLayout lay = bounds_topk_layout(xf);
+    Workspace rec;
+    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
+    if (rc) return rc;
+    rc = launch_prepack(c, X, y, nullptr, N, xf, lay, rec.as<float>());
+    if (rc) return rc;
+    return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xf, norm, M, k, wk, upper, lower, g);
+}
+
 int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
                        int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
                        const float* weights, float* upper, float* lower, float* g,

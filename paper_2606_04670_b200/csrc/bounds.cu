@@ -394,4 +394,161 @@ int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, in
     return v->launch(c, a, ff, flavour);
 }
 
+// ---------------------------------------------------------------------------------------------
+// NEXT-2: approximation with k > 1 neighbours:
+//   upper = sum_j wk[j] * (j-th smallest of y^k + M D^u),  lower = sum_j wk[j] * (j-th largest of y^k - M D^l).
+// The same fused pass; every query keeps its kTopK best upper and lower candidates sorted in registers.
+// The hot loop is the pair arithmetic plus one compare per side against the worst kept value; the
+// rare candidates that pass (rate ~ k ln(N)/N) are inserted by an unrolled compare-exchange chain.
+// ---------------------------------------------------------------------------------------------
+constexpr int kTopK = LIPFIT_MAX_TOPK;
+
+struct TopkWeights {
+    float w[kTopK];
+};
+
+template <int NORM, int DP, int R>
+__global__ void __launch_bounds__(128, 2)
+bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk) {
+    using Core = GenCore<NORM, DP>;
+    constexpr int THREADS = 128;
+    constexpr int RF = Core::RF;
+    constexpr int TILE = tile_records<RF>();
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+    const float inf = __int_as_float(0x7f800000);
+    for (int qb = blockIdx.x; qb < a.nqb; qb += gridDim.x) {
+        float q[R][DP];
+        float U[R][kTopK], L[R][kTopK];  // U ascending (U[K-1] = worst kept), L descending
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+            qi = qi < a.Q ? qi : a.Q - 1;
+            const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
+#pragma unroll
+            for (int j = 0; j < DP; ++j) q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+#pragma unroll
+            for (int j = 0; j < kTopK; ++j) {
+                U[r][j] = inf;
+                L[r][j] = -inf;
+            }
+        }
+        RecordStream<TILE> rs(a.rec, RF, 0, a.N, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            for (int j = 0; j < n; ++j) {
+                float x[RF];
+                load_record<RF>(s + j * RF, x);
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    float hi, lo;
+                    Core::pair(q[r], x, ff, a.M, hi, lo);
+                    if (hi < U[r][kTopK - 1]) {  // rare: insert into the sorted list
+                        U[r][kTopK - 1] = hi;
+#pragma unroll
+                        for (int i = kTopK - 1; i > 0; --i) {
+                            const float lo_ = fminf(U[r][i - 1], U[r][i]), hi_ = fmaxf(U[r][i - 1], U[r][i]);
+                            U[r][i - 1] = lo_;
+                            U[r][i] = hi_;
+                        }
+                    }
+                    if (lo > L[r][kTopK - 1]) {
+                        L[r][kTopK - 1] = lo;
+#pragma unroll
+                        for (int i = kTopK - 1; i > 0; --i) {
+                            const float hi_ = fmaxf(L[r][i - 1], L[r][i]), lo_ = fminf(L[r][i - 1], L[r][i]);
+                            L[r][i - 1] = hi_;
+                            L[r][i] = lo_;
+                        }
+                    }
+                }
+            }
+            rs.release(t);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+            if (qi < a.Q) {
+                float su = 0.f, sl = 0.f;
+#pragma unroll
+                for (int j = 0; j < kTopK; ++j) {  // slots past k have weight 0 (and may hold +-inf: skip them)
+                    if (wk.w[j] != 0.f) {
+                        su = fmaf(wk.w[j], U[r][j], su);
+                        sl = fmaf(wk.w[j], L[r][j], sl);
+                    }
+                }
+                if (a.upper) a.upper[qi] = su;
+                if (a.lower) a.lower[qi] = sl;
+                if (a.g) a.g[qi] = 0.5f * (su + sl);
+            }
+        }
+    }
+}
+
+namespace {
+
+template <int NORM, int DP>
+int launch_topk(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk) {
+    constexpr int R = DP <= 8 ? 2 : 1;
+    auto kern = bounds_topk_kernel<NORM, DP, R>;
+    int occ = 0;
+    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 128, 0));
+    if (occ < 1) occ = 1;
+    a.nqb = (a.Q + 128 * R - 1) / (128 * R);
+    const int slots = c.num_sms * occ;
+    KernelTimer kt(TK_BOUNDS, c.stream);
+    kern<<<a.nqb < slots ? a.nqb : slots, 128, 0, c.stream>>>(a, ff, wk);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+int topk_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
+
+}  // namespace
+
+RecLayout bounds_topk_layout(const Xform& xf) {
+    const int dp = topk_dp(xf.d);
+    return RecLayout{dp + 4, dp};
+}
+
+int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
+                       int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g) {
+    BoundsArgs a{};
+    a.rec = rec;
+    a.Xq = Xq;
+    a.upper = upper;
+    a.lower = lower;
+    a.g = g;
+    a.N = static_cast<int>(N);
+    a.Q = static_cast<int>(Q);
+    a.d = xf.d;
+    a.M = M;
+    a.xf = xf;
+    TopkWeights wk;
+    for (int j = 0; j < kTopK; ++j) wk.w[j] = j < k ? wk_host[j] : 0.f;
+    FreeFlags ff = make_free_flags(xf);
+    const int dp = topk_dp(xf.d);
+#define TOPK_GO(NORM)                                              \
+    do {                                                           \
+        if (dp == 4) return launch_topk<NORM, 4>(c, a, ff, wk);    \
+        if (dp == 8) return launch_topk<NORM, 8>(c, a, ff, wk);    \
+        if (dp == 16) return launch_topk<NORM, 16>(c, a, ff, wk);  \
+        return launch_topk<NORM, 32>(c, a, ff, wk);                \
+    } while (0)
+    if (norm == 1) TOPK_GO(1);
+    if (norm == 2) TOPK_GO(2);
+    TOPK_GO(3);
+#undef TOPK_GO
+}
+
 }  // namespace lipfit

@@ -30,6 +30,10 @@ int launch_prepack(const Ctx& c, const float* X, const float* y, const float* ep
 int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q,
                   const Xform& xf, int norm, float M, float* upper, float* lower, float* g);
 const char* bounds_variant_name(const Xform& xf, int norm);
+// NEXT-2: weighted sums of the k best upper / lower bound values; wk_host: host float[k]
+RecLayout bounds_topk_layout(const Xform& xf);
+int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
+                       int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g);
 
 // a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
