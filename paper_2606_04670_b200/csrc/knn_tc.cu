@@ -12,20 +12,26 @@
 // <= 3 * 2^-16 |q'_j x_j| per coordinate; the fp64 re-rank + certificate of knn.cu
 // turn the selected pools into the exact answer, whatever the key arithmetic was.
 //
-// Kernel (one CTA per SM, 320 threads, warp-specialised):
+// Kernel (one CTA per SM, 576 threads, warp-specialised):
 //   warp 8   TMA producer : 1-D bulk copies of pre-swizzled operand tiles (the pack kernels write the
 //                           global image in the canonical K-major SWIZZLE_128B shared-memory layout,
 //                           so no tensor map is needed) into a 4-stage ring; A (2 x 128 queries) once
 //                           per work item.
 //   warp 9   MMA issuer   : one thread; per B tile 2 x 4 tcgen05.mma (M=128, N=128, K=16) into
 //                           double-buffered TMEM accumulators (2 query halves x 2 stages x 128 columns).
-//   warps 0-7 epilogue    : tcgen05.ld 32 columns at a time (thread = query row), min-tree + one compare
-//                           against the query's threshold; rare hits append to the candidate pool /
-//                           compact it exactly as in knn.cu.
+//   warps 0-7 detectors   : tcgen05.ld 32 columns at a time (thread = query row), min-tree + one compare
+//                           against the query's threshold; a 32 x 32 block that contains a hit goes into a
+//                           shared-memory ring.
+//   warps 10-17 appenders : one per detector warp; own the thresholds and candidate pools of its 32
+//                           queries, append the hits of the ring blocks / compact the pools exactly as in
+//                           knn.cu, and publish lowered thresholds back through shared memory.
 #include <cuda_bf16.h>
 
 #include "knn_common.cuh"
 
+#ifndef LIPFIT_TC_SLEEP_NS
+#define LIPFIT_TC_SLEEP_NS 40
+#endif
 #ifndef LIPFIT_TC_EXPERIMENT
 #define LIPFIT_TC_EXPERIMENT 0  // 1, 2: timing experiments with invalid results (never in a product build)
 #endif
@@ -34,12 +40,14 @@ namespace lipfit {
 
 namespace {
 
-constexpr int kTcThreads = 320;
+constexpr int kTcThreads = 576;     // 8 detector warps, TMA warp, MMA warp, 8 appender warps
+constexpr int kTcRing = 3;          // hit blocks in flight between a detector warp and its appender warp
+constexpr int kTcBlockFloats = 32 * 32 + 32;  // one 32 x 32 key block [column][lane] + header
 constexpr int kTcStages = 4;
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
 constexpr size_t kTcSmemBytes = 1024 /*alignment slack*/ + 2 * kTcTileBytes + kTcStages * kTcTileBytes +
-                                8 * (kMaxP + 1) * sizeof(int2);
+                                8 * kTcRing * kTcBlockFloats * sizeof(float);
 
 // byte offset of 16-byte chunk c (0..7) of row r inside a K-major SWIZZLE_128B tile of 128-byte rows
 __host__ __device__ __forceinline__ uint32_t sw128_offset(int r, int c) {
@@ -49,6 +57,24 @@ __host__ __device__ __forceinline__ uint32_t sw128_offset(int r, int c) {
 // ---- PTX wrappers (tcgen05 / mbarrier) -------------------------------------------------------
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// Polling wait with a short sleep between polls: a dozen warps spinning on mbarrier.try_wait starve the
+// working warps of issue slots and shared-memory bandwidth (measured); only the MMA warp spins tightly.
+__device__ __forceinline__ void mbar_wait_sleep(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    for (;;) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (done) break;
+        __nanosleep(LIPFIT_TC_SLEEP_NS);
+    }
 }
 __device__ __forceinline__ void tc_fence_before() {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -287,14 +313,15 @@ __global__ void __launch_bounds__(kTcThreads, 1)
 knn_tc_select_kernel(const KnnTcArgs g) {
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t a_full, a_empty, b_full[kTcStages], b_empty[kTcStages], acc_full[2][2],
-        acc_empty[2][2];
+        acc_empty[2][2], r_full[8][kTcRing], r_empty[8][kTcRing];
+    __shared__ __align__(8) unsigned long long tau_s[8][32];  // (item << 32 | tau bits) published by the appenders
     __shared__ uint32_t s_tmem;
     // 1024-byte aligned carve-up (SWIZZLE_128B atoms are 1024 B)
     const uint32_t raw = smem_u32(smem_raw);
     unsigned char* base = smem_raw + ((1024u - (raw & 1023u)) & 1023u);
     unsigned char* sA = base;                                // 2 tiles
     unsigned char* sB = sA + 2 * kTcTileBytes;               // kTcStages tiles
-    int2* sC = reinterpret_cast<int2*>(sB + kTcStages * kTcTileBytes);  // 8 x [kMaxP + 1] compaction scratch
+    float* sR = reinterpret_cast<float*>(sB + kTcStages * kTcTileBytes);  // 8 rings of kTcRing hit blocks
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const KnnArgs& a = g.k;
@@ -308,7 +335,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         for (int h = 0; h < 2; ++h)
             for (int b = 0; b < 2; ++b) {
                 mbar_init(&acc_full[h][b], 1);
-                mbar_init(&acc_empty[h][b], 4);  // the 4 epilogue warps of the half
+                mbar_init(&acc_empty[h][b], 4);  // the 4 detector warps of the half
+            }
+        for (int w = 0; w < 8; ++w)
+            for (int r = 0; r < kTcRing; ++r) {
+                mbar_init(&r_full[w][r], 1);
+                mbar_init(&r_empty[w][r], 1);
             }
         mbar_fence_init();
     }
@@ -318,6 +350,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                      "r"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
+    if (threadIdx.x < 256) tau_s[threadIdx.x >> 5][threadIdx.x & 31] = 0xFFFFFFFF00000000ull;  // no item yet
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -348,12 +381,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
                 int qb, ch, tb, te;
                 decode(item, qb, ch, tb, te);
-                mbar_wait(&a_empty, (it & 1u) ^ 1u);
+                mbar_wait_sleep(&a_empty, (it & 1u) ^ 1u);
                 mbar_arrive_expect_tx(&a_full, 2 * kTcTileBytes);
                 bulk_g2s(sA, g.Aimg + static_cast<size_t>(qb) * 2 * kTcTileBytes, 2 * kTcTileBytes, &a_full);
                 for (int t = tb; t < te; ++t, ++gB) {
                     const uint32_t s = gB % kTcStages, u = gB / kTcStages;
-                    mbar_wait(&b_empty[s], (u & 1u) ^ 1u);
+                    mbar_wait_sleep(&b_empty[s], (u & 1u) ^ 1u);
                     mbar_arrive_expect_tx(&b_full[s], kTcTileBytes);
                     bulk_g2s(sB + s * kTcTileBytes, g.Bimg + static_cast<size_t>(t) * kTcTileBytes,
                              kTcTileBytes, &b_full[s]);
@@ -393,25 +426,43 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 tc_commit(&a_empty);
             }
         }
-    } else {
-        // ================= epilogue warps: h = query half, quad = TMEM lane quadrant =================
+    } else if (warp < 8) {
+        // ================= detector warps: h = query half, quad = TMEM lane quadrant =================
+        // They only FIND blocks of 32 x 32 keys that contain a key below some query's threshold and hand
+        // those blocks to their appender warp through a shared-memory ring, so the tensor pipe never waits
+        // for an append or a compaction (both are latency-bound: ~800 and ~6000 cycles per event).
         const int h = warp >> 2, quad = warp & 3;
-        int2* scr2 = sC + warp * (kMaxP + 1);
-        uint32_t gB = 0;
+        float* ring = sR + warp * kTcRing * kTcBlockFloats;
+        uint32_t gB = 0, nmsg = 0;
+        auto push = [&](const float (&v)[32], int kbase) {
+            const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+            mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
+            float* blk = ring + r * kTcBlockFloats;
+            if (kbase >= 0) {
+#pragma unroll
+                for (int c = 0; c < 32; ++c) blk[c * 32 + lane] = v[c];
+            }
+            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 32] = kbase;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&r_full[warp][r]);
+            ++nmsg;
+        };
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
             const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
             float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);  // real keys are far below 1e38
-            int fill = 0;
-            const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
-            int2* pool = a.pool + slot * a.P;
             for (int t = tb; t < te; ++t, ++gB) {
                 const uint32_t b = gB & 1u, ua = gB >> 1;
-                mbar_wait(&acc_full[h][b], ua & 1u);
+                {  // adopt the appender's latest threshold for this item (stale values only cost extra pushes)
+                    const unsigned long long ts = *reinterpret_cast<volatile unsigned long long*>(&tau_s[warp][lane]);
+                    if (static_cast<uint32_t>(ts >> 32) == static_cast<uint32_t>(item))
+                        tau = fminf(tau, __uint_as_float(static_cast<uint32_t>(ts)));
+                }
+                mbar_wait_sleep(&acc_full[h][b], ua & 1u);
                 tc_fence_after();
                 const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
-#pragma unroll 1  // ONE copy of the block code: the kernel must stay small enough for the instruction cache
+#pragma unroll 1
                 for (int cb = 0; cb < kTcBN / 32; ++cb) {
                     float v[32];
                     tc_ld32(trow + cb * 32, v);
@@ -428,10 +479,46 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (__any_sync(0xffffffffu, m < -1e30f)) tau = 0.f;
 #else
                     const float m = tc_min32(v);
-                    if (__any_sync(0xffffffffu, m < tau))  // rare after the first tiles
-                        tc_append32(a, v, t * kTcBN + cb * 32, tau, fill, pool, scr2, lane);
+                    if (__any_sync(0xffffffffu, m < tau)) push(v, t * kTcBN + cb * 32);
 #endif
                 }
+            }
+            float dummy[32];
+            push(dummy, -1);  // end of item: the appender writes fill / tau and moves on
+        }
+    } else {
+        // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
+        const int aw = warp - 10;  // paired detector warp
+        const int h = aw >> 2, quad = aw & 3;
+        const float* ring = sR + aw * kTcRing * kTcBlockFloats;
+        uint32_t nmsg = 0;
+        for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+            int qb, ch, tb, te;
+            decode(item, qb, ch, tb, te);
+            const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
+            float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);
+            int fill = 0;
+            const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
+            int2* pool = a.pool + slot * a.P;
+            for (;;) {
+                const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+                mbar_wait_sleep(&r_full[aw][r], u & 1u);
+                const float* blk = ring + r * kTcBlockFloats;
+                const int kbase = reinterpret_cast<const int*>(blk)[32 * 32];
+                float w[32];
+                if (kbase >= 0) {
+#pragma unroll
+                    for (int c = 0; c < 32; ++c) w[c] = blk[c * 32 + lane];
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&r_empty[aw][r]);
+                ++nmsg;
+                if (kbase < 0) break;
+                const float tau_before = tau;
+                tc_append32(a, w, kbase, tau, fill, pool, nullptr, lane);
+                if (__any_sync(0xffffffffu, tau != tau_before))  // a compaction lowered some threshold: publish
+                    tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
+                                      __float_as_uint(tau);
             }
 #if LIPFIT_TC_EXPERIMENT
             fill = 0;
