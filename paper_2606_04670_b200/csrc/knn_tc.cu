@@ -42,7 +42,7 @@ namespace {
 
 constexpr int kTcThreads = 576;     // 8 detector warps, TMA warp, MMA warp, 8 appender warps
 constexpr int kTcRing = 3;          // hit blocks in flight between a detector warp and its appender warp
-constexpr int kTcBlockFloats = 32 * 32 + 32;  // one 32 x 32 key block [column][lane] + header
+constexpr int kTcBlockFloats = 32 * 33 + 64;  // one 32 x 32 key block [query lane][33], 32 row minima, header
 constexpr int kTcStages = 4;
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
@@ -434,15 +434,16 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         const int h = warp >> 2, quad = warp & 3;
         float* ring = sR + warp * kTcRing * kTcBlockFloats;
         uint32_t gB = 0, nmsg = 0;
-        auto push = [&](const float (&v)[32], int kbase) {
+        auto push = [&](const float (&v)[32], float m, int kbase) {
             const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
             mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
             float* blk = ring + r * kTcBlockFloats;
             if (kbase >= 0) {
 #pragma unroll
-                for (int c = 0; c < 32; ++c) blk[c * 32 + lane] = v[c];
+                for (int c = 0; c < 32; ++c) blk[lane * 33 + c] = v[c];  // row = query lane, padded: conflict-free
+                blk[32 * 33 + lane] = m;                                 // the row's minimum
             }
-            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 32] = kbase;
+            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 33 + 32] = kbase;
             __syncwarp();
             if (lane == 0) mbar_arrive(&r_full[warp][r]);
             ++nmsg;
@@ -479,12 +480,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (__any_sync(0xffffffffu, m < -1e30f)) tau = 0.f;
 #else
                     const float m = tc_min32(v);
-                    if (__any_sync(0xffffffffu, m < tau)) push(v, t * kTcBN + cb * 32);
+                    if (__any_sync(0xffffffffu, m < tau)) push(v, m, t * kTcBN + cb * 32);
 #endif
                 }
             }
             float dummy[32];
-            push(dummy, -1);  // end of item: the appender writes fill / tau and moves on
+            push(dummy, 0.f, -1);  // end of item: the appender writes fill / tau and moves on
         }
     } else {
         // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
@@ -504,19 +505,41 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
                 mbar_wait_sleep(&r_full[aw][r], u & 1u);
                 const float* blk = ring + r * kTcBlockFloats;
-                const int kbase = reinterpret_cast<const int*>(blk)[32 * 32];
-                float w[32];
-                if (kbase >= 0) {
-#pragma unroll
-                    for (int c = 0; c < 32; ++c) w[c] = blk[c * 32 + lane];
+                const int kbase = reinterpret_cast<const int*>(blk)[32 * 33 + 32];
+                if (kbase < 0) {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&r_empty[aw][r]);
+                    ++nmsg;
+                    break;
+                }
+                // Rows (queries) of the block that still have a key below the CURRENT threshold; each such
+                // row is scanned by the whole warp (lane = column): ~20 instructions per row instead of a
+                // 32-column predicated pass by every lane.
+                unsigned hm = __ballot_sync(0xffffffffu, blk[32 * 33 + lane] < tau);
+                bool lowered = false;
+                while (hm) {
+                    const int L = __ffs(hm) - 1;
+                    hm &= hm - 1;
+                    float tauL = __shfl_sync(0xffffffffu, tau, L);
+                    int fillL = __shfl_sync(0xffffffffu, fill, L);
+                    int2* poolL = pool + static_cast<ptrdiff_t>(L - lane) * a.P;  // consecutive lanes = consecutive slots
+                    if (fillL > a.P - 32) {  // fewer than 32 free entries: compact (warp-cooperative radix select)
+                        __syncwarp();
+                        tauL = knn_compact(poolL, fillL, a.ksel, nullptr, lane);
+                        fillL = a.ksel;
+                        lowered = true;
+                        if (lane == L) tau = tauL;
+                    }
+                    const float val = blk[L * 33 + lane];
+                    const bool hit = val < tauL;
+                    const unsigned bm = __ballot_sync(0xffffffffu, hit);
+                    if (hit) poolL[fillL + __popc(bm & ((1u << lane) - 1u))] = make_int2(__float_as_int(val), kbase + lane);
+                    if (lane == L) fill = fillL + __popc(bm);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&r_empty[aw][r]);
                 ++nmsg;
-                if (kbase < 0) break;
-                const float tau_before = tau;
-                tc_append32(a, w, kbase, tau, fill, pool, nullptr, lane);
-                if (__any_sync(0xffffffffu, tau != tau_before))  // a compaction lowered some threshold: publish
+                if (lowered)  // a compaction lowered some threshold: publish for the detector
                     tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
                                       __float_as_uint(tau);
             }
