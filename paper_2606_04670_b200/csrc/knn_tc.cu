@@ -463,16 +463,9 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 mbar_wait_sleep(&acc_full[h][b], ua & 1u);
                 tc_fence_after();
                 const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
-#pragma unroll 1
-                for (int cb = 0; cb < kTcBN / 32; ++cb) {
-                    float v[32];
-                    tc_ld32(trow + cb * 32, v);
-                    tc_ld_wait();
-                    if (cb == kTcBN / 32 - 1) {  // last block is in registers: hand the TMEM stage back
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-                    }
+                // Software pipeline over the four 32-column blocks: the TMEM load of block cb+1 is in flight
+                // while block cb is reduced / pushed (two register buffers).
+                auto process = [&](const float (&v)[32], int cb) {
 #if LIPFIT_TC_EXPERIMENT == 1  // timing experiment: accumulators are read and dropped
                     if (v[0] == 12345.f && v[31] == 1.f) tau = 0.f;
 #elif LIPFIT_TC_EXPERIMENT == 2  // timing experiment: fast path only
@@ -482,7 +475,23 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const float m = tc_min32(v);
                     if (__any_sync(0xffffffffu, m < tau)) push(v, m, t * kTcBN + cb * 32);
 #endif
-                }
+                };
+                float va[32], vb[32];
+                tc_ld32(trow, va);
+                tc_ld_wait();
+                tc_ld32(trow + 32, vb);
+                process(va, 0);
+                tc_ld_wait();
+                tc_ld32(trow + 64, va);
+                process(vb, 1);
+                tc_ld_wait();
+                tc_ld32(trow + 96, vb);
+                process(va, 2);
+                tc_ld_wait();
+                tc_fence_before();  // all four blocks are in registers: hand the TMEM stage back
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+                process(vb, 3);
             }
             float dummy[32];
             push(dummy, 0.f, -1);  // end of item: the appender writes fill / tau and moves on
