@@ -101,7 +101,7 @@ int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const fl
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
-    RecLayout lay = bounds_layout(xf, norm);
+    RecLayout lay = bounds_layout(c, xf, norm, Q);
     if (lay.rf == 0) return LIPFIT_E_PARAM;
     const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
     Workspace rec;

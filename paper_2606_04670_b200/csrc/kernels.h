@@ -18,8 +18,10 @@ struct RecLayout {
     int rf, vslot;
     int cslot = -1;       // >= 0: slot of c' = 2 value - sum of the constrained coordinates (folded L1 bounds)
     bool mscale = false;  // true: the kernel family wants the coordinates pre-multiplied by M
+    bool dup = false;     // true: every float is stored twice (x0,x0,x1,x1,..): operands of packed f32x2 math;
+                          //       rf then counts the PHYSICAL floats, vslot / cslot stay logical
 };
-RecLayout bounds_layout(const Xform& xf, int norm);
+RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
 RecLayout smooth_layout(const Xform& xf, int norm);
 
 // a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].

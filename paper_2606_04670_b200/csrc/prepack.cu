@@ -142,6 +142,33 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
     }
 }
 
+// Duplicated layout for the packed-f32x2 kernels: logical record [x'_0..x'_{d-1}, value, c', 0..] of rf/2
+// floats, each stored twice, so that an LDS.128 yields two (x, x) register pairs ready for FADD2.
+__global__ void __launch_bounds__(256)
+prepack_dup_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xf, int rf, int vslot,
+                   int cslot, float* __restrict__ rec) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const float* src = X + static_cast<size_t>(k) * xf.d;
+    float* dst = rec + static_cast<size_t>(k) * rf;
+    const float v = y ? y[k] : 0.f;
+    float cval = 0.f;
+    if (cslot >= 0) {
+        float sc = 0.f;
+        for (int j = xf.dU; j < xf.d; ++j) sc += xf.sw[j] * src[xf.perm[j]];
+        cval = 2.f * v - sc;
+    }
+    for (int j0 = 0; j0 < rf / 2; j0 += 2) {
+        float t[2];
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            int j = j0 + c;
+            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : (j == cslot ? cval : 0.f));
+        }
+        *reinterpret_cast<float4*>(dst + 2 * j0) = make_float4(t[0], t[0], t[1], t[1]);
+    }
+}
+
 __global__ void __launch_bounds__(256)
 set_values_kernel(float* __restrict__ rec, int rf, int vslot, const float* __restrict__ y,
                   const float* __restrict__ eps, int N) {
@@ -159,6 +186,12 @@ axpy_kernel(float* __restrict__ y, const float* __restrict__ eps, int N) {
 int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
                    const Xform& xf, RecLayout lay, float* rec) {
     int n = static_cast<int>(N);
+    if (lay.dup) {
+        prepack_dup_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, n, xf, lay.rf, lay.vslot, lay.cslot, rec);
+        ++g_launches;
+        LIPFIT_CUDA(cudaGetLastError());
+        return LIPFIT_OK;
+    }
     prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, lay.cslot, rec);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
