@@ -235,11 +235,74 @@ __device__ __forceinline__ float2 sub2(float2 a, float2 b) {  // a - b, one FADD
     return __fadd2_rn(a, make_float2(-b.x, -b.y));
 }
 
-template <int DU, int DC, int RP, int THREADS, int MINB>
+// Packed policies: D coordinates, RFL logical floats per record, pair2() -> both candidates of both queries,
+// query_term2() -> per-query constants added to the lower bounds after the running maximum.
+template <int DU, int DC>
+struct PackedFoldL1 {
+    static constexpr int D = DU + DC;
+    static constexpr int RFL = record_floats(D + 1);
+    static __device__ __forceinline__ void pair2(const float2* qq, const float2* x, float2& hi, float2& lo) {
+        float2 acc = x[D];  // (y, y)
+#pragma unroll
+        for (int j = 0; j < DU; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            acc.x += fabsf(dlt.x);
+            acc.y += fabsf(dlt.y);
+        }
+#pragma unroll
+        for (int j = DU; j < D; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            acc = __fadd2_rn(acc, make_float2(fmaxf(dlt.x, 0.f), fmaxf(dlt.y, 0.f)));
+        }
+        hi = acc;
+        lo = sub2(x[D + 1], acc);  // c' - hi
+    }
+    static __device__ __forceinline__ float2 query_term2(const float2* qq) {
+        float2 sq = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = DU; j < D; ++j) {
+            sq.x += qq[j].x;
+            sq.y += qq[j].y;
+        }
+        return sq;
+    }
+};
+
+// Weighted Linf with the coordinates pre-multiplied by M: the subtractions and the two final additions are
+// FADD2, the maxima stay scalar (|.| and negation are free modifiers of FMNMX / FMNMX3):
+//   s = max_free |delta_j|,  hi = y + max(s, delta_c..),  lo = y - max(s, -delta_c..).
+template <int DU, int DC>
+struct PackedLinf {
+    static constexpr int D = DU + DC;
+    static constexpr int RFL = record_floats(D);
+    static __device__ __forceinline__ void pair2(const float2* qq, const float2* x, float2& hi, float2& lo) {
+        float2 sm = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < DU; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            sm.x = fmaxf(sm.x, fabsf(dlt.x));
+            sm.y = fmaxf(sm.y, fabsf(dlt.y));
+        }
+        float2 pu = sm, pl = sm;
+#pragma unroll
+        for (int j = DU; j < D; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            pu.x = fmaxf(pu.x, dlt.x);  // s >= 0 already: max(s, relu(d)) == max(s, d)
+            pu.y = fmaxf(pu.y, dlt.y);
+            pl.x = fmaxf(pl.x, -dlt.x);
+            pl.y = fmaxf(pl.y, -dlt.y);
+        }
+        hi = __fadd2_rn(x[D], pu);
+        lo = sub2(x[D], pl);
+    }
+    static __device__ __forceinline__ float2 query_term2(const float2*) { return make_float2(0.f, 0.f); }
+};
+
+template <class P2, int RP, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
-bounds_fold2_kernel(const BoundsArgs a) {
-    constexpr int D = DU + DC;
-    constexpr int RFL = record_floats(D + 1);  // logical floats per record
+bounds_packed_kernel(const BoundsArgs a) {
+    constexpr int D = P2::D;
+    constexpr int RFL = P2::RFL;               // logical floats per record
     constexpr int RF = 2 * RFL;                // physical (duplicated)
     constexpr int TILE = tile_records<RF>();
     constexpr int R = 2 * RP;
@@ -274,22 +337,6 @@ bounds_fold2_kernel(const BoundsArgs a) {
         const int begin = ch * a.chunk;
         const int end = min(a.N, begin + a.chunk);
         RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
-        auto pair2 = [&](const float2* qq, const float2* x, float2& hi, float2& lo) {
-            float2 acc = x[D];  // (y, y)
-#pragma unroll
-            for (int j = 0; j < DU; ++j) {
-                const float2 dlt = sub2(qq[j], x[j]);
-                acc.x += fabsf(dlt.x);
-                acc.y += fabsf(dlt.y);
-            }
-#pragma unroll
-            for (int j = DU; j < D; ++j) {
-                const float2 dlt = sub2(qq[j], x[j]);
-                acc = __fadd2_rn(acc, make_float2(fmaxf(dlt.x, 0.f), fmaxf(dlt.y, 0.f)));
-            }
-            hi = acc;
-            lo = sub2(x[D + 1], acc);  // c' - hi
-        };
         for (int t = 0; t < rs.ntiles; ++t) {
             const float* s = rs.acquire(t);
             const int n = rs.count(t);
@@ -308,8 +355,8 @@ bounds_fold2_kernel(const BoundsArgs a) {
 #pragma unroll
                 for (int rp = 0; rp < RP; ++rp) {
                     float2 hia, loa, hib, lob;
-                    pair2(q[rp], xa, hia, loa);
-                    pair2(q[rp], xb, hib, lob);
+                    P2::pair2(q[rp], xa, hia, loa);
+                    P2::pair2(q[rp], xb, hib, lob);
                     U[rp].x = fminf(fminf(U[rp].x, hia.x), hib.x);  // FMNMX3
                     U[rp].y = fminf(fminf(U[rp].y, hia.y), hib.y);
                     L[rp].x = fmaxf(fmaxf(L[rp].x, loa.x), lob.x);
@@ -327,7 +374,7 @@ bounds_fold2_kernel(const BoundsArgs a) {
 #pragma unroll
                 for (int rp = 0; rp < RP; ++rp) {
                     float2 hia, loa;
-                    pair2(q[rp], xa, hia, loa);
+                    P2::pair2(q[rp], xa, hia, loa);
                     U[rp].x = fminf(U[rp].x, hia.x);
                     U[rp].y = fminf(U[rp].y, hia.y);
                     L[rp].x = fmaxf(L[rp].x, loa.x);
@@ -338,13 +385,8 @@ bounds_fold2_kernel(const BoundsArgs a) {
         }
 #pragma unroll
         for (int rp = 0; rp < RP; ++rp) {
-            float sq0 = 0.f, sq1 = 0.f;  // the per-query constant of the folded lower bound
-#pragma unroll
-            for (int j = DU; j < D; ++j) {
-                sq0 += q[rp][j].x;
-                sq1 += q[rp][j].y;
-            }
-            const float Uv[2] = {U[rp].x, U[rp].y}, Lv[2] = {L[rp].x + sq0, L[rp].y + sq1};
+            const float2 sq = P2::query_term2(q[rp]);  // the per-query constant of the folded lower bound
+            const float Uv[2] = {U[rp].x, U[rp].y}, Lv[2] = {L[rp].x + sq.x, L[rp].y + sq.y};
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int qi = (qb * R + 2 * rp + e) * THREADS + static_cast<int>(threadIdx.x);
@@ -444,18 +486,16 @@ int launch_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     return launch_one<Core, 1, 128, 4>(c, a, ff);
 }
 
-template <int DU, int DC>
-int launch_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
-    using Core = FoldL1Core<DU, DC>;
-    if (flavour != 0) return launch_one<Core, 1, 128, 4>(c, a, ff);  // small Q: one query per thread, plain records
-    // throughput flavour: packed f32x2 kernel on duplicated records (the layout says which one was packed)
-    constexpr int RP = 4, THREADS = 128, R = 2 * RP;
-    auto kern = bounds_fold2_kernel<DU, DC, RP, THREADS, 2>;
+// throughput flavour of the packed f32x2 kernels: duplicated records (the layout says so)
+template <class P2, int RP>
+int launch_packed(const Ctx& c, BoundsArgs& a) {
+    constexpr int THREADS = 128, R = 2 * RP;
+    auto kern = bounds_packed_kernel<P2, RP, THREADS, 2>;
     int occ = 0;
     LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
-    constexpr int TILE = tile_records<2 * Core::RF>();
+    constexpr int TILE = tile_records<2 * P2::RFL>();
     a.nqb = (a.Q + THREADS * R - 1) / (THREADS * R);
     int want = (16 * slots + a.nqb - 1) / a.nqb;
     int max_ch = (a.N + 4 * TILE - 1) / (4 * TILE);
@@ -490,6 +530,22 @@ int launch_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     return LIPFIT_OK;
 }
 
+template <int DU, int DC>
+int launch_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    if (flavour != 0) return launch_one<FoldL1Core<DU, DC>, 1, 128, 4>(c, a, ff);  // small Q: plain records
+    return launch_packed<PackedFoldL1<DU, DC>, 4>(c, a);
+}
+
+// Linf with M folded into the coordinates (records [M x', y]): SpecCore<3,..> with M = 1 for small Q
+template <int DU, int DC>
+int launch_linf(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    if (flavour != 0) {
+        a.M = 1.f;
+        return launch_one<SpecCore<3, DU, DC>, 1, 128, 4>(c, a, ff);
+    }
+    return launch_packed<PackedLinf<DU, DC>, 4>(c, a);
+}
+
 template <int NORM, int DP>
 int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     using Core = GenCore<NORM, DP>;
@@ -501,7 +557,9 @@ int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
 #define SPEC(NORM, DU, DC, NAME) \
     { NORM, DU, DC, NAME, {record_floats(DU + DC), DU + DC}, &launch_spec<NORM, DU, DC> }
 #define FOLD(DU, DC, NAME) \
-    { 1, DU, DC, NAME, {record_floats(DU + DC + 1), DU + DC, DU + DC + 1, true}, &launch_fold<DU, DC> }
+    { 1, DU, DC, NAME, {record_floats(DU + DC + 1), DU + DC, DU + DC + 1, true, false, true}, &launch_fold<DU, DC> }
+#define LINF2(DU, DC, NAME) \
+    { 3, DU, DC, NAME, {record_floats(DU + DC), DU + DC, -1, true, false, true}, &launch_linf<DU, DC> }
 #define GEN(NORM, DP, NAME) \
     { NORM, DP, -1, NAME, {DP + 4, DP}, &launch_gen<NORM, DP> }
 
@@ -509,7 +567,7 @@ const Variant kVariants[] = {
     // shapes of BASELINE.json configs 1, 2, 3, 5 (+ the symmetric versions of the same dims)
     SPEC(2, 2, 0, "bounds<L2,U2,C0>"),
     FOLD(2, 2, "bounds<L1,U2,C2,folded>"),
-    SPEC(3, 7, 1, "bounds<Linf,U7,C1>"),
+    LINF2(7, 1, "bounds<Linf,U7,C1,packed>"),
     SPEC(2, 0, 5, "bounds<L2,U0,C5>"),
     SPEC(2, 3, 0, "bounds<L2,U3,C0>"),
     SPEC(2, 0, 3, "bounds<L2,U0,C3>"),
@@ -547,7 +605,7 @@ RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q) {
     const Variant* v = pick(xf, norm);
     if (!v) return RecLayout{0, 0};
     RecLayout lay = v->lay;
-    if (lay.cslot >= 0 && bounds_flavour(c, Q) == 0) {  // folded L1, throughput flavour: packed kernel, duplicated records
+    if (lay.packed && bounds_flavour(c, Q) == 0) {  // throughput flavour of a packed variant: duplicated records
         lay.rf *= 2;
         lay.dup = true;
     }

@@ -20,6 +20,7 @@ struct RecLayout {
     bool mscale = false;  // true: the kernel family wants the coordinates pre-multiplied by M
     bool dup = false;     // true: every float is stored twice (x0,x0,x1,x1,..): operands of packed f32x2 math;
                           //       rf then counts the PHYSICAL floats, vslot / cslot stay logical
+    bool packed = false;  // the variant has a packed-f32x2 throughput kernel (bounds_layout sets dup when it is used)
 };
 RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
 RecLayout smooth_layout(const Xform& xf, int norm);
