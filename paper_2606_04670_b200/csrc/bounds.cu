@@ -298,6 +298,40 @@ struct PackedLinf {
     static __device__ __forceinline__ float2 query_term2(const float2*) { return make_float2(0.f, 0.f); }
 };
 
+// Weighted L2 with the coordinates pre-multiplied by M: subtractions and squared accumulations are
+// FADD2 / FFMA2, the positive / negative parts stay scalar FMNMX, one MUFU.SQRT per bound and query.
+template <int DU, int DC>
+struct PackedL2 {
+    static constexpr int D = DU + DC;
+    static constexpr int RFL = record_floats(D);
+    static __device__ __forceinline__ void pair2(const float2* qq, const float2* x, float2& hi, float2& lo) {
+        float2 sm = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int j = 0; j < DU; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            sm = __ffma2_rn(dlt, dlt, sm);
+        }
+        if (DC == 0) {  // symmetric: both bounds share the distance
+            const float2 dist = make_float2(fast_sqrt(sm.x), fast_sqrt(sm.y));
+            hi = __fadd2_rn(x[D], dist);
+            lo = sub2(x[D], dist);
+            return;
+        }
+        float2 pu = sm, pl = sm;
+#pragma unroll
+        for (int j = DU; j < D; ++j) {
+            const float2 dlt = sub2(qq[j], x[j]);
+            const float2 r = make_float2(fmaxf(dlt.x, 0.f), fmaxf(dlt.y, 0.f));
+            const float2 m = make_float2(fminf(dlt.x, 0.f), fminf(dlt.y, 0.f));
+            pu = __ffma2_rn(r, r, pu);
+            pl = __ffma2_rn(m, m, pl);
+        }
+        hi = __fadd2_rn(x[D], make_float2(fast_sqrt(pu.x), fast_sqrt(pu.y)));
+        lo = sub2(x[D], make_float2(fast_sqrt(pl.x), fast_sqrt(pl.y)));
+    }
+    static __device__ __forceinline__ float2 query_term2(const float2*) { return make_float2(0.f, 0.f); }
+};
+
 template <class P2, int RP, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 bounds_packed_kernel(const BoundsArgs a) {
@@ -536,6 +570,16 @@ int launch_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     return launch_packed<PackedFoldL1<DU, DC>, 4>(c, a);
 }
 
+// L2 with M folded into the coordinates: SpecCore<2,..> with M = 1 for small Q
+template <int DU, int DC>
+int launch_l2p(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
+    if (flavour != 0) {
+        a.M = 1.f;
+        return launch_one<SpecCore<2, DU, DC>, 1, 128, 4>(c, a, ff);
+    }
+    return launch_packed<PackedL2<DU, DC>, 4>(c, a);
+}
+
 // Linf with M folded into the coordinates (records [M x', y]): SpecCore<3,..> with M = 1 for small Q
 template <int DU, int DC>
 int launch_linf(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
@@ -560,6 +604,8 @@ int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     { 1, DU, DC, NAME, {record_floats(DU + DC + 1), DU + DC, DU + DC + 1, true, false, true}, &launch_fold<DU, DC> }
 #define LINF2(DU, DC, NAME) \
     { 3, DU, DC, NAME, {record_floats(DU + DC), DU + DC, -1, true, false, true}, &launch_linf<DU, DC> }
+#define L2P(DU, DC, NAME) \
+    { 2, DU, DC, NAME, {record_floats(DU + DC), DU + DC, -1, true, false, true}, &launch_l2p<DU, DC> }
 #define GEN(NORM, DP, NAME) \
     { NORM, DP, -1, NAME, {DP + 4, DP}, &launch_gen<NORM, DP> }
 
@@ -568,7 +614,7 @@ const Variant kVariants[] = {
     SPEC(2, 2, 0, "bounds<L2,U2,C0>"),
     FOLD(2, 2, "bounds<L1,U2,C2,folded>"),
     LINF2(7, 1, "bounds<Linf,U7,C1,packed>"),
-    SPEC(2, 0, 5, "bounds<L2,U0,C5>"),
+    L2P(0, 5, "bounds<L2,U0,C5,packed>"),
     SPEC(2, 3, 0, "bounds<L2,U3,C0>"),
     SPEC(2, 0, 3, "bounds<L2,U0,C3>"),
     SPEC(1, 4, 0, "bounds<L1,U4,C0>"),

@@ -34,8 +34,8 @@ def test_status_strings_and_variant_names():
     assert L.bounds_variant(2, None, L2) == "bounds<L2,U2,C0>"
     assert L.bounds_variant(4, [1, 1, 0, 0], L1) == "bounds<L1,U2,C2,folded>"
     assert L.bounds_variant(8, [1] + [0] * 7, LINF) == "bounds<Linf,U7,C1,packed>"
-    assert L.bounds_variant(5, [1] * 5, L2) == "bounds<L2,U0,C5>"
-    assert L.bounds_variant(5, [-1] * 5, L2) == "bounds<L2,U0,C5>"     # mirrored coordinates (R2)
+    assert L.bounds_variant(5, [1] * 5, L2) == "bounds<L2,U0,C5,packed>"
+    assert L.bounds_variant(5, [-1] * 5, L2) == "bounds<L2,U0,C5,packed>"     # mirrored coordinates (R2)
     assert L.bounds_variant(9, None, L1).startswith("bounds_generic<L1,DP16")
     with pytest.raises(L.LipfitError):
         L.bounds_variant(33, None, L2)
