@@ -468,7 +468,7 @@ template <class Core, int R, int THREADS, int MINB>
 int launch_one(const Ctx& c, BoundsArgs& a, const FreeFlags& ff) {
     auto kern = bounds_kernel<Core, R, THREADS, MINB>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, THREADS, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     constexpr int TILE = tile_records<Core::RF>();
@@ -526,7 +526,7 @@ int launch_packed(const Ctx& c, BoundsArgs& a) {
     constexpr int THREADS = 128, R = 2 * RP;
     auto kern = bounds_packed_kernel<P2, RP, THREADS, 2>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, THREADS, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, THREADS, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     constexpr int TILE = tile_records<2 * P2::RFL>();
@@ -790,7 +790,7 @@ int launch_topk(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeig
     constexpr int R = DP <= 8 ? 2 : 1;
     auto kern = bounds_topk_kernel<NORM, DP, R>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 128, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, 128, 0));
     if (occ < 1) occ = 1;
     a.nqb = (a.Q + 128 * R - 1) / (128 * R);
     const int slots = c.num_sms * occ;

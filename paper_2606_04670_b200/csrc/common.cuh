@@ -52,6 +52,14 @@ struct Ctx {
 
 int make_ctx(void* cuda_stream, Ctx* ctx);  // LIPFIT_OK or LIPFIT_E_CUDA
 
+// cudaOccupancyMaxActiveBlocksPerMultiprocessor, cached per (kernel, block size, dynamic smem): the query costs
+// microseconds, which is the whole budget of the latency-bound calls (config 1).
+cudaError_t occupancy_cached(const void* func, int threads, size_t smem, int* occ);
+template <class K>
+inline cudaError_t occupancy_of(int* occ, K kern, int threads, size_t smem) {
+    return occupancy_cached(reinterpret_cast<const void*>(kern), threads, smem, occ);
+}
+
 inline int cuda_rc(cudaError_t e) {
     if (e == cudaSuccess) return LIPFIT_OK;
     return (e == cudaErrorMemoryAllocation) ? LIPFIT_E_NOMEM : LIPFIT_E_CUDA;

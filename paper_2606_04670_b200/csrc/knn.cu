@@ -568,7 +568,7 @@ int launch_select(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int slots_hint,
                                      static_cast<int>(smem)));
     if (query_only) {  // occupancy query used by the host to size the decomposition
         int occ = 0;
-        LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSelThreads, smem));
+        LIPFIT_CUDA(occupancy_of(&occ, kern, kSelThreads, smem));
         return occ < 1 ? 1 : occ;
     }
     long long ntiles = static_cast<long long>(a.nfull) + static_cast<long long>(a.ntail) * a.T;

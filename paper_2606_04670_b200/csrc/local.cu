@@ -298,7 +298,7 @@ int launch_table(const Ctx& c, TableArgs& a, const Knots& kn) {
     constexpr int R = local_r(DP);
     auto kern = local_table_kernel<NORM, DP, R>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLocThreads, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     local_schedule(a.N, kLocThreads * R, a.N, local_tile_records<DP + 4>(), slots, &a.nrb, &a.nch, &a.chunk);
@@ -316,7 +316,7 @@ int launch_eval(const Ctx& c, EvalArgs& a, const Knots& kn) {
     constexpr int R = local_r(DP);
     auto kern = local_eval_kernel<NORM, DP, R>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kLocThreads, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     local_schedule(a.Q, kLocThreads * R, a.N, local_tile_records<DP + 4 + kJ>(), slots, &a.nqb, &a.nch, &a.chunk);

@@ -3,6 +3,7 @@
 // ("a suitable modification to distance calculation, which avoids branching").
 // Pure streaming kernels (HBM-bound, microseconds).
 #include <cmath>
+#include <map>
 #include <mutex>
 
 #include "kernels.h"
@@ -62,11 +63,50 @@ int make_ctx(void* cuda_stream, Ctx* ctx) {
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     int dev = 0;
     LIPFIT_CUDA(cudaGetDevice(&dev));
-    int sms = 0;
-    LIPFIT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    static std::atomic<int> sm_cache[64];  // SM count per device ordinal (0 = not asked yet)
+    int sms = (dev >= 0 && dev < 64) ? sm_cache[dev].load() : 0;
+    if (sms == 0) {
+        LIPFIT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (dev >= 0 && dev < 64) sm_cache[dev].store(sms);
+    }
     ctx->device = dev;
     ctx->num_sms = sms;
     return LIPFIT_OK;
+}
+
+cudaError_t occupancy_cached(const void* func, int threads, size_t smem, int* occ) {
+    struct Key {
+        const void* f;
+        int t;
+        size_t s;
+        int dev;
+        bool operator<(const Key& o) const {
+            if (f != o.f) return f < o.f;
+            if (t != o.t) return t < o.t;
+            if (s != o.s) return s < o.s;
+            return dev < o.dev;
+        }
+    };
+    static std::mutex mu;
+    static std::map<Key, int> cache;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const Key k{func, threads, smem, dev};
+    {
+        std::lock_guard<std::mutex> lk(mu);
+        auto it = cache.find(k);
+        if (it != cache.end()) {
+            *occ = it->second;
+            return cudaSuccess;
+        }
+    }
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, func, threads, smem);
+    if (e == cudaSuccess) {
+        std::lock_guard<std::mutex> lk(mu);
+        cache[k] = *occ;
+    }
+    return e;
 }
 
 int make_xform(int32_t d, const int32_t* mono_mask, const float* weights, bool symmetric, bool flip,

@@ -574,7 +574,7 @@ template <class Acc, int R, int MODE>
 int launch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff) {
     auto kern = smooth_pairs_kernel<Acc, R, MODE>;
     int occ = 0;
-    LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSmThreads, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, kSmThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
     const int grid = a.nitems < slots ? a.nitems : slots;
@@ -704,7 +704,7 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
     if (packed) {
         auto kern = smooth_pairs_packed_kernel<5>;
         int occ = 0;
-        LIPFIT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kSmThreads, 0));
+        LIPFIT_CUDA(occupancy_of(&occ, kern, kSmThreads, 0));
         if (occ < 1) occ = 1;
         const int slots = c.num_sms * occ;
         KernelTimer kt(TK_SMOOTH_PAIRS, c.stream);
