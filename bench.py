@@ -450,6 +450,22 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
         out.update({k: r[k] for k in ("ms_per_step", "ms_min", "value", "kernel", "kernel_ms")})
         out["unit"] = UNIT
         out["roofline"] = _roofline(r["pairs"], LANE_OPS[c], r["kernel_ms"], sms, peaks)
+        if c == 1:
+            # latency-bound config: an isolated, L2-flushed step exposes the host launch latency; also report the
+            # steady state of back-to-back calls (inputs stay in L2; 200 calls between two events)
+            t = lambda a: torch.from_numpy(a).to(dev)
+            X, y, Xq = t(wl.X), t(wl.y), t(wl.Xq)
+            for _ in range(20):
+                L.lipfit_bounds(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(200):
+                L.lipfit_bounds(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
+            e1.record()
+            e1.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / 200
+            out["back_to_back"] = {"us_per_step": us, "value": r["pairs"] / (us * 1e-6) / 1e9, "unit": UNIT,
+                                   "note": "200 consecutive lipfit_bounds calls, no L2 flush"}
         if not args.no_cpu:
             rate, sample, cores, sel, ref = oracle_sample_rate(wl, 8.0)
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "sample": sample}
