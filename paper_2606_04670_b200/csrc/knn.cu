@@ -431,7 +431,9 @@ knn_rerank_kernel(const RerankArgs a) {
         myrank[s] = rank;
     }
     __syncwarp();
-    const double kth = skth[warp];
+    // fewer than k candidates cannot happen by construction (seeded thresholds keep >= ksel data below
+    // them); if it ever did, the query goes to the exact fallback with an unbounded candidate set
+    const double kth = total >= a.k ? skth[warp] : static_cast<double>(__int_as_float(0x7f800000));
     if (all_in || kth < lb) {
 #pragma unroll
         for (int s = 0; s < kMaxCand / 32; ++s) {

@@ -30,6 +30,27 @@ __host__ __device__ __forceinline__ size_t knn_pool_slot(int qslot, int c, int Q
                   : static_cast<size_t>(Qp) + static_cast<size_t>(c - 1) * Qtp + (qslot - nfullq);
 }
 
+// The rank-th smallest (1-based) of the 32 NE order-preserving integer keys a warp holds (NE per lane),
+// found bit by bit with warp votes; `need` = how many of the keys equal to it belong to the rank
+// smallest.  All 32 lanes must call it.
+template <int NE>
+__device__ __forceinline__ uint32_t knn_rank_select(const uint32_t (&key)[NE], int rank, int& need) {
+    uint32_t prefix = 0;
+    need = rank;  // rank still wanted among the keys that agree with `prefix` on the decided bits
+#pragma unroll 1
+    for (int bit = 31; bit >= 0; --bit) {
+        int cnt0 = 0;  // keys that agree with prefix above `bit` and have a 0 at `bit`
+#pragma unroll
+        for (int i = 0; i < NE; ++i)
+            cnt0 += __popc(__ballot_sync(0xffffffffu, ((key[i] ^ prefix) >> bit) == 0u));
+        if (need > cnt0) {
+            need -= cnt0;
+            prefix |= 1u << bit;
+        }
+    }
+    return prefix;
+}
+
 // Warp-cooperative compaction of one pool of n entries: keeps exactly the ksel entries with the
 // smallest keys in slots [0, ksel) (unordered; the re-rank sorts) and returns the ksel-th smallest key
 // (the new tau).  Register-resident radix select: every lane holds NE entries (n <= 32 NE), the
@@ -46,19 +67,8 @@ __device__ __forceinline__ float knn_compact_regs(int2* pool, int n, int ksel, i
         e[i] = c < n ? pool[c] : make_int2(0, 0);
         key[i] = c < n ? f2key(__int_as_float(e[i].x)) : 0xFFFFFFFFu;  // padding sorts last
     }
-    uint32_t prefix = 0;
-    int need = ksel;  // rank still wanted among the keys that agree with `prefix` on the decided bits
-#pragma unroll 1
-    for (int bit = 31; bit >= 0; --bit) {
-        int cnt0 = 0;  // keys that agree with prefix above `bit` and have a 0 at `bit`
-#pragma unroll
-        for (int i = 0; i < NE; ++i)
-            cnt0 += __popc(__ballot_sync(0xffffffffu, ((key[i] ^ prefix) >> bit) == 0u));
-        if (need > cnt0) {
-            need -= cnt0;
-            prefix |= 1u << bit;
-        }
-    }
+    int need;
+    const uint32_t prefix = knn_rank_select<NE>(key, ksel, need);
     // prefix = the ksel-th smallest key; `need` of the entries equal to it are kept
     const unsigned below = (1u << lane) - 1u;
     int base = 0, eqbase = 0;

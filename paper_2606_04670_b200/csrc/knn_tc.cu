@@ -35,6 +35,18 @@
 #ifndef LIPFIT_TC_EXPERIMENT
 #define LIPFIT_TC_EXPERIMENT 0  // 1, 2: timing experiments with invalid results (never in a product build)
 #endif
+#ifndef LIPFIT_TC_COUNT
+#define LIPFIT_TC_COUNT 0  // 1: CTA 0 prints per-warp event counts and wait cycles (diagnostic builds only)
+#endif
+#if LIPFIT_TC_COUNT
+#include <cstdio>
+#define TC_CLK(x) x
+#else
+#define TC_CLK(x)
+#endif
+#ifndef LIPFIT_TC_GROUP_A
+#define LIPFIT_TC_GROUP_A 4  // tiles per seeding minimum (see kTcTilesA)
+#endif
 
 namespace lipfit {
 
@@ -44,6 +56,19 @@ constexpr int kTcThreads = 576;     // 8 detector warps, TMA warp, MMA warp, 8 a
 constexpr int kTcRing = 3;          // hit blocks in flight between a detector warp and its appender warp
 constexpr int kTcBlockFloats = 32 * 33 + 64;  // one 32 x 32 key block [query lane][33], 32 row minima, header
 constexpr int kTcStages = 4;
+// Threshold seeding (phase A of a work item): the first kTcTilesA B tiles are multiplied once more up
+// front; the detectors only take the minimum key of every group of kTcGroupA tiles per query, 32 * kTcRing
+// minima in all, and the appender sets the query's starting threshold to the ksel-th smallest of them
+// (each minimum is the key of a different datum, so at least ksel data lie at or below it).  Without it
+// the first ~1 % of the tiles of an item carry half of its appends and compactions (the thresholds
+// start at +inf), a burst the appenders cannot absorb.
+constexpr int kTcGroupA = LIPFIT_TC_GROUP_A;
+constexpr int kTcTilesA = 32 * kTcRing * kTcGroupA;
+constexpr int kTcMinTilesA = 2 * kTcTilesA;  // shorter items are not worth the extra tiles
+constexpr int kTcMaxKselA = 64;              // of 96 minima
+__host__ __device__ __forceinline__ int tc_tiles_a(int tb, int te, int ksel) {
+    return (te - tb >= kTcMinTilesA && ksel <= kTcMaxKselA) ? kTcTilesA : 0;
+}
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
 constexpr size_t kTcSmemBytes = 1024 /*alignment slack*/ + 2 * kTcTileBytes + kTcStages * kTcTileBytes +
@@ -384,7 +409,9 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 mbar_wait_sleep(&a_empty, (it & 1u) ^ 1u);
                 mbar_arrive_expect_tx(&a_full, 2 * kTcTileBytes);
                 bulk_g2s(sA, g.Aimg + static_cast<size_t>(qb) * 2 * kTcTileBytes, 2 * kTcTileBytes, &a_full);
-                for (int t = tb; t < te; ++t, ++gB) {
+                const int nA = tc_tiles_a(tb, te, a.ksel);
+                for (int vt = -nA; vt < te - tb; ++vt, ++gB) {  // seeding tiles first, then the sweep
+                    const int t = tb + (vt < 0 ? vt + nA : vt);
                     const uint32_t s = gB % kTcStages, u = gB / kTcStages;
                     mbar_wait_sleep(&b_empty[s], (u & 1u) ^ 1u);
                     mbar_arrive_expect_tx(&b_full[s], kTcTileBytes);
@@ -404,7 +431,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 decode(item, qb, ch, tb, te);
                 mbar_wait(&a_full, it & 1u);
                 tc_fence_after();
-                for (int t = tb; t < te; ++t, ++gB) {
+                const int ntiles = te - tb + tc_tiles_a(tb, te, a.ksel);
+                for (int t = 0; t < ntiles; ++t, ++gB) {
                     const uint32_t s = gB % kTcStages, u = gB / kTcStages;
                     const uint32_t b = gB & 1u, ua = gB >> 1;
                     mbar_wait(&b_full[s], u & 1u);
@@ -434,9 +462,13 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         const int h = warp >> 2, quad = warp & 3;
         float* ring = sR + warp * kTcRing * kTcBlockFloats;
         uint32_t gB = 0, nmsg = 0;
+        TC_CLK(long long c_ring = 0; long long c_acc = 0; long long c_seed = 0; long long c_push = 0;
+               const long long c_start = clock64();)
         auto push = [&](const float (&v)[32], float m, int kbase) {
             const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+            TC_CLK(const long long c0 = clock64();)
             mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
+            TC_CLK(const long long c1 = clock64(); c_ring += c1 - c0;)
             float* blk = ring + r * kTcBlockFloats;
             if (kbase >= 0) {
 #pragma unroll
@@ -447,12 +479,62 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&r_full[warp][r]);
             ++nmsg;
+            TC_CLK(c_push += clock64() - c1;)
         };
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
             const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
             float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);  // real keys are far below 1e38
+            const int nA = tc_tiles_a(tb, te, a.ksel);
+            if (nA) {  // phase A: group minima of the first tiles -> ring (one column per group)
+                float gm = __int_as_float(0x7f800000);
+                for (int vt = 0; vt < nA; ++vt, ++gB) {
+                    const uint32_t b = gB & 1u, ua = gB >> 1;
+                    mbar_wait_sleep(&acc_full[h][b], ua & 1u);
+                    tc_fence_after();
+                    const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
+                    float va[32], vb[32];
+                    tc_ld32(trow, va);
+                    tc_ld_wait();
+                    tc_ld32(trow + 32, vb);
+                    gm = fminf(gm, tc_min32(va));
+                    tc_ld_wait();
+                    tc_ld32(trow + 64, va);
+                    gm = fminf(gm, tc_min32(vb));
+                    tc_ld_wait();
+                    tc_ld32(trow + 96, vb);
+                    gm = fminf(gm, tc_min32(va));
+                    tc_ld_wait();
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+                    gm = fminf(gm, tc_min32(vb));
+                    if ((vt + 1) % kTcGroupA == 0) {
+                        const int col = (vt / kTcGroupA) & 31;
+                        const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+                        if (col == 0) mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
+                        float* blk = ring + r * kTcBlockFloats;
+                        blk[lane * 33 + col] = gm;
+                        gm = __int_as_float(0x7f800000);
+                        if (col == 31) {
+                            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 33 + 32] = -2;
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&r_full[warp][r]);
+                            ++nmsg;
+                        }
+                    }
+                }
+                // the sweep starts from the appender's seeded threshold
+                TC_CLK(const long long c0 = clock64();)
+                for (;;) {
+                    const unsigned long long ts = *reinterpret_cast<volatile unsigned long long*>(&tau_s[warp][lane]);
+                    if (static_cast<uint32_t>(ts >> 32) == static_cast<uint32_t>(item)) break;
+                    __nanosleep(200);
+                }
+                __syncwarp();
+                TC_CLK(c_seed += clock64() - c0;)
+            }
             for (int t = tb; t < te; ++t, ++gB) {
                 const uint32_t b = gB & 1u, ua = gB >> 1;
                 {  // adopt the appender's latest threshold for this item (stale values only cost extra pushes)
@@ -460,7 +542,9 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (static_cast<uint32_t>(ts >> 32) == static_cast<uint32_t>(item))
                         tau = fminf(tau, __uint_as_float(static_cast<uint32_t>(ts)));
                 }
+                TC_CLK(const long long c0 = clock64();)
                 mbar_wait_sleep(&acc_full[h][b], ua & 1u);
+                TC_CLK(c_acc += clock64() - c0;)
                 tc_fence_after();
                 const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
                 // Software pipeline over the four 32-column blocks: the TMEM load of block cb+1 is in flight
@@ -496,12 +580,17 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             float dummy[32];
             push(dummy, 0.f, -1);  // end of item: the appender writes fill / tau and moves on
         }
+        TC_CLK(if (blockIdx.x == 0 && lane == 0)
+                   printf("det %d: total %lld wait_acc %lld wait_ring %lld wait_seed %lld push %lld msgs %u\n", warp,
+                          clock64() - c_start, c_acc, c_ring, c_seed, c_push, nmsg);)
     } else {
         // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
         const int aw = warp - 10;  // paired detector warp
         const int h = aw >> 2, quad = aw & 3;
         const float* ring = sR + aw * kTcRing * kTcBlockFloats;
         uint32_t nmsg = 0;
+        TC_CLK(long long c_idle = 0; long long c_comp = 0; long long c_seed = 0; long long n_rows = 0;
+               long long n_comp = 0; long long n_hits = 0; const long long c_start = clock64();)
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
@@ -510,9 +599,39 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             int fill = 0;
             const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
             int2* pool = a.pool + slot * a.P;
+            if (tc_tiles_a(tb, te, a.ksel)) {
+                // phase A: the kTcRing messages of group minima fill the whole ring; row L's 32 * kTcRing
+                // minima sit one per lane per slot.  tau = the next float above the ksel-th smallest, so
+                // that at least ksel data pass the strict `key < tau` test of the sweep.
+                for (int j = 0; j < kTcRing; ++j) {
+                    const uint32_t r = (nmsg + j) % kTcRing, u = (nmsg + j) / kTcRing;
+                    mbar_wait_sleep(&r_full[aw][r], u & 1u);
+                }
+                uint32_t seed = 0;
+                TC_CLK(const long long c0 = clock64();)
+#pragma unroll 2
+                for (int L = 0; L < 32; ++L) {
+                    uint32_t key[kTcRing];
+#pragma unroll
+                    for (int j = 0; j < kTcRing; ++j) key[j] = f2key(ring[j * kTcBlockFloats + L * 33 + lane]);
+                    int need;
+                    const uint32_t kth = knn_rank_select<kTcRing>(key, a.ksel, need);
+                    if (lane == L) seed = kth;
+                }
+                __syncwarp();
+                if (lane == 0)
+                    for (int j = 0; j < kTcRing; ++j) mbar_arrive(&r_empty[aw][j]);
+                nmsg += kTcRing;
+                TC_CLK(c_seed += clock64() - c0;)
+                tau = fminf(tau, key2f(seed + 1u));
+                tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
+                                  __float_as_uint(tau);
+            }
             for (;;) {
                 const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+                TC_CLK(const long long c0 = clock64();)
                 mbar_wait_sleep(&r_full[aw][r], u & 1u);
+                TC_CLK(c_idle += clock64() - c0;)
                 const float* blk = ring + r * kTcBlockFloats;
                 const int kbase = reinterpret_cast<const int*>(blk)[32 * 33 + 32];
                 if (kbase < 0) {
@@ -534,7 +653,9 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     int2* poolL = pool + static_cast<ptrdiff_t>(L - lane) * a.P;  // consecutive lanes = consecutive slots
                     if (fillL > a.P - 32) {  // fewer than 32 free entries: compact (warp-cooperative radix select)
                         __syncwarp();
+                        TC_CLK(const long long c1 = clock64();)
                         tauL = knn_compact(poolL, fillL, a.ksel, nullptr, lane);
+                        TC_CLK(c_comp += clock64() - c1; ++n_comp;)
                         fillL = a.ksel;
                         lowered = true;
                         if (lane == L) tau = tauL;
@@ -544,6 +665,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const unsigned bm = __ballot_sync(0xffffffffu, hit);
                     if (hit) poolL[fillL + __popc(bm & ((1u << lane) - 1u))] = make_int2(__float_as_int(val), kbase + lane);
                     if (lane == L) fill = fillL + __popc(bm);
+                    TC_CLK(++n_rows; n_hits += __popc(bm);)
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&r_empty[aw][r]);
@@ -559,6 +681,9 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             a.fill[slot] = fill;
             a.tau[slot] = tau;
         }
+        TC_CLK(if (blockIdx.x == 0 && lane == 0) printf(
+                   "app %d: total %lld idle %lld compact %lld (%lld) seed %lld rows %lld hits %lld msgs %u\n", aw,
+                   clock64() - c_start, c_idle, c_comp, n_comp, c_seed, n_rows, n_hits, nmsg);)
     }
     tc_fence_before();
     __syncthreads();

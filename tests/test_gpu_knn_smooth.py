@@ -147,6 +147,30 @@ def test_tensor_core_and_cuda_core_selection_agree(d):
     np.testing.assert_array_equal(a[1], b[1])
 
 
+@pytest.mark.parametrize("k", [32, 56])
+def test_tensor_core_threshold_seeding(k):
+    """Work items that sweep >= 768 B tiles seed their thresholds from group minima of the first tiles
+    (knn_tc.cu, phase A).  Full one-chunk items (seeded) and a chunked tail block (not seeded) in one
+    call; a sample of the queries against the oracle, all of them against the CUDA-core selection."""
+    import paper_2606_04670_b200 as L
+    N, Q, d = 100003, 148 * 256 + 100, 16
+    X, _, Xq = random_problem(77 + k, N, Q, d)
+    try:
+        gi, gd = _gpu_knn(X, Xq, k)
+        assert L.knn_fallbacks() == 0
+        L.knn_set_tensor_cores(False)
+        ci, cd = _gpu_knn(X, Xq, k)
+    finally:
+        L.knn_set_tensor_cores(True)
+    np.testing.assert_array_equal(gi, ci)
+    np.testing.assert_array_equal(gd, cd)
+    rows = np.r_[0:200, Q - 200:Q, np.arange(200, Q - 200, 97)[:300]]
+    oi, od = oracle.knn(X, Xq[rows], k)
+    np.testing.assert_array_equal(gi[rows], oi)
+    od32 = od.astype(np.float32)
+    assert np.all(np.abs(gd[rows] - od32) <= np.spacing(od32))
+
+
 def test_knn_host_and_errors():
     import paper_2606_04670_b200 as L
     X, _, Xq = random_problem(7, 2000, 100, 4)
