@@ -20,11 +20,14 @@
 //   warp 9   MMA issuer   : one thread; per B tile 2 x 4 tcgen05.mma (M=128, N=128, K=16) into
 //                           double-buffered TMEM accumulators (2 query halves x 2 stages x 128 columns).
 //   warps 0-7 detectors   : tcgen05.ld 32 columns at a time (thread = query row), min-tree + one compare
-//                           against the query's threshold; a 32 x 32 block that contains a hit goes into a
-//                           shared-memory ring.
+//                           against the query's threshold; every row of a 32 x 32 block that holds a key
+//                           below its threshold goes into a shared-memory ring as one 144-byte message.
 //   warps 10-17 appenders : one per detector warp; own the thresholds and candidate pools of its 32
-//                           queries, append the hits of the ring blocks / compact the pools exactly as in
-//                           knn.cu, and publish lowered thresholds back through shared memory.
+//                           queries, append the hits of the row messages (lane = column) / compact the
+//                           pools exactly as in knn.cu, and publish lowered thresholds back through shared
+//                           memory.
+// Every work item starts with a seeding phase (kTcTilesA tiles) that gives each query a finite threshold
+// before the sweep (see kTcGroupA).
 #include <cuda_bf16.h>
 
 #include "knn_common.cuh"
@@ -44,6 +47,9 @@
 #else
 #define TC_CLK(x)
 #endif
+#ifndef LIPFIT_TC_LDPAIR
+#define LIPFIT_TC_LDPAIR 0
+#endif
 #ifndef LIPFIT_TC_GROUP_A
 #define LIPFIT_TC_GROUP_A 4  // tiles per seeding minimum (see kTcTilesA)
 #endif
@@ -53,17 +59,31 @@ namespace lipfit {
 namespace {
 
 constexpr int kTcThreads = 576;     // 8 detector warps, TMA warp, MMA warp, 8 appender warps
-constexpr int kTcRing = 3;          // hit blocks in flight between a detector warp and its appender warp
-constexpr int kTcBlockFloats = 32 * 33 + 64;  // one 32 x 32 key block [query lane][33], 32 row minima, header
+// Detector -> appender ring: one message = one query row of a 32 x 32 key block that holds a key below the
+// query's threshold: 32 keys + (first datum index, row) in 36 floats (16-byte aligned; the stride keeps
+// the 128-bit row stores of different lanes on different banks).  Flow control: a head counter the
+// detector publishes, a tail counter the appender publishes.
+constexpr int kTcRowFloats = 36;
+#ifndef LIPFIT_TC_SLACK
+#define LIPFIT_TC_SLACK 32
+#endif
+// A pool is compacted back to its ksel best entries once it holds ksel + kTcSlack: the sooner, the lower the
+// thresholds the detectors test against (fewer messages) and the more compactions the appenders run.
+constexpr int kTcSlack = LIPFIT_TC_SLACK;
+static_assert(kTcSlack + 32 <= kTcPoolExtra, "a row message appends up to 32 entries");
+constexpr int kTcRing = 96;         // row messages in flight between a detector warp and its appender warp
+constexpr int kTcMinimaA = 96;      // seeding minima per query (phase A); they overlay the ring: 32 x 97 floats
+constexpr int kTcRingFloats = kTcRing * kTcRowFloats;
+static_assert(32 * (kTcMinimaA + 1) <= kTcRingFloats, "phase A minima overlay the ring");
 constexpr int kTcStages = 4;
 // Threshold seeding (phase A of a work item): the first kTcTilesA B tiles are multiplied once more up
-// front; the detectors only take the minimum key of every group of kTcGroupA tiles per query, 32 * kTcRing
+// front; the detectors only take the minimum key of every group of kTcGroupA tiles per query, kTcMinimaA
 // minima in all, and the appender sets the query's starting threshold to the ksel-th smallest of them
 // (each minimum is the key of a different datum, so at least ksel data lie at or below it).  Without it
 // the first ~1 % of the tiles of an item carry half of its appends and compactions (the thresholds
 // start at +inf), a burst the appenders cannot absorb.
 constexpr int kTcGroupA = LIPFIT_TC_GROUP_A;
-constexpr int kTcTilesA = 32 * kTcRing * kTcGroupA;
+constexpr int kTcTilesA = kTcMinimaA * kTcGroupA;
 constexpr int kTcMinTilesA = 2 * kTcTilesA;  // shorter items are not worth the extra tiles
 constexpr int kTcMaxKselA = 64;              // of 96 minima
 __host__ __device__ __forceinline__ int tc_tiles_a(int tb, int te, int ksel) {
@@ -72,7 +92,7 @@ __host__ __device__ __forceinline__ int tc_tiles_a(int tb, int te, int ksel) {
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
 constexpr size_t kTcSmemBytes = 1024 /*alignment slack*/ + 2 * kTcTileBytes + kTcStages * kTcTileBytes +
-                                8 * kTcRing * kTcBlockFloats * sizeof(float);
+                                8 * kTcRingFloats * sizeof(float);
 
 // byte offset of 16-byte chunk c (0..7) of row r inside a K-major SWIZZLE_128B tile of 128-byte rows
 __host__ __device__ __forceinline__ uint32_t sw128_offset(int r, int c) {
@@ -100,6 +120,19 @@ __device__ __forceinline__ void mbar_wait_sleep(uint64_t* bar, uint32_t parity) 
         if (done) break;
         __nanosleep(LIPFIT_TC_SLEEP_NS);
     }
+}
+// release / acquire on a shared-memory word (CTA scope): the flags of the detector <-> appender ring
+__device__ __forceinline__ void st_release_s(volatile void* p, uint32_t v) {
+#ifdef LIPFIT_TC_NOFENCE
+    asm volatile("st.volatile.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(const_cast<void*>(p))), "r"(v) : "memory");
+#else
+    asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(const_cast<void*>(p))), "r"(v) : "memory");
+#endif
+}
+__device__ __forceinline__ uint32_t ld_acquire_s(const volatile void* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(const_cast<void*>(p))) : "memory");
+    return v;
 }
 __device__ __forceinline__ void tc_fence_before() {
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -338,15 +371,17 @@ __global__ void __launch_bounds__(kTcThreads, 1)
 knn_tc_select_kernel(const KnnTcArgs g) {
     extern __shared__ unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t a_full, a_empty, b_full[kTcStages], b_empty[kTcStages], acc_full[2][2],
-        acc_empty[2][2], r_full[8][kTcRing], r_empty[8][kTcRing];
+        acc_empty[2][2];
     __shared__ __align__(8) unsigned long long tau_s[8][32];  // (item << 32 | tau bits) published by the appenders
+    __shared__ volatile uint32_t head_s[8], tail_s[8];  // ring counters (messages written / consumed)
+    __shared__ volatile int seed_s[8];                  // item whose phase A minima are complete
     __shared__ uint32_t s_tmem;
     // 1024-byte aligned carve-up (SWIZZLE_128B atoms are 1024 B)
     const uint32_t raw = smem_u32(smem_raw);
     unsigned char* base = smem_raw + ((1024u - (raw & 1023u)) & 1023u);
     unsigned char* sA = base;                                // 2 tiles
     unsigned char* sB = sA + 2 * kTcTileBytes;               // kTcStages tiles
-    float* sR = reinterpret_cast<float*>(sB + kTcStages * kTcTileBytes);  // 8 rings of kTcRing hit blocks
+    float* sR = reinterpret_cast<float*>(sB + kTcStages * kTcTileBytes);  // 8 rings of kTcRing row messages
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const KnnArgs& a = g.k;
@@ -362,11 +397,11 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 mbar_init(&acc_full[h][b], 1);
                 mbar_init(&acc_empty[h][b], 4);  // the 4 detector warps of the half
             }
-        for (int w = 0; w < 8; ++w)
-            for (int r = 0; r < kTcRing; ++r) {
-                mbar_init(&r_full[w][r], 1);
-                mbar_init(&r_empty[w][r], 1);
-            }
+        for (int w = 0; w < 8; ++w) {
+            head_s[w] = 0;
+            tail_s[w] = 0;
+            seed_s[w] = -1;
+        }
         mbar_fence_init();
     }
     if (warp == 8) {  // the whole warp allocates all 512 TMEM columns of this SM
@@ -460,26 +495,41 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         // those blocks to their appender warp through a shared-memory ring, so the tensor pipe never waits
         // for an append or a compaction (both are latency-bound: ~800 and ~6000 cycles per event).
         const int h = warp >> 2, quad = warp & 3;
-        float* ring = sR + warp * kTcRing * kTcBlockFloats;
-        uint32_t gB = 0, nmsg = 0;
+        float* ring = sR + warp * kTcRingFloats;
+        uint32_t gB = 0, head = 0, hslot = 0, tail_seen = 0;
         TC_CLK(long long c_ring = 0; long long c_acc = 0; long long c_seed = 0; long long c_push = 0;
-               const long long c_start = clock64();)
-        auto push = [&](const float (&v)[32], float m, int kbase) {
-            const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
+               long long n_push = 0; const long long c_start = clock64();)
+        // room for n more messages (the appender's tail counter only grows)
+        auto reserve = [&](uint32_t n) {
             TC_CLK(const long long c0 = clock64();)
-            mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
-            TC_CLK(const long long c1 = clock64(); c_ring += c1 - c0;)
-            float* blk = ring + r * kTcBlockFloats;
-            if (kbase >= 0) {
-#pragma unroll
-                for (int c = 0; c < 32; ++c) blk[lane * 33 + c] = v[c];  // row = query lane, padded: conflict-free
-                blk[32 * 33 + lane] = m;                                 // the row's minimum
+            while (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) {
+                tail_seen = ld_acquire_s(&tail_s[warp]);
+                if (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) __nanosleep(LIPFIT_TC_SLEEP_NS);
             }
-            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 33 + 32] = kbase;
+            TC_CLK(c_ring += clock64() - c0;)
+        };
+        auto publish = [&](uint32_t n) {
+            head += n;
+            hslot += n;
+            if (hslot >= static_cast<uint32_t>(kTcRing)) hslot -= kTcRing;
             __syncwarp();
-            if (lane == 0) mbar_arrive(&r_full[warp][r]);
-            ++nmsg;
-            TC_CLK(c_push += clock64() - c1;)
+            if (lane == 0) st_release_s(&head_s[warp], head);
+        };
+        // the rows `hm` of a 32 x 32 block (thread = row) go to the appender, one message each
+        auto push = [&](const float (&v)[32], unsigned hm, int kbase) {
+            const uint32_t n = __popc(hm);
+            reserve(n);
+            TC_CLK(const long long c1 = clock64();)
+            if ((hm >> lane) & 1u) {
+                uint32_t sl = hslot + __popc(hm & ((1u << lane) - 1u));
+                if (sl >= static_cast<uint32_t>(kTcRing)) sl -= kTcRing;
+                float4* p = reinterpret_cast<float4*>(ring + sl * kTcRowFloats);
+#pragma unroll
+                for (int c = 0; c < 8; ++c) p[c] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+                *reinterpret_cast<int2*>(p + 8) = make_int2(kbase, lane);
+            }
+            publish(n);
+            TC_CLK(c_push += clock64() - c1; ++n_push;)
         };
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
@@ -487,45 +537,35 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             const int qslot = qb * kTcQueries + h * 128 + quad * 32 + lane;
             float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);  // real keys are far below 1e38
             const int nA = tc_tiles_a(tb, te, a.ksel);
-            if (nA) {  // phase A: group minima of the first tiles -> ring (one column per group)
+            if (nA) {  // phase A: group minima of the first tiles, [row][kTcMinimaA + 1] over the drained ring
+                TC_CLK(const long long c00 = clock64();)
+                while (ld_acquire_s(&tail_s[warp]) != head) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                tail_seen = head;
+                TC_CLK(c_ring += clock64() - c00;)
                 float gm = __int_as_float(0x7f800000);
                 for (int vt = 0; vt < nA; ++vt, ++gB) {
                     const uint32_t b = gB & 1u, ua = gB >> 1;
                     mbar_wait_sleep(&acc_full[h][b], ua & 1u);
                     tc_fence_after();
                     const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
-                    float va[32], vb[32];
-                    tc_ld32(trow, va);
-                    tc_ld_wait();
-                    tc_ld32(trow + 32, vb);
-                    gm = fminf(gm, tc_min32(va));
-                    tc_ld_wait();
-                    tc_ld32(trow + 64, va);
-                    gm = fminf(gm, tc_min32(vb));
-                    tc_ld_wait();
-                    tc_ld32(trow + 96, vb);
-                    gm = fminf(gm, tc_min32(va));
-                    tc_ld_wait();
+                    float va[32];  // one buffer: phase A is 5 % of the tiles, two buffers spill here
+#pragma unroll
+                    for (int cb = 0; cb < 4; ++cb) {
+                        tc_ld32(trow + 32 * cb, va);
+                        tc_ld_wait();
+                        gm = fminf(gm, tc_min32(va));
+                    }
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-                    gm = fminf(gm, tc_min32(vb));
                     if ((vt + 1) % kTcGroupA == 0) {
-                        const int col = (vt / kTcGroupA) & 31;
-                        const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
-                        if (col == 0) mbar_wait_sleep(&r_empty[warp][r], (u & 1u) ^ 1u);
-                        float* blk = ring + r * kTcBlockFloats;
-                        blk[lane * 33 + col] = gm;
+                        ring[lane * (kTcMinimaA + 1) + vt / kTcGroupA] = gm;
                         gm = __int_as_float(0x7f800000);
-                        if (col == 31) {
-                            if (lane == 0) reinterpret_cast<int*>(blk)[32 * 33 + 32] = -2;
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(&r_full[warp][r]);
-                            ++nmsg;
-                        }
                     }
                 }
-                // the sweep starts from the appender's seeded threshold
+                __syncwarp();
+                if (lane == 0) st_release_s(&seed_s[warp], static_cast<uint32_t>(item));
+                // the sweep starts from the appender's seeded threshold (and the ring is free again)
                 TC_CLK(const long long c0 = clock64();)
                 for (;;) {
                     const unsigned long long ts = *reinterpret_cast<volatile unsigned long long*>(&tau_s[warp][lane]);
@@ -557,10 +597,25 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (__any_sync(0xffffffffu, m < -1e30f)) tau = 0.f;
 #else
                     const float m = tc_min32(v);
-                    if (__any_sync(0xffffffffu, m < tau)) push(v, m, t * kTcBN + cb * 32);
+                    const unsigned hm = __ballot_sync(0xffffffffu, m < tau);
+                    if (hm) push(v, hm, t * kTcBN + cb * 32);
 #endif
                 };
                 float va[32], vb[32];
+#if LIPFIT_TC_LDPAIR
+                tc_ld32(trow, va);
+                tc_ld32(trow + 32, vb);
+                tc_ld_wait();
+                process(va, 0);
+                process(vb, 1);
+                tc_ld32(trow + 64, va);
+                tc_ld32(trow + 96, vb);
+                tc_ld_wait();
+                tc_fence_before();  // all four blocks are in registers: hand the TMEM stage back
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+                process(va, 2);
+#else
                 tc_ld32(trow, va);
                 tc_ld_wait();
                 tc_ld32(trow + 32, vb);
@@ -575,22 +630,25 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 tc_fence_before();  // all four blocks are in registers: hand the TMEM stage back
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+#endif
                 process(vb, 3);
             }
-            float dummy[32];
-            push(dummy, 0.f, -1);  // end of item: the appender writes fill / tau and moves on
+            // end of item: the appender writes fill / tau and moves on
+            reserve(1);
+            if (lane == 0) *reinterpret_cast<int2*>(ring + hslot * kTcRowFloats + 32) = make_int2(-1, 0);
+            publish(1);
         }
         TC_CLK(if (blockIdx.x == 0 && lane == 0)
-                   printf("det %d: total %lld wait_acc %lld wait_ring %lld wait_seed %lld push %lld msgs %u\n", warp,
-                          clock64() - c_start, c_acc, c_ring, c_seed, c_push, nmsg);)
+                   printf("det %d: total %lld wait_acc %lld wait_ring %lld wait_seed %lld push %lld (%lld) msgs %u\n",
+                          warp, clock64() - c_start, c_acc, c_ring, c_seed, c_push, n_push, head);)
     } else {
         // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
         const int aw = warp - 10;  // paired detector warp
         const int h = aw >> 2, quad = aw & 3;
-        const float* ring = sR + aw * kTcRing * kTcBlockFloats;
-        uint32_t nmsg = 0;
-        TC_CLK(long long c_idle = 0; long long c_comp = 0; long long c_seed = 0; long long n_rows = 0;
-               long long n_comp = 0; long long n_hits = 0; const long long c_start = clock64();)
+        const float* ring = sR + aw * kTcRingFloats;
+        uint32_t tail = 0, tslot = 0, head_seen = 0;
+        TC_CLK(long long c_idle = 0; long long c_comp = 0; long long c_seed = 0; long long n_comp = 0;
+               long long n_hits = 0; const long long c_start = clock64();)
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
@@ -600,79 +658,66 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             const size_t slot = knn_pool_slot(qslot, ch, a.Qp, a.Qtp, a.nfullq);
             int2* pool = a.pool + slot * a.P;
             if (tc_tiles_a(tb, te, a.ksel)) {
-                // phase A: the kTcRing messages of group minima fill the whole ring; row L's 32 * kTcRing
-                // minima sit one per lane per slot.  tau = the next float above the ksel-th smallest, so
-                // that at least ksel data pass the strict `key < tau` test of the sweep.
-                for (int j = 0; j < kTcRing; ++j) {
-                    const uint32_t r = (nmsg + j) % kTcRing, u = (nmsg + j) / kTcRing;
-                    mbar_wait_sleep(&r_full[aw][r], u & 1u);
-                }
+                // phase A: row L's kTcMinimaA group minima sit at ring[L][.], one per lane per 32.  tau = the
+                // next float above the ksel-th smallest, so that at least ksel data pass the strict
+                // `key < tau` test of the sweep.
+                TC_CLK(const long long c00 = clock64();)
+                while (ld_acquire_s(&seed_s[aw]) != static_cast<uint32_t>(item)) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                TC_CLK(const long long c0 = clock64(); c_idle += c0 - c00;)
                 uint32_t seed = 0;
-                TC_CLK(const long long c0 = clock64();)
 #pragma unroll 2
                 for (int L = 0; L < 32; ++L) {
-                    uint32_t key[kTcRing];
+                    uint32_t key[kTcMinimaA / 32];
 #pragma unroll
-                    for (int j = 0; j < kTcRing; ++j) key[j] = f2key(ring[j * kTcBlockFloats + L * 33 + lane]);
+                    for (int j = 0; j < kTcMinimaA / 32; ++j)
+                        key[j] = f2key(ring[L * (kTcMinimaA + 1) + j * 32 + lane]);
                     int need;
-                    const uint32_t kth = knn_rank_select<kTcRing>(key, a.ksel, need);
+                    const uint32_t kth = knn_rank_select<kTcMinimaA / 32>(key, a.ksel, need);
                     if (lane == L) seed = kth;
                 }
                 __syncwarp();
-                if (lane == 0)
-                    for (int j = 0; j < kTcRing; ++j) mbar_arrive(&r_empty[aw][j]);
-                nmsg += kTcRing;
                 TC_CLK(c_seed += clock64() - c0;)
                 tau = fminf(tau, key2f(seed + 1u));
                 tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
                                   __float_as_uint(tau);
             }
             for (;;) {
-                const uint32_t r = nmsg % kTcRing, u = nmsg / kTcRing;
-                TC_CLK(const long long c0 = clock64();)
-                mbar_wait_sleep(&r_full[aw][r], u & 1u);
-                TC_CLK(c_idle += clock64() - c0;)
-                const float* blk = ring + r * kTcBlockFloats;
-                const int kbase = reinterpret_cast<const int*>(blk)[32 * 33 + 32];
-                if (kbase < 0) {
+                if (head_seen == tail) {
+                    TC_CLK(const long long c0 = clock64();)
+                    while ((head_seen = ld_acquire_s(&head_s[aw])) == tail) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                    TC_CLK(c_idle += clock64() - c0;)
+                }
+                const float* p = ring + tslot * kTcRowFloats;
+                const int2 hd = *reinterpret_cast<const int2*>(p + 32);  // (first datum index, row)
+                const float val = p[lane];                               // lane = column
+                ++tail;
+                if (++tslot == static_cast<uint32_t>(kTcRing)) tslot = 0;
+                if (hd.x < 0) {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&r_empty[aw][r]);
-                    ++nmsg;
+                    if (lane == 0) st_release_s(&tail_s[aw], tail);
                     break;
                 }
-                // Rows (queries) of the block that still have a key below the CURRENT threshold; each such
-                // row is scanned by the whole warp (lane = column): ~20 instructions per row instead of a
-                // 32-column predicated pass by every lane.
-                unsigned hm = __ballot_sync(0xffffffffu, blk[32 * 33 + lane] < tau);
-                bool lowered = false;
-                while (hm) {
-                    const int L = __ffs(hm) - 1;
-                    hm &= hm - 1;
-                    float tauL = __shfl_sync(0xffffffffu, tau, L);
-                    int fillL = __shfl_sync(0xffffffffu, fill, L);
-                    int2* poolL = pool + static_cast<ptrdiff_t>(L - lane) * a.P;  // consecutive lanes = consecutive slots
-                    if (fillL > a.P - 32) {  // fewer than 32 free entries: compact (warp-cooperative radix select)
-                        __syncwarp();
-                        TC_CLK(const long long c1 = clock64();)
-                        tauL = knn_compact(poolL, fillL, a.ksel, nullptr, lane);
-                        TC_CLK(c_comp += clock64() - c1; ++n_comp;)
-                        fillL = a.ksel;
-                        lowered = true;
-                        if (lane == L) tau = tauL;
-                    }
-                    const float val = blk[L * 33 + lane];
-                    const bool hit = val < tauL;
-                    const unsigned bm = __ballot_sync(0xffffffffu, hit);
-                    if (hit) poolL[fillL + __popc(bm & ((1u << lane) - 1u))] = make_int2(__float_as_int(val), kbase + lane);
-                    if (lane == L) fill = fillL + __popc(bm);
-                    TC_CLK(++n_rows; n_hits += __popc(bm);)
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&r_empty[aw][r]);
-                ++nmsg;
-                if (lowered)  // a compaction lowered some threshold: publish for the detector
+                const int L = hd.y;
+                float tauL = __shfl_sync(0xffffffffu, tau, L);
+                int fillL = __shfl_sync(0xffffffffu, fill, L);
+                int2* poolL = pool + static_cast<ptrdiff_t>(L - lane) * a.P;  // consecutive lanes = consecutive slots
+                if (fillL >= a.ksel + kTcSlack) {  // compact (warp-cooperative radix select): lowers tau
+                    __syncwarp();
+                    TC_CLK(const long long c1 = clock64();)
+                    tauL = knn_compact(poolL, fillL, a.ksel, nullptr, lane);
+                    TC_CLK(c_comp += clock64() - c1; ++n_comp;)
+                    fillL = a.ksel;
+                    if (lane == L) tau = tauL;
+                    // publish the lowered threshold for the detector
                     tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
                                       __float_as_uint(tau);
+                }
+                const bool hit = val < tauL;
+                const unsigned bm = __ballot_sync(0xffffffffu, hit);
+                if (hit) poolL[fillL + __popc(bm & ((1u << lane) - 1u))] = make_int2(__float_as_int(val), hd.x + lane);
+                if (lane == L) fill = fillL + __popc(bm);
+                if (lane == 0) st_release_s(&tail_s[aw], tail);  // every lane's read of the message fed the ballot above
+                TC_CLK(n_hits += __popc(bm);)
             }
 #if LIPFIT_TC_EXPERIMENT
             fill = 0;
@@ -682,8 +727,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             a.tau[slot] = tau;
         }
         TC_CLK(if (blockIdx.x == 0 && lane == 0) printf(
-                   "app %d: total %lld idle %lld compact %lld (%lld) seed %lld rows %lld hits %lld msgs %u\n", aw,
-                   clock64() - c_start, c_idle, c_comp, n_comp, c_seed, n_rows, n_hits, nmsg);)
+                   "app %d: total %lld idle %lld compact %lld (%lld) seed %lld hits %lld msgs %u\n", aw,
+                   clock64() - c_start, c_idle, c_comp, n_comp, c_seed, n_hits, tail);)
     }
     tc_fence_before();
     __syncthreads();
