@@ -548,8 +548,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     mbar_wait_sleep(&acc_full[h][b], ua & 1u);
                     tc_fence_after();
                     const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
-                    float va[32];  // one buffer: phase A is 5 % of the tiles, two buffers spill here
-#pragma unroll
+                    float va[32];  // one buffer, rolled loop: ptxas spills a buffer in any unrolled form
+#pragma unroll 1
                     for (int cb = 0; cb < 4; ++cb) {
                         tc_ld32(trow + 32 * cb, va);
                         tc_ld_wait();
