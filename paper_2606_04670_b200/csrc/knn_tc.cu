@@ -58,7 +58,7 @@ namespace lipfit {
 
 namespace {
 
-constexpr int kTcThreads = 576;     // 8 detector warps, TMA warp, MMA warp, 8 appender warps
+constexpr int kTcThreads = 608;     // 8 detector warps, TMA warp, MMA warp (half 0), 8 appender warps, MMA warp (half 1)
 // Detector -> appender ring: one message = one query row of a 32 x 32 key block that holds a key below the
 // query's threshold: 32 keys + (first datum index, row) in 36 floats (16-byte aligned; the stride keeps
 // the 128-bit row stores of different lanes on different banks).  Flow control: a head counter the
@@ -387,10 +387,10 @@ knn_tc_select_kernel(const KnnTcArgs g) {
     const KnnArgs& a = g.k;
     if (threadIdx.x == 0) {
         mbar_init(&a_full, 1);
-        mbar_init(&a_empty, 1);
+        mbar_init(&a_empty, 2);  // both MMA issuers
         for (int s = 0; s < kTcStages; ++s) {
             mbar_init(&b_full[s], 1);
-            mbar_init(&b_empty[s], 1);
+            mbar_init(&b_empty[s], 2);
         }
         for (int h = 0; h < 2; ++h)
             for (int b = 0; b < 2; ++b) {
@@ -455,12 +455,14 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 }
             }
         }
-    } else if (warp == 9) {
-        // ================= MMA issuer =================
+    } else if (warp == 9 || warp == 18) {
+        // ================= MMA issuers: one thread per query half =================
+        // Two issuers so that a half whose detectors are held up (pushes, a full ring) does not block the
+        // other half's accumulator stages; they share the B ring and drift at most kTcStages tiles apart.
         if (lane == 0) {
+            const int h = warp == 9 ? 0 : 1;
             uint32_t gB = 0, it = 0;
-            const uint64_t adesc0 = tc_smem_desc(smem_u32(sA));
-            const uint64_t adesc1 = tc_smem_desc(smem_u32(sA + kTcTileBytes));
+            const uint64_t ad = tc_smem_desc(smem_u32(sA + h * kTcTileBytes));
             for (int item = blockIdx.x; item < nitems; item += gridDim.x, ++it) {
                 int qb, ch, tb, te;
                 decode(item, qb, ch, tb, te);
@@ -471,19 +473,14 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const uint32_t s = gB % kTcStages, u = gB / kTcStages;
                     const uint32_t b = gB & 1u, ua = gB >> 1;
                     mbar_wait(&b_full[s], u & 1u);
+                    mbar_wait(&acc_empty[h][b], (ua & 1u) ^ 1u);
                     tc_fence_after();
                     const uint64_t bdesc = tc_smem_desc(smem_u32(sB + s * kTcTileBytes));
+                    const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        mbar_wait(&acc_empty[h][b], (ua & 1u) ^ 1u);
-                        tc_fence_after();
-                        const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
-                        const uint64_t ad = h ? adesc1 : adesc0;
-#pragma unroll
-                        for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
-                            tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
-                        tc_commit(&acc_full[h][b]);
-                    }
+                    for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
+                        tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
+                    tc_commit(&acc_full[h][b]);
                     tc_commit(&b_empty[s]);
                 }
                 tc_commit(&a_empty);
@@ -641,7 +638,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         TC_CLK(if (blockIdx.x == 0 && lane == 0)
                    printf("det %d: total %lld wait_acc %lld wait_ring %lld wait_seed %lld push %lld (%lld) msgs %u\n",
                           warp, clock64() - c_start, c_acc, c_ring, c_seed, c_push, n_push, head);)
-    } else {
+    } else if (warp < 18) {
         // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
         const int aw = warp - 10;  // paired detector warp
         const int h = aw >> 2, quad = aw & 3;
