@@ -478,7 +478,10 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const uint64_t bdesc = tc_smem_desc(smem_u32(sB + s * kTcTileBytes));
                     const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
 #pragma unroll
-                    for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
+#ifndef LIPFIT_TC_KSTEPS
+#define LIPFIT_TC_KSTEPS (kTcK / 16)
+#endif
+                    for (int k = 0; k < LIPFIT_TC_KSTEPS; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
                         tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
                     tc_commit(&acc_full[h][b]);
                     tc_commit(&b_empty[s]);
@@ -599,6 +602,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
 #endif
                 };
                 float va[32], vb[32];
+#if LIPFIT_TC_EXPERIMENT == 3  // timing experiment: MMA only, accumulators never read
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
+                continue;
+#endif
 #if LIPFIT_TC_LDPAIR
                 tc_ld32(trow, va);
                 tc_ld32(trow + 32, vb);
