@@ -98,7 +98,7 @@ __device__ __forceinline__ float knn_compact(int2* pool, int n, int ksel, int2*,
 // certificate.  slots = CTAs of the persistent grid.
 constexpr int kTcQueries = 256;  // queries per work item
 constexpr int kTcBN = 128;       // data records per B tile
-constexpr int kTcPoolExtra = 64; // pools of the tensor-core path hold ksel + 64 entries (see tc_append32)
+constexpr int kTcPoolExtra = 64; // pools of the tensor-core path hold ksel + 64 entries (knn_tc.cu: kTcSlack)
 int knn_tc_slots(const Ctx& c);
 int launch_knn_tc_select(const Ctx& c, const float* X, const float* Xq, KnnArgs& a, float* mu_dev,
                          uint32_t* stats);

@@ -6,8 +6,10 @@
 //     key = ||x_c||^2 - 2 q_c . x_c      ( = ||q - x||^2 - ||q_c||^2 : same order as the distance )
 // as ONE bf16 GEMM with K = 64 and fp32 accumulation in tensor memory.  fp32 values are split
 // v = hi + lo (two bf16, 16 significant bits) and the operand rows are
-//     A (query) = [ hi(-2 q_c) | hi(-2 q_c) | lo(-2 q_c) | 1 1 1 0.. ]      16 + 16 + 16 + 16 = 64 bf16
+//     A (query) = [ hi(-2 q_c) | hi(-2 q_c) | lo(-2 q_c) | 1 1 1 0.. ]      d + d + d + 3 of the 64 bf16 of a row
 //     B (datum) = [ hi(x_c)    | lo(x_c)    | hi(x_c)    | x2_h x2_m x2_l 0.. ]   (||x_c||^2 in 3 bf16)
+// and only the ceil((3 d + 3) / 16) K steps that hold non-zero columns are multiplied (d = 16: 4, d <= 15: 3,
+// d <= 9: 2, d <= 4: 1)
 // so A.B = hi.hi + hi.lo + lo.hi + ||x_c||^2: the dropped lo.lo terms and the split residue are
 // <= 3 * 2^-16 |q'_j x_j| per coordinate; the fp64 re-rank + certificate of knn.cu
 // turn the selected pools into the exact answer, whatever the key arithmetic was.
@@ -34,6 +36,9 @@
 
 #ifndef LIPFIT_TC_SLEEP_NS
 #define LIPFIT_TC_SLEEP_NS 40
+#endif
+#ifndef LIPFIT_TC_POLL_NS
+#define LIPFIT_TC_POLL_NS 100  // back-off of the ring-counter polls (shared-memory loads: keep them rare)
 #endif
 #ifndef LIPFIT_TC_EXPERIMENT
 #define LIPFIT_TC_EXPERIMENT 0  // 1, 2: timing experiments with invalid results (never in a product build)
@@ -118,7 +123,7 @@ __device__ __forceinline__ void mbar_wait_sleep(uint64_t* bar, uint32_t parity) 
             : "r"(smem_u32(bar)), "r"(parity)
             : "memory");
         if (done) break;
-        __nanosleep(LIPFIT_TC_SLEEP_NS);
+        __nanosleep(LIPFIT_TC_POLL_NS);
     }
 }
 // release / acquire on a shared-memory word (CTA scope): the flags of the detector <-> appender ring
@@ -248,20 +253,22 @@ knn_tc_pack_b_kernel(const float* __restrict__ X, int N, int Npad, Xform xf, con
                 s2 += static_cast<double>(xc) * static_cast<double>(xc);
                 __nv_bfloat16 hi, lo;
                 split2(xc, hi, lo);
-                row[j] = hi;
-                row[16 + j] = lo;
-                row[32 + j] = hi;
+                if (j < xf.d) {
+                    row[j] = hi;
+                    row[xf.d + j] = lo;
+                    row[2 * xf.d + j] = hi;
+                }
             }
             x2f = static_cast<float>(s2);
             const __nv_bfloat16 h = __float2bfloat16_rn(x2f);
             const float r1 = x2f - __bfloat162float(h);
             const __nv_bfloat16 m = __float2bfloat16_rn(r1);
             const __nv_bfloat16 l = __float2bfloat16_rn(r1 - __bfloat162float(m));
-            row[48] = h;
-            row[49] = m;
-            row[50] = l;
+            row[3 * xf.d] = h;
+            row[3 * xf.d + 1] = m;
+            row[3 * xf.d + 2] = l;
         } else {
-            row[48] = __float2bfloat16_rn(3.0e38f);
+            row[3 * xf.d] = __float2bfloat16_rn(3.0e38f);
         }
         store_row(img + static_cast<size_t>(k / kTcBN) * kTcTileBytes, k % kTcBN, row);
     }
@@ -293,11 +300,13 @@ knn_tc_pack_a_kernel(const float* __restrict__ Xq, int Q, int Qp, Xform xf, cons
             if (j < xf.d) qc = xf.sw[j] * src[xf.perm[j]] - mu[j];
             __nv_bfloat16 hi, lo;
             split2(-2.f * qc, hi, lo);
-            row[j] = hi;
-            row[16 + j] = hi;
-            row[32 + j] = lo;
+            if (j < xf.d) {
+                row[j] = hi;
+                row[xf.d + j] = hi;
+                row[2 * xf.d + j] = lo;
+            }
         }
-        row[48] = row[49] = row[50] = __float2bfloat16_rn(1.f);
+        row[3 * xf.d] = row[3 * xf.d + 1] = row[3 * xf.d + 2] = __float2bfloat16_rn(1.f);
     }
     store_row(img + static_cast<size_t>(q / 128) * kTcTileBytes, q % 128, row);
 }
@@ -311,50 +320,9 @@ struct KnnTcArgs {
     const unsigned char* Aimg;  // [Qp/128] tiles of 128 query rows
     const unsigned char* Bimg;  // [ntilesB] tiles of 128 data rows
     int ntilesB;
+    int ksteps;                 // K steps (16 bf16 each) that hold non-zero operand columns
     KnnArgs k;                  // pools, schedule (query blocks of kTcQueries), N, Q, ksel, P
 };
-
-// Epilogue slow path for 32 keys of one query (this lane's row): v[c] is the key of datum kbase + c.
-// Entered warp-uniformly when some lane of the warp has a key below its threshold.  Pools of the
-// tensor-core path have P = ksel + 64 entries and are compacted (warp-cooperatively) as soon as
-// fewer than 32 entries are free, so the 32 predicated appends below always fit: no loop, no
-// shared-memory staging.  Padding rows (index >= N) carry key 3e38 > the initial threshold 1e38.
-__device__ __forceinline__ void tc_append32(const KnnArgs& a, const float (&v)[32], int kbase, float& tau,
-                                            int& fill, int2* pool, int2* scr2, int lane) {
-    const int P = a.P;
-    unsigned fm = __ballot_sync(0xffffffffu, fill > P - 32);
-    if (fm) {
-        __syncwarp();  // orders earlier appends before the cooperative reads below
-        while (fm) {
-            const int src = __ffs(fm) - 1;
-            fm &= fm - 1;
-            int2* pq = pool + static_cast<ptrdiff_t>(src - lane) * P;  // consecutive lanes = consecutive slots
-            const int n = __shfl_sync(0xffffffffu, fill, src);
-            const float nt = knn_compact(pq, n, a.ksel, scr2, lane);
-            if (lane == src) {
-                tau = nt;
-                fill = a.ksel;
-            }
-        }
-    }
-#pragma unroll
-    for (int c = 0; c < 32; ++c) {
-        const float val = v[c];
-        // predicated store + predicated increment: 32 divergent branches here cost far more than the work
-        int inc;
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "setp.lt.f32 p, %1, %2;\n\t"
-            "@p st.global.v2.b32 [%3], {%4, %5};\n\t"
-            "selp.s32 %0, 1, 0, p;\n\t"
-            "}\n"
-            : "=r"(inc)
-            : "f"(val), "f"(tau), "l"(pool + fill), "r"(__float_as_int(val)), "r"(kbase + c)
-            : "memory");
-        fill += inc;
-    }
-}
 
 // min of 32 values as a depth-4 tree of 3-input minima (FMNMX3)
 __device__ __forceinline__ float tc_min32(const float (&v)[32]) {
@@ -479,10 +447,11 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
 #pragma unroll
 #ifndef LIPFIT_TC_KSTEPS
-#define LIPFIT_TC_KSTEPS (kTcK / 16)
+#define LIPFIT_TC_KSTEPS g.ksteps
 #endif
-                    for (int k = 0; k < LIPFIT_TC_KSTEPS; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
-                        tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
+#pragma unroll
+                    for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
+                        if (k < LIPFIT_TC_KSTEPS) tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
                     tc_commit(&acc_full[h][b]);
                     tc_commit(&b_empty[s]);
                 }
@@ -504,7 +473,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             TC_CLK(const long long c0 = clock64();)
             while (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) {
                 tail_seen = ld_acquire_s(&tail_s[warp]);
-                if (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                if (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) __nanosleep(LIPFIT_TC_POLL_NS);
             }
             TC_CLK(c_ring += clock64() - c0;)
         };
@@ -539,7 +508,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             const int nA = tc_tiles_a(tb, te, a.ksel);
             if (nA) {  // phase A: group minima of the first tiles, [row][kTcMinimaA + 1] over the drained ring
                 TC_CLK(const long long c00 = clock64();)
-                while (ld_acquire_s(&tail_s[warp]) != head) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                while (ld_acquire_s(&tail_s[warp]) != head) __nanosleep(LIPFIT_TC_POLL_NS);
                 tail_seen = head;
                 TC_CLK(c_ring += clock64() - c00;)
                 float gm = __int_as_float(0x7f800000);
@@ -668,7 +637,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 // next float above the ksel-th smallest, so that at least ksel data pass the strict
                 // `key < tau` test of the sweep.
                 TC_CLK(const long long c00 = clock64();)
-                while (ld_acquire_s(&seed_s[aw]) != static_cast<uint32_t>(item)) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                while (ld_acquire_s(&seed_s[aw]) != static_cast<uint32_t>(item)) __nanosleep(LIPFIT_TC_POLL_NS);
                 TC_CLK(const long long c0 = clock64(); c_idle += c0 - c00;)
                 uint32_t seed = 0;
 #pragma unroll 2
@@ -690,7 +659,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             for (;;) {
                 if (head_seen == tail) {
                     TC_CLK(const long long c0 = clock64();)
-                    while ((head_seen = ld_acquire_s(&head_s[aw])) == tail) __nanosleep(LIPFIT_TC_SLEEP_NS);
+                    while ((head_seen = ld_acquire_s(&head_s[aw])) == tail) __nanosleep(LIPFIT_TC_POLL_NS);
                     TC_CLK(c_idle += clock64() - c0;)
                 }
                 const float* p = ring + tslot * kTcRowFloats;
@@ -767,6 +736,7 @@ int launch_knn_tc_select(const Ctx& c, const float* X, const float* Xq, KnnArgs&
     g.Aimg = wa.as<unsigned char>();
     g.Bimg = wb.as<unsigned char>();
     g.ntilesB = ntilesB;
+    g.ksteps = (3 * a.xf.d + 3 + 15) / 16;
     g.k = a;
     LIPFIT_CUDA(cudaFuncSetAttribute(knn_tc_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      static_cast<int>(kTcSmemBytes)));
