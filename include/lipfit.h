@@ -16,7 +16,10 @@
  *     everything and do the host<->device copies themselves.
  *   - `cuda_stream` is a cudaStream_t (NULL = default stream).  Internal
  *     workspace comes from cudaMallocAsync on that stream and is released
- *     (stream-ordered) before the call returns.
+ *     (stream-ordered) before the call returns.  The first call on a device sets
+ *     the release threshold of that device's default memory pool to "keep", so
+ *     released workspaces stay cached in the pool across synchronisations
+ *     (cudaMemPoolTrimTo on the default pool hands them back to the driver).
  *   - Every function returns LIPFIT_OK (0) or a negative lipfit_status; no
  *     exception crosses the boundary; apart from an atomic launch counter there is
  *     no global mutable state, so calls on distinct streams are thread-safe.

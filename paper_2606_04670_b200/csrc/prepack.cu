@@ -65,8 +65,18 @@ int make_ctx(void* cuda_stream, Ctx* ctx) {
     LIPFIT_CUDA(cudaGetDevice(&dev));
     static std::atomic<int> sm_cache[64];  // SM count per device ordinal (0 = not asked yet)
     int sms = (dev >= 0 && dev < 64) ? sm_cache[dev].load() : 0;
-    if (sms == 0) {
+    if (sms == 0) {  // first call on this device
         LIPFIT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        // Workspaces come from the device's default stream-ordered pool (common.cuh: Workspace).  Its
+        // default release threshold is 0: every synchronisation hands the freed workspaces back to
+        // the driver and the next call pays for mapping them again (tens of ms for the 0.5 GB of
+        // kNN pools).  Keep them cached in the pool instead.
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        (void)cudaGetLastError();
         if (dev >= 0 && dev < 64) sm_cache[dev].store(sms);
     }
     ctx->device = dev;
