@@ -47,7 +47,7 @@ UNIT = "Gpairs/s"
 LANE_OPS = {1: 9, 2: 13, "2survey": 18, 3: 21, 4: 17, "4direct": 33, "5s": 18, "5s_survey": 26, "5b": 31}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md); null where no capture of this kernel version exists.
-NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2,folded>": 30_431_744, "knn_tc_select": 2_954_589_000, "knn_select<dot>": 5_975_622_000,
+NCU_TRAFFIC_BYTES = {"bounds<L1,U2,C2,folded>": 30_431_744, "knn_tc_select": 2_853_554_000, "knn_select<dot>": 5_975_622_000,
                      "smooth_pairs<L2,U0,C5>": 14_425_600}
 FP32_LANES_PER_SM = 128
 

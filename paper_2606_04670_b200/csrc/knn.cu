@@ -651,7 +651,11 @@ double knn_last_key_error_ratio() {
 void knn_set_tensor_cores(int on) { g_knn_tc.store(on ? 1 : 0); }
 
 const char* knn_variant_name(const Xform& xf, int norm) {
-    if (use_tc(xf, norm)) return "knn_tc_select<bf16x3,K64>";
+    if (use_tc(xf, norm)) {  // K = 16 bf16 per K step, ceil((3 d + 3) / 16) steps (knn_tc.cu)
+        static const char* const names[4] = {"knn_tc_select<bf16x3,K16>", "knn_tc_select<bf16x3,K32>",
+                                             "knn_tc_select<bf16x3,K48>", "knn_tc_select<bf16x3,K64>"};
+        return names[(3 * xf.d + 3 + 15) / 16 - 1];
+    }
     return (norm == 2 && xf.dC == 0) ? "knn_select<dot>" : "knn_select<diff>";
 }
 
