@@ -251,7 +251,7 @@ def bench_bounds(torch, L, wl, steps, warmup, l2buf, dev, lane_ops, do_e2e=True)
         outs = tuple(torch.empty(wl.Q, dtype=torch.float32).pin_memory().numpy() for _ in range(3))
         sp = torch.cuda.current_stream().cuda_stream
         hfn = lambda: L.lipfit_bounds_host(Xh, yh, Xqh, wl.M, wl.mask, wl.norm, wl.weights, outs, sp)
-        hms = _time_steps(torch, hfn, max(1, steps), min(warmup, 2), l2buf)
+        hms = _time_steps(torch, hfn, max(1, steps), warmup, l2buf)
         res["e2e"] = {"value": pairs / (np.mean(hms) * 1e-3) / 1e9, "unit": UNIT,
                       "ms_per_step": float(np.mean(hms)),
                       "h2d_bytes_per_step": int(Xh.nbytes + yh.nbytes + Xqh.nbytes),
@@ -471,15 +471,15 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
             out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "sample": sample}
             out["parity"] = parity_bounds(wl, r["outputs"], sel, ref)
     elif c == 4:
-        r = bench_knn(torch, L, wl, steps, 1, l2buf, dev, tensor_cores=True)
+        r = bench_knn(torch, L, wl, steps, max(3, args.warmup), l2buf, dev, tensor_cores=True)
         out.update({k: r[k] for k in ("ms_per_step", "value", "kernel_ms", "kernel")})
         out["unit"] = UNIT
         out["step"] = "lipfit_knn = operand images + tensor-core selection + fp64 re-rank / certificate + exact fallback"
         out["exact_fallback_queries"] = r["fallbacks"]
         out["key_error_over_bound"] = r["key_error_over_bound"]
-        out["roofline"] = _roofline_tensor(r["pairs"], 64, r["kernel_ms"], peaks)
+        out["roofline"] = _roofline_tensor(r["pairs"], 16 * ((3 * wl.d + 3 + 15) // 16), r["kernel_ms"], peaks)
         # the CUDA-core selection kernel (tensor cores switched off), same outputs
-        rc = bench_knn(torch, L, wl, max(1, min(steps, 2)), 1, l2buf, dev, tensor_cores=False)
+        rc = bench_knn(torch, L, wl, max(1, min(steps, 2)), max(3, args.warmup), l2buf, dev, tensor_cores=False)
         out["cuda_core_selection"] = {k: rc[k] for k in ("ms_per_step", "value", "kernel_ms", "kernel")}
         out["cuda_core_selection"]["roofline"] = _roofline(rc["pairs"], LANE_OPS[4], rc["kernel_ms"], sms, peaks)
         out["cuda_core_selection"]["roofline"]["frac_direct_difference_form_33ops"] = (
