@@ -409,7 +409,7 @@ def run_gpu(args):
         "e2e": {"value": world * r2["pairs"] / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
                 "h2d_bytes_per_step": r2["e2e"]["h2d_bytes_per_step"],
                 "d2h_bytes_per_step": r2["e2e"]["d2h_bytes_per_step"], "ms_per_step": e2e_ms},
-        "gpu_launches": r2["gpu_launches"] * args.steps,
+        "gpu_launches": r2["gpu_launches"],
         "roofline": _roofline(r2["pairs"], LANE_OPS[2], r2["kernel_ms"], sms, peaks, r2["kernel"]),
         "peaks": peaks_how,
     }
