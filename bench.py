@@ -320,22 +320,24 @@ def bench_local(torch, L, l2buf, dev, sms, peaks, args):
     pi_d, pk_d = t(pi), t(pk)
     knots = L.lipfit_distance_quantiles(X, pi_d, pk_d, L.LIPFIT_LOCAL_KNOTS, wl.norm)
     f_tab = lambda: L.lipfit_local_lipschitz(X, y, knots, wl.norm)
-    ms_tab = _time_steps(torch, f_tab, max(1, min(args.steps, 3)), 2, l2buf)
+    ms_tab = _time_steps(torch, f_tab, max(1, min(args.steps, 3)), 3, l2buf)
     k_tab, _ = _kernel_ms(L, 4, f_tab, 1)
     table = f_tab()
     f_ev = lambda: L.lipfit_values_local(X, y, Xq, knots, table, wl.norm)
-    ms_ev = _time_steps(torch, f_ev, max(1, min(args.steps, 3)), 2, l2buf)
+    ms_ev = _time_steps(torch, f_ev, max(1, min(args.steps, 3)), 3, l2buf)
     k_ev, _ = _kernel_ms(L, 5, f_ev, 1)
     # executed lane-ops per pair (d = 5 padded to 8 coordinates, J = 16 knots):
-    #   table: 8 sub + 8 fma + sqrt + |dy| + divide (~8) + 15 (compare + max) pairs + last max + nn update ~ 60
-    #   eval : 8 sub + 8 fma + sqrt + 15 (compare + select) + guard 2 + 2 fma-like + min + max ~ 53
+    #   table: 8 sub + 8 fma + |dy| 2 + two-level knot search (6 compares + 5 adds) + MUFU sqrt + 2 mul + raise test
+    #          + nearest-neighbour test 3 ~ 36 on the fast path (IEEE sqrt / divide only for pairs that raise a bin)
+    #   eval : 8 sub + 8 fma + knot search 11 + MUFU sqrt + guard 2 + mul + add + sub + min + max + index math ~ 39
+    #          (counted in the SASS of local_eval_kernel<2,8,4>: 157 arithmetic instructions per record of 4 pairs)
     out = {"workload": "config 5 data (d=5, N=200000), Q=1000000, L2, J=16 knots from 1e6 sampled pairs",
            "table": {"ms_per_step": float(np.mean(ms_tab)), "kernel_ms": k_tab,
                      "value": wl.N * (wl.N - 1) / (np.mean(ms_tab) * 1e-3) / 1e9, "unit": "G ordered pairs/s",
-                     "roofline": _roofline(wl.N * wl.N, 60, k_tab, sms, peaks)},
+                     "roofline": _roofline(wl.N * wl.N, 36, k_tab, sms, peaks)},
            "evaluate": {"ms_per_step": float(np.mean(ms_ev)), "kernel_ms": k_ev,
                         "value": wl.N * wl.Q / (np.mean(ms_ev) * 1e-3) / 1e9, "unit": UNIT,
-                        "roofline": _roofline(wl.N * wl.Q, 53, k_ev, sms, peaks)}}
+                        "roofline": _roofline(wl.N * wl.Q, 39, k_ev, sms, peaks)}}
     if not args.no_cpu:
         sel = oracle_subset(wl.Q, 400)
         rows = oracle_subset(wl.N, 64)

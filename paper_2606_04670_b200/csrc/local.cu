@@ -4,8 +4,8 @@
 //       max_{i != k, D(x^k,x^i) <= t_j} |y_k - y_i| / D), last knot = +inf -- an all-pairs pass, J running
 //       maxima per row in registers, nothing of size N x N stored;
 //   (3) evaluation: Eq.(2),(3) with M replaced by M_k(D(x, x^k)): the fused bounds pass
-//       with the table row riding in the packed record and a compare/select chain for the knot lookup
-//       (the paper's torch.searchsorted).
+//       with the table row riding in the packed record and a two-level knot lookup (3 + 3 compares, the
+//       paper's torch.searchsorted) that indexes the row in shared memory.
 // Radial, symmetric weighted distance D(a,b) = ||w (a - b)||_p; J is fixed at LIPFIT_LOCAL_KNOTS = 16.
 #include <cub/device/device_radix_sort.cuh>
 
@@ -36,6 +36,23 @@ __device__ __forceinline__ void local_load_record(const float* s, float* x) {
         x[4 * c + 2] = v.z;
         x[4 * c + 3] = v.w;
     }
+}
+
+// Knot lookup (the paper's searchsorted): index of the first knot t_j >= D among t_0..t_{J-2}, J-1 if none
+// = number of those knots below D (they are sorted).  Two levels of 3 compares instead of a chain of 15
+// compare/selects: which quarter (knots 3, 7, 11 from the constant bank), then the quarter's three knots as
+// one 16-byte shared-memory word.
+static_assert(kJ == 16, "two levels of four");
+__device__ __forceinline__ void local_knot_groups(const Knots& kn, float4* sk4) {
+    if (threadIdx.x < 4) {
+        const int q = threadIdx.x;
+        sk4[q] = make_float4(kn.t[4 * q], kn.t[4 * q + 1], kn.t[4 * q + 2], 0.f);
+    }
+}
+__device__ __forceinline__ int local_knot_index(float D, const Knots& kn, const float4* sk4) {
+    const int q = (D > kn.t[3] ? 1 : 0) + (D > kn.t[7] ? 1 : 0) + (D > kn.t[11] ? 1 : 0);
+    const float4 g = sk4[q];
+    return 4 * q + (D > g.x ? 1 : 0) + (D > g.y ? 1 : 0) + (D > g.z ? 1 : 0);
 }
 
 template <int RF>
@@ -87,13 +104,24 @@ struct TableArgs {
     int N, nrb, nch, chunk;
 };
 
+// records per shared-memory tile of the table kernel: its per-thread bins take R * kJ * 512 B of the 48 KB
+template <int RF>
+__host__ __device__ constexpr int local_table_tile() {
+    return RF <= 8 ? 128 : local_tile_records<RF>() / 2;
+}
+
 template <int NORM, int DP, int R>
 __global__ void __launch_bounds__(kLocThreads, 2)
 local_table_kernel(const TableArgs a, const Knots kn) {
     constexpr int RF = DP + 4;
-    constexpr int TILE = local_tile_records<RF>();
+    constexpr int TILE = local_table_tile<RF>();
     __shared__ __align__(128) float sbuf[2 * TILE * RF];
     __shared__ __align__(8) uint64_t bars[2];
+    // running maxima per (row, bin) in thread-private shared memory ([r][j][thread]: conflict-free): a pair
+    // raises ONE bin (the first knot >= its distance); the cumulative table is a prefix maximum at the end
+    __shared__ float sM[R * kJ * kLocThreads];
+    __shared__ float4 sk4[4];
+    local_knot_groups(kn, sk4);
     if (threadIdx.x == 0) {
         mbar_init(&bars[0], 1);
         mbar_init(&bars[1], 1);
@@ -105,7 +133,8 @@ local_table_kernel(const TableArgs a, const Knots kn) {
     const int ntiles = a.nrb * a.nch;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int rb = tile / a.nch, ch = tile - rb * a.nch;
-        float xi[R][DP], yi[R], M[R][kJ], dmin[R], rnn[R];
+        float xi[R][DP], yi[R], dmin[R], dmin2[R], rnn[R];
+        float* myM = sM + threadIdx.x;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             int i = (rb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
@@ -115,8 +144,9 @@ local_table_kernel(const TableArgs a, const Knots kn) {
             for (int j = 0; j < DP; ++j) xi[r][j] = __ldg(src + j);
             yi[r] = __ldg(src + DP);
 #pragma unroll
-            for (int j = 0; j < kJ; ++j) M[r][j] = 0.f;
+            for (int j = 0; j < kJ; ++j) myM[(r * kJ + j) * kLocThreads] = 0.f;
             dmin[r] = inf;
+            dmin2[r] = inf;
             rnn[r] = 0.f;
         }
         const int begin = ch * a.chunk;
@@ -130,20 +160,29 @@ local_table_kernel(const TableArgs a, const Knots kn) {
                 local_load_record<DP + 4>(s + jrec * RF, x);
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const float D = local_finish<NORM>(PairAccU<NORM, DP, 0>::run(xi[r], x));
+                    // L2: the knots of this kernel are squared (launch_local_lipschitz): bins from the squared
+                    // distance.  The IEEE square root and quotient of the ratio are only taken by the pairs that
+                    // can raise their bin (ratio > M  <=>  dy > M D, tested with the 2-ulp MUFU root and a
+                    // 2^-20 margin so that no raise is missed) or that are a nearest neighbour so far: a few
+                    // hundred of the N pairs of a row.
+                    const float acc = PairAccU<NORM, DP, 0>::run(xi[r], x);
                     const float dy = fabsf(yi[r] - x[DP]);
-                    // self / duplicate (D = 0, same value): ratio 0 changes nothing; different value at D = 0: +inf
-                    const float ratio = D > 0.f ? __fdiv_rn(dy, D) : (dy > 0.f ? inf : 0.f);
-#pragma unroll
-                    for (int j = 0; j < kJ - 1; ++j)
-                        if (D <= kn.t[j]) M[r][j] = fmaxf(M[r][j], ratio);
-                    M[r][kJ - 1] = fmaxf(M[r][kJ - 1], ratio);
-                    const bool valid = (D > 0.f) || (dy > 0.f);
-                    if (valid && D < dmin[r]) {
-                        dmin[r] = D;
-                        rnn[r] = ratio;
-                    } else if (valid && D == dmin[r]) {
-                        rnn[r] = fmaxf(rnn[r], ratio);
+                    float* pb = myM + (r * kJ + local_knot_index(acc, kn, sk4)) * kLocThreads;
+                    const float Mb = *pb;
+                    const float Da = NORM == 2 ? fast_sqrt(acc) : acc;
+                    const bool valid = (acc > 0.f) || (dy > 0.f);  // not the row itself / an exact duplicate
+                    if (dy > Mb * Da * (1.f - 0x1p-20f) || (valid && acc <= dmin2[r])) {
+                        const float D = local_finish<NORM>(acc);
+                        // duplicate position with a different value: +inf
+                        const float ratio = D > 0.f ? __fdiv_rn(dy, D) : (dy > 0.f ? inf : 0.f);
+                        *pb = fmaxf(Mb, ratio);
+                        if (valid && acc < dmin2[r]) {
+                            dmin2[r] = acc;
+                            dmin[r] = D;
+                            rnn[r] = ratio;
+                        } else if (valid && acc == dmin2[r]) {
+                            rnn[r] = fmaxf(rnn[r], ratio);
+                        }
                     }
                 }
             }
@@ -153,9 +192,12 @@ local_table_kernel(const TableArgs a, const Knots kn) {
         for (int r = 0; r < R; ++r) {
             const int i = (rb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
             if (i < a.N) {
+                float m = 0.f;
 #pragma unroll
-                for (int j = 0; j < kJ; ++j)
-                    if (M[r][j] > 0.f) atomicMax(a.tab + static_cast<size_t>(i) * kJ + j, __float_as_uint(M[r][j]));
+                for (int j = 0; j < kJ; ++j) {
+                    m = fmaxf(m, myM[(r * kJ + j) * kLocThreads]);
+                    if (m > 0.f) atomicMax(a.tab + static_cast<size_t>(i) * kJ + j, __float_as_uint(m));
+                }
                 const unsigned long long key = (static_cast<unsigned long long>(__float_as_uint(dmin[r])) << 32) |
                                                static_cast<unsigned long long>(~__float_as_uint(rnn[r]));
                 atomicMin(a.nn + i, key);
@@ -208,6 +250,8 @@ local_eval_kernel(const EvalArgs a, const Knots kn) {
     constexpr int TILE = local_tile_records<RF>();
     __shared__ __align__(128) float sbuf[2 * TILE * RF];
     __shared__ __align__(8) uint64_t bars[2];
+    __shared__ float4 sk4[4];
+    local_knot_groups(kn, sk4);
     if (threadIdx.x == 0) {
         mbar_init(&bars[0], 1);
         mbar_init(&bars[1], 1);
@@ -236,15 +280,17 @@ local_eval_kernel(const EvalArgs a, const Knots kn) {
             const float* s = rs.acquire(t);
             const int n = rs.count(t);
             for (int jrec = 0; jrec < n; ++jrec) {
-                float x[RF];
-                local_load_record<RF>(s + jrec * RF, x);
+                float x[DP + 4];
+                local_load_record<DP + 4>(s + jrec * RF, x);
                 const float yk = x[DP];
+                const float* mk = s + jrec * RF + DP + 4;  // the datum's step table stays in shared memory
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
-                    const float D = local_finish<NORM>(PairAccU<NORM, DP, 0>::run(q[r], x));
-                    float Mk = x[DP + 4 + kJ - 1];  // first knot with D <= t_j, the last one if none
-#pragma unroll
-                    for (int j = kJ - 2; j >= 0; --j) Mk = (D <= kn.t[j]) ? x[DP + 4 + j] : Mk;
+                    // L2: the knots of this kernel are squared (launch_values_local), so the bin is decided on
+                    // the squared distance and the square root (one MUFU, <= 2 ulp) only scales M_k
+                    const float acc = PairAccU<NORM, DP, 0>::run(q[r], x);
+                    const float Mk = mk[local_knot_index(acc, kn, sk4)];
+                    const float D = NORM == 2 ? fast_sqrt(acc) : acc;
                     const float MD = D > 0.f ? Mk * D : 0.f;  // M_k may be +inf at a duplicate: inf * 0 := 0
                     U[r] = fminf(U[r], yk + MD);
                     L[r] = fmaxf(L[r], yk - MD);
@@ -301,7 +347,7 @@ int launch_table(const Ctx& c, TableArgs& a, const Knots& kn) {
     LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
-    local_schedule(a.N, kLocThreads * R, a.N, local_tile_records<DP + 4>(), slots, &a.nrb, &a.nch, &a.chunk);
+    local_schedule(a.N, kLocThreads * R, a.N, local_table_tile<DP + 4>(), slots, &a.nrb, &a.nch, &a.chunk);
     const long long nt = static_cast<long long>(a.nrb) * a.nch;
     KernelTimer kt(TK_LOCAL_TABLE, c.stream);
     kern<<<static_cast<int>(nt < slots ? nt : slots), kLocThreads, 0, c.stream>>>(a, kn);
@@ -394,8 +440,9 @@ int launch_local_lipschitz(const Ctx& c, const float* X, const float* y, int64_t
     if ((rc = launch_prepack(c, X, y, nullptr, N, xf, lay, wrec.as<float>()))) return rc;
     LIPFIT_CUDA(cudaMemsetAsync(wtab.p, 0, sizeof(uint32_t) * static_cast<size_t>(N) * kJ, c.stream));
     LIPFIT_CUDA(cudaMemsetAsync(wnn.p, 0xFF, sizeof(unsigned long long) * static_cast<size_t>(N), c.stream));
-    Knots kn;
-    for (int j = 0; j < kJ; ++j) kn.t[j] = knots_host[j];
+    Knots kn;  // L2: squared knots, correctly rounded (the kernel bins squared distances)
+    for (int j = 0; j < kJ; ++j)
+        kn.t[j] = norm == 2 ? static_cast<float>(static_cast<double>(knots_host[j]) * knots_host[j]) : knots_host[j];
     TableArgs a{};
     a.rec = wrec.as<float>();
     a.tab = wtab.as<uint32_t>();
@@ -422,8 +469,9 @@ int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N6
     local_eval_pack_kernel<<<(N + 255) / 256, 256, 0, c.stream>>>(X, y, table, N, xf, dp, wrec.as<float>());
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
-    Knots kn;
-    for (int j = 0; j < kJ; ++j) kn.t[j] = knots_host[j];
+    Knots kn;  // L2: squared knots, correctly rounded (the kernel compares squared distances with them)
+    for (int j = 0; j < kJ; ++j)
+        kn.t[j] = norm == 2 ? static_cast<float>(static_cast<double>(knots_host[j]) * knots_host[j]) : knots_host[j];
     EvalArgs a{};
     a.rec = wrec.as<float>();
     a.Xq = Xq;
