@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- measures the LipFit hot path on B200 (contract: task prompt, "Measurement").
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--configs 2[,1,3,4,5]]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--configs 2[,1,3,4,5,6,7,8]]
 
 One "step" = one pass of the hot path over one batch of synthetic input of the bench workload:
 BASELINE.json configs[1] (d=4, N=1e5 data, Q=1e6 queries, weighted L1, mask [+1,+1,0,0], M=8) through
@@ -444,7 +444,7 @@ def run_gpu(args):
 
 def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
     import oracle
-    wl = make_workload(5 if c == 6 else c)
+    wl = make_workload({6: 5, 7: 2, 8: 5}.get(c, c))
     steps = max(1, min(args.steps, 3)) if c in (3, 4) else args.steps
     out = {}
     if c in (1, 3):
@@ -504,6 +504,43 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
                              "queries": int(len(sel))}
     elif c == 6:
         out.update(bench_local(torch, L, l2buf, dev, sms, peaks, args))
+    elif c == 7:
+        # NEXT-2: weighted sums of the k = 4 best bound values on the config 2 workload
+        wk = np.array([0.4, 0.3, 0.2, 0.1], dtype=np.float32)
+        t = lambda a: torch.from_numpy(a).to(dev)
+        X, y, Xq = t(wl.X), t(wl.y), t(wl.Xq)
+        fn = lambda: L.lipfit_bounds_topk(X, y, Xq, wl.M, wk, wl.mask, wl.norm, wl.weights)
+        ms = _time_steps(torch, fn, steps, 3, l2buf)
+        pairs = wl.N * wl.Q
+        out.update({"workload": "config 2 data and queries, k = 4 best bounds with weights [0.4, 0.3, 0.2, 0.1]",
+                    "ms_per_step": float(np.mean(ms)), "value": pairs / (np.mean(ms) * 1e-3) / 1e9, "unit": UNIT,
+                    "kernel": "bounds_topk<L1,DP4> (generic distance, 2 x 8 sorted lists in registers)"})
+        if not args.no_cpu:
+            sel = oracle_subset(wl.Q, 2000)
+            ref = oracle.bounds_topk(wl.X, wl.y, wl.Xq[sel], wl.M, wk, wl.mask, wl.norm, wl.weights)
+            out["parity"] = parity_bounds(wl, fn(), sel, ref)
+    elif c == 8:
+        # NEXT-3: smallest consistent Lipschitz constant of the config 5 data
+        t = lambda a: torch.from_numpy(a).to(dev)
+        X, y = t(wl.X), t(wl.y)
+        # (symmetric distance: under the config's monotone mask the noisy data violate monotonicity, L = +inf)
+        fn = lambda: L.lipfit_lipschitz_constant(X, y, None, wl.norm, wl.weights)
+        ms = _time_steps(torch, fn, steps, 3, l2buf)
+        kms, _ = _kernel_ms(L, 3, fn, 1)
+        pairs = wl.N * (wl.N - 1)
+        out.update({"workload": "config 5 data (d=5, N=200000, L2), symmetric distance",
+                    "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+                    "unit": "G ordered pairs/s (each unordered pair is visited once)",
+                    "L": float(fn().cpu().numpy()[0]),
+                    # fast path per visited unordered pair (source count, d = 5 symmetric L2): 5 sub + 5 fma + dy +
+                    # |dy| + 2 mul + 1 compare of dy^2 against L^2 D^2 + loop share ~ 16; survivors take the fp64 ratio
+                    "roofline": _roofline(pairs // 2, 16, kms, sms, peaks)})
+        if not args.no_cpu:
+            # the oracle is O(N^2) on the host: compare on the first 20000 data (4e8 ordered pairs)
+            n = 20000
+            ref = oracle.lipschitz_constant(wl.X[:n], wl.y[:n], None, wl.norm, wl.weights)
+            got = float(L.lipfit_lipschitz_constant(t(wl.X[:n]), t(wl.y[:n]), None, wl.norm, wl.weights).cpu().numpy()[0])
+            out["parity"] = {"data": n, "oracle": ref, "gpu": got, "ok": bool(got == float(np.float32(ref)))}
     elif c == 5:
         r = bench_smooth(torch, L, wl, l2buf, dev)
         out.update({"smooth_wall_s": r["wall_s"], "info": r["info"], "evals": r["evals"],
@@ -536,7 +573,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--configs", default="2",
-                    help="comma list of BASELINE.json configs to report (2 always); 6 = local Lipschitz (NEXT-1)")
+                    help="comma list of BASELINE.json configs to report (2 always); 6 = local Lipschitz (NEXT-1), "
+                         "7 = top-k bounds (NEXT-2), 8 = Lipschitz constant (NEXT-3)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
