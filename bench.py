@@ -444,7 +444,7 @@ def run_gpu(args):
 
 def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
     import oracle
-    wl = make_workload({6: 5, 7: 2, 8: 5}.get(c, c))
+    wl = make_workload({6: 5, 7: 2, 8: 5, 9: 2, 10: 3, 11: 5}.get(c, c))
     steps = max(1, min(args.steps, 3)) if c in (3, 4) else args.steps
     out = {}
     if c in (1, 3):
@@ -519,6 +519,34 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
             sel = oracle_subset(wl.Q, 2000)
             ref = oracle.bounds_topk(wl.X, wl.y, wl.Xq[sel], wl.M, wk, wl.mask, wl.norm, wl.weights)
             out["parity"] = parity_bounds(wl, fn(), sel, ref)
+    elif c in (9, 10, 11):
+        # NEXT-4(ii): bounds with EXACT spatial pruning on the config 2 / 3 / 5 workloads.  "Effective" pairs/s =
+        # Q N / step time (the work the unpruned path would do), reported beside the pairs actually evaluated;
+        # never mixed into the brute-force roofline numbers above.
+        t = lambda a: torch.from_numpy(a).to(dev)
+        X, y, Xq = t(wl.X), t(wl.y), t(wl.Xq)
+        fn = lambda: L.lipfit_bounds_pruned(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
+        steps_p = max(1, min(args.steps, 3)) if c == 10 else args.steps
+        ms = _time_steps(torch, fn, steps_p, 3, l2buf)
+        kms, _ = _kernel_ms(L, 6, fn, 1)
+        *outs, evaluated = L.lipfit_bounds_pruned(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights, count_pairs=True)
+        pairs = wl.N * wl.Q
+        fb = lambda: L.lipfit_bounds(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
+        ms_b = _time_steps(torch, fb, 1 if c == 10 else 2, 1, l2buf)
+        ub = fb()
+        out.update({"workload": "config %d data and queries" % {9: 2, 10: 3, 11: 5}[c],
+                    "ms_per_step": float(np.mean(ms)), "kernel_ms": kms,
+                    "value": pairs / (np.mean(ms) * 1e-3) / 1e9, "unit": "effective " + UNIT,
+                    "pairs_evaluated": int(evaluated), "fraction_evaluated": evaluated / pairs,
+                    "evaluated_rate_gpairs_s": evaluated / (kms * 1e-3) / 1e9,
+                    "unpruned_ms_per_step": float(np.mean(ms_b)),
+                    "speedup_over_unpruned": float(np.mean(ms_b) / np.mean(ms)),
+                    "max_abs_diff_vs_unpruned": max(float((a - b).abs().max()) for a, b in zip(outs, ub)),
+                    "kernel": "bounds_pruned<norm,DP> (Morton-sorted 32-datum tiles, box tests, generic distance)"})
+        if not args.no_cpu:
+            sel = oracle_subset(wl.Q, 2000 if c != 10 else 96)
+            ref = oracle.bounds(wl.X, wl.y, wl.Xq[sel], wl.M, wl.mask, wl.norm, wl.weights)
+            out["parity"] = parity_bounds(wl, outs, sel, ref)
     elif c == 8:
         # NEXT-3: smallest consistent Lipschitz constant of the config 5 data
         t = lambda a: torch.from_numpy(a).to(dev)
@@ -574,7 +602,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--configs", default="2",
                     help="comma list of BASELINE.json configs to report (2 always); 6 = local Lipschitz (NEXT-1), "
-                         "7 = top-k bounds (NEXT-2), 8 = Lipschitz constant (NEXT-3)")
+                         "7 = top-k bounds (NEXT-2), 8 = Lipschitz constant (NEXT-3), 9 / 10 / 11 = exactly pruned bounds on the "
+                         "config 2 / 3 / 5 workloads (NEXT-4(ii))")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -96,6 +96,24 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
                        const float* wk /* host[k] */, float* upper, float* lower, float* g,
                        void* cuda_stream);
 
+/* ---- NEXT-4(ii): the same upper / lower / g as lipfit_bounds, evaluated with EXACT spatial pruning ----
+ * (the exact counterpart of the heuristic of PAPER.md:214-218, which keeps only data close to the
+ * query).  Data and queries are sorted along a Morton curve of the transformed coordinates; tiles of
+ * 32 data carry a bounding box and the range of their values; a tile is skipped for a group of
+ * queries when  ymin + M dlb^u >= every running upper bound  and  ymax - M dlb^l <= every running
+ * lower bound  of the group (dlb = smallest possible distance between the boxes), which proves that
+ * no datum of the tile can change a minimum of Eq.(2) or a maximum of Eq.(3).  The result is the
+ * min / max over ALL N data of the per-pair fp32 arithmetic; only the number of pairs evaluated
+ * changes (by orders of magnitude for low d, not at all in the worst case).
+ * Arguments, layout, ownership and error behaviour as lipfit_bounds.  pairs_evaluated: HOST int64
+ * or NULL; when non-NULL the call synchronises the stream and stores the number of (query, datum)
+ * pairs whose distance was actually computed (Q N for the unpruned path). */
+int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d,
+                         const float* Xq, int64_t Q, float M,
+                         const int32_t* mono_mask, int32_t norm, const float* weights,
+                         float* upper, float* lower, float* g, int64_t* pairs_evaluated /* host */,
+                         void* cuda_stream);
+
 /* ---- k nearest data per query by distance (d_(1) <= d_(2) <= ...) -------------
  * side 0: symmetric weighted norm, mask ignored; +1: D^u; -1: D^l.
  * idx [Q*k] int32 and dist [Q*k] fp32, row-major, ascending distance per query.
@@ -207,7 +225,7 @@ const char* lipfit_version(void);
 int64_t lipfit_launch_count(void);
 /* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
  * resets the accumulators and makes every later launch of the three dominant kernels
- * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation) bracketed by CUDA events on
+ * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation, 6 = pruned bounds) bracketed by CUDA events on
  * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
  * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);

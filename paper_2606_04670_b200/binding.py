@@ -25,6 +25,7 @@ EXPORTS = [
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
     "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
+    "lipfit_bounds_pruned",
 ]
 LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
@@ -67,6 +68,7 @@ def load():
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
     lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
     lib.lipfit_lbfgs.argtypes = [i64, P, EVAL_FN, P, i32, f64, i32, P]
+    lib.lipfit_bounds_pruned.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, P, P, P, P, P]
     lib.lipfit_bounds_topk.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, i32, P, P, P, P, P]
     lib.lipfit_distance_quantiles.argtypes = [P, i64, i32, i32, P, P, P, i64, i32, P, P]
     lib.lipfit_local_lipschitz.argtypes = [P, P, i64, i32, i32, P, P, i32, P, P]
@@ -202,6 +204,25 @@ def lipfit_bounds(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, wei
                               ptr["g"], _stream(stream))
     _check(rc, "lipfit_bounds")
     return outs["upper"], outs["lower"], outs["g"]
+
+
+def lipfit_bounds_pruned(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                         count_pairs: bool = False, stream=None):
+    """(upper, lower, g[, pairs_evaluated]) as lipfit_bounds, evaluated with exact spatial pruning."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    if Xq.shape[1] != d or y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    m, w = _host_params(d, mono_mask, weights)
+    outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    n = C.c_int64(0)
+    rc = load().lipfit_bounds_pruned(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(m),
+                                     int(norm), _np_ptr(w), outs[0].data_ptr(), outs[1].data_ptr(),
+                                     outs[2].data_ptr(), C.byref(n) if count_pairs else None, _stream(stream))
+    _check(rc, "lipfit_bounds_pruned")
+    return (*outs, int(n.value)) if count_pairs else tuple(outs)
 
 
 def lipfit_bounds_topk(X, y, Xq, M: float, wk, mono_mask=None, norm: int = LIPFIT_L2, weights=None,

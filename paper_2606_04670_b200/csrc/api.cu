@@ -112,6 +112,42 @@ int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const fl
     return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g);
 }
 
+int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
+                         float* lower, float* g, int64_t* pairs_evaluated, void* cuda_stream) {
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    if (!X || !y) return LIPFIT_E_NULL;
+    if (Q == 0) {
+        if (pairs_evaluated) *pairs_evaluated = 0;
+        return LIPFIT_OK;
+    }
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    Workspace stats;
+    if (pairs_evaluated) {
+        rc = stats.alloc(2 * sizeof(unsigned long long), c.stream);
+        if (rc) return rc;
+        LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 2 * sizeof(unsigned long long), c.stream));
+    }
+    rc = launch_bounds_pruned(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g,
+                              stats.as<unsigned long long>());
+    if (rc) return rc;
+    if (pairs_evaluated) {
+        unsigned long long h[2] = {0, 0};
+        LIPFIT_CUDA(cudaMemcpyAsync(h, stats.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+        LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+        *pairs_evaluated = static_cast<int64_t>(h[0]) * 1024;
+    }
+    return LIPFIT_OK;
+}
+
 int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                        float M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
                        const float* wk, float* upper, float* lower, float* g, void* cuda_stream) {

@@ -38,6 +38,12 @@ RecLayout bounds_topk_layout(const Xform& xf);
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                        int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g);
 
+// NEXT-4(ii): bounds with exact spatial pruning (prune.cu); X, Xq: ORIGINAL row-major arrays.
+// stats_dev: device uint64[2] (zeroed by the caller) or NULL: [0] += tiles of 32 x 32 pairs evaluated.
+int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
+                         const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
+                         unsigned long long* stats_dev);
+
 // a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                int norm, int k, int32_t* idx, float* dist);

@@ -1,0 +1,458 @@
+// prune.cu -- NEXT-4(ii): Eq.(2),(3) PAPER.md:103-116 evaluated EXACTLY with spatial pruning.
+//
+// The paper prunes with a heuristic ("only the data within M/3 ..." PAPER.md:214-218).  Here the
+// pruning is exact: data and queries are sorted along a Morton curve of the packed coordinates;
+// 32 consecutive data form a tile with a bounding box [lo, hi] and the range [ymin, ymax] of its
+// values, 32 consecutive queries form a warp with a bounding box.  For a tile t and a set of
+// queries B
+//     y^k + M D^u(q, x^k) >= ymin_t + M dlb^u(B, t)      for every q in B, k in t
+//     y^k - M D^l(q, x^k) <= ymax_t - M dlb^l(B, t)
+// where dlb is the norm of the componentwise smallest possible |delta| / relu(+-delta) between
+// the two boxes.  A tile whose first quantity is not below the largest running upper bound of B
+// and whose second is not above the smallest running lower bound of B cannot change any running
+// extremum and is skipped.  Two stages: (1) lane = tile, warp box against tile box with the
+// warp-wide extrema; (2) per surviving tile, lane = query, the query point against the tile box
+// with the lane's own running bounds, the tile is evaluated if any lane needs it.  Running bounds
+// are seeded from the tile(s) at the queries' own Morton position.
+//
+// Exactness in fp32: a pair is evaluated as fmaf(M, D, y) with D the rounded norm; the box
+// distance is scaled by (1 - 1e-5), which covers the rounding of both norms ((DP + 3) 2^-24 each),
+// and fmaf is monotone in its addend and multiplicand, so the computed tile bound never exceeds a
+// computed pair value of that tile: the result is the min / max over all N data of the same
+// per-pair arithmetic, whatever was skipped.
+#include <cub/device/device_radix_sort.cuh>
+
+#include "kernels.h"
+
+namespace lipfit {
+
+namespace {
+
+constexpr int kTile = 32;  // data per tile = lanes per warp
+
+struct PruneGrid {
+    int bits;  // Morton bits per packed coordinate
+    int d;
+};
+
+// ---- coordinate ranges of the packed data -----------------------------------------------------
+__global__ void prune_range_init_kernel(uint32_t* keys) {
+    int j = threadIdx.x;
+    if (j < kMaxDim) {
+        keys[j] = 0xFFFFFFFFu;      // running minimum
+        keys[kMaxDim + j] = 0u;     // running maximum
+    }
+}
+
+__global__ void __launch_bounds__(256)
+prune_range_kernel(const float* __restrict__ X, int N, Xform xf, uint32_t* __restrict__ keys) {
+    __shared__ uint32_t smin[kMaxDim], smax[kMaxDim];
+    if (threadIdx.x < kMaxDim) {
+        smin[threadIdx.x] = 0xFFFFFFFFu;
+        smax[threadIdx.x] = 0u;
+    }
+    __syncthreads();
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
+        const float* src = X + static_cast<size_t>(k) * xf.d;
+        for (int j = 0; j < xf.d; ++j) {
+            uint32_t key = f2key(xf.sw[j] * src[xf.perm[j]]);
+            atomicMin(&smin[j], key);
+            atomicMax(&smax[j], key);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < xf.d) {
+        atomicMin(&keys[threadIdx.x], smin[threadIdx.x]);
+        atomicMax(&keys[kMaxDim + threadIdx.x], smax[threadIdx.x]);
+    }
+}
+
+// Morton key of one point: cell index per coordinate inside the data range (clamped), bits
+// interleaved, coordinate 0 most significant within a level.
+__device__ __forceinline__ uint64_t morton_key(const float* __restrict__ src, const Xform& xf,
+                                               const uint32_t* __restrict__ keys, int bits) {
+    uint32_t cell[kMaxDim];
+    const float cells = static_cast<float>(1u << bits);
+    for (int j = 0; j < xf.d; ++j) {
+        float lo = key2f(keys[j]), hi = key2f(keys[kMaxDim + j]);
+        float v = xf.sw[j] * src[xf.perm[j]];
+        float w = hi - lo;
+        float t = w > 0.f ? (v - lo) / w * cells : 0.f;
+        t = fminf(fmaxf(t, 0.f), cells - 1.f);
+        cell[j] = static_cast<uint32_t>(t);
+    }
+    uint64_t key = 0;
+    for (int b = bits - 1; b >= 0; --b)
+        for (int j = 0; j < xf.d; ++j) key = (key << 1) | ((cell[j] >> b) & 1u);
+    return key;
+}
+
+__global__ void __launch_bounds__(256)
+prune_keys_kernel(const float* __restrict__ P, int n, Xform xf, const uint32_t* __restrict__ keys, int bits,
+                  uint64_t* __restrict__ out, int32_t* __restrict__ ids) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    out[k] = morton_key(P + static_cast<size_t>(k) * xf.d, xf, keys, bits);
+    ids[k] = k;
+}
+
+// ---- sorted records and tile boxes: one warp per tile, lane = record --------------------------
+// rec : ntiles * 32 records of RF = DP + 4 floats [x'_0 .. x'_{DP-1}, y, 0, 0, 0]; the last tile is
+//       filled up with copies of the last datum (they change no minimum or maximum)
+// box : ntiles * (2 DP + 4) floats [lo_0 .. lo_{DP-1}, hi_0 .. hi_{DP-1}, ymin, ymax, 0, 0]
+template <int DP>
+__global__ void __launch_bounds__(128)
+prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xf,
+                    const int32_t* __restrict__ order, int ntiles, float* __restrict__ rec,
+                    float* __restrict__ box) {
+    constexpr int RF = DP + 4, BF = 2 * DP + 4;
+    const int lane = threadIdx.x & 31;
+    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (t >= ntiles) return;
+    int pos = t * kTile + lane;
+    if (pos >= N) pos = N - 1;
+    const int k = order[pos];
+    const float* src = X + static_cast<size_t>(k) * xf.d;
+    float v[DP];
+#pragma unroll
+    for (int j = 0; j < DP; ++j) v[j] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : 0.f;
+    const float yv = y[k];
+    float4* dst = reinterpret_cast<float4*>(rec + (static_cast<size_t>(t) * kTile + lane) * RF);
+#pragma unroll
+    for (int j = 0; j < DP; j += 4) dst[j >> 2] = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+    dst[DP >> 2] = make_float4(yv, 0.f, 0.f, 0.f);
+    float* b = box + static_cast<size_t>(t) * BF;
+#pragma unroll
+    for (int j = 0; j < DP; ++j) {
+        float lo = v[j], hi = v[j];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        if (lane == 0) {
+            b[j] = lo;
+            b[DP + j] = hi;
+        }
+    }
+    float ylo = yv, yhi = yv;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        ylo = fminf(ylo, __shfl_xor_sync(0xffffffffu, ylo, o));
+        yhi = fmaxf(yhi, __shfl_xor_sync(0xffffffffu, yhi, o));
+    }
+    if (lane == 0) {
+        b[2 * DP] = ylo;
+        b[2 * DP + 1] = yhi;
+        b[2 * DP + 2] = 0.f;
+        b[2 * DP + 3] = 0.f;
+    }
+}
+
+// ---- box distances -----------------------------------------------------------------------------
+// Smallest possible D^u and D^l between a query box [qlo, qhi] and a tile box [tlo, thi]
+// (delta = q - x):  a = qlo - thi <= delta <= qhi - tlo = -b.
+//   unconstrained: |delta| >= max(a, b, 0) on both sides
+//   constrained  : relu(delta) >= max(a, 0),  relu(-delta) >= max(b, 0)
+template <int NORM, int DP>
+__device__ __forceinline__ void box_lb(const float* __restrict__ qlo, const float* __restrict__ qhi,
+                                       const float* __restrict__ tb, const FreeFlags& ff, float& du,
+                                       float& dl) {
+    float pu = 0.f, pl = 0.f;
+#pragma unroll
+    for (int j = 0; j < DP; ++j) {
+        float a = qlo[j] - tb[DP + j];
+        float b = tb[j] - qhi[j];
+        float u = fmaxf(fmaxf(a, ff.fr[j] * b), 0.f);
+        float l = fmaxf(fmaxf(b, ff.fr[j] * a), 0.f);
+        if (NORM == 1) {
+            pu += u;
+            pl += l;
+        }
+        if (NORM == 2) {
+            pu = fmaf(u, u, pu);
+            pl = fmaf(l, l, pl);
+        }
+        if (NORM == 3) {
+            pu = fmaxf(pu, u);
+            pl = fmaxf(pl, l);
+        }
+    }
+    constexpr float kShrink = 1.f - 1e-5f;  // covers the rounding of this norm and of the pair's norm
+    du = (NORM == 2 ? fast_sqrt(pu) : pu) * kShrink;
+    dl = (NORM == 2 ? fast_sqrt(pl) : pl) * kShrink;
+}
+
+struct PruneArgs {
+    const float* Xq;
+    const int32_t* qorder;     // sorted position -> original query
+    const uint64_t* qkeys;     // sorted Morton keys of the queries
+    const uint64_t* dkeys;     // sorted Morton keys of the data
+    const float* rec;
+    const float* box;
+    int N, Q, ntiles;
+    float M;
+    Xform xf;
+    FreeFlags ff;
+    float *upper, *lower, *g;
+    unsigned long long* stats;  // [0] tiles evaluated (x 1024 pairs), [1] stage-1 survivors
+};
+
+template <int NORM, int DP>
+__device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, const float* q,
+                                          const FreeFlags& ff, float M, float& U, float& L) {
+    constexpr int RF = DP + 4;
+    const float4* r4 = reinterpret_cast<const float4*>(rec + static_cast<size_t>(t) * kTile * RF);
+#pragma unroll 4
+    for (int r = 0; r < kTile; ++r) {
+        float x[DP];
+#pragma unroll
+        for (int j = 0; j < DP; j += 4) {
+            float4 v = __ldg(r4 + r * (RF / 4) + (j >> 2));
+            x[j] = v.x;
+            x[j + 1] = v.y;
+            x[j + 2] = v.z;
+            x[j + 3] = v.w;
+        }
+        const float yv = __ldg(r4 + r * (RF / 4) + (DP >> 2)).x;
+        float au, al;
+        PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+        U = fminf(U, fmaf(M, PairAccGeneric<NORM, DP>::finish(au), yv));
+        L = fmaxf(L, fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), yv));
+    }
+}
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+template <int NORM, int DP>
+__global__ void __launch_bounds__(128)
+bounds_pruned_kernel(const PruneArgs a) {
+    constexpr int BF = 2 * DP + 4;
+    const int lane = threadIdx.x & 31;
+    const int nwarps = (a.Q + 31) >> 5;
+    unsigned long long n_eval = 0, n_surv = 0;
+    for (int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < nwarps;
+         w += gridDim.x * (blockDim.x >> 5)) {
+        const int pos = min(w * 32 + lane, a.Q - 1);
+        const bool live = (w * 32 + lane) < a.Q;
+        const int qi = a.qorder[pos];
+        const float* src = a.Xq + static_cast<size_t>(qi) * a.xf.d;
+        float q[DP];
+#pragma unroll
+        for (int j = 0; j < DP; ++j) q[j] = (j < a.xf.d) ? a.xf.sw[j] * src[a.xf.perm[j]] : 0.f;
+        float qlo[DP], qhi[DP];
+#pragma unroll
+        for (int j = 0; j < DP; ++j) {
+            qlo[j] = warp_min(q[j]);
+            qhi[j] = warp_max(q[j]);
+        }
+        // seed: the tile at the lane's own Morton position among the data
+        int mytile;
+        {
+            const uint64_t key = a.qkeys[pos];
+            int lo = 0, hi = a.N;  // first datum with key >= the query's
+            while (lo < hi) {
+                int mid = (lo + hi) >> 1;
+                if (a.dkeys[mid] < key) lo = mid + 1;
+                else hi = mid;
+            }
+            mytile = min(lo, a.N - 1) / kTile;
+        }
+        float U = __int_as_float(0x7f800000), L = __int_as_float(0xff800000);
+        {
+            unsigned todo = 0xffffffffu;
+            while (todo) {
+                const int t = __shfl_sync(0xffffffffu, mytile, __ffs(todo) - 1);
+                eval_tile<NORM, DP>(a.rec, t, q, a.ff, a.M, U, L);
+                ++n_eval;
+                todo &= ~__ballot_sync(0xffffffffu, mytile == t);
+            }
+        }
+        float Umax = warp_max(U), Lmin = warp_min(L);
+        for (int tb = 0; tb < a.ntiles; tb += 32) {
+            const int t = tb + lane;
+            bool need = false;
+            if (t < a.ntiles) {
+                const float* b = a.box + static_cast<size_t>(t) * BF;
+                float tbx[2 * DP];
+#pragma unroll
+                for (int j = 0; j < 2 * DP; j += 4) {
+                    float4 v = __ldg(reinterpret_cast<const float4*>(b + j));
+                    tbx[j] = v.x;
+                    tbx[j + 1] = v.y;
+                    tbx[j + 2] = v.z;
+                    tbx[j + 3] = v.w;
+                }
+                const float4 yy = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
+                float du, dl;
+                box_lb<NORM, DP>(qlo, qhi, tbx, a.ff, du, dl);
+                need = (fmaf(a.M, du, yy.x) < Umax) || (fmaf(-a.M, dl, yy.y) > Lmin);
+            }
+            unsigned surv = __ballot_sync(0xffffffffu, need);
+            if (!surv) continue;
+            bool any_eval = false;
+            while (surv) {
+                const int s = __ffs(surv) - 1;
+                surv &= surv - 1;
+                const int ts = tb + s;
+                ++n_surv;
+                if (__any_sync(0xffffffffu, mytile == ts)) continue;  // evaluated as a seed
+                // stage 2: the lane's own query against the tile box, with its own running bounds
+                const float* b = a.box + static_cast<size_t>(ts) * BF;
+                float tbx[2 * DP];
+#pragma unroll
+                for (int j = 0; j < 2 * DP; j += 4) {
+                    float4 v = __ldg(reinterpret_cast<const float4*>(b + j));
+                    tbx[j] = v.x;
+                    tbx[j + 1] = v.y;
+                    tbx[j + 2] = v.z;
+                    tbx[j + 3] = v.w;
+                }
+                const float4 yy = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
+                float du, dl;
+                box_lb<NORM, DP>(q, q, tbx, a.ff, du, dl);
+                const bool mine = (fmaf(a.M, du, yy.x) < U) || (fmaf(-a.M, dl, yy.y) > L);
+                if (!__any_sync(0xffffffffu, mine)) continue;
+                eval_tile<NORM, DP>(a.rec, ts, q, a.ff, a.M, U, L);
+                ++n_eval;
+                any_eval = true;
+            }
+            if (any_eval) {
+                Umax = warp_max(U);
+                Lmin = warp_min(L);
+            }
+        }
+        if (live) {
+            if (a.upper) a.upper[qi] = U;
+            if (a.lower) a.lower[qi] = L;
+            if (a.g) a.g[qi] = 0.5f * (U + L);
+        }
+    }
+    if (a.stats && lane == 0) {
+        atomicAdd(&a.stats[0], n_eval);
+        atomicAdd(&a.stats[1], n_surv);
+    }
+}
+
+template <int NORM, int DP>
+int launch_pruned_t(const Ctx& c, const float* X, const float* y, int N, const int32_t* dorder, int ntiles,
+                    float* rec, float* box, const PruneArgs& a) {
+    prune_gather_kernel<DP><<<(ntiles + 3) / 4, 128, 0, c.stream>>>(X, y, N, a.xf, dorder, ntiles, rec, box);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    const int nwarps = (a.Q + 31) / 32;
+    int occ = 0;
+    LIPFIT_CUDA(occupancy_of(&occ, bounds_pruned_kernel<NORM, DP>, 128, 0));
+    if (occ < 1) occ = 1;
+    int grid = (nwarps + 3) / 4;
+    const int cap = c.num_sms * occ * 4;  // a few waves: warps differ in the number of surviving tiles
+    if (grid > cap) grid = cap;
+    KernelTimer kt(TK_BOUNDS_PRUNED, c.stream);
+    bounds_pruned_kernel<NORM, DP><<<grid, 128, 0, c.stream>>>(a);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+template <int NORM>
+int launch_pruned_n(int dp, const Ctx& c, const float* X, const float* y, int N, const int32_t* dorder,
+                    int ntiles, float* rec, float* box, const PruneArgs& a) {
+    switch (dp) {
+        case 4: return launch_pruned_t<NORM, 4>(c, X, y, N, dorder, ntiles, rec, box, a);
+        case 8: return launch_pruned_t<NORM, 8>(c, X, y, N, dorder, ntiles, rec, box, a);
+        case 16: return launch_pruned_t<NORM, 16>(c, X, y, N, dorder, ntiles, rec, box, a);
+        default: return launch_pruned_t<NORM, 32>(c, X, y, N, dorder, ntiles, rec, box, a);
+    }
+}
+
+// Morton keys of n points, sorted; order[i] = original index of the i-th point along the curve.
+int sorted_keys(const Ctx& c, const float* P, int n, const Xform& xf, const uint32_t* range, int bits,
+                Workspace& keys_sorted, Workspace& order) {
+    Workspace keys_in, ids_in, tmp;
+    int rc = keys_in.alloc(sizeof(uint64_t) * n, c.stream);
+    if (rc) return rc;
+    if ((rc = ids_in.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    if ((rc = keys_sorted.alloc(sizeof(uint64_t) * n, c.stream))) return rc;
+    if ((rc = order.alloc(sizeof(int32_t) * n, c.stream))) return rc;
+    prune_keys_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(P, n, xf, range, bits, keys_in.as<uint64_t>(),
+                                                             ids_in.as<int32_t>());
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    size_t tmp_bytes = 0;
+    const int end_bit = bits * xf.d > 0 ? bits * xf.d : 1;
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys_in.as<uint64_t>(),
+                                                keys_sorted.as<uint64_t>(), ids_in.as<int32_t>(),
+                                                order.as<int32_t>(), n, 0, end_bit, c.stream));
+    if ((rc = tmp.alloc(tmp_bytes, c.stream))) return rc;
+    LIPFIT_CUDA(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, keys_in.as<uint64_t>(),
+                                                keys_sorted.as<uint64_t>(), ids_in.as<int32_t>(),
+                                                order.as<int32_t>(), n, 0, end_bit, c.stream));
+    return LIPFIT_OK;
+}
+
+}  // namespace
+
+int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N64, const float* Xq,
+                         int64_t Q64, const Xform& xf, int norm, float M, float* upper, float* lower,
+                         float* g, unsigned long long* stats_dev) {
+    const int N = static_cast<int>(N64), Q = static_cast<int>(Q64);
+    const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
+    int bits = 63 / xf.d;
+    if (bits > 16) bits = 16;
+    const int ntiles = (N + kTile - 1) / kTile;
+
+    Workspace range, dkeys, dorder, qkeys, qorder, rec, box;
+    int rc = range.alloc(sizeof(uint32_t) * 2 * kMaxDim, c.stream);
+    if (rc) return rc;
+    prune_range_init_kernel<<<1, 32, 0, c.stream>>>(range.as<uint32_t>());
+    int rgrid = (N + 255) / 256;
+    if (rgrid > c.num_sms * 8) rgrid = c.num_sms * 8;
+    prune_range_kernel<<<rgrid, 256, 0, c.stream>>>(X, N, xf, range.as<uint32_t>());
+    g_launches += 2;
+    LIPFIT_CUDA(cudaGetLastError());
+    if ((rc = sorted_keys(c, X, N, xf, range.as<uint32_t>(), bits, dkeys, dorder))) return rc;
+    if ((rc = sorted_keys(c, Xq, Q, xf, range.as<uint32_t>(), bits, qkeys, qorder))) return rc;
+    if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
+    if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
+
+    PruneArgs a;
+    a.Xq = Xq;
+    a.qorder = qorder.as<int32_t>();
+    a.qkeys = qkeys.as<uint64_t>();
+    a.dkeys = dkeys.as<uint64_t>();
+    a.rec = rec.as<float>();
+    a.box = box.as<float>();
+    a.N = N;
+    a.Q = Q;
+    a.ntiles = ntiles;
+    a.M = M;
+    a.xf = xf;
+    a.ff = make_free_flags(xf);
+    a.upper = upper;
+    a.lower = lower;
+    a.g = g;
+    a.stats = stats_dev;
+    switch (norm) {
+        case LIPFIT_L1:
+            return launch_pruned_n<1>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
+                                      box.as<float>(), a);
+        case LIPFIT_L2:
+            return launch_pruned_n<2>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
+                                      box.as<float>(), a);
+        default:
+            return launch_pruned_n<3>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
+                                      box.as<float>(), a);
+    }
+}
+
+}  // namespace lipfit
