@@ -105,9 +105,11 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
  * no datum of the tile can change a minimum of Eq.(2) or a maximum of Eq.(3).  The result is the
  * min / max over ALL N data of the per-pair fp32 arithmetic; only the number of pairs evaluated
  * changes (by orders of magnitude for low d, not at all in the worst case).
- * Arguments, layout, ownership and error behaviour as lipfit_bounds.  pairs_evaluated: HOST int64
- * or NULL; when non-NULL the call synchronises the stream and stores the number of (query, datum)
- * pairs whose distance was actually computed (Q N for the unpruned path). */
+ * Arguments, layout, ownership and error behaviour as lipfit_bounds.  pairs_evaluated: HOST int64[3]
+ * or NULL; when non-NULL the call synchronises the stream and stores [0] the number of (query, datum)
+ * pairs whose distance was actually computed (Q N for the unpruned path), [1] the number of
+ * (query group, tile) combinations that passed the box-to-box test, [2] the number of (query, tile)
+ * combinations whose own point-to-box test asked for an evaluated tile (diagnostics). */
 int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d,
                          const float* Xq, int64_t Q, float M,
                          const int32_t* mono_mask, int32_t norm, const float* weights,

@@ -217,12 +217,14 @@ def lipfit_bounds_pruned(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_
         raise ValueError("shape mismatch")
     m, w = _host_params(d, mono_mask, weights)
     outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
-    n = C.c_int64(0)
+    n = (C.c_int64 * 3)()
     rc = load().lipfit_bounds_pruned(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(m),
                                      int(norm), _np_ptr(w), outs[0].data_ptr(), outs[1].data_ptr(),
-                                     outs[2].data_ptr(), C.byref(n) if count_pairs else None, _stream(stream))
+                                     outs[2].data_ptr(), n if count_pairs else None, _stream(stream))
     _check(rc, "lipfit_bounds_pruned")
-    return (*outs, int(n.value)) if count_pairs else tuple(outs)
+    if count_pairs == "all":
+        return (*outs, [int(v) for v in n])
+    return (*outs, int(n[0])) if count_pairs else tuple(outs)
 
 
 def lipfit_bounds_topk(X, y, Xq, M: float, wk, mono_mask=None, norm: int = LIPFIT_L2, weights=None,

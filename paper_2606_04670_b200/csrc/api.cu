@@ -123,7 +123,7 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
     if (rc) return rc;
     if (!X || !y) return LIPFIT_E_NULL;
     if (Q == 0) {
-        if (pairs_evaluated) *pairs_evaluated = 0;
+        if (pairs_evaluated) pairs_evaluated[0] = pairs_evaluated[1] = pairs_evaluated[2] = 0;
         return LIPFIT_OK;
     }
     if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
@@ -132,18 +132,20 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
     if (rc) return rc;
     Workspace stats;
     if (pairs_evaluated) {
-        rc = stats.alloc(2 * sizeof(unsigned long long), c.stream);
+        rc = stats.alloc(4 * sizeof(unsigned long long), c.stream);
         if (rc) return rc;
-        LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 2 * sizeof(unsigned long long), c.stream));
+        LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 4 * sizeof(unsigned long long), c.stream));
     }
     rc = launch_bounds_pruned(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g,
                               stats.as<unsigned long long>());
     if (rc) return rc;
     if (pairs_evaluated) {
-        unsigned long long h[2] = {0, 0};
+        unsigned long long h[4] = {0, 0, 0, 0};
         LIPFIT_CUDA(cudaMemcpyAsync(h, stats.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
         LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
-        *pairs_evaluated = static_cast<int64_t>(h[0]) * 1024;
+        pairs_evaluated[0] = static_cast<int64_t>(h[0]) * 1024;
+        pairs_evaluated[1] = static_cast<int64_t>(h[1]);
+        pairs_evaluated[2] = static_cast<int64_t>(h[2]);
     }
     return LIPFIT_OK;
 }

@@ -39,7 +39,8 @@ int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* X
                        int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g);
 
 // NEXT-4(ii): bounds with exact spatial pruning (prune.cu); X, Xq: ORIGINAL row-major arrays.
-// stats_dev: device uint64[2] (zeroed by the caller) or NULL: [0] += tiles of 32 x 32 pairs evaluated.
+// stats_dev: device uint64[3] (zeroed by the caller) or NULL: [0] += tiles of 32 x 32 pairs evaluated,
+// [1] += tiles that passed the warp-box test, [2] += lanes whose own test asked for an evaluated tile.
 int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
                          const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
                          unsigned long long* stats_dev);

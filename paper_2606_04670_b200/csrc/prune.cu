@@ -30,11 +30,6 @@ namespace {
 
 constexpr int kTile = 32;  // data per tile = lanes per warp
 
-struct PruneGrid {
-    int bits;  // Morton bits per packed coordinate
-    int d;
-};
-
 // ---- coordinate ranges of the packed data -----------------------------------------------------
 __global__ void prune_range_init_kernel(uint32_t* keys) {
     int j = threadIdx.x;
@@ -100,9 +95,10 @@ prune_keys_kernel(const float* __restrict__ P, int n, Xform xf, const uint32_t* 
 // rec : ntiles * 32 records of RF = DP + 4 floats [x'_0 .. x'_{DP-1}, y, 0, 0, 0]; the last tile is
 //       filled up with copies of the last datum (they change no minimum or maximum)
 // box : ntiles * (2 DP + 4) floats [lo_0 .. lo_{DP-1}, hi_0 .. hi_{DP-1}, ymin, ymax, 0, 0]
+// xfp: the PADDED transform of launch_bounds_pruned (DP packed coordinates), dsrc: floats per source row.
 template <int DP>
 __global__ void __launch_bounds__(128)
-prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xf,
+prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xfp, int dsrc,
                     const int32_t* __restrict__ order, int ntiles, float* __restrict__ rec,
                     float* __restrict__ box) {
     constexpr int RF = DP + 4, BF = 2 * DP + 4;
@@ -112,10 +108,10 @@ prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, in
     int pos = t * kTile + lane;
     if (pos >= N) pos = N - 1;
     const int k = order[pos];
-    const float* src = X + static_cast<size_t>(k) * xf.d;
+    const float* src = X + static_cast<size_t>(k) * dsrc;
     float v[DP];
 #pragma unroll
-    for (int j = 0; j < DP; ++j) v[j] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : 0.f;
+    for (int j = 0; j < DP; ++j) v[j] = xfp.sw[j] * src[xfp.perm[j]];
     const float yv = y[k];
     float4* dst = reinterpret_cast<float4*>(rec + (static_cast<size_t>(t) * kTile + lane) * RF);
 #pragma unroll
@@ -154,7 +150,8 @@ prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, in
 // (delta = q - x):  a = qlo - thi <= delta <= qhi - tlo = -b.
 //   unconstrained: |delta| >= max(a, b, 0) on both sides
 //   constrained  : relu(delta) >= max(a, 0),  relu(-delta) >= max(b, 0)
-template <int NORM, int DP>
+// DC >= 0: the last DC packed coordinates are the constrained ones (compile time); DC < 0: runtime flags.
+template <int NORM, int DP, int DC>
 __device__ __forceinline__ void box_lb(const float* __restrict__ qlo, const float* __restrict__ qhi,
                                        const float* __restrict__ tb, const FreeFlags& ff, float& du,
                                        float& dl) {
@@ -163,8 +160,16 @@ __device__ __forceinline__ void box_lb(const float* __restrict__ qlo, const floa
     for (int j = 0; j < DP; ++j) {
         float a = qlo[j] - tb[DP + j];
         float b = tb[j] - qhi[j];
-        float u = fmaxf(fmaxf(a, ff.fr[j] * b), 0.f);
-        float l = fmaxf(fmaxf(b, ff.fr[j] * a), 0.f);
+        float u, l;
+        if (DC < 0) {
+            u = fmaxf(fmaxf(a, ff.fr[j] * b), 0.f);
+            l = fmaxf(fmaxf(b, ff.fr[j] * a), 0.f);
+        } else if (j < DP - DC) {
+            u = l = fmaxf(fmaxf(a, b), 0.f);
+        } else {
+            u = fmaxf(a, 0.f);
+            l = fmaxf(b, 0.f);
+        }
         if (NORM == 1) {
             pu += u;
             pl += l;
@@ -190,15 +195,21 @@ struct PruneArgs {
     const uint64_t* dkeys;     // sorted Morton keys of the data
     const float* rec;
     const float* box;
-    int N, Q, ntiles;
+    int N, Q, ntiles, dsrc;
     float M;
-    Xform xf;
+    Xform xfp;                 // padded transform: [unconstrained, zero padding, constrained], DP coordinates
     FreeFlags ff;
     float *upper, *lower, *g;
-    unsigned long long* stats;  // [0] tiles evaluated (x 1024 pairs), [1] stage-1 survivors
+    unsigned long long* stats;  // [0] tiles evaluated (x 1024 pairs), [1] stage-1 survivors, [2] lanes that needed them
 };
 
-template <int NORM, int DP>
+template <int NORM, int DP, int DC>
+__device__ __forceinline__ void pair_acc(const float* q, const float* x, const FreeFlags& ff, float& au, float& al) {
+    if (DC < 0) PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+    else PairAcc<NORM, DP - (DC < 0 ? 0 : DC), (DC < 0 ? 0 : DC)>::run(q, x, au, al);
+}
+
+template <int NORM, int DP, int DC>
 __device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, const float* q,
                                           const FreeFlags& ff, float M, float& U, float& L) {
     constexpr int RF = DP + 4;
@@ -216,7 +227,7 @@ __device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, 
         }
         const float yv = __ldg(r4 + r * (RF / 4) + (DP >> 2)).x;
         float au, al;
-        PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+        pair_acc<NORM, DP, DC>(q, x, ff, au, al);
         U = fminf(U, fmaf(M, PairAccGeneric<NORM, DP>::finish(au), yv));
         L = fmaxf(L, fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), yv));
     }
@@ -233,22 +244,23 @@ __device__ __forceinline__ float warp_min(float v) {
     return v;
 }
 
-template <int NORM, int DP>
+template <int NORM, int DP, int DC>
 __global__ void __launch_bounds__(128)
 bounds_pruned_kernel(const PruneArgs a) {
     constexpr int BF = 2 * DP + 4;
     const int lane = threadIdx.x & 31;
     const int nwarps = (a.Q + 31) >> 5;
-    unsigned long long n_eval = 0, n_surv = 0;
+    const int nchunks = (a.ntiles + 31) >> 5;
+    unsigned long long n_eval = 0, n_surv = 0, n_mine = 0;
     for (int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < nwarps;
          w += gridDim.x * (blockDim.x >> 5)) {
         const int pos = min(w * 32 + lane, a.Q - 1);
         const bool live = (w * 32 + lane) < a.Q;
         const int qi = a.qorder[pos];
-        const float* src = a.Xq + static_cast<size_t>(qi) * a.xf.d;
+        const float* src = a.Xq + static_cast<size_t>(qi) * a.dsrc;
         float q[DP];
 #pragma unroll
-        for (int j = 0; j < DP; ++j) q[j] = (j < a.xf.d) ? a.xf.sw[j] * src[a.xf.perm[j]] : 0.f;
+        for (int j = 0; j < DP; ++j) q[j] = a.xfp.sw[j] * src[a.xfp.perm[j]];
         float qlo[DP], qhi[DP];
 #pragma unroll
         for (int j = 0; j < DP; ++j) {
@@ -272,13 +284,21 @@ bounds_pruned_kernel(const PruneArgs a) {
             unsigned todo = 0xffffffffu;
             while (todo) {
                 const int t = __shfl_sync(0xffffffffu, mytile, __ffs(todo) - 1);
-                eval_tile<NORM, DP>(a.rec, t, q, a.ff, a.M, U, L);
+                eval_tile<NORM, DP, DC>(a.rec, t, q, a.ff, a.M, U, L);
                 ++n_eval;
                 todo &= ~__ballot_sync(0xffffffffu, mytile == t);
             }
         }
         float Umax = warp_max(U), Lmin = warp_min(L);
-        for (int tb = 0; tb < a.ntiles; tb += 32) {
+        // chunks of 32 tiles, from the chunk of the seed outwards along the curve (near tiles first: the
+        // running bounds tighten early)
+        const int c0 = __shfl_sync(0xffffffffu, mytile, 0) >> 5;
+        int up = c0, down = c0 - 1;
+        for (int i = 0; i < nchunks; ++i) {
+            int chunk;
+            if (down < 0 || (up < nchunks && (i & 1) == 0)) chunk = up++;
+            else chunk = down--;
+            const int tb = chunk << 5;
             const int t = tb + lane;
             bool need = false;
             if (t < a.ntiles) {
@@ -294,7 +314,7 @@ bounds_pruned_kernel(const PruneArgs a) {
                 }
                 const float4 yy = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
                 float du, dl;
-                box_lb<NORM, DP>(qlo, qhi, tbx, a.ff, du, dl);
+                box_lb<NORM, DP, DC>(qlo, qhi, tbx, a.ff, du, dl);
                 need = (fmaf(a.M, du, yy.x) < Umax) || (fmaf(-a.M, dl, yy.y) > Lmin);
             }
             unsigned surv = __ballot_sync(0xffffffffu, need);
@@ -319,11 +339,13 @@ bounds_pruned_kernel(const PruneArgs a) {
                 }
                 const float4 yy = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
                 float du, dl;
-                box_lb<NORM, DP>(q, q, tbx, a.ff, du, dl);
+                box_lb<NORM, DP, DC>(q, q, tbx, a.ff, du, dl);
                 const bool mine = (fmaf(a.M, du, yy.x) < U) || (fmaf(-a.M, dl, yy.y) > L);
-                if (!__any_sync(0xffffffffu, mine)) continue;
-                eval_tile<NORM, DP>(a.rec, ts, q, a.ff, a.M, U, L);
+                const unsigned who = __ballot_sync(0xffffffffu, mine);
+                if (!who) continue;
+                eval_tile<NORM, DP, DC>(a.rec, ts, q, a.ff, a.M, U, L);
                 ++n_eval;
+                n_mine += __popc(who);
                 any_eval = true;
             }
             if (any_eval) {
@@ -340,38 +362,56 @@ bounds_pruned_kernel(const PruneArgs a) {
     if (a.stats && lane == 0) {
         atomicAdd(&a.stats[0], n_eval);
         atomicAdd(&a.stats[1], n_surv);
+        atomicAdd(&a.stats[2], n_mine);
     }
 }
 
-template <int NORM, int DP>
-int launch_pruned_t(const Ctx& c, const float* X, const float* y, int N, const int32_t* dorder, int ntiles,
-                    float* rec, float* box, const PruneArgs& a) {
-    prune_gather_kernel<DP><<<(ntiles + 3) / 4, 128, 0, c.stream>>>(X, y, N, a.xf, dorder, ntiles, rec, box);
+struct PruneLaunch {
+    const float *X, *y;
+    const int32_t* dorder;
+    float *rec, *box;
+};
+
+template <int NORM, int DP, int DC>
+int launch_pruned_t(const Ctx& c, const PruneLaunch& pl, const PruneArgs& a) {
+    prune_gather_kernel<DP><<<(a.ntiles + 3) / 4, 128, 0, c.stream>>>(pl.X, pl.y, a.N, a.xfp, a.dsrc, pl.dorder,
+                                                                     a.ntiles, pl.rec, pl.box);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
-    const int nwarps = (a.Q + 31) / 32;
-    int occ = 0;
-    LIPFIT_CUDA(occupancy_of(&occ, bounds_pruned_kernel<NORM, DP>, 128, 0));
-    if (occ < 1) occ = 1;
-    int grid = (nwarps + 3) / 4;
-    const int cap = c.num_sms * occ * 4;  // a few waves: warps differ in the number of surviving tiles
-    if (grid > cap) grid = cap;
+    // one warp per group of 32 queries, every CTA launched: the groups differ in the number of surviving
+    // tiles, the hardware scheduler balances them
+    const int grid = ((a.Q + 31) / 32 + 3) / 4;
     KernelTimer kt(TK_BOUNDS_PRUNED, c.stream);
-    bounds_pruned_kernel<NORM, DP><<<grid, 128, 0, c.stream>>>(a);
+    bounds_pruned_kernel<NORM, DP, DC><<<grid, 128, 0, c.stream>>>(a);
     kt.stop();
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     return LIPFIT_OK;
 }
 
+template <int NORM, int DP, int DC>
+struct PruneDispatchDC {
+    static int run(int dc, const Ctx& c, const PruneLaunch& pl, const PruneArgs& a) {
+        if (dc == DC) return launch_pruned_t<NORM, DP, DC>(c, pl, a);
+        return PruneDispatchDC<NORM, DP, DC - 1>::run(dc, c, pl, a);
+    }
+};
+template <int NORM, int DP>
+struct PruneDispatchDC<NORM, DP, -1> {
+    static int run(int, const Ctx& c, const PruneLaunch& pl, const PruneArgs& a) {
+        return launch_pruned_t<NORM, DP, -1>(c, pl, a);
+    }
+};
+
+// DP <= 8: the number of constrained coordinates is a compile-time constant of the kernel (no flag
+// arithmetic per pair); DP = 16, 32: runtime flags.
 template <int NORM>
-int launch_pruned_n(int dp, const Ctx& c, const float* X, const float* y, int N, const int32_t* dorder,
-                    int ntiles, float* rec, float* box, const PruneArgs& a) {
+int launch_pruned_n(int dp, int dc, const Ctx& c, const PruneLaunch& pl, const PruneArgs& a) {
     switch (dp) {
-        case 4: return launch_pruned_t<NORM, 4>(c, X, y, N, dorder, ntiles, rec, box, a);
-        case 8: return launch_pruned_t<NORM, 8>(c, X, y, N, dorder, ntiles, rec, box, a);
-        case 16: return launch_pruned_t<NORM, 16>(c, X, y, N, dorder, ntiles, rec, box, a);
-        default: return launch_pruned_t<NORM, 32>(c, X, y, N, dorder, ntiles, rec, box, a);
+        case 4: return PruneDispatchDC<NORM, 4, 4>::run(dc, c, pl, a);
+        case 8: return PruneDispatchDC<NORM, 8, 8>::run(dc, c, pl, a);
+        case 16: return launch_pruned_t<NORM, 16, -1>(c, pl, a);
+        default: return launch_pruned_t<NORM, 32, -1>(c, pl, a);
     }
 }
 
@@ -425,6 +465,22 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
     if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
     if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
 
+    // padded transform: unconstrained coordinates, zero padding up to DP, constrained coordinates last
+    Xform xfp = xf;
+    xfp.d = dp;
+    const int npad = dp - xf.d;
+    for (int j = 0; j < dp; ++j) {
+        if (j < xf.dU) continue;
+        if (j < xf.dU + npad) {
+            xfp.perm[j] = 0;
+            xfp.sw[j] = 0.f;
+        } else {
+            xfp.perm[j] = xf.perm[j - npad];
+            xfp.sw[j] = xf.sw[j - npad];
+        }
+    }
+    xfp.dU = xf.dU + npad;
+
     PruneArgs a;
     a.Xq = Xq;
     a.qorder = qorder.as<int32_t>();
@@ -435,23 +491,19 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
     a.N = N;
     a.Q = Q;
     a.ntiles = ntiles;
+    a.dsrc = xf.d;
     a.M = M;
-    a.xf = xf;
-    a.ff = make_free_flags(xf);
+    a.xfp = xfp;
+    a.ff = make_free_flags(xfp);
     a.upper = upper;
     a.lower = lower;
     a.g = g;
     a.stats = stats_dev;
+    PruneLaunch pl{X, y, dorder.as<int32_t>(), rec.as<float>(), box.as<float>()};
     switch (norm) {
-        case LIPFIT_L1:
-            return launch_pruned_n<1>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
-                                      box.as<float>(), a);
-        case LIPFIT_L2:
-            return launch_pruned_n<2>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
-                                      box.as<float>(), a);
-        default:
-            return launch_pruned_n<3>(dp, c, X, y, N, dorder.as<int32_t>(), ntiles, rec.as<float>(),
-                                      box.as<float>(), a);
+        case LIPFIT_L1: return launch_pruned_n<1>(dp, xf.dC, c, pl, a);
+        case LIPFIT_L2: return launch_pruned_n<2>(dp, xf.dC, c, pl, a);
+        default: return launch_pruned_n<3>(dp, xf.dC, c, pl, a);
     }
 }
 
