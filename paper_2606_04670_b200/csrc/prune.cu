@@ -209,23 +209,35 @@ __device__ __forceinline__ void pair_acc(const float* q, const float* x, const F
     else PairAcc<NORM, DP - (DC < 0 ? 0 : DC), (DC < 0 ? 0 : DC)>::run(q, x, au, al);
 }
 
+// One tile against the warp's 32 queries.  Every lane fetches ONE record of the tile (coalesced, a single
+// L2 round trip per tile), the warp parks the 32 records in its own shared-memory slab as float4 columns
+// (sm[c * 32 + r] = 16-byte word c of record r: conflict-free stores, broadcast loads), then every lane
+// runs its query against all 32 records.
 template <int NORM, int DP, int DC>
-__device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, const float* q,
-                                          const FreeFlags& ff, float M, float& U, float& L) {
-    constexpr int RF = DP + 4;
-    const float4* r4 = reinterpret_cast<const float4*>(rec + static_cast<size_t>(t) * kTile * RF);
-#pragma unroll 4
+__device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, float4* __restrict__ sm,
+                                          const float* q, const FreeFlags& ff, float M, float& U, float& L) {
+    constexpr int RF = DP + 4, W = RF / 4;
+    const int lane = threadIdx.x & 31;
+    const float4* g = reinterpret_cast<const float4*>(rec + static_cast<size_t>(t) * kTile * RF) + lane * W;
+    float4 v[W];
+#pragma unroll
+    for (int c = 0; c < W; ++c) v[c] = __ldg(g + c);
+    __syncwarp();  // every lane has finished reading the previous tile
+#pragma unroll
+    for (int c = 0; c < W; ++c) sm[c * 32 + lane] = v[c];
+    __syncwarp();
+#pragma unroll 8
     for (int r = 0; r < kTile; ++r) {
         float x[DP];
 #pragma unroll
         for (int j = 0; j < DP; j += 4) {
-            float4 v = __ldg(r4 + r * (RF / 4) + (j >> 2));
-            x[j] = v.x;
-            x[j + 1] = v.y;
-            x[j + 2] = v.z;
-            x[j + 3] = v.w;
+            const float4 xv = sm[(j >> 2) * 32 + r];
+            x[j] = xv.x;
+            x[j + 1] = xv.y;
+            x[j + 2] = xv.z;
+            x[j + 3] = xv.w;
         }
-        const float yv = __ldg(r4 + r * (RF / 4) + (DP >> 2)).x;
+        const float yv = sm[(W - 1) * 32 + r].x;
         float au, al;
         pair_acc<NORM, DP, DC>(q, x, ff, au, al);
         U = fminf(U, fmaf(M, PairAccGeneric<NORM, DP>::finish(au), yv));
@@ -248,6 +260,8 @@ template <int NORM, int DP, int DC>
 __global__ void __launch_bounds__(128)
 bounds_pruned_kernel(const PruneArgs a) {
     constexpr int BF = 2 * DP + 4;
+    __shared__ float4 slab[4][(DP + 4) / 4 * 32];
+    float4* sm = slab[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
     const int nwarps = (a.Q + 31) >> 5;
     const int nchunks = (a.ntiles + 31) >> 5;
@@ -284,7 +298,7 @@ bounds_pruned_kernel(const PruneArgs a) {
             unsigned todo = 0xffffffffu;
             while (todo) {
                 const int t = __shfl_sync(0xffffffffu, mytile, __ffs(todo) - 1);
-                eval_tile<NORM, DP, DC>(a.rec, t, q, a.ff, a.M, U, L);
+                eval_tile<NORM, DP, DC>(a.rec, t, sm, q, a.ff, a.M, U, L);
                 ++n_eval;
                 todo &= ~__ballot_sync(0xffffffffu, mytile == t);
             }
@@ -343,7 +357,7 @@ bounds_pruned_kernel(const PruneArgs a) {
                 const bool mine = (fmaf(a.M, du, yy.x) < U) || (fmaf(-a.M, dl, yy.y) > L);
                 const unsigned who = __ballot_sync(0xffffffffu, mine);
                 if (!who) continue;
-                eval_tile<NORM, DP, DC>(a.rec, ts, q, a.ff, a.M, U, L);
+                eval_tile<NORM, DP, DC>(a.rec, ts, sm, q, a.ff, a.M, U, L);
                 ++n_eval;
                 n_mine += __popc(who);
                 any_eval = true;
