@@ -534,6 +534,12 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
         fb = lambda: L.lipfit_bounds(X, y, Xq, wl.M, wl.mask, wl.norm, wl.weights)
         ms_b = _time_steps(torch, fb, 1 if c == 10 else 2, 1, l2buf)
         ub = fb()
+        d_async = max(float((a - b).abs().max()) for a, b in zip(outs, ub))
+        torch.cuda.synchronize()
+        d_sync = max(float((a - b).abs().max()) for a, b in zip(outs, ub))
+        if d_async != d_sync:
+            print(f"bench.py: config {c}: unpruned outputs changed after a synchronize ({d_async} -> {d_sync})",
+                  file=sys.stderr)
         out.update({"workload": "config %d data and queries" % {9: 2, 10: 3, 11: 5}[c],
                     "ms_per_step": float(np.mean(ms)), "kernel_ms": kms,
                     "value": pairs / (np.mean(ms) * 1e-3) / 1e9, "unit": "effective " + UNIT,
@@ -541,7 +547,7 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
                     "evaluated_rate_gpairs_s": evaluated / (kms * 1e-3) / 1e9,
                     "unpruned_ms_per_step": float(np.mean(ms_b)),
                     "speedup_over_unpruned": float(np.mean(ms_b) / np.mean(ms)),
-                    "max_abs_diff_vs_unpruned": max(float((a - b).abs().max()) for a, b in zip(outs, ub)),
+                    "max_abs_diff_vs_unpruned": d_sync,
                     "kernel": "bounds_pruned<norm,DP> (Morton-sorted 32-datum tiles, box tests, generic distance)"})
         if not args.no_cpu:
             sel = oracle_subset(wl.Q, 2000 if c != 10 else 96)

@@ -97,8 +97,8 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
                        void* cuda_stream);
 
 /* ---- NEXT-4(ii): the same upper / lower / g as lipfit_bounds, evaluated with EXACT spatial pruning ----
- * (the exact counterpart of the heuristic of PAPER.md:214-218, which keeps only data close to the
- * query).  Data and queries are sorted along a Morton curve of the transformed coordinates; tiles of
+ * (the paper evaluates every bound in time "proportional to N", and prunes only
+ * heuristically, pairs of the smoothing problem).  Data and queries are sorted along a Morton curve of the transformed coordinates; tiles of
  * 32 data carry a bounding box and the range of their values; a tile is skipped for a group of
  * queries when  ymin + M dlb^u >= every running upper bound  and  ymax - M dlb^l <= every running
  * lower bound  of the group (dlb = smallest possible distance between the boxes), which proves that

