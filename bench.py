@@ -444,7 +444,7 @@ def run_gpu(args):
 
 def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
     import oracle
-    wl = make_workload({6: 5, 7: 2, 8: 5, 9: 2, 10: 3, 11: 5}.get(c, c))
+    wl = make_workload({6: 5, 7: 2, 8: 5, 9: 2, 10: 3, 11: 5, 12: 5}.get(c, c))
     steps = max(1, min(args.steps, 3)) if c in (3, 4) else args.steps
     out = {}
     if c in (1, 3):
@@ -553,6 +553,52 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
             sel = oracle_subset(wl.Q, 2000 if c != 10 else 96)
             ref = oracle.bounds(wl.X, wl.y, wl.Xq[sel], wl.M, wl.mask, wl.norm, wl.weights)
             out["parity"] = parity_bounds(wl, outs, sel, ref)
+    elif c == 12:
+        # Eq.(7) objective / gradient of config 5 with exact pruning (the exact counterpart of the M/3 heuristic,
+        # PAPER.md:214-218), beside the unpruned all-pairs pass, at eps = 0 and at a random eps (sigma 0.05)
+        t = lambda a: torch.from_numpy(a).to(dev)
+        X, y = t(wl.X), t(wl.y)
+        eps = t((0.05 * np.random.default_rng(7).standard_normal(wl.N)).astype(np.float32))
+        pairs = wl.N * (wl.N - 1)
+        out.update({"workload": "config 5 data (d=5, N=200000, L2, all coordinates monotone, M=3, p=1)",
+                    "unit": "effective G ordered pairs of Eq.(7) per second"})
+        for name, e in (("eps0", None), ("eps_random", eps)):
+            fn = lambda: L.lipfit_smooth_objective_pruned(X, y, wl.M, e, wl.mask, wl.norm, None, wl.p)
+            fu = lambda: L.lipfit_smooth_objective(X, y, wl.M, e, wl.mask, wl.norm, None, wl.p)
+            ms = _time_steps(torch, fn, args.steps, 3, l2buf)
+            kms, _ = _kernel_ms(L, 7, fn, 1)
+            ms_u = _time_steps(torch, fu, 2, 1, l2buf)
+            F, g, evaluated = L.lipfit_smooth_objective_pruned(X, y, wl.M, e, wl.mask, wl.norm, None, wl.p,
+                                                               count_pairs=True)
+            Fu, gu = fu()
+            torch.cuda.synchronize()
+            out[name] = {"ms_per_step": float(np.mean(ms)), "kernel_ms": kms,
+                         "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+                         "pairs_evaluated": int(evaluated), "fraction_evaluated": evaluated / pairs,
+                         "unpruned_ms_per_step": float(np.mean(ms_u)),
+                         "speedup_over_unpruned": float(np.mean(ms_u) / np.mean(ms)),
+                         "F": F, "F_rel_diff_vs_unpruned": abs(F - Fu) / Fu,
+                         "grad_rel_diff_vs_unpruned": float((g - gu).abs().max() / gu.abs().max())}
+        out["value"] = out["eps0"]["value"]
+        out["ms_per_step"] = out["eps0"]["ms_per_step"]
+        # the same data without the monotone mask (symmetric distance): only near pairs can violate
+        fs = lambda: L.lipfit_smooth_objective_pruned(X, y, wl.M, None, None, wl.norm, None, wl.p)
+        fsu = lambda: L.lipfit_smooth_objective(X, y, wl.M, None, None, wl.norm, None, wl.p)
+        ms = _time_steps(torch, fs, args.steps, 3, l2buf)
+        ms_u = _time_steps(torch, fsu, 2, 1, l2buf)
+        Fs, gs, ev = L.lipfit_smooth_objective_pruned(X, y, wl.M, None, None, wl.norm, None, wl.p, count_pairs=True)
+        Fsu, gsu = fsu()
+        torch.cuda.synchronize()
+        out["eps0_no_mask"] = {"ms_per_step": float(np.mean(ms)), "unpruned_ms_per_step": float(np.mean(ms_u)),
+                               "speedup_over_unpruned": float(np.mean(ms_u) / np.mean(ms)),
+                               "fraction_evaluated": ev / pairs, "F_rel_diff_vs_unpruned": abs(Fs - Fsu) / Fsu,
+                               "grad_rel_diff_vs_unpruned": float((gs - gsu).abs().max() / gsu.abs().max())}
+        if not args.no_cpu:
+            rows = oracle_subset(wl.N, 64)
+            g_ref, _ = oracle.smooth_rows(wl.X, wl.y, wl.M, np.zeros(wl.N), rows, wl.mask, wl.norm, None, wl.p)
+            _, g0 = L.lipfit_smooth_objective_pruned(X, y, wl.M, None, wl.mask, wl.norm, None, wl.p)
+            err = float(np.abs(g0.cpu().numpy()[rows] - g_ref).max() / np.abs(g_ref).max())
+            out["parity"] = {"gradient_rows": int(len(rows)), "max_rel_err": err, "tol": 1e-5, "ok": bool(err <= 1e-5)}
     elif c == 8:
         # NEXT-3: smallest consistent Lipschitz constant of the config 5 data
         t = lambda a: torch.from_numpy(a).to(dev)
@@ -609,7 +655,7 @@ def main():
     ap.add_argument("--configs", default="2",
                     help="comma list of BASELINE.json configs to report (2 always); 6 = local Lipschitz (NEXT-1), "
                          "7 = top-k bounds (NEXT-2), 8 = Lipschitz constant (NEXT-3), 9 / 10 / 11 = exactly pruned bounds on the "
-                         "config 2 / 3 / 5 workloads (NEXT-4(ii))")
+                         "config 2 / 3 / 5 workloads, 12 = exactly pruned smoothing objective (NEXT-4(ii))")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

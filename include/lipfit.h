@@ -116,6 +116,20 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d,
                          float* upper, float* lower, float* g, int64_t* pairs_evaluated /* host */,
                          void* cuda_stream);
 
+/* ---- Eq.(7) PAPER.md:197 objective and gradient with the same exact pruning -----------------------
+ * Same F and grad as lipfit_smooth_objective (same reading of Eq.(5),(6)).  From datum i's side the two
+ * penalty terms of the pair (i,k) are the violations of the upper bound  z_k + M d_s(x^k,x^i)  and of the
+ * lower bound  z_k - M d_s(x^i,x^k)  at x^i, so a tile B of data is skipped for the data of a tile A when
+ * zmin_B + M dlb^u >= zmax_A  and  zmax_B - M dlb^l <= zmin_A : every term of that tile pair is exactly 0.
+ * This is the exact counterpart of the M/3 pair-removal heuristic of PAPER.md:214-218.
+ * X [N*d], y [N], eps [N] (device, eps may be NULL = 0); *F HOST double (required; the call
+ * synchronises); grad [N] device fp32 or NULL; pairs_evaluated HOST int64 or NULL (ordered pairs whose
+ * distances were computed, N(N-1) for the unpruned pass). */
+int lipfit_smooth_objective_pruned(const float* X, const float* y, int64_t N, int32_t d, float M,
+                                   const int32_t* mono_mask, int32_t norm, const float* weights, float p,
+                                   const float* eps, double* F /* host */, float* grad,
+                                   int64_t* pairs_evaluated /* host */, void* cuda_stream);
+
 /* ---- k nearest data per query by distance (d_(1) <= d_(2) <= ...) -------------
  * side 0: symmetric weighted norm, mask ignored; +1: D^u; -1: D^l.
  * idx [Q*k] int32 and dist [Q*k] fp32, row-major, ascending distance per query.
@@ -227,7 +241,7 @@ const char* lipfit_version(void);
 int64_t lipfit_launch_count(void);
 /* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
  * resets the accumulators and makes every later launch of the three dominant kernels
- * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation, 6 = pruned bounds) bracketed by CUDA events on
+ * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation, 6 = pruned bounds, 7 = pruned smoothing pass) bracketed by CUDA events on
  * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
  * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);

@@ -25,7 +25,7 @@ EXPORTS = [
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
     "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
-    "lipfit_bounds_pruned",
+    "lipfit_bounds_pruned", "lipfit_smooth_objective_pruned",
 ]
 LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
@@ -64,6 +64,7 @@ def load():
     lib.lipfit_bounds_host.argtypes = lib.lipfit_bounds.argtypes
     lib.lipfit_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, P]
     lib.lipfit_knn_host.argtypes = lib.lipfit_knn.argtypes
+    lib.lipfit_smooth_objective_pruned.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, P, P, P, P, P]
     lib.lipfit_smooth_objective.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, P, P, P, P]
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
     lib.lipfit_smooth_host.argtypes = lib.lipfit_smooth.argtypes
@@ -277,6 +278,28 @@ def lipfit_smooth_objective(X, y, M: float, eps=None, mono_mask=None, norm: int 
         None if grad is None else C.c_void_p(grad.data_ptr()), _stream(stream))
     _check(rc, "lipfit_smooth_objective")
     return float(F.value), grad
+
+
+def lipfit_smooth_objective_pruned(X, y, M: float, eps=None, mono_mask=None, norm: int = LIPFIT_L2,
+                                   weights=None, p: float = 1.0, want_grad: bool = True, count_pairs: bool = False,
+                                   stream=None):
+    """(F, grad[, pairs_evaluated]) as lipfit_smooth_objective, evaluated with exact spatial pruning."""
+    torch = _torch()
+    X, y = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y")
+    N, d = X.shape
+    m, w = _host_params(d, mono_mask, weights)
+    if eps is not None:
+        eps = _dev_f32(eps, 1, "eps")
+    grad = torch.empty(N, dtype=torch.float32, device=X.device) if want_grad else None
+    F = C.c_double(0.0)
+    n = C.c_int64(0)
+    rc = load().lipfit_smooth_objective_pruned(
+        X.data_ptr(), y.data_ptr(), N, d, float(M), _np_ptr(m), int(norm), _np_ptr(w), float(p),
+        None if eps is None else C.c_void_p(eps.data_ptr()), C.cast(C.byref(F), C.c_void_p),
+        None if grad is None else C.c_void_p(grad.data_ptr()),
+        C.cast(C.byref(n), C.c_void_p) if count_pairs else None, _stream(stream))
+    _check(rc, "lipfit_smooth_objective_pruned")
+    return (float(F.value), grad, int(n.value)) if count_pairs else (float(F.value), grad)
 
 
 def lipfit_lipschitz_constant(X, y, mono_mask=None, norm: int = LIPFIT_L2, weights=None, stream=None):

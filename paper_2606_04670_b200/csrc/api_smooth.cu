@@ -3,6 +3,8 @@
 #include <cmath>
 #include <vector>
 
+#include <cstring>
+
 #include "kernels.h"
 #include "lbfgs.h"
 
@@ -70,6 +72,35 @@ int lipfit_smooth_objective(const float* X, const float* y, int64_t N, int32_t d
         LIPFIT_CUDA(cudaMemcpyAsync(F, fdev.p, sizeof(double), cudaMemcpyDeviceToHost, c.stream));
         LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
     }
+    return LIPFIT_OK;
+}
+
+int lipfit_smooth_objective_pruned(const float* X, const float* y, int64_t N, int32_t d, float M,
+                                   const int32_t* mono_mask, int32_t norm, const float* weights, float p,
+                                   const float* eps, double* F, float* grad, int64_t* pairs_evaluated,
+                                   void* cuda_stream) {
+    int rc = check_common(X, y, N, d, M, norm, p);
+    if (rc) return rc;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    if (!F) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    Workspace fdev;
+    rc = fdev.alloc(sizeof(double) + 2 * sizeof(unsigned long long), c.stream);
+    if (rc) return rc;
+    LIPFIT_CUDA(cudaMemsetAsync(fdev.p, 0, sizeof(double) + 2 * sizeof(unsigned long long), c.stream));
+    unsigned long long* stats = reinterpret_cast<unsigned long long*>(fdev.as<double>() + 1);
+    rc = launch_smooth_objective_pruned(c, X, y, eps, N, xf, norm, M, p, fdev.as<double>(), grad,
+                                        pairs_evaluated ? stats : nullptr);
+    if (rc) return rc;
+    unsigned long long h[3] = {0, 0, 0};
+    LIPFIT_CUDA(cudaMemcpyAsync(h, fdev.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+    LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+    std::memcpy(F, &h[0], sizeof(double));
+    if (pairs_evaluated) *pairs_evaluated = static_cast<int64_t>(h[1]) * 1024;
     return LIPFIT_OK;
 }
 

@@ -33,7 +33,7 @@ extern std::atomic<int64_t> g_launches;
 
 // Optional per-kernel device timing of the three dominant kernels (lipfit_set_timing): when on,
 // the launch is bracketed by CUDA events on its own stream and the call waits for it.
-enum TimedKernel { TK_BOUNDS = 0, TK_KNN_SELECT = 1, TK_SMOOTH_PAIRS = 2, TK_LIPCONST_PAIRS = 3, TK_LOCAL_TABLE = 4, TK_LOCAL_EVAL = 5, TK_BOUNDS_PRUNED = 6, TK_COUNT = 7 };
+enum TimedKernel { TK_BOUNDS = 0, TK_KNN_SELECT = 1, TK_SMOOTH_PAIRS = 2, TK_LIPCONST_PAIRS = 3, TK_LOCAL_TABLE = 4, TK_LOCAL_EVAL = 5, TK_BOUNDS_PRUNED = 6, TK_SMOOTH_PRUNED = 7, TK_COUNT = 8 };
 struct KernelTimer {
     int which;
     cudaStream_t s;

@@ -45,6 +45,12 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
                          const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
                          unsigned long long* stats_dev);
 
+// Eq.(7) objective / gradient with the same exact pruning (prune.cu).  F_dev: device double (required,
+// zeroed here); grad: device float in the original order or NULL; eps may be NULL.
+int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
+                                   const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
+                                   unsigned long long* stats_dev);
+
 // a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                int norm, int k, int32_t* idx, float* dist);

@@ -98,9 +98,9 @@ prune_keys_kernel(const float* __restrict__ P, int n, Xform xf, const uint32_t* 
 // xfp: the PADDED transform of launch_bounds_pruned (DP packed coordinates), dsrc: floats per source row.
 template <int DP>
 __global__ void __launch_bounds__(128)
-prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xfp, int dsrc,
-                    const int32_t* __restrict__ order, int ntiles, float* __restrict__ rec,
-                    float* __restrict__ box) {
+prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, const float* __restrict__ eps,
+                    int N, Xform xfp, int dsrc, const int32_t* __restrict__ order, int ntiles,
+                    float* __restrict__ rec, float* __restrict__ box) {
     constexpr int RF = DP + 4, BF = 2 * DP + 4;
     const int lane = threadIdx.x & 31;
     const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -112,7 +112,7 @@ prune_gather_kernel(const float* __restrict__ X, const float* __restrict__ y, in
     float v[DP];
 #pragma unroll
     for (int j = 0; j < DP; ++j) v[j] = xfp.sw[j] * src[xfp.perm[j]];
-    const float yv = y[k];
+    const float yv = eps ? y[k] + eps[k] : y[k];  // smoothing: z = y + eps
     float4* dst = reinterpret_cast<float4*>(rec + (static_cast<size_t>(t) * kTile + lane) * RF);
 #pragma unroll
     for (int j = 0; j < DP; j += 4) dst[j >> 2] = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
@@ -389,8 +389,8 @@ struct PruneLaunch {
 
 template <int NORM, int DP, int DC>
 int launch_pruned_t(const Ctx& c, const PruneLaunch& pl, const PruneArgs& a) {
-    prune_gather_kernel<DP><<<(a.ntiles + 3) / 4, 128, 0, c.stream>>>(pl.X, pl.y, a.N, a.xfp, a.dsrc, pl.dorder,
-                                                                     a.ntiles, pl.rec, pl.box);
+    prune_gather_kernel<DP><<<(a.ntiles + 3) / 4, 128, 0, c.stream>>>(pl.X, pl.y, nullptr, a.N, a.xfp, a.dsrc,
+                                                                     pl.dorder, a.ntiles, pl.rec, pl.box);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     // one warp per group of 32 queries, every CTA launched: the groups differ in the number of surviving
@@ -455,6 +455,218 @@ int sorted_keys(const Ctx& c, const float* P, int n, const Xform& xf, const uint
     return LIPFIT_OK;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Smoothing objective / gradient, Eq.(5)-(7) PAPER.md:189-198, with the same exact pruning.
+// From datum i's side (reading R12):  V_ik = (z_i - (z_k + M D^u(x^i, k)))_+  is i's violation of the
+// upper bound set by k, V_ki = ((z_k - M D^l(x^i, k)) - z_i)_+  its violation of the lower bound, so
+//   F = ||eps||^2 / p + sum_i sum_k (V_ik^2 + V_ki^2),   dF/deps_i = 2 eps_i / p + 4 sum_k (V_ik - V_ki),
+// i.e. the bounds pass with the data as queries and a different reduction.  A tile B is skipped for
+// the data of tile A when  zmin_B + M dlb^u >= zmax_A  and  zmax_B - M dlb^l <= zmin_A : then every
+// V_ik and V_ki with i in A, k in B is exactly 0 in the kernel's own arithmetic (same argument as above).
+// One warp per tile A, lane = datum i (coordinates and z_i in registers); pair terms in fp32, the sums
+// of a tile's 32 terms go into fp64 accumulators.
+struct SmoothPruneArgs {
+    const float* rec;
+    const float* box;
+    const int32_t* order;
+    const float* eps;  // original order, may be NULL
+    int N, ntiles;
+    float M, p;
+    FreeFlags ff;
+    double* F;         // device, zeroed
+    float* grad;       // original order, may be NULL
+    unsigned long long* stats;
+};
+
+template <int NORM, int DP, int DC>
+__global__ void __launch_bounds__(128)
+smooth_pruned_kernel(const SmoothPruneArgs a) {
+    constexpr int RF = DP + 4, W = RF / 4, BF = 2 * DP + 4;
+    __shared__ float4 slab[4][W * 32];
+    float4* sm = slab[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const int nchunks = (a.ntiles + 31) >> 5;
+    const int A = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (A >= a.ntiles) return;
+    const int pos = A * kTile + lane;
+    const bool live = pos < a.N;
+    float q[DP], zi;
+    {
+        const float4* g = reinterpret_cast<const float4*>(a.rec + static_cast<size_t>(pos) * RF);
+#pragma unroll
+        for (int j = 0; j < DP; j += 4) {
+            const float4 v = __ldg(g + (j >> 2));
+            q[j] = v.x;
+            q[j + 1] = v.y;
+            q[j + 2] = v.z;
+            q[j + 3] = v.w;
+        }
+        zi = __ldg(g + (W - 1)).x;
+    }
+    float qlo[DP], qhi[DP];
+    const float* ba = a.box + static_cast<size_t>(A) * BF;
+#pragma unroll
+    for (int j = 0; j < DP; ++j) {
+        qlo[j] = __ldg(ba + j);
+        qhi[j] = __ldg(ba + DP + j);
+    }
+    const float zminA = __ldg(ba + 2 * DP), zmaxA = __ldg(ba + 2 * DP + 1);
+    double Fi = 0.0, gi = 0.0;
+    unsigned long long n_eval = 0;
+    for (int chunk = 0; chunk < nchunks; ++chunk) {
+        const int tb = chunk << 5;
+        const int t = tb + lane;
+        bool need = false;
+        if (t < a.ntiles) {
+            const float* b = a.box + static_cast<size_t>(t) * BF;
+            float tbx[2 * DP];
+#pragma unroll
+            for (int j = 0; j < 2 * DP; j += 4) {
+                float4 v = __ldg(reinterpret_cast<const float4*>(b + j));
+                tbx[j] = v.x;
+                tbx[j + 1] = v.y;
+                tbx[j + 2] = v.z;
+                tbx[j + 3] = v.w;
+            }
+            const float4 zz = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
+            float du, dl;
+            box_lb<NORM, DP, DC>(qlo, qhi, tbx, a.ff, du, dl);
+            need = (fmaf(a.M, du, zz.x) < zmaxA) || (fmaf(-a.M, dl, zz.y) > zminA);
+        }
+        unsigned surv = __ballot_sync(0xffffffffu, need);
+        while (surv) {
+            const int s = __ffs(surv) - 1;
+            surv &= surv - 1;
+            const int ts = tb + s;
+            const float* b = a.box + static_cast<size_t>(ts) * BF;
+            float tbx[2 * DP];
+#pragma unroll
+            for (int j = 0; j < 2 * DP; j += 4) {
+                float4 v = __ldg(reinterpret_cast<const float4*>(b + j));
+                tbx[j] = v.x;
+                tbx[j + 1] = v.y;
+                tbx[j + 2] = v.z;
+                tbx[j + 3] = v.w;
+            }
+            const float4 zz = __ldg(reinterpret_cast<const float4*>(b + 2 * DP));
+            float du, dl;
+            box_lb<NORM, DP, DC>(q, q, tbx, a.ff, du, dl);
+            const bool mine = (fmaf(a.M, du, zz.x) < zi) || (fmaf(-a.M, dl, zz.y) > zi);
+            if (!__any_sync(0xffffffffu, mine)) continue;
+            // evaluate tile ts (only its real records: the filled-up tail of the last tile is left out)
+            const float4* g = reinterpret_cast<const float4*>(a.rec + static_cast<size_t>(ts) * kTile * RF) + lane * W;
+            float4 v[W];
+#pragma unroll
+            for (int c = 0; c < W; ++c) v[c] = __ldg(g + c);
+            __syncwarp();
+#pragma unroll
+            for (int c = 0; c < W; ++c) sm[c * 32 + lane] = v[c];
+            __syncwarp();
+            const int n = min(kTile, a.N - ts * kTile);
+            float fs = 0.f, gs = 0.f;
+#pragma unroll 4
+            for (int r = 0; r < n; ++r) {
+                float x[DP];
+#pragma unroll
+                for (int j = 0; j < DP; j += 4) {
+                    const float4 xv = sm[(j >> 2) * 32 + r];
+                    x[j] = xv.x;
+                    x[j + 1] = xv.y;
+                    x[j + 2] = xv.z;
+                    x[j + 3] = xv.w;
+                }
+                const float zk = sm[(W - 1) * 32 + r].x;
+                float au, al;
+                pair_acc<NORM, DP, DC>(q, x, a.ff, au, al);
+                const float v1 = fmaxf(zi - fmaf(a.M, PairAccGeneric<NORM, DP>::finish(au), zk), 0.f);
+                const float v2 = fmaxf(fmaf(-a.M, PairAccGeneric<NORM, DP>::finish(al), zk) - zi, 0.f);
+                fs = fmaf(v1, v1, fs);
+                fs = fmaf(v2, v2, fs);
+                gs += v1 - v2;
+            }
+            Fi += static_cast<double>(fs);
+            gi += static_cast<double>(gs);
+            ++n_eval;
+        }
+    }
+    if (live) {
+        const int orig = a.order[pos];
+        const double e = a.eps ? static_cast<double>(a.eps[orig]) : 0.0;
+        Fi += e * e / static_cast<double>(a.p);
+        if (a.grad) a.grad[orig] = static_cast<float>(2.0 * e / static_cast<double>(a.p) + 4.0 * gi);
+    } else {
+        Fi = 0.0;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) Fi += __shfl_xor_sync(0xffffffffu, Fi, o);
+    if (lane == 0) {
+        atomicAdd(a.F, Fi);
+        if (a.stats) atomicAdd(&a.stats[0], n_eval);
+    }
+}
+
+template <int NORM, int DP, int DC>
+int launch_smooth_pruned_t(const Ctx& c, const PruneLaunch& pl, const Xform& xfp, int dsrc, const float* eps,
+                           const SmoothPruneArgs& a) {
+    prune_gather_kernel<DP><<<(a.ntiles + 3) / 4, 128, 0, c.stream>>>(pl.X, pl.y, eps, a.N, xfp, dsrc, pl.dorder,
+                                                                     a.ntiles, pl.rec, pl.box);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    KernelTimer kt(TK_SMOOTH_PRUNED, c.stream);
+    smooth_pruned_kernel<NORM, DP, DC><<<(a.ntiles + 3) / 4, 128, 0, c.stream>>>(a);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
+template <int NORM, int DP, int DC>
+struct SmoothDispatchDC {
+    static int run(int dc, const Ctx& c, const PruneLaunch& pl, const Xform& xfp, int dsrc, const float* eps,
+                   const SmoothPruneArgs& a) {
+        if (dc == DC) return launch_smooth_pruned_t<NORM, DP, DC>(c, pl, xfp, dsrc, eps, a);
+        return SmoothDispatchDC<NORM, DP, DC - 1>::run(dc, c, pl, xfp, dsrc, eps, a);
+    }
+};
+template <int NORM, int DP>
+struct SmoothDispatchDC<NORM, DP, -1> {
+    static int run(int, const Ctx& c, const PruneLaunch& pl, const Xform& xfp, int dsrc, const float* eps,
+                   const SmoothPruneArgs& a) {
+        return launch_smooth_pruned_t<NORM, DP, -1>(c, pl, xfp, dsrc, eps, a);
+    }
+};
+
+template <int NORM>
+int launch_smooth_pruned_n(int dp, int dc, const Ctx& c, const PruneLaunch& pl, const Xform& xfp, int dsrc,
+                           const float* eps, const SmoothPruneArgs& a) {
+    switch (dp) {
+        case 4: return SmoothDispatchDC<NORM, 4, 4>::run(dc, c, pl, xfp, dsrc, eps, a);
+        case 8: return SmoothDispatchDC<NORM, 8, 8>::run(dc, c, pl, xfp, dsrc, eps, a);
+        case 16: return launch_smooth_pruned_t<NORM, 16, -1>(c, pl, xfp, dsrc, eps, a);
+        default: return launch_smooth_pruned_t<NORM, 32, -1>(c, pl, xfp, dsrc, eps, a);
+    }
+}
+
+// padded transform: unconstrained coordinates, zero padding up to dp, constrained coordinates last
+Xform padded_xform(const Xform& xf, int dp) {
+    Xform xfp = xf;
+    xfp.d = dp;
+    const int npad = dp - xf.d;
+    for (int j = 0; j < dp; ++j) {
+        if (j < xf.dU) continue;
+        if (j < xf.dU + npad) {
+            xfp.perm[j] = 0;
+            xfp.sw[j] = 0.f;
+        } else {
+            xfp.perm[j] = xf.perm[j - npad];
+            xfp.sw[j] = xf.sw[j - npad];
+        }
+    }
+    xfp.dU = xf.dU + npad;
+    return xfp;
+}
+
 }  // namespace
 
 int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N64, const float* Xq,
@@ -480,21 +692,7 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
     if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
     if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
 
-    // padded transform: unconstrained coordinates, zero padding up to DP, constrained coordinates last
-    Xform xfp = xf;
-    xfp.d = dp;
-    const int npad = dp - xf.d;
-    for (int j = 0; j < dp; ++j) {
-        if (j < xf.dU) continue;
-        if (j < xf.dU + npad) {
-            xfp.perm[j] = 0;
-            xfp.sw[j] = 0.f;
-        } else {
-            xfp.perm[j] = xf.perm[j - npad];
-            xfp.sw[j] = xf.sw[j - npad];
-        }
-    }
-    xfp.dU = xf.dU + npad;
+    const Xform xfp = padded_xform(xf, dp);
 
     PruneArgs a;
     a.Xq = Xq;
@@ -521,5 +719,49 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
         default: return launch_pruned_n<3>(dp, xf.dC, c, pl, a);
     }
 }
+
+int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N64,
+                                   const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
+                                   unsigned long long* stats_dev) {
+    const int N = static_cast<int>(N64);
+    const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
+    int bits = 32 / xf.d;
+    if (bits > 16) bits = 16;
+    const int ntiles = (N + kTile - 1) / kTile;
+    Workspace range, dkeys, dorder, rec, box;
+    int rc = range.alloc(sizeof(uint32_t) * 2 * kMaxDim, c.stream);
+    if (rc) return rc;
+    prune_range_init_kernel<<<1, 32, 0, c.stream>>>(range.as<uint32_t>());
+    int rgrid = (N + 255) / 256;
+    if (rgrid > c.num_sms * 8) rgrid = c.num_sms * 8;
+    prune_range_kernel<<<rgrid, 256, 0, c.stream>>>(X, N, xf, range.as<uint32_t>());
+    g_launches += 2;
+    LIPFIT_CUDA(cudaGetLastError());
+    if ((rc = sorted_keys(c, X, N, xf, range.as<uint32_t>(), bits, dkeys, dorder))) return rc;
+    if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
+    if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
+    LIPFIT_CUDA(cudaMemsetAsync(F_dev, 0, sizeof(double), c.stream));
+    const Xform xfp = padded_xform(xf, dp);
+    SmoothPruneArgs a;
+    a.rec = rec.as<float>();
+    a.box = box.as<float>();
+    a.order = dorder.as<int32_t>();
+    a.eps = eps;
+    a.N = N;
+    a.ntiles = ntiles;
+    a.M = M;
+    a.p = p;
+    a.ff = make_free_flags(xfp);
+    a.F = F_dev;
+    a.grad = grad;
+    a.stats = stats_dev;
+    PruneLaunch pl{X, y, dorder.as<int32_t>(), rec.as<float>(), box.as<float>()};
+    switch (norm) {
+        case LIPFIT_L1: return launch_smooth_pruned_n<1>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
+        case LIPFIT_L2: return launch_smooth_pruned_n<2>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
+        default: return launch_smooth_pruned_n<3>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
+    }
+}
+
 
 }  // namespace lipfit

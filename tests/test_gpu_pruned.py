@@ -95,3 +95,67 @@ def test_config2_full_sampled():
     ub, lb, gb = L.lipfit_bounds(_dev(wl.X), _dev(wl.y), _dev(wl.Xq), wl.M, wl.mask, wl.norm, wl.weights)
     assert np.abs(up - ub.cpu().numpy()).max() <= tol and np.abs(lo - lb.cpu().numpy()).max() <= tol
     assert pairs < 0.2 * wl.N * wl.Q
+
+
+# ---- Eq.(7) objective / gradient with the same pruning (lipfit_smooth_objective_pruned) -------------------
+def _check_smooth(X, y, M, eps, mask, norm, w=None, p=1.0):
+    import paper_2606_04670_b200 as L
+    N = X.shape[0]
+    e64 = np.zeros(N) if eps is None else eps.astype(np.float64)
+    F, grad, pairs = L.lipfit_smooth_objective_pruned(_dev(X), _dev(y), M, None if eps is None else _dev(eps), mask,
+                                                      norm, w, p, count_pairs=True)
+    Fo, go = oracle.smooth_objective(X, y, M, e64, mask, norm, w, p)
+    assert abs(F - Fo) <= 1e-5 * max(Fo, 1e-30)                          # SURVEY.md §8(c) acceptance rule (S)
+    assert np.abs(grad.cpu().numpy() - go).max() <= 1e-5 * max(np.abs(go).max(), 1e-30)
+    assert pairs % 1024 == 0
+    return F, grad, pairs
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("d,mask", [(1, [1]), (2, None), (3, [1, -1, 0]), (5, [1] * 5), (8, [1] + [0] * 7),
+                                    (12, [1, 0] * 6), (21, None)])
+def test_smooth_objective_shapes(norm, d, mask):
+    X, y, _ = random_problem(300 + d, 1500 + d, 1, d)                    # ragged last tile
+    rng = np.random.default_rng(d)
+    w = (0.25 + np.arange(d) % 3).astype(np.float32)
+    _check_smooth(X, y, 1.25, None, mask, norm, w, 1.0)
+    _check_smooth(X, y, 6.0, (0.3 * rng.standard_normal(X.shape[0])).astype(np.float32), mask, norm, None, 2.5)
+
+
+def test_smooth_objective_config5_and_unpruned():
+    import paper_2606_04670_b200 as L
+    wl = make_workload(5, N=20000, Q=1)
+    rng = np.random.default_rng(3)
+    for eps in (None, (0.05 * rng.standard_normal(wl.N)).astype(np.float32)):
+        F, grad, pairs = _check_smooth(wl.X, wl.y, wl.M, eps, wl.mask, wl.norm, None, wl.p)
+        Fu, gu = L.lipfit_smooth_objective(_dev(wl.X), _dev(wl.y), wl.M, None if eps is None else _dev(eps), wl.mask,
+                                           wl.norm, None, wl.p)
+        assert abs(F - Fu) <= 1e-5 * Fu and float((grad - gu).abs().max()) <= 1e-5 * float(gu.abs().max())
+        assert pairs <= 625 * 625 * 1024                                 # at most every tile pair
+    # without the monotone mask only near pairs can violate (noise 0.05 against M d): the pruning bites
+    *_, pairs_sym = _check_smooth(wl.X, wl.y, wl.M, None, None, wl.norm, None, wl.p)
+    assert pairs_sym < 0.5 * wl.N * wl.N
+
+
+def test_smooth_objective_edges():
+    X, y, _ = random_problem(11, 40, 1, 2)
+    _check_smooth(X[:1], y[:1], 1.0, None, None, L2)                     # N = 1: F = 0
+    _check_smooth(X[:2], y[:2], 0.5, None, [1, 0], L1)
+    _check_smooth(X[:33], y[:33], 0.5, None, [-1, 1], LINF)              # one full tile + one datum
+    _check_smooth(np.repeat(X[:3], 20, axis=0), (np.arange(60) % 7).astype(np.float32), 2.0, None, None, L2)
+    _check_smooth(X, y, 0.0, None, None, L2)                             # M = 0: every ordered pair violates
+
+
+def test_smooth_objective_config5_full_vs_unpruned():
+    """Config 5 at full N, in the launch configuration bench.py --configs 12 times: the pruned pass against
+    the (oracle-checked, tests/test_gpu_full_configs.py) unpruned pass, and sampled gradient rows against the oracle."""
+    import paper_2606_04670_b200 as L
+    wl = make_workload(5, Q=1)
+    X, y = _dev(wl.X), _dev(wl.y)
+    F, grad, pairs = L.lipfit_smooth_objective_pruned(X, y, wl.M, None, wl.mask, wl.norm, None, wl.p, count_pairs=True)
+    Fu, gu = L.lipfit_smooth_objective(X, y, wl.M, None, wl.mask, wl.norm, None, wl.p)
+    assert abs(F - Fu) <= 1e-5 * Fu and float((grad - gu).abs().max()) <= 1e-5 * float(gu.abs().max())
+    rows = oracle_subset(wl.N, 48)
+    g_ref, _ = oracle.smooth_rows(wl.X, wl.y, wl.M, np.zeros(wl.N), rows, wl.mask, wl.norm, None, wl.p)
+    assert np.abs(grad.cpu().numpy()[rows] - g_ref).max() <= 1e-5 * np.abs(g_ref).max()
+    assert pairs < 0.5 * wl.N * wl.N                                     # measured: 0.22 (all coordinates monotone)
