@@ -593,6 +593,13 @@ def run_other_config(torch, L, c, args, l2buf, dev, sms, peaks):
                                "speedup_over_unpruned": float(np.mean(ms_u) / np.mean(ms)),
                                "fraction_evaluated": ev / pairs, "F_rel_diff_vs_unpruned": abs(Fs - Fsu) / Fsu,
                                "grad_rel_diff_vs_unpruned": float((gs - gsu).abs().max() / gsu.abs().max())}
+        # lipfit_smooth on the same data without a mask runs the pruned pass (N >= 8192, no constrained coordinate)
+        ys = y.clone()
+        t0 = time.perf_counter()
+        _, info_s = L.lipfit_smooth(X, ys, wl.M, None, wl.norm, None, wl.p, wl.max_iter, 1e-6)
+        torch.cuda.synchronize()
+        out["smooth_no_mask"] = {"wall_s": time.perf_counter() - t0, "info": info_s,
+                                 "ms_per_evaluation_incl_host": 1e3 * (time.perf_counter() - t0) / max(info_s["evals"], 1)}
         if not args.no_cpu:
             rows = oracle_subset(wl.N, 64)
             g_ref, _ = oracle.smooth_rows(wl.X, wl.y, wl.M, np.zeros(wl.N), rows, wl.mask, wl.norm, None, wl.p)

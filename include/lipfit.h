@@ -122,6 +122,8 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d,
  * lower bound  z_k - M d_s(x^i,x^k)  at x^i, so a tile B of data is skipped for the data of a tile A when
  * zmin_B + M dlb^u >= zmax_A  and  zmax_B - M dlb^l <= zmin_A : every term of that tile pair is exactly 0.
  * This is the exact counterpart of the M/3 pair-removal heuristic of PAPER.md:214-218.
+ * lipfit_smooth evaluates Eq.(7) with this pass when no coordinate is constrained and N >= 8192 (where it
+ * wins by an order of magnitude), with the all-pairs pass otherwise.
  * X [N*d], y [N], eps [N] (device, eps may be NULL = 0); *F HOST double (required; the call
  * synchronises); grad [N] device fp32 or NULL; pairs_evaluated HOST int64 or NULL (ordered pairs whose
  * distances were computed, N(N-1) for the unpruned pass). */

@@ -131,13 +131,18 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
     rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>());
     if (rc) return rc;
 
+    const bool use_pruned = smooth_prefers_pruned(xf, N);
     std::vector<double> viol;  // max violation seen by each evaluation
     auto eval = [&](const double* x, double* f, double* g) -> int {
         float* eh = eps_h.as<float>();
         for (size_t i = 0; i < n; ++i) eh[i] = static_cast<float>(x[i]);
         LIPFIT_CUDA(cudaMemcpyAsync(eps_d.p, eh, sizeof(float) * n, cudaMemcpyHostToDevice, c.stream));
-        int r = launch_smooth_objective(c, rec.as<float>(), y_inout, eps_d.as<float>(), N, xf, norm, p,
-                                        fv_d.as<double>(), grad_d.as<float>(), fv_d.as<double>() + 1);
+        int r = use_pruned
+                    ? launch_smooth_objective_pruned(c, X, y_inout, eps_d.as<float>(), N, xf, norm, M, p,
+                                                     fv_d.as<double>(), grad_d.as<float>(), nullptr,
+                                                     fv_d.as<double>() + 1)
+                    : launch_smooth_objective(c, rec.as<float>(), y_inout, eps_d.as<float>(), N, xf, norm, p,
+                                              fv_d.as<double>(), grad_d.as<float>(), fv_d.as<double>() + 1);
         if (r) return r;
         LIPFIT_CUDA(cudaMemcpyAsync(grad_h.p, grad_d.p, sizeof(float) * n, cudaMemcpyDeviceToHost,
                                     c.stream));

@@ -49,7 +49,10 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
 // zeroed here); grad: device float in the original order or NULL; eps may be NULL.
 int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
                                    const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
-                                   unsigned long long* stats_dev);
+                                   unsigned long long* stats_dev, double* maxviol_dev = nullptr);
+// lipfit_smooth evaluates Eq.(7) with the pruned pass when it wins: no constrained coordinate (the
+// dominated orthant of a monotone mask defeats the box test) and enough data to fill the chip
+inline bool smooth_prefers_pruned(const Xform& xf, int64_t N) { return xf.dC == 0 && N >= 8192; }
 
 // a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,

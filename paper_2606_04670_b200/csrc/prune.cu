@@ -475,6 +475,7 @@ struct SmoothPruneArgs {
     float M, p;
     FreeFlags ff;
     double* F;         // device, zeroed
+    double* maxviol;   // device, zeroed, may be NULL: max over pairs of V_ik
     float* grad;       // original order, may be NULL
     unsigned long long* stats;
 };
@@ -513,6 +514,7 @@ smooth_pruned_kernel(const SmoothPruneArgs a) {
     }
     const float zminA = __ldg(ba + 2 * DP), zmaxA = __ldg(ba + 2 * DP + 1);
     double Fi = 0.0, gi = 0.0;
+    float vmax = 0.f;
     unsigned long long n_eval = 0;
     for (int chunk = 0; chunk < nchunks; ++chunk) {
         const int tb = chunk << 5;
@@ -584,6 +586,7 @@ smooth_pruned_kernel(const SmoothPruneArgs a) {
                 fs = fmaf(v1, v1, fs);
                 fs = fmaf(v2, v2, fs);
                 gs += v1 - v2;
+                vmax = fmaxf(vmax, fmaxf(v1, v2));
             }
             Fi += static_cast<double>(fs);
             gi += static_cast<double>(gs);
@@ -597,11 +600,17 @@ smooth_pruned_kernel(const SmoothPruneArgs a) {
         if (a.grad) a.grad[orig] = static_cast<float>(2.0 * e / static_cast<double>(a.p) + 4.0 * gi);
     } else {
         Fi = 0.0;
+        vmax = 0.f;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) Fi += __shfl_xor_sync(0xffffffffu, Fi, o);
+    vmax = warp_max(vmax);
     if (lane == 0) {
         atomicAdd(a.F, Fi);
+        // non-negative doubles order like their bit patterns
+        if (a.maxviol)
+            atomicMax(reinterpret_cast<unsigned long long*>(a.maxviol),
+                      static_cast<unsigned long long>(__double_as_longlong(static_cast<double>(vmax))));
         if (a.stats) atomicAdd(&a.stats[0], n_eval);
     }
 }
@@ -722,7 +731,7 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
 
 int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N64,
                                    const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
-                                   unsigned long long* stats_dev) {
+                                   unsigned long long* stats_dev, double* maxviol_dev) {
     const int N = static_cast<int>(N64);
     const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
     int bits = 32 / xf.d;
@@ -741,6 +750,7 @@ int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y,
     if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
     if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
     LIPFIT_CUDA(cudaMemsetAsync(F_dev, 0, sizeof(double), c.stream));
+    if (maxviol_dev) LIPFIT_CUDA(cudaMemsetAsync(maxviol_dev, 0, sizeof(double), c.stream));
     const Xform xfp = padded_xform(xf, dp);
     SmoothPruneArgs a;
     a.rec = rec.as<float>();
@@ -753,6 +763,7 @@ int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y,
     a.p = p;
     a.ff = make_free_flags(xfp);
     a.F = F_dev;
+    a.maxviol = maxviol_dev;
     a.grad = grad;
     a.stats = stats_dev;
     PruneLaunch pl{X, y, dorder.as<int32_t>(), rec.as<float>(), box.as<float>()};

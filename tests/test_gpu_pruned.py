@@ -159,3 +159,25 @@ def test_smooth_objective_config5_full_vs_unpruned():
     g_ref, _ = oracle.smooth_rows(wl.X, wl.y, wl.M, np.zeros(wl.N), rows, wl.mask, wl.norm, None, wl.p)
     assert np.abs(grad.cpu().numpy()[rows] - g_ref).max() <= 1e-5 * np.abs(g_ref).max()
     assert pairs < 0.5 * wl.N * wl.N                                     # measured: 0.22 (all coordinates monotone)
+
+
+def test_lipfit_smooth_uses_the_pruned_pass_without_a_mask():
+    """lipfit_smooth with no constrained coordinate and N >= 8192 evaluates Eq.(7) with the pruned pass: its
+    report must agree with the oracle's objective / max violation at the returned eps, the returned eps must be a
+    stationary point of the (oracle-checked) all-pairs pass, and the violations must shrink."""
+    import torch
+    import paper_2606_04670_b200 as L
+    wl = make_workload(5, N=9000, Q=1)
+    X, yd = _dev(wl.X), _dev(wl.y)
+    eps, info = L.lipfit_smooth(X, yd, wl.M, None, wl.norm, None, wl.p, max_iter=200, tol_grad=1e-6)
+    torch.cuda.synchronize()
+    e = eps.cpu().numpy()
+    np.testing.assert_allclose(e + wl.y, yd.cpu().numpy(), atol=1e-6)    # y <- y + eps (PAPER.md:234)
+    Fo, go = oracle.smooth_objective(wl.X, wl.y, wl.M, e.astype(np.float64), None, wl.norm, None, wl.p)
+    F0o, _ = oracle.smooth_objective(wl.X, wl.y, wl.M, np.zeros(wl.N), None, wl.norm, None, wl.p)
+    assert abs(info["F"] - Fo) <= 1e-5 * Fo and abs(info["F0"] - F0o) <= 1e-5 * F0o
+    assert info["F"] < info["F0"] and info["max_violation"] < info["max_violation0"]
+    assert abs(info["max_violation0"] - oracle.max_violation(wl.X, wl.y, wl.M, None, None, wl.norm)) <= 1e-5
+    assert np.abs(go).max() <= 1e-3 * max(1.0, info["gnorm_inf"] * 1e3)  # stationary for the oracle's gradient too
+    Fu, gu = L.lipfit_smooth_objective(X, _dev(wl.y), wl.M, eps, None, wl.norm, None, wl.p)
+    assert abs(Fu - info["F"]) <= 1e-5 * Fu                              # SURVEY.md §8(c) rule (S), both passes
