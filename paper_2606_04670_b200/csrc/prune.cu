@@ -224,24 +224,31 @@ __device__ __forceinline__ void eval_tile(const float* __restrict__ rec, int t, 
     for (int c = 0; c < W; ++c) v[c] = __ldg(g + c);
     __syncwarp();  // every lane has finished reading the previous tile
 #pragma unroll
-    for (int c = 0; c < W; ++c) sm[c * 32 + lane] = v[c];
+    for (int c = 0; c < W - 1; ++c) sm[c * 32 + lane] = v[c];
+    // the 32 values packed into eight 16-byte words: one load serves four records
+    reinterpret_cast<float*>(sm + (W - 1) * 32)[lane] = v[W - 1].x;
     __syncwarp();
-#pragma unroll 8
-    for (int r = 0; r < kTile; ++r) {
-        float x[DP];
+#pragma unroll 2
+    for (int r0 = 0; r0 < kTile; r0 += 4) {
+        const float4 y4 = sm[(W - 1) * 32 + (r0 >> 2)];
+        const float yv4[4] = {y4.x, y4.y, y4.z, y4.w};
 #pragma unroll
-        for (int j = 0; j < DP; j += 4) {
-            const float4 xv = sm[(j >> 2) * 32 + r];
-            x[j] = xv.x;
-            x[j + 1] = xv.y;
-            x[j + 2] = xv.z;
-            x[j + 3] = xv.w;
+        for (int u = 0; u < 4; ++u) {
+            const int r = r0 + u;
+            float x[DP];
+#pragma unroll
+            for (int j = 0; j < DP; j += 4) {
+                const float4 xv = sm[(j >> 2) * 32 + r];
+                x[j] = xv.x;
+                x[j + 1] = xv.y;
+                x[j + 2] = xv.z;
+                x[j + 3] = xv.w;
+            }
+            float au, al;
+            pair_acc<NORM, DP, DC>(q, x, ff, au, al);
+            U = fminf(U, fmaf(M, PairAccGeneric<NORM, DP>::finish(au), yv4[u]));
+            L = fmaxf(L, fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), yv4[u]));
         }
-        const float yv = sm[(W - 1) * 32 + r].x;
-        float au, al;
-        pair_acc<NORM, DP, DC>(q, x, ff, au, al);
-        U = fminf(U, fmaf(M, PairAccGeneric<NORM, DP>::finish(au), yv));
-        L = fmaxf(L, fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), yv));
     }
 }
 
