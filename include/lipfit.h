@@ -14,15 +14,23 @@
  *     `mono_mask` and `weights` are HOST arrays of length d (read during the
  *     call; NULL = all 0 / all 1).  The `*_host` variants take HOST pointers for
  *     everything and do the host<->device copies themselves.
- *   - `cuda_stream` is a cudaStream_t (NULL = default stream).  Internal
- *     workspace comes from cudaMallocAsync on that stream and is released
- *     (stream-ordered) before the call returns.  The first call on a device sets
- *     the release threshold of that device's default memory pool to "keep", so
- *     released workspaces stay cached in the pool across synchronisations
- *     (cudaMemPoolTrimTo on the default pool hands them back to the driver).
- *   - Every function returns LIPFIT_OK (0) or a negative lipfit_status; no
- *     exception crosses the boundary; apart from an atomic launch counter there is
- *     no global mutable state, so calls on distinct streams are thread-safe.
+ *   - `cuda_stream` is a cudaStream_t (NULL = default stream).  Internal workspace comes from a
+ *     PRIVATE stream-ordered memory pool of the library (cudaMemPoolCreate, one per device, created on
+ *     first use), is allocated on that stream and released (stream-ordered) before the call returns.
+ *     The pool keeps released workspaces cached across synchronisations (so that back-to-back calls do
+ *     not re-map them); lipfit_release_workspace() hands them back to the driver.  The device's default
+ *     memory pool and the caller's allocator are never touched.
+ *   - Every function returns LIPFIT_OK (0) or a negative lipfit_status; no exception crosses the
+ *     boundary.
+ *   - Thread safety.  The compute entry points keep no per-call state outside their arguments, so
+ *     calls from different host threads on different streams may run concurrently.  Process-wide
+ *     state is exactly: (1) the private memory pools and the caches of device attributes / occupancy
+ *     (mutex-protected, invisible to results); (2) the monotone launch counter lipfit_launch_count
+ *     (atomic); (3) the DIAGNOSTIC timing switch lipfit_set_timing / lipfit_get_timing: process-wide
+ *     accumulators under a mutex, every thread's launches add to them while the switch is on, and a
+ *     timed launch blocks its calling thread -- meant for single-threaded measurement (bench.py), not
+ *     for production use.  Nothing else is global: kernel-selection options and per-call diagnostics
+ *     of kNN are arguments of lipfit_knn_ex, not settings.
  *   - lipfit_bounds / lipfit_knn / lipfit_smooth_objective(F==NULL) are
  *     asynchronous on `cuda_stream`; lipfit_smooth and the *_host variants
  *     synchronise the stream before returning.
@@ -149,6 +157,29 @@ int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64
                     const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
                     int32_t k, int32_t* idx, float* dist, void* cuda_stream);
 
+/* lipfit_knn with per-call options and diagnostics (nothing process-wide is read or written).
+ * flags: LIPFIT_KNN_NO_TENSOR_CORES keeps the selection of symmetric L2, d <= 16 on the CUDA cores
+ *   (FFMA2 cross-term kernel) instead of the tcgen05 bf16x3 GEMM of csrc/knn_tc.cu; the results are
+ *   identical (both feed the same exact re-rank).  Unknown bits: LIPFIT_E_PARAM.
+ * info: HOST pointer or NULL.  When non-NULL the call synchronises the stream and fills
+ *   fallbacks        queries whose superset certificate failed and that were therefore answered by the
+ *                    exact fp64 scan (0 on typical data),
+ *   key_error_ratio  largest observed |selection key - exact fp64 key| / the certificate's error bound E
+ *                    over every pool candidate of this call (the bound is sound iff <= 1; the tests
+ *                    assert it on every kNN case),
+ *   tensor_cores     1 if the tcgen05 selection kernel ran. */
+#define LIPFIT_KNN_NO_TENSOR_CORES 1
+typedef struct lipfit_knn_info {
+    int64_t fallbacks;
+    double key_error_ratio;
+    int32_t tensor_cores;
+    int32_t reserved;
+} lipfit_knn_info;
+int lipfit_knn_ex(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                  const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
+                  int32_t k, int32_t* idx, float* dist, int32_t flags, lipfit_knn_info* info /* host */,
+                  void* cuda_stream);
+
 /* ---- Penalty smoothing, Eq.(5)-(7) PAPER.md:189-198 ---------------------------------------
  * F(eps) = ||eps||^2/p + sum_{i!=k} (z_i - z_k - M d_s(x^k,x^i))_+^2
  *                      + sum_{i!=k} (z_k - z_i - M d_s(x^i,x^k))_+^2,   z = y + eps,
@@ -241,27 +272,20 @@ const char* lipfit_version(void);
 /* Number of kernel launches this library has issued since load (all threads); used by
  * bench.py's gpu_launches.  Monotone counter, not reset. */
 int64_t lipfit_launch_count(void);
-/* Device timing of the dominant kernels, for roofline reports (bench.py).  lipfit_set_timing(1)
- * resets the accumulators and makes every later launch of the three dominant kernels
- * (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs, 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation, 6 = pruned bounds, 7 = pruned smoothing pass) bracketed by CUDA events on
- * its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off (default).
- * lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
+/* Returns the cached workspaces of the current device's private pool to the driver
+ * (cudaMemPoolTrimTo(pool, 0)); workspaces of calls still in flight are unaffected. */
+int lipfit_release_workspace(void);
+/* Device timing of the dominant kernels, for roofline reports (bench.py).  PROCESS-WIDE diagnostic
+ * (see "Thread safety" above).  lipfit_set_timing(1) resets the accumulators and makes every later launch
+ * of the dominant kernels (which: 0 = fused bounds, 1 = kNN selection, 2 = smoothing all-pairs,
+ * 3 = Lipschitz-constant all-pairs, 4 = local step tables, 5 = local evaluation, 6 = pruned bounds,
+ * 7 = pruned smoothing pass, 8 = kNN re-rank, 9 = top-k bounds, 10 = region-monotone bounds) bracketed by
+ * CUDA events on its own stream; such calls wait for that kernel.  lipfit_set_timing(0) switches it off
+ * (default).  lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);
 int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches);
-/* Number of queries of the most recent lipfit_knn / lipfit_knn_host call (any thread) whose
- * superset certificate failed and that were therefore answered by the exact fp64 fallback
- * scan; valid once that call's stream has been synchronised.  0 on typical data. */
-int64_t lipfit_knn_fallbacks(void);
-/* Largest observed |selection key - exact fp64 key| divided by the certificate's error bound E,
- * over every pool candidate of that call (same validity rule).  The bound is sound iff this
- * stays <= 1; the tests assert it on every kNN case. */
-double lipfit_knn_key_error_ratio(void);
-/* Selection kernel choice for symmetric L2 with d <= 16: 1 (default) = tensor cores (tcgen05 bf16x3
- * cross-term GEMM, csrc/knn_tc.cu), 0 = CUDA-core FFMA2 kernel.  Process-wide; results are identical
- * (both feed the same exact re-rank). */
-void lipfit_knn_set_tensor_cores(int32_t on);
-/* Name of the selection kernel lipfit_knn would use for (d, side, norm). */
-int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, char* out, int32_t cap);
+/* Name of the selection kernel lipfit_knn_ex would use for (d, side, norm, flags). */
+int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, int32_t flags, char* out, int32_t cap);
 /* Name of the kernel variant lipfit_bounds would dispatch to for (d, mask, norm), e.g.
  * "bounds<L1,U2,C2,R8>" or "bounds_generic<L2,DP8>"; writes at most `cap` bytes incl. NUL. */
 int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, char* out, int32_t cap);

@@ -36,6 +36,10 @@ def load():
         lib.oracle_values_local.argtypes = [P, P, i64, i32, P, i64, i32, P, P, i32, P, P, P, P]
         lib.oracle_bounds_topk.argtypes = [P, P, i64, i32, P, i64, f64, P, i32, P, i32, P, P, P, P]
         lib.oracle_bounds_topk.restype = C.c_int
+        lib.oracle_local_lipschitz_rows.argtypes = [P, P, i64, i32, i32, P, P, i32, P, i64, P]
+        lib.oracle_local_lipschitz_rows.restype = C.c_int
+        lib.oracle_bounds_region.argtypes = [P, P, i64, i32, P, i64, f64, P, P, P, i32, P, P, P, P]
+        lib.oracle_bounds_region.restype = C.c_int
         for fn in (lib.oracle_distance_quantiles, lib.oracle_local_lipschitz, lib.oracle_values_local):
             fn.restype = C.c_int
         for fn in (lib.oracle_bounds, lib.oracle_knn, lib.oracle_smooth_objective,
@@ -195,6 +199,38 @@ def local_lipschitz(X, y, knots, norm=2, weights=None):
     if rc:
         raise ValueError(f"oracle_local_lipschitz rc={rc}")
     return table
+
+
+def local_lipschitz_rows(X, y, knots, rows, norm=2, weights=None):
+    """table rows [len(rows), J] (float64) of the step functions M_k of the listed data only."""
+    X, y = _f32(X, 2), _f32(y, 1)
+    N, d = X.shape
+    _, w = _params(d, None, weights)
+    knots = np.ascontiguousarray(knots, dtype=np.float64)
+    rows = np.ascontiguousarray(rows, dtype=np.int64)
+    out = np.empty((len(rows), len(knots)), dtype=np.float64)
+    rc = load().oracle_local_lipschitz_rows(_ptr(X), _ptr(y), N, d, int(norm), _ptr(w), _ptr(knots), len(knots),
+                                            _ptr(rows), len(rows), _ptr(out))
+    if rc:
+        raise ValueError(f"oracle_local_lipschitz_rows rc={rc}")
+    return out
+
+
+def bounds_region(X, y, Xq, M, mon, a, b, norm=2, weights=None):
+    """(upper, lower, g) under monotonicity on parts of the domain (reading R26)."""
+    X, y, Xq = _f32(X, 2), _f32(y, 1), _f32(Xq, 2)
+    N, d = X.shape
+    Q = Xq.shape[0]
+    _, w = _params(d, None, weights)
+    mon = None if mon is None else np.ascontiguousarray(mon, dtype=np.int32).reshape(d)
+    a = None if a is None else np.ascontiguousarray(a, dtype=np.float32).reshape(d)
+    b = None if b is None else np.ascontiguousarray(b, dtype=np.float32).reshape(d)
+    U, L, G = (np.empty(Q, dtype=np.float64) for _ in range(3))
+    rc = load().oracle_bounds_region(_ptr(X), _ptr(y), N, d, _ptr(Xq), Q, float(np.float32(M)), _ptr(mon), _ptr(a), _ptr(b),
+                                     int(norm), _ptr(w), _ptr(U), _ptr(L), _ptr(G))
+    if rc:
+        raise ValueError(f"oracle_bounds_region rc={rc}")
+    return U, L, G
 
 
 def values_local(X, y, Xq, knots, table, norm=2, weights=None):

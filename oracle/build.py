@@ -3,6 +3,7 @@
 Usage: python -m oracle.build      (also called by __graft_entry__.build() and,
 on demand, by oracle.load() when the library is missing or stale).
 No -march=native: the .so travels to a different host with the gpurun snapshot.
+FLAGS is what bench.py reports beside the cpu_baseline.
 """
 from __future__ import annotations
 
@@ -32,11 +33,13 @@ def is_fresh() -> bool:
         return False
 
 
+FLAGS = ["-O2", "-std=c11", "-fopenmp", "-fno-fast-math"]
+
+
 def build(force: bool = False) -> str:
     if not force and is_fresh():
         return LIB
-    cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fno-fast-math", "-shared", "-fPIC",
-           "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC[0], "-lm"]
+    cmd = ["gcc", *FLAGS, "-shared", "-fPIC", "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC[0], "-lm"]
     subprocess.run(cmd, check=True, cwd=HERE)
     os.replace(LIB + ".tmp", LIB)
     with open(STAMP, "w") as f:

@@ -334,6 +334,30 @@ int oracle_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm
  * the same distance: the largest of their ratios) and the LAST knot is treated as +infinity, so the
  * last column is the maximum over all data (R21).  A different value at zero distance gives +infinity;
  * an equal value at zero distance (a duplicate) is ignored. */
+/* One row of the table: the step function M_k of datum k, see oracle_local_lipschitz. */
+static void local_lipschitz_row(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                                const float* weights, const double* knots, int32_t J, int64_t k, double* M) {
+    for (int32_t j = 0; j < J; ++j) M[j] = 0.0;
+    double dmin = INFINITY, rnn = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (i == k) continue;
+        double D = radial_distance(X + k * d, X + i * d, d, norm, weights);
+        double dy = fabs((double)y[k] - (double)y[i]);
+        if (D == 0.0 && dy == 0.0) continue; /* duplicate datum */
+        double ratio = (D > 0.0) ? dy / D : INFINITY;
+        if (D < dmin) {
+            dmin = D;
+            rnn = ratio;
+        } else if (D == dmin && ratio > rnn) {
+            rnn = ratio;
+        }
+        for (int32_t j = 0; j < J; ++j)
+            if ((j == J - 1 || D <= knots[j]) && ratio > M[j]) M[j] = ratio;
+    }
+    for (int32_t j = 0; j < J; ++j)
+        if (rnn > M[j]) M[j] = rnn;
+}
+
 int oracle_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
                            const float* weights, const double* knots, int32_t J, double* table) {
     int rc = check_common(X, N, d, NULL, norm, weights);
@@ -341,28 +365,24 @@ int oracle_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d,
     if (!y || !knots || !table) return -1;
     if (J < 1) return -3;
 #pragma omp parallel for schedule(static)
-    for (int64_t k = 0; k < N; ++k) {
-        double* M = table + k * J;
-        for (int32_t j = 0; j < J; ++j) M[j] = 0.0;
-        double dmin = INFINITY, rnn = 0.0;
-        for (int64_t i = 0; i < N; ++i) {
-            if (i == k) continue;
-            double D = radial_distance(X + k * d, X + i * d, d, norm, weights);
-            double dy = fabs((double)y[k] - (double)y[i]);
-            if (D == 0.0 && dy == 0.0) continue; /* duplicate datum */
-            double ratio = (D > 0.0) ? dy / D : INFINITY;
-            if (D < dmin) {
-                dmin = D;
-                rnn = ratio;
-            } else if (D == dmin && ratio > rnn) {
-                rnn = ratio;
-            }
-            for (int32_t j = 0; j < J; ++j)
-                if ((j == J - 1 || D <= knots[j]) && ratio > M[j]) M[j] = ratio;
-        }
-        for (int32_t j = 0; j < J; ++j)
-            if (rnn > M[j]) M[j] = rnn;
-    }
+    for (int64_t k = 0; k < N; ++k)
+        local_lipschitz_row(X, y, N, d, norm, weights, knots, J, k, table + k * J);
+    return 0;
+}
+
+/* The same rows for a list of data only (full-size parity samples): table_rows[r*J + j] = M_{rows[r]}. */
+int oracle_local_lipschitz_rows(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                                const float* weights, const double* knots, int32_t J, const int64_t* rows,
+                                int64_t R, double* table_rows) {
+    int rc = check_common(X, N, d, NULL, norm, weights);
+    if (rc) return rc;
+    if (!y || !knots || !table_rows || (R > 0 && !rows)) return -1;
+    if (J < 1 || R < 0) return -3;
+    for (int64_t r = 0; r < R; ++r)
+        if (rows[r] < 0 || rows[r] >= N) return -3;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < R; ++r)
+        local_lipschitz_row(X, y, N, d, norm, weights, knots, J, rows[r], table_rows + r * J);
     return 0;
 }
 
@@ -452,3 +472,94 @@ int oracle_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
     return bad ? -6 : 0;
 }
 
+
+/* ---- Monotonicity on parts of the domain, PAPER.md:147-167 (section 4.2), reading R26 of DESIGN.md ----
+ * Per coordinate i the line is cut into A: t <= a_i, AB: a_i <= t <= b_i, B: t >= b_i, and
+ *   mon_i = 0: unrestricted,        1: case I   (increasing on A and B),  2: case II (decreasing on A and B),
+ *           3: case III (decreasing on A, increasing on B),               4: case IV (increasing on A, decreasing on B);
+ * AB is unrestricted in every case.  The paper withholds the formula ("can be expressed through components
+ * of the distance vector"); R26 derives it.  Walking coordinate i from the datum's x^k_i to
+ * the query's x_i, f can only GROW on the part of the way where it is not known to fall in the direction
+ * of travel, and can only FALL on the part where it is not known to grow:
+ *   u_i = w_i * (length of the way inside AB
+ *                + length inside A if f may grow there in the direction of travel
+ *                + length inside B if f may grow there in the direction of travel),
+ *   l_i = the same with "fall" for "grow",
+ *   f(x) <= y^k + M ||u||_p,   f(x) >= y^k - M ||l||_p,   then Eq.(2),(3) unchanged.
+ * "f may grow in the direction of travel" = travelling up through an increasing region, or down through a
+ * decreasing one.  a_i = -inf / b_i = +inf are allowed (empty A / empty B). */
+static void region_distances(const float* x, const float* xk, int32_t d, const int32_t* mon,
+                             const float* a, const float* b, int32_t norm, const float* w,
+                             double* Du, double* Dl) {
+    double au = 0.0, al = 0.0;
+    for (int i = 0; i < d; ++i) {
+        double from = (double)xk[i], to = (double)x[i];
+        double lo = fmin(from, to), hi = fmax(from, to);
+        int m = mon ? mon[i] : 0;
+        double cu, cl;
+        if (m == 0) {
+            cu = hi - lo;
+            cl = hi - lo;
+        } else {
+            double ai = (double)a[i], bi = (double)b[i];
+            double lenA = fmax(0.0, fmin(hi, ai) - lo);            /* part of [lo, hi] inside A  */
+            double lenB = fmax(0.0, hi - fmax(lo, bi));            /* part inside B              */
+            double lenM = fmax(0.0, fmin(hi, bi) - fmax(lo, ai));  /* part inside AB             */
+            int incA = (m == 1 || m == 4), incB = (m == 1 || m == 3); /* f increasing on A / on B */
+            int up = (to >= from);                                 /* direction of travel        */
+            int growA = up ? incA : !incA, growB = up ? incB : !incB;
+            cu = lenM + (growA ? lenA : 0.0) + (growB ? lenB : 0.0);
+            cl = lenM + (growA ? 0.0 : lenA) + (growB ? 0.0 : lenB);
+        }
+        double wi = w ? (double)w[i] : 1.0;
+        cu *= wi;
+        cl *= wi;
+        if (norm == 1) {
+            au += cu;
+            al += cl;
+        } else if (norm == 2) {
+            au += cu * cu;
+            al += cl * cl;
+        } else {
+            au = fmax(au, cu);
+            al = fmax(al, cl);
+        }
+    }
+    if (norm == 2) {
+        au = sqrt(au);
+        al = sqrt(al);
+    }
+    *Du = au;
+    *Dl = al;
+}
+
+int oracle_bounds_region(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         double M, const int32_t* mon, const float* a, const float* b, int32_t norm,
+                         const float* weights, double* upper, double* lower, double* g) {
+    int rc = check_common(X, N, d, NULL, norm, weights);
+    if (rc) return rc;
+    if (!y || (Q > 0 && !Xq)) return -1;
+    if (Q < 0) return -3;
+    if (!(M >= 0.0) || !isfinite(M)) return -4;
+    for (int i = 0; i < d; ++i) {
+        int m = mon ? mon[i] : 0;
+        if (m < 0 || m > 4) return -4;
+        if (m != 0 && (!a || !b || !(a[i] <= b[i]))) return -4; /* also rejects NaN */
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < Q; ++q) {
+        double U = INFINITY, L = -INFINITY;
+        for (int64_t k = 0; k < N; ++k) {
+            double Du, Dl;
+            region_distances(Xq + q * d, X + k * d, d, mon, a, b, norm, weights, &Du, &Dl);
+            double hi = (double)y[k] + M * Du;
+            double lo = (double)y[k] - M * Dl;
+            if (hi < U) U = hi;
+            if (lo > L) L = lo;
+        }
+        if (upper) upper[q] = U;
+        if (lower) lower[q] = L;
+        if (g) g[q] = 0.5 * (U + L);
+    }
+    return 0;
+}

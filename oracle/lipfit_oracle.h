@@ -13,7 +13,9 @@
  * enclosure of the generator, Lipschitz and monotone properties, 1-D closed
  * forms, scipy cdist / cKDTree special cases, metamorphic relations, N=2
  * smoothing closed form, finite-difference gradient, brute force on tiny
- * inputs.  The one thing left "parity unpinned" by design is the LBFGS
+ * inputs; for region monotonicity (oracle_bounds_region, R26) the limits a = b and
+ * a = -inf, b = +inf, admissible 1-D functions (enclosure and attainment) and an
+ * independent NumPy integration of the "may grow" indicator along the way.  The one thing left "parity unpinned" by design is the LBFGS
  * TRAJECTORY of smoothing (the minimiser itself is unique and is pinned).
  *
  * All inputs are fp32 arrays on the host (the same arrays the GPU gets); every
@@ -85,6 +87,10 @@ int oracle_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm
 /* table[k*J+j] = value of the step function M_k on (t_{j-1}, t_j] (last knot = +inf). */
 int oracle_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
                            const float* weights, const double* knots, int32_t J, double* table);
+/* Rows rows[0..R) of the same table only: table_rows[r*J+j] = M_{rows[r]} on (t_{j-1}, t_j]. */
+int oracle_local_lipschitz_rows(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
+                                const float* weights, const double* knots, int32_t J, const int64_t* rows,
+                                int64_t R, double* table_rows);
 /* Eq.(2),(3) with M -> M_k(D(x, x^k)). */
 int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                         int32_t norm, const float* weights, const double* knots, int32_t J,
@@ -95,6 +101,16 @@ int oracle_values_local(const float* X, const float* y, int64_t N, int32_t d, co
 int oracle_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                        double M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
                        const float* wk, double* upper, double* lower, double* g);
+
+/* Eq.(2),(3) under monotonicity on parts of the domain (cases I-IV; reading R26):
+ * mon[i] in {0,1,2,3,4} (0 = unrestricted, 1..4 = case I..IV), a[i] <= b[i] (a = -inf / b = +inf allowed)
+ * for every coordinate with mon[i] != 0.  Per coordinate, walking from x^k_i to x_i,
+ *   u_i = w_i (length of the way in AB + length in A / B where f may grow in the direction of travel),
+ *   l_i = w_i (length of the way in AB + length in A / B where f may fall in the direction of travel),
+ * upper = min_k (y^k + M ||u||_p), lower = max_k (y^k - M ||l||_p), g their midpoint. */
+int oracle_bounds_region(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         double M, const int32_t* mon, const float* a, const float* b, int32_t norm,
+                         const float* weights, double* upper, double* lower, double* g);
 
 int oracle_num_threads(void);
 

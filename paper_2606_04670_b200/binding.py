@@ -21,14 +21,21 @@ EXPORTS = [
     "lipfit_bounds", "lipfit_bounds_host", "lipfit_knn", "lipfit_knn_host",
     "lipfit_smooth_objective", "lipfit_smooth", "lipfit_smooth_host", "lipfit_lbfgs",
     "lipfit_status_string", "lipfit_version", "lipfit_launch_count", "lipfit_bounds_variant",
-    "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_fallbacks",
-    "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host",
-    "lipfit_knn_key_error_ratio", "lipfit_knn_set_tensor_cores", "lipfit_knn_variant",
+    "lipfit_set_timing", "lipfit_get_timing", "lipfit_knn_ex", "lipfit_release_workspace",
+    "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host", "lipfit_knn_variant",
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
     "lipfit_bounds_pruned", "lipfit_smooth_objective_pruned",
 ]
 LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
+LIPFIT_KNN_NO_TENSOR_CORES = 1
+
+
+__all__ = [n for n in EXPORTS if n not in ("lipfit_status_string", "lipfit_version", "lipfit_launch_count",
+                                           "lipfit_bounds_variant", "lipfit_set_timing", "lipfit_get_timing",
+                                           "lipfit_knn_variant", "lipfit_release_workspace")] + [
+    "LIPFIT_L1", "LIPFIT_L2", "LIPFIT_LINF", "LIPFIT_MAX_DIM", "LIPFIT_MAX_K", "LIPFIT_MAX_TOPK",
+    "LIPFIT_LOCAL_KNOTS", "LIPFIT_KNN_NO_TENSOR_CORES"]
 
 
 class LipfitError(RuntimeError):
@@ -45,6 +52,15 @@ class SmoothInfo(C.Structure):
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class KnnInfo(C.Structure):
+    _fields_ = [("fallbacks", C.c_int64), ("key_error_ratio", C.c_double), ("tensor_cores", C.c_int32),
+                ("reserved", C.c_int32)]
+
+    def as_dict(self):
+        return {"fallbacks": int(self.fallbacks), "key_error_ratio": float(self.key_error_ratio),
+                "tensor_cores": bool(self.tensor_cores)}
 
 
 EVAL_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double),
@@ -64,6 +80,7 @@ def load():
     lib.lipfit_bounds_host.argtypes = lib.lipfit_bounds.argtypes
     lib.lipfit_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, P]
     lib.lipfit_knn_host.argtypes = lib.lipfit_knn.argtypes
+    lib.lipfit_knn_ex.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, i32, P, P]
     lib.lipfit_smooth_objective_pruned.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, P, P, P, P, P]
     lib.lipfit_smooth_objective.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, P, P, P, P]
     lib.lipfit_smooth.argtypes = [P, P, i64, i32, f32, P, i32, P, f32, i32, f64, P, P, P]
@@ -84,13 +101,8 @@ def load():
     lib.lipfit_version.restype = C.c_char_p
     lib.lipfit_launch_count.restype = C.c_int64
     lib.lipfit_set_timing.restype = None
-    lib.lipfit_knn_key_error_ratio.argtypes = []
-    lib.lipfit_knn_key_error_ratio.restype = C.c_double
-    lib.lipfit_knn_set_tensor_cores.argtypes = [i32]
-    lib.lipfit_knn_set_tensor_cores.restype = None
-    lib.lipfit_knn_variant.argtypes = [i32, i32, i32, C.c_char_p, i32]
-    lib.lipfit_knn_fallbacks.argtypes = []
-    lib.lipfit_knn_fallbacks.restype = i64
+    lib.lipfit_knn_variant.argtypes = [i32, i32, i32, i32, C.c_char_p, i32]
+    lib.lipfit_release_workspace.argtypes = []
     lib.lipfit_set_timing.argtypes = [i32]
     lib.lipfit_get_timing.argtypes = [i32, P, P]
     _lib = lib
@@ -109,23 +121,15 @@ def launch_count() -> int:
     return int(load().lipfit_launch_count())
 
 
-def knn_fallbacks() -> int:
-    """Queries of the last lipfit_knn call answered by the exact fp64 fallback (after a sync)."""
-    return int(load().lipfit_knn_fallbacks())
+def release_workspace() -> None:
+    """Hands the cached workspaces of the library's private memory pool back to the driver."""
+    _check(load().lipfit_release_workspace(), "lipfit_release_workspace")
 
 
-def knn_key_error_ratio() -> float:
-    """Largest observed selection-key error / certificate bound of the last lipfit_knn call (<= 1)."""
-    return float(load().lipfit_knn_key_error_ratio())
-
-
-def knn_set_tensor_cores(on: bool) -> None:
-    load().lipfit_knn_set_tensor_cores(1 if on else 0)
-
-
-def knn_variant(d: int, side: int = 0, norm: int = LIPFIT_L2) -> str:
+def knn_variant(d: int, side: int = 0, norm: int = LIPFIT_L2, tensor_cores: bool = True) -> str:
     buf = C.create_string_buffer(96)
-    _check(load().lipfit_knn_variant(d, side, norm, buf, 96), "lipfit_knn_variant")
+    _check(load().lipfit_knn_variant(d, side, norm, 0 if tensor_cores else LIPFIT_KNN_NO_TENSOR_CORES, buf, 96),
+           "lipfit_knn_variant")
     return buf.value.decode()
 
 
@@ -243,6 +247,26 @@ def lipfit_bounds_topk(X, y, Xq, M: float, wk, mono_mask=None, norm: int = LIPFI
                                    outs[1].data_ptr(), outs[2].data_ptr(), _stream(stream))
     _check(rc, "lipfit_bounds_topk")
     return tuple(outs)
+
+
+def lipfit_knn_ex(X, Xq, k: int, mono_mask=None, side: int = 0, norm: int = LIPFIT_L2, weights=None,
+                  tensor_cores: bool = True, want_info: bool = True, stream=None):
+    """(idx, dist, info dict or None) through lipfit_knn_ex: per-call kernel choice and diagnostics
+    (want_info=True synchronises the stream)."""
+    torch = _torch()
+    X, Xq = _dev_f32(X, 2, "X"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    m, w = _host_params(d, mono_mask, weights)
+    idx = torch.empty((Q, k), dtype=torch.int32, device=X.device)
+    dist = torch.empty((Q, k), dtype=torch.float32, device=X.device)
+    info = KnnInfo()
+    rc = load().lipfit_knn_ex(X.data_ptr(), N, d, Xq.data_ptr(), Q, _np_ptr(m), int(side), int(norm),
+                              _np_ptr(w), int(k), idx.data_ptr(), dist.data_ptr(),
+                              0 if tensor_cores else LIPFIT_KNN_NO_TENSOR_CORES,
+                              C.cast(C.byref(info), C.c_void_p) if want_info else None, _stream(stream))
+    _check(rc, "lipfit_knn_ex")
+    return idx, dist, (info.as_dict() if want_info else None)
 
 
 def lipfit_knn(X, Xq, k: int, mono_mask=None, side: int = 0, norm: int = LIPFIT_L2, weights=None,

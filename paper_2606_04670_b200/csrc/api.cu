@@ -70,18 +70,17 @@ int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, cha
     return LIPFIT_OK;
 }
 
-int64_t lipfit_knn_fallbacks(void) { return knn_last_fallbacks(); }
-double lipfit_knn_key_error_ratio(void) { return knn_last_key_error_ratio(); }
-void lipfit_knn_set_tensor_cores(int32_t on) { knn_set_tensor_cores(on); }
-int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, char* out, int32_t cap) {
+int lipfit_release_workspace(void) { return workspace_release(); }
+
+int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, int32_t flags, char* out, int32_t cap) {
     if (!out || cap < 1) return LIPFIT_E_NULL;
-    if (check_norm(norm) || side < -1 || side > 1) return LIPFIT_E_PARAM;
+    if (check_norm(norm) || side < -1 || side > 1 || (flags & ~LIPFIT_KNN_NO_TENSOR_CORES)) return LIPFIT_E_PARAM;
     if (d < 1 || d > LIPFIT_MAX_DIM) return LIPFIT_E_DIM;
     Xform xf;
     std::vector<int32_t> mask(static_cast<size_t>(d), side == 0 ? 0 : 1);  // any constrained coordinate => one-sided
     int rc = make_xform(d, mask.data(), nullptr, side == 0, false, &xf);
     if (rc) return rc;
-    std::strncpy(out, knn_variant_name(xf, norm), static_cast<size_t>(cap) - 1);
+    std::strncpy(out, knn_variant_name(xf, norm, !(flags & LIPFIT_KNN_NO_TENSOR_CORES)), static_cast<size_t>(cap) - 1);
     out[cap - 1] = '\0';
     return LIPFIT_OK;
 }
@@ -89,6 +88,7 @@ int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, char* out, int32_t
 int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                   float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
                   float* lower, float* g, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
@@ -104,17 +104,19 @@ int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const fl
     RecLayout lay = bounds_layout(c, xf, norm, Q);
     if (lay.rf == 0) return LIPFIT_E_PARAM;
     const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
+    const float* centre = lay.mscale ? X : nullptr;          // ... and those are translated to the first datum
     Workspace rec;
     rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
     if (rc) return rc;
-    rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>());
+    rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>(), centre);
     if (rc) return rc;
-    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g);
+    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g, centre);
 }
 
 int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                          float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
                          float* lower, float* g, int64_t* pairs_evaluated, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds_pruned");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
@@ -153,6 +155,7 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
 int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                        float M, const int32_t* mono_mask, int32_t norm, const float* weights, int32_t k,
                        const float* wk, float* upper, float* lower, float* g, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds_topk");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (k < 1 || k > LIPFIT_MAX_TOPK || k > N) return LIPFIT_E_SIZE;
@@ -182,6 +185,7 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, con
                        int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
                        const float* weights, float* upper, float* lower, float* g,
                        void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds_host");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
@@ -212,10 +216,18 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, con
 int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
                const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights, int32_t k,
                int32_t* idx, float* dist, void* cuda_stream) {
+    return lipfit_knn_ex(X, N, d, Xq, Q, mono_mask, side, norm, weights, k, idx, dist, 0, nullptr, cuda_stream);
+}
+
+int lipfit_knn_ex(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                  const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights, int32_t k,
+                  int32_t* idx, float* dist, int32_t flags, lipfit_knn_info* info, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_knn_ex");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (k < 1 || k > N || k > LIPFIT_MAX_K) return LIPFIT_E_SIZE;
-    if (check_norm(norm) || side < -1 || side > 1) return LIPFIT_E_PARAM;
+    if (check_norm(norm) || side < -1 || side > 1 || (flags & ~LIPFIT_KNN_NO_TENSOR_CORES)) return LIPFIT_E_PARAM;
+    if (info) *info = lipfit_knn_info{0, 0.0, 0, 0};
     Xform xf;
     rc = make_xform(d, mono_mask, weights, side == 0, side < 0, &xf);
     if (rc) return rc;
@@ -225,12 +237,13 @@ int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
-    return launch_knn(c, X, N, Xq, Q, xf, norm, k, idx, dist);
+    return launch_knn(c, X, N, Xq, Q, xf, norm, k, idx, dist, !(flags & LIPFIT_KNN_NO_TENSOR_CORES), info);
 }
 
 int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,
                     const int32_t* mono_mask, int32_t side, int32_t norm, const float* weights,
                     int32_t k, int32_t* idx, float* dist, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_knn_host");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (k < 1 || k > N || k > LIPFIT_MAX_K) return LIPFIT_E_SIZE;
@@ -261,6 +274,7 @@ int lipfit_knn_host(const float* X, int64_t N, int32_t d, const float* Xq, int64
 int lipfit_distance_quantiles(const float* X, int64_t N, int32_t d, int32_t norm, const float* weights,
                               const int32_t* pair_i, const int32_t* pair_k, int64_t S, int32_t J, float* knots,
                               void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_distance_quantiles");
     int rc = check_sizes(N, d, 0);
     if (rc) return rc;
     if (check_norm(norm)) return LIPFIT_E_PARAM;
@@ -294,6 +308,7 @@ static int check_knots(const float* knots, int32_t J) {
 int lipfit_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d, int32_t norm,
                            const float* weights, const float* knots, int32_t J, float* table,
                            void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_local_lipschitz");
     int rc = check_sizes(N, d, 0);
     if (rc) return rc;
     if (check_norm(norm)) return LIPFIT_E_PARAM;
@@ -310,6 +325,7 @@ int lipfit_local_lipschitz(const float* X, const float* y, int64_t N, int32_t d,
 int lipfit_values_local(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
                         int32_t norm, const float* weights, const float* knots, int32_t J, const float* table,
                         float* upper, float* lower, float* g, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_values_local");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm)) return LIPFIT_E_PARAM;

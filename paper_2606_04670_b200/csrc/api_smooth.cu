@@ -48,6 +48,7 @@ extern "C" {
 int lipfit_smooth_objective(const float* X, const float* y, int64_t N, int32_t d, float M,
                             const int32_t* mono_mask, int32_t norm, const float* weights, float p,
                             const float* eps, double* F, float* grad, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_smooth_objective");
     int rc = check_common(X, y, N, d, M, norm, p);
     if (rc) return rc;
     Xform xf;
@@ -63,7 +64,7 @@ int lipfit_smooth_objective(const float* X, const float* y, int64_t N, int32_t d
     if (rc) return rc;
     rc = fdev.alloc(sizeof(double) * 2, c.stream);
     if (rc) return rc;
-    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>());
+    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>(), X /* centre */);
     if (rc) return rc;
     rc = launch_smooth_objective(c, rec.as<float>(), y, eps, N, xf, norm, p,
                                  F ? fdev.as<double>() : nullptr, grad, nullptr);
@@ -79,6 +80,7 @@ int lipfit_smooth_objective_pruned(const float* X, const float* y, int64_t N, in
                                    const int32_t* mono_mask, int32_t norm, const float* weights, float p,
                                    const float* eps, double* F, float* grad, int64_t* pairs_evaluated,
                                    void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_smooth_objective_pruned");
     int rc = check_common(X, y, N, d, M, norm, p);
     if (rc) return rc;
     Xform xf;
@@ -108,6 +110,7 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
                   const int32_t* mono_mask, int32_t norm, const float* weights, float p,
                   int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,
                   void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_smooth");
     int rc = check_common(X, y_inout, N, d, M, norm, p);
     if (rc) return rc;
     if (max_iter < 0 || !(tol_grad >= 0.0)) return LIPFIT_E_PARAM;
@@ -128,7 +131,7 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
     if ((rc = eps_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = grad_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = fv_h.alloc(sizeof(double) * 2))) return rc;
-    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>());
+    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>(), X /* centre */);
     if (rc) return rc;
 
     const bool use_pruned = smooth_prefers_pruned(xf, N);
@@ -194,6 +197,7 @@ int lipfit_smooth_host(const float* X, float* y_inout, int64_t N, int32_t d, flo
                        const int32_t* mono_mask, int32_t norm, const float* weights, float p,
                        int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,
                        void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_smooth_host");
     int rc = check_common(X, y_inout, N, d, M, norm, p);
     if (rc) return rc;
     if (max_iter < 0 || !(tol_grad >= 0.0)) return LIPFIT_E_PARAM;
@@ -219,6 +223,7 @@ int lipfit_smooth_host(const float* X, float* y_inout, int64_t N, int32_t d, flo
 int lipfit_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t d,
                               const int32_t* mono_mask, int32_t norm, const float* weights, float* L,
                               void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_lipschitz_constant");
     int rc = check_common(X, y, N, d, 0.f, norm, 1.f);
     if (rc) return rc;
     if (!L) return LIPFIT_E_NULL;
@@ -240,6 +245,7 @@ int lipfit_lipschitz_constant(const float* X, const float* y, int64_t N, int32_t
 int lipfit_lipschitz_constant_host(const float* X, const float* y, int64_t N, int32_t d,
                                    const int32_t* mono_mask, int32_t norm, const float* weights,
                                    float* L, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_lipschitz_constant_host");
     int rc = check_common(X, y, N, d, 0.f, norm, 1.f);
     if (rc) return rc;
     if (!L) return LIPFIT_E_NULL;
@@ -263,6 +269,7 @@ int lipfit_lipschitz_constant_host(const float* X, const float* y, int64_t N, in
 
 int lipfit_lbfgs(int64_t n, double* x, lipfit_eval_fn fn, void* user, int32_t max_iter,
                  double tol_grad, int32_t history, lipfit_smooth_info* info) {
+    NvtxRange nvtx_range("lipfit_lbfgs");
     if (!x || !fn) return LIPFIT_E_NULL;
     if (n < 1 || n > 0x7fffffffLL || max_iter < 0 || history < 1 || !(tol_grad >= 0.0))
         return LIPFIT_E_SIZE;

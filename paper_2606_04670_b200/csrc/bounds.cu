@@ -16,6 +16,7 @@ namespace lipfit {
 struct BoundsArgs {
     const float* rec;
     const float* Xq;
+    const float* centre;  // translation applied to the records (launch_prepack) or NULL
     float* upper;
     float* lower;
     float* g;
@@ -162,10 +163,12 @@ bounds_kernel(const BoundsArgs a, const FreeFlags ff) {
             const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
 #pragma unroll
             for (int j = 0; j < D; ++j) {
-                if (Core::kGeneric)
+                if (Core::kGeneric) {
                     q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
-                else
-                    q[r][j] = a.xf.sw[j] * __ldg(src + a.xf.perm[j]);
+                } else {
+                    const int o = a.xf.perm[j];
+                    q[r][j] = a.xf.sw[j] * (a.centre ? __ldg(src + o) - __ldg(a.centre + o) : __ldg(src + o));
+                }
             }
             U[r] = __int_as_float(0x7f800000);
             L[r] = __int_as_float(0xff800000);
@@ -363,8 +366,11 @@ bounds_packed_kernel(const BoundsArgs a) {
             const float* s0 = a.Xq + static_cast<size_t>(q0) * a.d;
             const float* s1 = a.Xq + static_cast<size_t>(q1) * a.d;
 #pragma unroll
-            for (int j = 0; j < D; ++j)
-                q[rp][j] = make_float2(a.xf.sw[j] * __ldg(s0 + a.xf.perm[j]), a.xf.sw[j] * __ldg(s1 + a.xf.perm[j]));
+            for (int j = 0; j < D; ++j) {
+                const int o = a.xf.perm[j];
+                const float cj = a.centre ? __ldg(a.centre + o) : 0.f;  // x - 0 is exact
+                q[rp][j] = make_float2(a.xf.sw[j] * (__ldg(s0 + o) - cj), a.xf.sw[j] * (__ldg(s1 + o) - cj));
+            }
             U[rp] = make_float2(__int_as_float(0x7f800000), __int_as_float(0x7f800000));
             L[rp] = make_float2(__int_as_float(0xff800000), __int_as_float(0xff800000));
         }
@@ -664,12 +670,15 @@ const char* bounds_variant_name(const Xform& xf, int norm) {
 }
 
 int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q,
-                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g) {
+                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
+                  const float* centre) {
     const Variant* v = pick(xf, norm);
     if (!v) return LIPFIT_E_PARAM;
+    if (centre && v->dC < 0) return LIPFIT_E_PARAM;  // the generic kernels take untranslated records
     BoundsArgs a{};
     a.rec = rec;
     a.Xq = Xq;
+    a.centre = centre;
     a.upper = upper;
     a.lower = lower;
     a.g = g;
@@ -794,7 +803,7 @@ int launch_topk(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeig
     if (occ < 1) occ = 1;
     a.nqb = (a.Q + 128 * R - 1) / (128 * R);
     const int slots = c.num_sms * occ;
-    KernelTimer kt(TK_BOUNDS, c.stream);
+    KernelTimer kt(TK_BOUNDS_TOPK, c.stream);
     kern<<<a.nqb < slots ? a.nqb : slots, 128, 0, c.stream>>>(a, ff, wk);
     kt.stop();
     ++g_launches;

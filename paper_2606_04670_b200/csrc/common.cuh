@@ -7,6 +7,8 @@
 
 #include <atomic>
 
+#include <nvtx3/nvToolsExt.h>  // header-only NVTX v3: a no-op unless a profiler injects itself
+
 #include "../../include/lipfit.h"
 
 namespace lipfit {
@@ -33,7 +35,8 @@ extern std::atomic<int64_t> g_launches;
 
 // Optional per-kernel device timing of the three dominant kernels (lipfit_set_timing): when on,
 // the launch is bracketed by CUDA events on its own stream and the call waits for it.
-enum TimedKernel { TK_BOUNDS = 0, TK_KNN_SELECT = 1, TK_SMOOTH_PAIRS = 2, TK_LIPCONST_PAIRS = 3, TK_LOCAL_TABLE = 4, TK_LOCAL_EVAL = 5, TK_BOUNDS_PRUNED = 6, TK_SMOOTH_PRUNED = 7, TK_COUNT = 8 };
+enum TimedKernel { TK_BOUNDS = 0, TK_KNN_SELECT = 1, TK_SMOOTH_PAIRS = 2, TK_LIPCONST_PAIRS = 3, TK_LOCAL_TABLE = 4, TK_LOCAL_EVAL = 5, TK_BOUNDS_PRUNED = 6, TK_SMOOTH_PRUNED = 7,
+                   TK_KNN_RERANK = 8, TK_BOUNDS_TOPK = 9, TK_BOUNDS_REGION = 10, TK_COUNT = 11 };
 struct KernelTimer {
     int which;
     cudaStream_t s;
@@ -42,6 +45,14 @@ struct KernelTimer {
     KernelTimer(int which_, cudaStream_t s_);
     void stop();  // call right after the launch
     ~KernelTimer();
+};
+
+// NVTX range around an entry point of the C ABI (visible in Nsight Systems / ncu --nvtx).
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+    NvtxRange(const NvtxRange&) = delete;
+    NvtxRange& operator=(const NvtxRange&) = delete;
 };
 
 struct Ctx {
@@ -74,13 +85,20 @@ inline int cuda_rc(cudaError_t e) {
         }                                                  \
     } while (0)
 
+// The library's PRIVATE stream-ordered memory pool of the current device (created on first use, release
+// threshold "keep": freed workspaces stay cached across synchronisations until lipfit_release_workspace()).
+// The device's default pool, which the host application may use, is never touched.
+cudaError_t workspace_pool(cudaMemPool_t* pool);
+
 // Stream-ordered workspace that frees itself (stream-ordered) when it goes out of scope.
 struct Workspace {
     void* p = nullptr;
     cudaStream_t s = nullptr;
     int alloc(size_t bytes, cudaStream_t stream) {
         s = stream;
-        cudaError_t e = cudaMallocAsync(&p, bytes ? bytes : 16, stream);
+        cudaMemPool_t pool;
+        cudaError_t e = workspace_pool(&pool);
+        if (e == cudaSuccess) e = cudaMallocFromPoolAsync(&p, bytes ? bytes : 16, pool, stream);
         if (e != cudaSuccess) {
             (void)cudaGetLastError();
             p = nullptr;

@@ -26,12 +26,19 @@ RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
 RecLayout smooth_layout(const Xform& xf, int norm);
 
 // a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].
+// centre: device float[d] in the ORIGINAL coordinate order or NULL.  When given, the packed coordinates are
+// sw_j (x - centre): the kernel families that pre-multiply the coordinates by M (layouts with mscale, the
+// smoothing records) round M w x before subtracting, an absolute error ~2^-24 M |x| per coordinate -- after
+// the translation it scales with the spread of the data instead of their offset from the origin.  The
+// callers pass the first datum X[0 .. d) (any point near the data does; distances are translation
+// invariant).  The consumer must translate its queries by the same centre.
 int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
-                   const Xform& xf, RecLayout lay, float* rec);
+                   const Xform& xf, RecLayout lay, float* rec, const float* centre = nullptr);
 
 // a2: fused bounds.  rec: packed records; Xq: ORIGINAL row-major queries (transformed on load).
 int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q,
-                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g);
+                  const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
+                  const float* centre = nullptr);
 const char* bounds_variant_name(const Xform& xf, int norm);
 // NEXT-2: weighted sums of the k best upper / lower bound values; wk_host: host float[k]
 RecLayout bounds_topk_layout(const Xform& xf);
@@ -54,17 +61,11 @@ int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y,
 // dominated orthant of a monotone mask defeats the box test) and enough data to fill the chip
 inline bool smooth_prefers_pruned(const Xform& xf, int64_t N) { return xf.dC == 0 && N >= 8192; }
 
-// a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.
+// a3: fused distance + top-k selection (fp32) followed by the fp64 re-rank.  allow_tc = false keeps the
+// selection on the CUDA cores; info (host, may be NULL): per-call diagnostics, the call then synchronises.
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
-               int norm, int k, int32_t* idx, float* dist);
-const char* knn_variant_name(const Xform& xf, int norm);
-// queries of the most recent completed lipfit_knn call that needed the exact fp64 fallback
-int64_t knn_last_fallbacks();
-// largest observed |selection key - exact fp64 key| / certificate bound E over all pool candidates of
-// the most recent completed call (must stay <= 1; the tests assert it)
-double knn_last_key_error_ratio();
-// 1 (default): symmetric L2 with d <= 16 selects on the tensor cores; 0: CUDA-core selection everywhere
-void knn_set_tensor_cores(int on);
+               int norm, int k, int32_t* idx, float* dist, bool allow_tc, lipfit_knn_info* info);
+const char* knn_variant_name(const Xform& xf, int norm, bool allow_tc);
 
 // a4: all-pairs objective/gradient.  base: packed records whose coordinates are PRE-MULTIPLIED BY M
 // (prepack with scale_xform(xf, M)); their value slot is ignored, z = y + eps is formed per call.
@@ -92,6 +93,9 @@ int launch_set_values(const Ctx& c, float* rec, RecLayout lay, const float* y, c
                       int64_t N);
 // y[k] += eps[k]
 int launch_axpy(const Ctx& c, float* y, const float* eps, int64_t N);
+
+// cudaMemPoolTrimTo(private pool of the current device, 0)
+int workspace_release();
 
 void timing_set(int on);
 int timing_get(int which, double* ms, long long* n);

@@ -615,43 +615,14 @@ int dispatch(const Ctx& c, KnnArgs& a, const FreeFlags& ff, int norm, bool onesi
                     : dispatch_dp<3, false>(c, a, ff, dp, slots, query_only);
 }
 
-// pinned host words written stream-ordered at the end of every call: [0] exact-fallback queries,
-// [1] bits of the largest observed key error / bound
-int32_t* fallback_word() {
-    static int32_t* h = [] {
-        int32_t* p = nullptr;
-        if (cudaMallocHost(&p, 2 * sizeof(int32_t)) != cudaSuccess) {
-            (void)cudaGetLastError();
-            return static_cast<int32_t*>(nullptr);
-        }
-        p[0] = p[1] = 0;
-        return p;
-    }();
-    return h;
+bool use_tc(const Xform& xf, int norm, bool allow_tc) {
+    return allow_tc && norm == 2 && xf.dC == 0 && xf.d <= 16;
 }
-
-std::atomic<int> g_knn_tc{1};
-
-bool use_tc(const Xform& xf, int norm) { return norm == 2 && xf.dC == 0 && xf.d <= 16 && g_knn_tc.load() != 0; }
 
 }  // namespace
 
-int64_t knn_last_fallbacks() {
-    int32_t* h = fallback_word();
-    return h ? static_cast<int64_t>(*reinterpret_cast<volatile int32_t*>(h)) : -1;
-}
-double knn_last_key_error_ratio() {
-    int32_t* h = fallback_word();
-    if (!h) return -1.0;
-    const int32_t bits = *reinterpret_cast<volatile int32_t*>(h + 1);
-    float f;
-    memcpy(&f, &bits, sizeof(f));
-    return static_cast<double>(f);
-}
-void knn_set_tensor_cores(int on) { g_knn_tc.store(on ? 1 : 0); }
-
-const char* knn_variant_name(const Xform& xf, int norm) {
-    if (use_tc(xf, norm)) {  // K = 16 bf16 per K step, ceil((3 d + 3) / 16) steps (knn_tc.cu)
+const char* knn_variant_name(const Xform& xf, int norm, bool allow_tc) {
+    if (use_tc(xf, norm, allow_tc)) {  // K = 16 bf16 per K step, ceil((3 d + 3) / 16) steps (knn_tc.cu)
         static const char* const names[4] = {"knn_tc_select<bf16x3,K16>", "knn_tc_select<bf16x3,K32>",
                                              "knn_tc_select<bf16x3,K48>", "knn_tc_select<bf16x3,K64>"};
         return names[(3 * xf.d + 3 + 15) / 16 - 1];
@@ -660,7 +631,7 @@ const char* knn_variant_name(const Xform& xf, int norm) {
 }
 
 int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
-               int norm, int k, int32_t* idx, float* dist) {
+               int norm, int k, int32_t* idx, float* dist, bool allow_tc, lipfit_knn_info* info) {
     KnnArgs a{};
     const int dp = knn_dp(xf.d);
     const int rf = dp + 4;
@@ -673,7 +644,7 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     a.xf = xf;
     a.ksel = static_cast<int>(N < k + kKnnMargin ? N : k + kKnnMargin);
     a.P = 2 * a.ksel;
-    const bool tc = use_tc(xf, norm);  // tensor-core selection (knn_tc.cu)
+    const bool tc = use_tc(xf, norm, allow_tc);  // tensor-core selection (knn_tc.cu)
     if (tc) a.P = a.ksel + kTcPoolExtra;
     const int qper = tc ? kTcQueries : kSelThreads * knn_r(dp);
     a.nqb = (a.Q + qper - 1) / qper;
@@ -760,17 +731,27 @@ int launch_knn(const Ctx& c, const float* X, int64_t N, const float* Xq, int64_t
     r.norm = norm;
     r.dot = tc ? 2 : (dot ? 1 : 0);
     r.xf = xf;
-    knn_rerank_kernel<<<(a.Q + kRerankWarps - 1) / kRerankWarps, kRerankWarps * 32, 0, c.stream>>>(r);
+    {
+        KernelTimer kt(TK_KNN_RERANK, c.stream);
+        knn_rerank_kernel<<<(a.Q + kRerankWarps - 1) / kRerankWarps, kRerankWarps * 32, 0, c.stream>>>(r);
+        kt.stop();
+    }
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     int egrid = a.Q < 2 * c.num_sms ? a.Q : 2 * c.num_sms;
     knn_exact_kernel<<<egrid, kExactThreads, 0, c.stream>>>(r);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
-    // introspection (lipfit_knn_fallbacks): copied to pinned host memory, stream-ordered, no sync
-    if (int32_t* h = fallback_word()) {
-        LIPFIT_CUDA(cudaMemcpyAsync(h, stats + 2, sizeof(int32_t), cudaMemcpyDeviceToHost, c.stream));
-        LIPFIT_CUDA(cudaMemcpyAsync(h + 1, stats + 4, sizeof(int32_t), cudaMemcpyDeviceToHost, c.stream));
+    if (info) {  // per-call diagnostics: the caller asked for them, so this call synchronises
+        uint32_t h[8] = {};
+        LIPFIT_CUDA(cudaMemcpyAsync(h, stats, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+        LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+        float ratio;
+        memcpy(&ratio, &h[4], sizeof(ratio));
+        info->fallbacks = static_cast<int64_t>(static_cast<int32_t>(h[2]));
+        info->key_error_ratio = static_cast<double>(ratio);
+        info->tensor_cores = tc ? 1 : 0;
+        info->reserved = 0;
     }
     return LIPFIT_OK;
 }

@@ -14,13 +14,14 @@
 // <= 3 * 2^-16 |q'_j x_j| per coordinate; the fp64 re-rank + certificate of knn.cu
 // turn the selected pools into the exact answer, whatever the key arithmetic was.
 //
-// Kernel (one CTA per SM, 576 threads, warp-specialised):
+// Kernel (one CTA per SM, 608 threads = 19 warps, warp-specialised):
 //   warp 8   TMA producer : 1-D bulk copies of pre-swizzled operand tiles (the pack kernels write the
 //                           global image in the canonical K-major SWIZZLE_128B shared-memory layout,
 //                           so no tensor map is needed) into a 4-stage ring; A (2 x 128 queries) once
 //                           per work item.
-//   warp 9   MMA issuer   : one thread; per B tile 2 x 4 tcgen05.mma (M=128, N=128, K=16) into
-//                           double-buffered TMEM accumulators (2 query halves x 2 stages x 128 columns).
+//   warps 9, 18 MMA issuers: one thread each, one per query half (so a held-up half does not block the
+//                           other): per B tile up to 4 tcgen05.mma (M=128, N=128, K=16) into double-
+//                           buffered TMEM accumulators (2 query halves x 2 stages x 128 columns).
 //   warps 0-7 detectors   : tcgen05.ld 32 columns at a time (thread = query row), min-tree + one compare
 //                           against the query's threshold; every row of a 32 x 32 block that holds a key
 //                           below its threshold goes into a shared-memory ring as one 144-byte message.
@@ -34,30 +35,8 @@
 
 #include "knn_common.cuh"
 
-#ifndef LIPFIT_TC_SLEEP_NS
-#define LIPFIT_TC_SLEEP_NS 40
-#endif
-#ifndef LIPFIT_TC_POLL_NS
-#define LIPFIT_TC_POLL_NS 100  // back-off of the ring-counter polls (shared-memory loads: keep them rare)
-#endif
-#ifndef LIPFIT_TC_EXPERIMENT
-#define LIPFIT_TC_EXPERIMENT 0  // 1, 2: timing experiments with invalid results (never in a product build)
-#endif
-#ifndef LIPFIT_TC_COUNT
-#define LIPFIT_TC_COUNT 0  // 1: CTA 0 prints per-warp event counts and wait cycles (diagnostic builds only)
-#endif
-#if LIPFIT_TC_COUNT
-#include <cstdio>
-#define TC_CLK(x) x
-#else
-#define TC_CLK(x)
-#endif
-#ifndef LIPFIT_TC_LDPAIR
-#define LIPFIT_TC_LDPAIR 0
-#endif
-#ifndef LIPFIT_TC_GROUP_A
-#define LIPFIT_TC_GROUP_A 4  // tiles per seeding minimum (see kTcTilesA)
-#endif
+// back-off of the ring-counter / mbarrier polls (shared-memory loads: keep them rare)
+#define LIPFIT_TC_POLL_NS 100
 
 namespace lipfit {
 
@@ -69,12 +48,9 @@ constexpr int kTcThreads = 608;     // 8 detector warps, TMA warp, MMA warp (hal
 // the 128-bit row stores of different lanes on different banks).  Flow control: a head counter the
 // detector publishes, a tail counter the appender publishes.
 constexpr int kTcRowFloats = 36;
-#ifndef LIPFIT_TC_SLACK
-#define LIPFIT_TC_SLACK 32
-#endif
 // A pool is compacted back to its ksel best entries once it holds ksel + kTcSlack: the sooner, the lower the
 // thresholds the detectors test against (fewer messages) and the more compactions the appenders run.
-constexpr int kTcSlack = LIPFIT_TC_SLACK;
+constexpr int kTcSlack = 32;
 static_assert(kTcSlack + 32 <= kTcPoolExtra, "a row message appends up to 32 entries");
 constexpr int kTcRing = 96;         // row messages in flight between a detector warp and its appender warp
 constexpr int kTcMinimaA = 96;      // seeding minima per query (phase A); they overlay the ring: 32 x 97 floats
@@ -87,7 +63,7 @@ constexpr int kTcStages = 4;
 // (each minimum is the key of a different datum, so at least ksel data lie at or below it).  Without it
 // the first ~1 % of the tiles of an item carry half of its appends and compactions (the thresholds
 // start at +inf), a burst the appenders cannot absorb.
-constexpr int kTcGroupA = LIPFIT_TC_GROUP_A;
+constexpr int kTcGroupA = 4;  // tiles per seeding minimum
 constexpr int kTcTilesA = kTcMinimaA * kTcGroupA;
 constexpr int kTcMinTilesA = 2 * kTcTilesA;  // shorter items are not worth the extra tiles
 constexpr int kTcMaxKselA = 64;              // of 96 minima
@@ -128,11 +104,7 @@ __device__ __forceinline__ void mbar_wait_sleep(uint64_t* bar, uint32_t parity) 
 }
 // release / acquire on a shared-memory word (CTA scope): the flags of the detector <-> appender ring
 __device__ __forceinline__ void st_release_s(volatile void* p, uint32_t v) {
-#ifdef LIPFIT_TC_NOFENCE
-    asm volatile("st.volatile.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(const_cast<void*>(p))), "r"(v) : "memory");
-#else
     asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(const_cast<void*>(p))), "r"(v) : "memory");
-#endif
 }
 __device__ __forceinline__ uint32_t ld_acquire_s(const volatile void* p) {
     uint32_t v;
@@ -446,12 +418,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     const uint64_t bdesc = tc_smem_desc(smem_u32(sB + s * kTcTileBytes));
                     const uint32_t dcol = tmem + (h * 2 + b) * kTcBN;
 #pragma unroll
-#ifndef LIPFIT_TC_KSTEPS
-#define LIPFIT_TC_KSTEPS g.ksteps
-#endif
-#pragma unroll
                     for (int k = 0; k < kTcK / 16; ++k)  // 32 bytes (16 bf16) per K step: +2 in the address field
-                        if (k < LIPFIT_TC_KSTEPS) tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
+                        if (k < g.ksteps) tc_mma(dcol, ad + 2 * k, bdesc + 2 * k, kTcIdesc, k > 0 ? 1u : 0u);
                     tc_commit(&acc_full[h][b]);
                     tc_commit(&b_empty[s]);
                 }
@@ -466,16 +434,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         const int h = warp >> 2, quad = warp & 3;
         float* ring = sR + warp * kTcRingFloats;
         uint32_t gB = 0, head = 0, hslot = 0, tail_seen = 0;
-        TC_CLK(long long c_ring = 0; long long c_acc = 0; long long c_seed = 0; long long c_push = 0;
-               long long n_push = 0; const long long c_start = clock64();)
         // room for n more messages (the appender's tail counter only grows)
         auto reserve = [&](uint32_t n) {
-            TC_CLK(const long long c0 = clock64();)
             while (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) {
                 tail_seen = ld_acquire_s(&tail_s[warp]);
                 if (head + n - tail_seen > static_cast<uint32_t>(kTcRing)) __nanosleep(LIPFIT_TC_POLL_NS);
             }
-            TC_CLK(c_ring += clock64() - c0;)
         };
         auto publish = [&](uint32_t n) {
             head += n;
@@ -488,7 +452,6 @@ knn_tc_select_kernel(const KnnTcArgs g) {
         auto push = [&](const float (&v)[32], unsigned hm, int kbase) {
             const uint32_t n = __popc(hm);
             reserve(n);
-            TC_CLK(const long long c1 = clock64();)
             if ((hm >> lane) & 1u) {
                 uint32_t sl = hslot + __popc(hm & ((1u << lane) - 1u));
                 if (sl >= static_cast<uint32_t>(kTcRing)) sl -= kTcRing;
@@ -498,7 +461,6 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 *reinterpret_cast<int2*>(p + 8) = make_int2(kbase, lane);
             }
             publish(n);
-            TC_CLK(c_push += clock64() - c1; ++n_push;)
         };
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
@@ -507,10 +469,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             float tau = qslot < a.Q ? 1.0e38f : __int_as_float(0xff800000);  // real keys are far below 1e38
             const int nA = tc_tiles_a(tb, te, a.ksel);
             if (nA) {  // phase A: group minima of the first tiles, [row][kTcMinimaA + 1] over the drained ring
-                TC_CLK(const long long c00 = clock64();)
                 while (ld_acquire_s(&tail_s[warp]) != head) __nanosleep(LIPFIT_TC_POLL_NS);
                 tail_seen = head;
-                TC_CLK(c_ring += clock64() - c00;)
                 float gm = __int_as_float(0x7f800000);
                 for (int vt = 0; vt < nA; ++vt, ++gB) {
                     const uint32_t b = gB & 1u, ua = gB >> 1;
@@ -535,14 +495,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 __syncwarp();
                 if (lane == 0) st_release_s(&seed_s[warp], static_cast<uint32_t>(item));
                 // the sweep starts from the appender's seeded threshold (and the ring is free again)
-                TC_CLK(const long long c0 = clock64();)
                 for (;;) {
                     const unsigned long long ts = *reinterpret_cast<volatile unsigned long long*>(&tau_s[warp][lane]);
                     if (static_cast<uint32_t>(ts >> 32) == static_cast<uint32_t>(item)) break;
                     __nanosleep(200);
                 }
                 __syncwarp();
-                TC_CLK(c_seed += clock64() - c0;)
             }
             for (int t = tb; t < te; ++t, ++gB) {
                 const uint32_t b = gB & 1u, ua = gB >> 1;
@@ -551,46 +509,17 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (static_cast<uint32_t>(ts >> 32) == static_cast<uint32_t>(item))
                         tau = fminf(tau, __uint_as_float(static_cast<uint32_t>(ts)));
                 }
-                TC_CLK(const long long c0 = clock64();)
                 mbar_wait_sleep(&acc_full[h][b], ua & 1u);
-                TC_CLK(c_acc += clock64() - c0;)
                 tc_fence_after();
                 const uint32_t trow = tmem + (static_cast<uint32_t>(quad * 32) << 16) + (h * 2 + b) * kTcBN;
                 // Software pipeline over the four 32-column blocks: the TMEM load of block cb+1 is in flight
                 // while block cb is reduced / pushed (two register buffers).
                 auto process = [&](const float (&v)[32], int cb) {
-#if LIPFIT_TC_EXPERIMENT == 1  // timing experiment: accumulators are read and dropped
-                    if (v[0] == 12345.f && v[31] == 1.f) tau = 0.f;
-#elif LIPFIT_TC_EXPERIMENT == 2  // timing experiment: fast path only
-                    const float m = tc_min32(v);
-                    if (__any_sync(0xffffffffu, m < -1e30f)) tau = 0.f;
-#else
                     const float m = tc_min32(v);
                     const unsigned hm = __ballot_sync(0xffffffffu, m < tau);
                     if (hm) push(v, hm, t * kTcBN + cb * 32);
-#endif
                 };
                 float va[32], vb[32];
-#if LIPFIT_TC_EXPERIMENT == 3  // timing experiment: MMA only, accumulators never read
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-                continue;
-#endif
-#if LIPFIT_TC_LDPAIR
-                tc_ld32(trow, va);
-                tc_ld32(trow + 32, vb);
-                tc_ld_wait();
-                process(va, 0);
-                process(vb, 1);
-                tc_ld32(trow + 64, va);
-                tc_ld32(trow + 96, vb);
-                tc_ld_wait();
-                tc_fence_before();  // all four blocks are in registers: hand the TMEM stage back
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-                process(va, 2);
-#else
                 tc_ld32(trow, va);
                 tc_ld_wait();
                 tc_ld32(trow + 32, vb);
@@ -605,7 +534,6 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 tc_fence_before();  // all four blocks are in registers: hand the TMEM stage back
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-#endif
                 process(vb, 3);
             }
             // end of item: the appender writes fill / tau and moves on
@@ -613,17 +541,12 @@ knn_tc_select_kernel(const KnnTcArgs g) {
             if (lane == 0) *reinterpret_cast<int2*>(ring + hslot * kTcRowFloats + 32) = make_int2(-1, 0);
             publish(1);
         }
-        TC_CLK(if (blockIdx.x == 0 && lane == 0)
-                   printf("det %d: total %lld wait_acc %lld wait_ring %lld wait_seed %lld push %lld (%lld) msgs %u\n",
-                          warp, clock64() - c_start, c_acc, c_ring, c_seed, c_push, n_push, head);)
     } else if (warp < 18) {
         // ================= appender warps: own the thresholds and pools of the paired detector's queries ====
         const int aw = warp - 10;  // paired detector warp
         const int h = aw >> 2, quad = aw & 3;
         const float* ring = sR + aw * kTcRingFloats;
         uint32_t tail = 0, tslot = 0, head_seen = 0;
-        TC_CLK(long long c_idle = 0; long long c_comp = 0; long long c_seed = 0; long long n_comp = 0;
-               long long n_hits = 0; const long long c_start = clock64();)
         for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
             int qb, ch, tb, te;
             decode(item, qb, ch, tb, te);
@@ -636,9 +559,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 // phase A: row L's kTcMinimaA group minima sit at ring[L][.], one per lane per 32.  tau = the
                 // next float above the ksel-th smallest, so that at least ksel data pass the strict
                 // `key < tau` test of the sweep.
-                TC_CLK(const long long c00 = clock64();)
                 while (ld_acquire_s(&seed_s[aw]) != static_cast<uint32_t>(item)) __nanosleep(LIPFIT_TC_POLL_NS);
-                TC_CLK(const long long c0 = clock64(); c_idle += c0 - c00;)
                 uint32_t seed = 0;
 #pragma unroll 2
                 for (int L = 0; L < 32; ++L) {
@@ -651,16 +572,13 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     if (lane == L) seed = kth;
                 }
                 __syncwarp();
-                TC_CLK(c_seed += clock64() - c0;)
                 tau = fminf(tau, key2f(seed + 1u));
                 tau_s[aw][lane] = (static_cast<unsigned long long>(static_cast<uint32_t>(item)) << 32) |
                                   __float_as_uint(tau);
             }
             for (;;) {
                 if (head_seen == tail) {
-                    TC_CLK(const long long c0 = clock64();)
                     while ((head_seen = ld_acquire_s(&head_s[aw])) == tail) __nanosleep(LIPFIT_TC_POLL_NS);
-                    TC_CLK(c_idle += clock64() - c0;)
                 }
                 const float* p = ring + tslot * kTcRowFloats;
                 const int2 hd = *reinterpret_cast<const int2*>(p + 32);  // (first datum index, row)
@@ -678,9 +596,7 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 int2* poolL = pool + static_cast<ptrdiff_t>(L - lane) * a.P;  // consecutive lanes = consecutive slots
                 if (fillL >= a.ksel + kTcSlack) {  // compact (warp-cooperative radix select): lowers tau
                     __syncwarp();
-                    TC_CLK(const long long c1 = clock64();)
                     tauL = knn_compact(poolL, fillL, a.ksel, nullptr, lane);
-                    TC_CLK(c_comp += clock64() - c1; ++n_comp;)
                     fillL = a.ksel;
                     if (lane == L) tau = tauL;
                     // publish the lowered threshold for the detector
@@ -692,18 +608,10 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 if (hit) poolL[fillL + __popc(bm & ((1u << lane) - 1u))] = make_int2(__float_as_int(val), hd.x + lane);
                 if (lane == L) fill = fillL + __popc(bm);
                 if (lane == 0) st_release_s(&tail_s[aw], tail);  // every lane's read of the message fed the ballot above
-                TC_CLK(n_hits += __popc(bm);)
             }
-#if LIPFIT_TC_EXPERIMENT
-            fill = 0;
-            tau = __int_as_float(0x7f800000);
-#endif
             a.fill[slot] = fill;
             a.tau[slot] = tau;
         }
-        TC_CLK(if (blockIdx.x == 0 && lane == 0) printf(
-                   "app %d: total %lld idle %lld compact %lld (%lld) seed %lld hits %lld msgs %u\n", aw,
-                   clock64() - c_start, c_idle, c_comp, n_comp, c_seed, n_hits, tail);)
     }
     tc_fence_before();
     __syncthreads();

@@ -67,20 +67,51 @@ int make_ctx(void* cuda_stream, Ctx* ctx) {
     int sms = (dev >= 0 && dev < 64) ? sm_cache[dev].load() : 0;
     if (sms == 0) {  // first call on this device
         LIPFIT_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-        // Workspaces come from the device's default stream-ordered pool (common.cuh: Workspace).  Its
-        // default release threshold is 0: every synchronisation hands the freed workspaces back to
-        // the driver and the next call pays for mapping them again (tens of ms for the 0.5 GB of
-        // kNN pools).  Keep them cached in the pool instead.
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long keep = ~0ull;
-            (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-        (void)cudaGetLastError();
         if (dev >= 0 && dev < 64) sm_cache[dev].store(sms);
     }
     ctx->device = dev;
     ctx->num_sms = sms;
+    return LIPFIT_OK;
+}
+
+// Workspaces come from a pool of the library's own (common.cuh: Workspace).  A pool's default release
+// threshold is 0: every synchronisation would hand the freed workspaces back to the driver and the next
+// call would pay for mapping them again (0.2-0.6 ms on the 25 us config 1 step, tens of ms for the 0.5 GB
+// of kNN pools), so this pool keeps them until lipfit_release_workspace().
+namespace {
+std::mutex g_pool_mu;
+cudaMemPool_t g_pools[64] = {};
+}  // namespace
+
+cudaError_t workspace_pool(cudaMemPool_t* pool) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p = nullptr;
+        e = cudaMemPoolCreate(&p, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ull;
+        (void)cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_pools[dev] = p;
+    }
+    *pool = g_pools[dev];
+    return cudaSuccess;
+}
+
+int workspace_release() {
+    int dev = 0;
+    LIPFIT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return LIPFIT_E_CUDA;
+    std::lock_guard<std::mutex> lk(g_pool_mu);
+    if (g_pools[dev]) LIPFIT_CUDA(cudaMemPoolTrimTo(g_pools[dev], 0));
     return LIPFIT_OK;
 }
 
@@ -168,17 +199,22 @@ FreeFlags make_free_flags(const Xform& xf) {
 __global__ void __launch_bounds__(256)
 prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
                const float* __restrict__ eps, int N, Xform xf, int rf, int vslot, int cslot,
-               float* __restrict__ rec) {
+               const float* __restrict__ centre, float* __restrict__ rec) {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     const float* src = X + static_cast<size_t>(k) * xf.d;
     float* dst = rec + static_cast<size_t>(k) * rf;
     float v = y ? y[k] : 0.f;
     if (eps) v += eps[k];
+    // packed coordinate j = sw_j (x_perm(j) - centre_perm(j)); centre == NULL: no translation
+    auto coord = [&](int j) {
+        const int o = xf.perm[j];
+        return xf.sw[j] * (centre ? src[o] - __ldg(centre + o) : src[o]);
+    };
     float cval = 0.f;
     if (cslot >= 0) {  // c' = 2 y - sum of the constrained (packed) coordinates, see bounds.cu FoldL1Core
         float sc = 0.f;
-        for (int j = xf.dU; j < xf.d; ++j) sc += xf.sw[j] * src[xf.perm[j]];
+        for (int j = xf.dU; j < xf.d; ++j) sc += coord(j);
         cval = 2.f * v - sc;
     }
     for (int j0 = 0; j0 < rf; j0 += 4) {
@@ -186,7 +222,7 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             int j = j0 + c;
-            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : (j == cslot ? cval : 0.f));
+            t[c] = (j < xf.d) ? coord(j) : (j == vslot ? v : (j == cslot ? cval : 0.f));
         }
         *reinterpret_cast<float4*>(dst + j0) = make_float4(t[0], t[1], t[2], t[3]);
     }
@@ -196,16 +232,20 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
 // floats, each stored twice, so that an LDS.128 yields two (x, x) register pairs ready for FADD2.
 __global__ void __launch_bounds__(256)
 prepack_dup_kernel(const float* __restrict__ X, const float* __restrict__ y, int N, Xform xf, int rf, int vslot,
-                   int cslot, float* __restrict__ rec) {
+                   int cslot, const float* __restrict__ centre, float* __restrict__ rec) {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     const float* src = X + static_cast<size_t>(k) * xf.d;
     float* dst = rec + static_cast<size_t>(k) * rf;
     const float v = y ? y[k] : 0.f;
+    auto coord = [&](int j) {
+        const int o = xf.perm[j];
+        return xf.sw[j] * (centre ? src[o] - __ldg(centre + o) : src[o]);
+    };
     float cval = 0.f;
     if (cslot >= 0) {
         float sc = 0.f;
-        for (int j = xf.dU; j < xf.d; ++j) sc += xf.sw[j] * src[xf.perm[j]];
+        for (int j = xf.dU; j < xf.d; ++j) sc += coord(j);
         cval = 2.f * v - sc;
     }
     for (int j0 = 0; j0 < rf / 2; j0 += 2) {
@@ -213,7 +253,7 @@ prepack_dup_kernel(const float* __restrict__ X, const float* __restrict__ y, int
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             int j = j0 + c;
-            t[c] = (j < xf.d) ? xf.sw[j] * src[xf.perm[j]] : (j == vslot ? v : (j == cslot ? cval : 0.f));
+            t[c] = (j < xf.d) ? coord(j) : (j == vslot ? v : (j == cslot ? cval : 0.f));
         }
         *reinterpret_cast<float4*>(dst + 2 * j0) = make_float4(t[0], t[0], t[1], t[1]);
     }
@@ -234,15 +274,17 @@ axpy_kernel(float* __restrict__ y, const float* __restrict__ eps, int N) {
 }
 
 int launch_prepack(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
-                   const Xform& xf, RecLayout lay, float* rec) {
+                   const Xform& xf, RecLayout lay, float* rec, const float* centre) {
     int n = static_cast<int>(N);
     if (lay.dup) {
-        prepack_dup_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, n, xf, lay.rf, lay.vslot, lay.cslot, rec);
+        prepack_dup_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, n, xf, lay.rf, lay.vslot, lay.cslot, centre,
+                                                                  rec);
         ++g_launches;
         LIPFIT_CUDA(cudaGetLastError());
         return LIPFIT_OK;
     }
-    prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, lay.cslot, rec);
+    prepack_kernel<<<(n + 255) / 256, 256, 0, c.stream>>>(X, y, eps, n, xf, lay.rf, lay.vslot, lay.cslot, centre,
+                                                          rec);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     return LIPFIT_OK;

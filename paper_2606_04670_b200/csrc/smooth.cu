@@ -12,8 +12,10 @@
 //       only V_ik can be non-zero: one one-sided distance per pair, no sign select;
 //   (3) pre-filters on the squared quantity (L2: sum (M u_j)^2 < (z_i - z_k)^2, no square root); the
 //       rare surviving pairs (~1e-5 of all) take a slow path that forms V, adds V^2 to F, +V to row i
-//       and -V to row k.  Gradient sums are kept in 2^-40 fixed point (64-bit integer atomics): exact,
-//       hence independent of the order of the atomics -- an evaluation is bit-reproducible.
+//       and -V to row k.  Gradient sums are kept in fixed point (64-bit integer atomics): exact, hence
+//       independent of the order of the atomics -- an evaluation is bit-reproducible.  The scale is
+//       2^e, e = min(40, 62 - ceil(log2(N (z_max - z_min)))), chosen per evaluation from the sorted z:
+//       every V is <= z_max - z_min, so no row sum can reach 2^62 whatever the magnitude of the data.
 // Kernel shape as in bounds.cu: R rows per thread in registers, data tiles through shared memory via
 // the TMA engine (decoupled 4-stage pipe); work items (row block, data chunk) of the lower triangle
 // are handed out by an atomic counter.
@@ -31,11 +33,12 @@ constexpr int kSmThreads = 128;
 constexpr int kSmWarps = kSmThreads / 32;
 constexpr int kSmStages = 4;
 constexpr int kSmChunk = 4096;  // data records per work item (multiple of every tile size)
-constexpr double kFix = 1099511627776.0;  // 2^40
+constexpr int kFixMaxExp = 40;  // finest fixed-point scale of the gradient sums (2^-40)
 
 struct SmoothArgs {
     const float* rec;         // sorted records [N][RF]
-    unsigned long long* gfix; // [N] sum_k (V_ik - V_ki) of sorted position i, 2^-40 fixed point
+    unsigned long long* gfix; // [N] sum_k (V_ik - V_ki) of sorted position i, fixed point with scale fix[0]
+    const double* fix;        // [2] fixed-point scale 2^e and its inverse (written by the gather kernel)
     double* fpart;            // [nitems] sum of V^2 over the item
     float* vpart;             // [nitems] max V over the item
     int* counter;             // work counter
@@ -78,6 +81,7 @@ __device__ __forceinline__ void smooth_hit(const SmoothArgs& a, const float (&ac
                                            const bool (&pass)[R], int kpos, long long (&grow)[R],
                                            double& fd, float& vmax) {
     long long col = 0;
+    const double kFix = __ldg(a.fix);
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         if (pass[r]) {
@@ -477,9 +481,20 @@ smooth_z_kernel(const float* __restrict__ y, const float* __restrict__ eps, int 
 __global__ void __launch_bounds__(256)
 smooth_gather_kernel(const float* __restrict__ base, const int32_t* __restrict__ perm,
                      const float* __restrict__ zs, int N, int rf, int vslot, float* __restrict__ rec,
-                     unsigned long long* __restrict__ gfix, uint32_t* __restrict__ amax, int dup) {
+                     unsigned long long* __restrict__ gfix, uint32_t* __restrict__ amax, int dup,
+                     double* __restrict__ fix) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
+    if (j == 0 && fix) {
+        // fixed-point scale of this evaluation's gradient sums: |sum_k V| <= (N-1) (z_max - z_min) < 2^ex
+        const double r = static_cast<double>(N) * (static_cast<double>(zs[N - 1]) - static_cast<double>(zs[0]));
+        int ex = 0;
+        if (r > 0.0 && r < 1.0e300) (void)frexp(r, &ex);
+        int e = 62 - ex;
+        if (e > kFixMaxExp) e = kFixMaxExp;
+        fix[0] = ldexp(1.0, e);
+        fix[1] = ldexp(1.0, -e);
+    }
     if (dup) {  // duplicated layout (x, x) for the packed kernel: 2 rf floats per record
         const float* src = base + static_cast<size_t>(perm[j]) * rf;
         float4* dst = reinterpret_cast<float4*>(rec + static_cast<size_t>(j) * 2 * rf);
@@ -512,9 +527,10 @@ __global__ void lipconst_final_kernel(const unsigned long long* __restrict__ lma
     *L = static_cast<float>(__longlong_as_double(static_cast<long long>(*lmax)));
 }
 
-// grad[perm[j]] = 2 eps / p + 4 * gfix[j] * 2^-40; per-block partial of sum eps^2.
+// grad[perm[j]] = 2 eps / p + 4 * gfix[j] / scale; per-block partial of sum eps^2.
 __global__ void __launch_bounds__(256)
-smooth_grad_kernel(const unsigned long long* __restrict__ gfix, const int32_t* __restrict__ perm, int N,
+smooth_grad_kernel(const unsigned long long* __restrict__ gfix, const double* __restrict__ fix,
+                   const int32_t* __restrict__ perm, int N,
                    const float* __restrict__ eps, float p, float* __restrict__ grad,
                    double* __restrict__ e2part) {
     __shared__ double red[8];
@@ -522,7 +538,7 @@ smooth_grad_kernel(const unsigned long long* __restrict__ gfix, const int32_t* _
     double e = 0.0;
     if (j < N) {
         const int i = perm[j];
-        const double s = static_cast<double>(static_cast<long long>(gfix[j])) / kFix;
+        const double s = static_cast<double>(static_cast<long long>(gfix[j])) * fix[1];
         e = eps ? static_cast<double>(eps[i]) : 0.0;
         if (grad) grad[i] = static_cast<float>(2.0 * e / static_cast<double>(p) + 4.0 * s);
     }
@@ -666,8 +682,9 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
                                                 static_cast<float*>(nullptr),
                                                 static_cast<const int32_t*>(nullptr),
                                                 static_cast<int32_t*>(nullptr), N, 0, 32, c.stream));
-    Workspace wz, wzs, wi, wperm, wsort, wrec, wg, wf, wv, we, wc;
+    Workspace wz, wzs, wi, wperm, wsort, wrec, wg, wf, wv, we, wc, wfix;
     int rc;
+    if ((rc = wfix.alloc(sizeof(double) * 2, c.stream))) return rc;
     if ((rc = wz.alloc(sizeof(float) * n, c.stream))) return rc;
     if ((rc = wzs.alloc(sizeof(float) * n, c.stream))) return rc;
     if ((rc = wi.alloc(sizeof(int32_t) * n, c.stream))) return rc;
@@ -689,7 +706,8 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
                                                 c.stream));
     smooth_gather_kernel<<<nblk, 256, 0, c.stream>>>(base, wperm.as<int32_t>(), wzs.as<float>(), N, lay.rf,
                                                      lay.vslot, wrec.as<float>(),
-                                                     wg.as<unsigned long long>(), nullptr, packed ? 1 : 0);
+                                                     wg.as<unsigned long long>(), nullptr, packed ? 1 : 0,
+                                                     wfix.as<double>());
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     LIPFIT_CUDA(cudaMemsetAsync(wc.p, 0, sizeof(int), c.stream));
@@ -697,6 +715,7 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
     // ---- (2),(3) lower-triangle pairs ----
     a.rec = wrec.as<float>();
     a.gfix = wg.as<unsigned long long>();
+    a.fix = wfix.as<double>();
     a.fpart = wf.as<double>();
     a.vpart = wv.as<float>();
     a.counter = wc.as<int>();
@@ -718,7 +737,7 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
     }
     if (rc) return rc;
 
-    smooth_grad_kernel<<<nblk, 256, 0, c.stream>>>(a.gfix, wperm.as<int32_t>(), N, eps, p, grad,
+    smooth_grad_kernel<<<nblk, 256, 0, c.stream>>>(a.gfix, a.fix, wperm.as<int32_t>(), N, eps, p, grad,
                                                    we.as<double>());
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
@@ -774,7 +793,8 @@ int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, c
     smooth_gather_kernel<<<nblk, 256, 0, c.stream>>>(base, wperm.as<int32_t>(), wzs.as<float>(), N, lay.rf,
                                                      lay.vslot, wrec.as<float>(),
                                                      wg.as<unsigned long long>(),
-                                                     reinterpret_cast<uint32_t*>(wl.as<unsigned long long>() + 1), 0);
+                                                     reinterpret_cast<uint32_t*>(wl.as<unsigned long long>() + 1), 0,
+                                                     nullptr);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     LIPFIT_CUDA(cudaMemsetAsync(wc.p, 0, sizeof(int), c.stream));

@@ -24,15 +24,19 @@ def _gpu_bounds(X, y, Xq, M, mask, norm, w=None, want=("upper", "lower", "g")):
     return f(up), f(lo), f(g)
 
 
-def _check(X, y, Xq, M, mask, norm, w=None, tol_scale=1.0):
+def _check(X, y, Xq, M, mask, norm, w=None, stated=False):
+    """stated=True (config-shaped inputs, inputs.make_workload): the bar is north_star's
+    1e-5 * (max y - min y) and nothing else.  stated=False (inputs.random_problem: unstructured normal
+    data whose M*D can dwarf the range of y): the fp32 rounding of the winning candidate y + M*D itself,
+    (d+4) * 2^-24 * max|H|, is added (DESIGN.md §6 derives it and names the tests that use it)."""
     U, L_, g = oracle.bounds(X, y, Xq, M, mask, norm, w)
     up, lo, gg = _gpu_bounds(X, y, Xq, M, mask, norm, w)
     rng = float(np.max(y) - np.min(y)) if len(y) > 1 else 1.0
     rng = max(rng, 1e-30)
-    # 1e-5 * range is the stated bar; for M*D far above the data range the fp32 rounding of the
-    # candidate y + M*D itself (2^-24 relative) is added.
-    mag = np.maximum(np.abs(U), np.abs(L_)).max() if len(U) else 0.0
-    tol = tol_scale * (1e-5 * rng + (np.shape(X)[1] + 4) * 2.0 ** -24 * mag)
+    tol = 1e-5 * rng
+    if not stated:
+        mag = np.maximum(np.abs(U), np.abs(L_)).max() if len(U) else 0.0
+        tol += (np.shape(X)[1] + 4) * 2.0 ** -24 * mag
     assert np.abs(up - U).max(initial=0) <= tol, (np.abs(up - U).max(), tol)
     assert np.abs(lo - L_).max(initial=0) <= tol, (np.abs(lo - L_).max(), tol)
     assert np.abs(gg - g).max(initial=0) <= tol
@@ -41,7 +45,7 @@ def _check(X, y, Xq, M, mask, norm, w=None, tol_scale=1.0):
 
 def test_config1_full():
     wl = make_workload(1)
-    up, lo, g = _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm)
+    up, lo, g = _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, stated=True)
     assert np.all(lo <= up + 1e-5 * wl.y_range)            # consistent data: sandwich (P2)
     # interpolation (P1) within the fp32 tolerance
     up, lo, g = _gpu_bounds(wl.X, wl.y, wl.X, wl.M, wl.mask, wl.norm)
@@ -53,7 +57,20 @@ def test_config1_full():
 def test_configs_scaled(cfg, N, Q):
     # sizes span several shared-memory tiles, a ragged tail, the direct and the chunked (atomic) paths
     wl = make_workload(cfg, N=N, Q=Q)
-    _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights, stated=True)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+@pytest.mark.parametrize("offset", [1.0e3, -2.5e2])
+def test_configs_far_from_the_origin(cfg, offset):
+    """The kernel families that fold M into the coordinates (configs 2, 3, 5) translate data and queries to
+    the first datum before scaling (csrc/prepack.cu), so the stated bar also holds for data that sit far
+    from the origin: the same workload shifted by `offset` in every coordinate."""
+    for N, Q in ((6000, 3000), (700, 310000)):      # one query per thread / the packed-f32x2 throughput kernels
+        wl = make_workload(cfg, N=N, Q=Q)
+        X = (wl.X.astype(np.float64) + offset).astype(np.float32)
+        Xq = (wl.Xq.astype(np.float64) + offset).astype(np.float32)
+        _check(X, wl.y, Xq, wl.M, wl.mask, wl.norm, wl.weights, stated=True)
 
 
 @pytest.mark.parametrize("norm", NORMS)
@@ -69,12 +86,16 @@ def test_generic_and_specialised_shapes(norm, d, mask):
 
 @pytest.mark.parametrize("Q", [1, 31, 127, 128, 129, 1025])
 def test_ragged_query_counts(Q):
+    wl = make_workload(2, N=1000, Q=Q)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights, stated=True)
     X, y, Xq = random_problem(7, 1000, Q, 4)
     _check(X, y, Xq, 2.0, [1, 1, 0, 0], L1)
 
 
 @pytest.mark.parametrize("N", [1, 2, 511, 512, 513, 1027])
 def test_ragged_data_counts(N):
+    wl = make_workload(1, N=N, Q=300)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wl.mask, wl.norm, wl.weights, stated=True)
     X, y, Xq = random_problem(8, N, 300, 2)
     _check(X, y, Xq, 4.0, [0, 0], L2)
 

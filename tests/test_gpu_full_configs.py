@@ -52,9 +52,9 @@ def test_config4_full():
     import torch
     import paper_2606_04670_b200 as L
     wl = make_workload(4)
-    idx, dist = L.lipfit_knn(_dev(wl.X), _dev(wl.Xq), wl.k, None, 0, wl.norm)
-    torch.cuda.synchronize()
-    assert L.knn_fallbacks() <= wl.Q // 1000                  # the certificate holds almost everywhere
+    idx, dist, info = L.lipfit_knn_ex(_dev(wl.X), _dev(wl.Xq), wl.k, None, 0, wl.norm)
+    assert info["fallbacks"] <= wl.Q // 1000                  # the certificate holds almost everywhere
+    assert info["key_error_ratio"] <= 1.0 and info["tensor_cores"]
     idx, dist = idx.cpu().numpy(), dist.cpu().numpy()
     sel = oracle_subset(wl.Q, 48)
     oi, od = oracle.knn(wl.X, wl.Xq[sel], wl.k, None, 0, wl.norm)

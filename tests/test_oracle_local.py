@@ -124,3 +124,18 @@ def test_duplicates_and_degenerate_inputs():
     assert np.all(np.isinf(T[2]) == False) and T[2, 1] == pytest.approx(2.0)
     U, L, G = oracle.values_local(X, y, X[2:3], np.array([0.5, 2.0]), T, L2)
     assert U[0] == 3.0 and L[0] == 3.0                              # inf * 0 := 0 at the datum itself
+
+
+def test_rows_variant_equals_the_full_table():
+    """oracle.local_lipschitz_rows (full-size parity samples) is the same loop over a list of data: its rows
+    equal the rows of the whole table bit for bit, which the brute-force pin above fixes."""
+    X, y, _ = _problem(91, 700, 1, 4)
+    w = np.array([1.0, 0.5, 2.0, 1.0], np.float32)
+    pi, pk = sample_pairs(5, 700, 5000)
+    for norm in NORMS:
+        knots = oracle.distance_quantiles(X, pi, pk, 16, norm, w)
+        full = oracle.local_lipschitz(X, y, knots, norm, w)
+        rows = np.array([0, 699, 13, 13, 350], np.int64)
+        np.testing.assert_array_equal(oracle.local_lipschitz_rows(X, y, knots, rows, norm, w), full[rows])
+    with pytest.raises(ValueError):
+        oracle.local_lipschitz_rows(X, y, knots, [700], L2, w)
