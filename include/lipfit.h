@@ -78,7 +78,8 @@ enum lipfit_status {
  * Q = 0 returns LIPFIT_OK and writes nothing.  M = 0 is allowed.  Inconsistent data
  * (lower > upper somewhere) are not an error.
  * Steps on the device: a1 prepack (permute / mirror / weight the coordinates, build records)
- * then a2 fused distance + running min/max; the Q x N distance matrix is never formed. */
+ * then a2 fused distance + running min/max; the Q x N distance matrix is never formed.
+ * Evaluation policy LIPFIT_BOUNDS_AUTO (see lipfit_bounds_ex). */
 int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d,
                   const float* Xq, int64_t Q, float M,
                   const int32_t* mono_mask /* host[d] or NULL */, int32_t norm,
@@ -91,6 +92,51 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d,
                        const float* Xq, int64_t Q, float M,
                        const int32_t* mono_mask, int32_t norm, const float* weights,
                        float* upper, float* lower, float* g, void* cuda_stream);
+
+/* ---- Evaluation policy of Eq.(2),(3) -------------------------------------------------------------
+ * The result of lipfit_bounds is always the minimum / maximum over ALL N data (within the fp32 tolerance
+ * of DESIGN.md section 6, whichever pass computes it); the policy only chooses how many pairs are visited:
+ *   LIPFIT_BOUNDS_BRUTE   every (query, datum) pair, the fused all-pairs kernels (step a2): N Q pair
+ *                         evaluations "proportional to N" per query as in PAPER.md:130.
+ *   LIPFIT_BOUNDS_PRUNED  exact spatial pruning (NEXT-4(ii), see lipfit_bounds_pruned below).
+ *   LIPFIT_BOUNDS_AUTO    what lipfit_bounds / lipfit_bounds_host do: PRUNED when d <= 8, N >= 8192,
+ *                         Q >= 4096 and N Q >= 2^32 (few enough coordinates for bounding boxes to separate,
+ *                         enough pairs to pay for two radix sorts: 9.7x / 5.3x / 2.0x on the config 2 / 5 / 3
+ *                         workloads), BRUTE otherwise.  Pruning cannot help when M D is small against the
+ *                         spread of y everywhere (M = 0 in the limit): PRUNED then visits every pair at about
+ *                         half the all-pairs rate; callers who know that pass LIPFIT_BOUNDS_BRUTE.
+ * pairs_evaluated: HOST int64[3] or NULL, as in lipfit_bounds_pruned ([0] = N Q under BRUTE); non-NULL
+ * synchronises the stream.  Unknown policy: LIPFIT_E_PARAM. */
+enum lipfit_bounds_policy { LIPFIT_BOUNDS_AUTO = 0, LIPFIT_BOUNDS_BRUTE = 1, LIPFIT_BOUNDS_PRUNED = 2 };
+int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q, float M,
+                     const int32_t* mono_mask, int32_t norm, const float* weights,
+                     float* upper, float* lower, float* g, int32_t policy,
+                     int64_t* pairs_evaluated /* host[3] or NULL */, void* cuda_stream);
+int lipfit_bounds_host_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                          float M, const int32_t* mono_mask, int32_t norm, const float* weights,
+                          float* upper, float* lower, float* g, int32_t policy,
+                          int64_t* pairs_evaluated /* host[3] or NULL */, void* cuda_stream);
+
+/* ---- NEXT-4(iii): Eq.(2),(3) under monotonicity on PARTS of the domain (section 4.2) ----
+ * "Partition the domain with respect to each variable i into the intervals A: x_i <= a_i, AB: a_i <= x_i <= b_i,
+ * B: x_i >= b_i" and "Case I: f increasing on A, B, unrestricted on AB.  Case II: f decreasing on A, B ...
+ * Case III: f decreasing on A, increasing on B ...  Case IV: f increasing on A, decreasing on B";
+ * the package passes `mon in {0,1,2,3,4}^dim` and `a, b in R^dim`.  The paper does not print the
+ * modified bounds ("can be expressed through components of the distance vector"); reading R26
+ * of DESIGN.md derives them: walking coordinate i from the datum x^k_i to the query x_i,
+ *   u_i = w_i (length of the way in AB + length in A / in B where f may GROW in the direction of travel)
+ *   l_i = w_i (length of the way in AB + length in A / in B where f may FALL in the direction of travel)
+ * ("may grow" = travelling up through an increasing region or down through a decreasing one), and
+ *   upper[q] = min_k (y[k] + M ||u||_p),  lower[q] = max_k (y[k] - M ||l||_p),  g = (upper + lower) / 2.
+ * mon: HOST int32[d] or NULL (= all 0), 0 = unrestricted, 1..4 = case I..IV.  a, b: HOST float[d], required
+ * when some mon[i] != 0, a[i] <= b[i]; a[i] = -inf (no region A) and b[i] = +inf (no region B) are allowed;
+ * entries of coordinates with mon[i] = 0 are ignored.  a = b with case I / II is lipfit_bounds with mask
+ * +1 / -1 (Eq.(4)).  Every pair is visited (no pruning).  Other arguments, layout, ownership, error
+ * behaviour and asynchrony as lipfit_bounds; bad mon / a > b / NaN: LIPFIT_E_PARAM. */
+int lipfit_bounds_region(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         float M, const int32_t* mon /* host[d] or NULL */, const float* a /* host[d] */,
+                         const float* b /* host[d] */, int32_t norm, const float* weights /* host[d] or NULL */,
+                         float* upper, float* lower, float* g, void* cuda_stream);
 
 /* ---- Approximation with k > 1 neighbours ("Extra features" 2) -------
  *   upper[q] = sum_j wk[j] * (j-th smallest of y[k] + M D^u(q,k)),
@@ -113,6 +159,7 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
  * no datum of the tile can change a minimum of Eq.(2) or a maximum of Eq.(3).  The result is the
  * min / max over ALL N data of the per-pair fp32 arithmetic; only the number of pairs evaluated
  * changes (by orders of magnitude for low d, not at all in the worst case).
+ * Equivalent to lipfit_bounds_ex(..., LIPFIT_BOUNDS_PRUNED, pairs_evaluated, stream).
  * Arguments, layout, ownership and error behaviour as lipfit_bounds.  pairs_evaluated: HOST int64[3]
  * or NULL; when non-NULL the call synchronises the stream and stores [0] the number of (query, datum)
  * pairs whose distance was actually computed (Q N for the unpruned path), [1] the number of

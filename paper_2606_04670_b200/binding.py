@@ -25,7 +25,9 @@ EXPORTS = [
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host", "lipfit_knn_variant",
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
     "lipfit_bounds_pruned", "lipfit_smooth_objective_pruned",
+    "lipfit_bounds_ex", "lipfit_bounds_host_ex", "lipfit_bounds_region",
 ]
+LIPFIT_BOUNDS_AUTO, LIPFIT_BOUNDS_BRUTE, LIPFIT_BOUNDS_PRUNED = 0, 1, 2
 LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
 LIPFIT_KNN_NO_TENSOR_CORES = 1
@@ -35,7 +37,8 @@ __all__ = [n for n in EXPORTS if n not in ("lipfit_status_string", "lipfit_versi
                                            "lipfit_bounds_variant", "lipfit_set_timing", "lipfit_get_timing",
                                            "lipfit_knn_variant", "lipfit_release_workspace")] + [
     "LIPFIT_L1", "LIPFIT_L2", "LIPFIT_LINF", "LIPFIT_MAX_DIM", "LIPFIT_MAX_K", "LIPFIT_MAX_TOPK",
-    "LIPFIT_LOCAL_KNOTS", "LIPFIT_KNN_NO_TENSOR_CORES"]
+    "LIPFIT_LOCAL_KNOTS", "LIPFIT_KNN_NO_TENSOR_CORES", "LIPFIT_BOUNDS_AUTO", "LIPFIT_BOUNDS_BRUTE",
+    "LIPFIT_BOUNDS_PRUNED"]
 
 
 class LipfitError(RuntimeError):
@@ -78,6 +81,9 @@ def load():
     P, i64, i32, f32, f64 = C.c_void_p, C.c_int64, C.c_int32, C.c_float, C.c_double
     lib.lipfit_bounds.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, P, P, P, P]
     lib.lipfit_bounds_host.argtypes = lib.lipfit_bounds.argtypes
+    lib.lipfit_bounds_ex.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, P, P, P, i32, P, P]
+    lib.lipfit_bounds_host_ex.argtypes = lib.lipfit_bounds_ex.argtypes
+    lib.lipfit_bounds_region.argtypes = [P, P, i64, i32, P, i64, f32, P, P, P, i32, P, P, P, P, P]
     lib.lipfit_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, P]
     lib.lipfit_knn_host.argtypes = lib.lipfit_knn.argtypes
     lib.lipfit_knn_ex.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, i32, P, P]
@@ -189,6 +195,46 @@ def _stream(stream):
     torch = _torch()
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def lipfit_bounds_ex(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                     policy: int = LIPFIT_BOUNDS_AUTO, count_pairs: bool = False, stream=None):
+    """(upper, lower, g[, pairs_evaluated list of 3]) through lipfit_bounds_ex with an explicit evaluation
+    policy (LIPFIT_BOUNDS_AUTO / BRUTE / PRUNED); count_pairs=True synchronises."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    if Xq.shape[1] != d or y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    m, w = _host_params(d, mono_mask, weights)
+    outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    n = (C.c_int64 * 3)()
+    rc = load().lipfit_bounds_ex(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(m),
+                                 int(norm), _np_ptr(w), outs[0].data_ptr(), outs[1].data_ptr(),
+                                 outs[2].data_ptr(), int(policy), n if count_pairs else None, _stream(stream))
+    _check(rc, "lipfit_bounds_ex")
+    return (*outs, [int(v) for v in n]) if count_pairs else tuple(outs)
+
+
+def lipfit_bounds_region(X, y, Xq, M: float, mon, a, b, norm: int = LIPFIT_L2, weights=None, stream=None):
+    """(upper, lower, g) under monotonicity on parts of the domain: mon in {0..4}^d
+    (0 unrestricted, 1..4 = case I..IV), thresholds a <= b per coordinate (host arrays)."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    if Xq.shape[1] != d or y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    mon_h, w = _host_params(d, mon, weights)
+    a_h = None if a is None else np.ascontiguousarray(a, dtype=np.float32).reshape(d)
+    b_h = None if b is None else np.ascontiguousarray(b, dtype=np.float32).reshape(d)
+    outs = [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    rc = load().lipfit_bounds_region(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(mon_h),
+                                     _np_ptr(a_h), _np_ptr(b_h), int(norm), _np_ptr(w), outs[0].data_ptr(),
+                                     outs[1].data_ptr(), outs[2].data_ptr(), _stream(stream))
+    _check(rc, "lipfit_bounds_region")
+    return tuple(outs)
 
 
 def lipfit_bounds(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
@@ -430,14 +476,25 @@ def lipfit_bounds_host(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2
                        out=None, stream_ptr: Optional[int] = None):
     """numpy in / numpy out through lipfit_bounds_host.  `out` may be a preallocated (e.g. pinned)
     tuple of three float32 arrays of length Q."""
+    return lipfit_bounds_host_ex(X, y, Xq, M, mono_mask, norm, weights, out, stream_ptr, None)
+
+
+def lipfit_bounds_host_ex(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None,
+                          out=None, stream_ptr: Optional[int] = None, policy: Optional[int] = LIPFIT_BOUNDS_AUTO):
+    """As lipfit_bounds_host with an explicit evaluation policy (policy=None: the plain entry point)."""
     X, y, Xq = _host_f32(X, 2), _host_f32(y, 1), _host_f32(Xq, 2)
     N, d = X.shape
     Q = Xq.shape[0]
     m, w = _host_params(d, mono_mask, weights)
     up, lo, g = out if out is not None else (np.empty(Q, np.float32) for _ in range(3))
-    rc = load().lipfit_bounds_host(_np_ptr(X), _np_ptr(y), N, d, _np_ptr(Xq), Q, float(M), _np_ptr(m),
-                                   int(norm), _np_ptr(w), _np_ptr(up), _np_ptr(lo), _np_ptr(g),
-                                   C.c_void_p(stream_ptr or 0))
+    if policy is None:
+        rc = load().lipfit_bounds_host(_np_ptr(X), _np_ptr(y), N, d, _np_ptr(Xq), Q, float(M), _np_ptr(m),
+                                       int(norm), _np_ptr(w), _np_ptr(up), _np_ptr(lo), _np_ptr(g),
+                                       C.c_void_p(stream_ptr or 0))
+    else:
+        rc = load().lipfit_bounds_host_ex(_np_ptr(X), _np_ptr(y), N, d, _np_ptr(Xq), Q, float(M), _np_ptr(m),
+                                          int(norm), _np_ptr(w), _np_ptr(up), _np_ptr(lo), _np_ptr(g),
+                                          int(policy), None, C.c_void_p(stream_ptr or 0))
     _check(rc, "lipfit_bounds_host")
     return up, lo, g
 

@@ -85,41 +85,16 @@ int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, int32_t flags, cha
     return LIPFIT_OK;
 }
 
-int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
-                  float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
-                  float* lower, float* g, void* cuda_stream) {
+// lipfit_bounds_ex: Eq.(2),(3) with an explicit evaluation policy (include/lipfit.h).
+int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q, float M,
+                     const int32_t* mono_mask, int32_t norm, const float* weights, float* upper, float* lower,
+                     float* g, int32_t policy, int64_t* pairs_evaluated, void* cuda_stream) {
     NvtxRange nvtx_range("lipfit_bounds");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
-    Xform xf;
-    rc = make_xform(d, mono_mask, weights, false, false, &xf);
-    if (rc) return rc;
-    if (!X || !y) return LIPFIT_E_NULL;
-    if (Q == 0) return LIPFIT_OK;
-    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
-    Ctx c;
-    rc = make_ctx(cuda_stream, &c);
-    if (rc) return rc;
-    RecLayout lay = bounds_layout(c, xf, norm, Q);
-    if (lay.rf == 0) return LIPFIT_E_PARAM;
-    const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
-    const float* centre = lay.mscale ? X : nullptr;          // ... and those are translated to the first datum
-    Workspace rec;
-    rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
-    if (rc) return rc;
-    rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>(), centre);
-    if (rc) return rc;
-    return launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g, centre);
-}
-
-int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
-                         float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
-                         float* lower, float* g, int64_t* pairs_evaluated, void* cuda_stream) {
-    NvtxRange nvtx_range("lipfit_bounds_pruned");
-    int rc = check_sizes(N, d, Q);
-    if (rc) return rc;
-    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    if (policy != LIPFIT_BOUNDS_AUTO && policy != LIPFIT_BOUNDS_BRUTE && policy != LIPFIT_BOUNDS_PRUNED)
+        return LIPFIT_E_PARAM;
     Xform xf;
     rc = make_xform(d, mono_mask, weights, false, false, &xf);
     if (rc) return rc;
@@ -132,6 +107,26 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
+    const bool pruned = policy == LIPFIT_BOUNDS_PRUNED || (policy == LIPFIT_BOUNDS_AUTO && bounds_prefers_pruned(xf, N, Q));
+    if (!pruned) {
+        RecLayout lay = bounds_layout(c, xf, norm, Q);
+        if (lay.rf == 0) return LIPFIT_E_PARAM;
+        const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
+        const float* centre = lay.mscale ? X : nullptr;          // ... and those are translated to the first datum
+        Workspace rec;
+        rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
+        if (rc) return rc;
+        rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>(), centre);
+        if (rc) return rc;
+        rc = launch_bounds(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, upper, lower, g, centre);
+        if (rc) return rc;
+        if (pairs_evaluated) {
+            LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+            pairs_evaluated[0] = N * Q;
+            pairs_evaluated[1] = pairs_evaluated[2] = 0;
+        }
+        return LIPFIT_OK;
+    }
     Workspace stats;
     if (pairs_evaluated) {
         rc = stats.alloc(4 * sizeof(unsigned long long), c.stream);
@@ -139,7 +134,7 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
         LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 4 * sizeof(unsigned long long), c.stream));
     }
     rc = launch_bounds_pruned(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g,
-                              stats.as<unsigned long long>());
+                              pairs_evaluated ? stats.as<unsigned long long>() : nullptr);
     if (rc) return rc;
     if (pairs_evaluated) {
         unsigned long long h[4] = {0, 0, 0, 0};
@@ -150,6 +145,45 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
         pairs_evaluated[2] = static_cast<int64_t>(h[2]);
     }
     return LIPFIT_OK;
+}
+
+int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                  float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
+                  float* lower, float* g, void* cuda_stream) {
+    return lipfit_bounds_ex(X, y, N, d, Xq, Q, M, mono_mask, norm, weights, upper, lower, g, LIPFIT_BOUNDS_AUTO,
+                            nullptr, cuda_stream);
+}
+
+int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
+                         float* lower, float* g, int64_t* pairs_evaluated, void* cuda_stream) {
+    return lipfit_bounds_ex(X, y, N, d, Xq, Q, M, mono_mask, norm, weights, upper, lower, g, LIPFIT_BOUNDS_PRUNED,
+                            pairs_evaluated, cuda_stream);
+}
+
+int lipfit_bounds_region(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                         float M, const int32_t* mon, const float* a, const float* b, int32_t norm,
+                         const float* weights, float* upper, float* lower, float* g, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds_region");
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    for (int i = 0; i < d; ++i) {
+        const int m = mon ? mon[i] : 0;
+        if (m < 0 || m > 4) return LIPFIT_E_PARAM;
+        if (m != 0) {
+            if (!a || !b) return LIPFIT_E_NULL;
+            if (!(a[i] <= b[i]) || a[i] == INFINITY || b[i] == -INFINITY) return LIPFIT_E_PARAM;  // also NaN
+        }
+        if (weights && !(weights[i] >= 0.f && std::isfinite(weights[i]))) return LIPFIT_E_PARAM;
+    }
+    if (!X || !y) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    return launch_bounds_region(c, X, y, N, d, Xq, Q, M, mon, a, b, norm, weights, upper, lower, g);
 }
 
 int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
@@ -181,18 +215,23 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
     return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xf, norm, M, k, wk, upper, lower, g);
 }
 
-int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
-                       int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
-                       const float* weights, float* upper, float* lower, float* g,
-                       void* cuda_stream) {
+int lipfit_bounds_host_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
+                          int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
+                          const float* weights, float* upper, float* lower, float* g, int32_t policy,
+                          int64_t* pairs_evaluated, void* cuda_stream) {
     NvtxRange nvtx_range("lipfit_bounds_host");
     int rc = check_sizes(N, d, Q);
     if (rc) return rc;
     if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    if (policy != LIPFIT_BOUNDS_AUTO && policy != LIPFIT_BOUNDS_BRUTE && policy != LIPFIT_BOUNDS_PRUNED)
+        return LIPFIT_E_PARAM;
     Xform xf;
     if ((rc = make_xform(d, mono_mask, weights, false, false, &xf))) return rc;
     if (!X || !y || (Q > 0 && !Xq)) return LIPFIT_E_NULL;
-    if (Q == 0) return LIPFIT_OK;
+    if (Q == 0) {
+        if (pairs_evaluated) pairs_evaluated[0] = pairs_evaluated[1] = pairs_evaluated[2] = 0;
+        return LIPFIT_OK;
+    }
     cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
     Workspace dX, dy, dXq, dout;
     if ((rc = to_device(dX, X, static_cast<size_t>(N) * d, s))) return rc;
@@ -202,8 +241,8 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, con
     float* du = upper ? dout.as<float>() : nullptr;
     float* dl = lower ? dout.as<float>() + Q : nullptr;
     float* dg = g ? dout.as<float>() + 2 * Q : nullptr;
-    rc = lipfit_bounds(dX.as<float>(), dy.as<float>(), N, d, dXq.as<float>(), Q, M, mono_mask, norm,
-                       weights, du, dl, dg, cuda_stream);
+    rc = lipfit_bounds_ex(dX.as<float>(), dy.as<float>(), N, d, dXq.as<float>(), Q, M, mono_mask, norm,
+                          weights, du, dl, dg, policy, pairs_evaluated, cuda_stream);
     if (rc) return rc;
     const size_t ob = sizeof(float) * static_cast<size_t>(Q);
     if (upper && Q) LIPFIT_CUDA(cudaMemcpyAsync(upper, du, ob, cudaMemcpyDeviceToHost, s));
@@ -211,6 +250,14 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, con
     if (g && Q) LIPFIT_CUDA(cudaMemcpyAsync(g, dg, ob, cudaMemcpyDeviceToHost, s));
     LIPFIT_CUDA(cudaStreamSynchronize(s));
     return LIPFIT_OK;
+}
+
+int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
+                       int64_t Q, float M, const int32_t* mono_mask, int32_t norm,
+                       const float* weights, float* upper, float* lower, float* g,
+                       void* cuda_stream) {
+    return lipfit_bounds_host_ex(X, y, N, d, Xq, Q, M, mono_mask, norm, weights, upper, lower, g,
+                                 LIPFIT_BOUNDS_AUTO, nullptr, cuda_stream);
 }
 
 int lipfit_knn(const float* X, int64_t N, int32_t d, const float* Xq, int64_t Q,

@@ -457,6 +457,14 @@ bounds_finalize_kernel(const uint32_t* __restrict__ keyU, const uint32_t* __rest
     if (g) g[qi] = 0.5f * (U + L);
 }
 
+int launch_bounds_finalize(const Ctx& c, const uint32_t* keyU, const uint32_t* keyL, int Q, float* upper,
+                           float* lower, float* g) {
+    bounds_finalize_kernel<<<(Q + 255) / 256, 256, 0, c.stream>>>(keyU, keyL, Q, upper, lower, g);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Host dispatch
 // ---------------------------------------------------------------------------------------------

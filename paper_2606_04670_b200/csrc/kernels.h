@@ -40,6 +40,14 @@ int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, in
                   const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
                   const float* centre = nullptr);
 const char* bounds_variant_name(const Xform& xf, int norm);
+// partial extrema of data chunks (order-preserving keys, atomicMin / atomicMax) -> upper / lower / g
+int launch_bounds_finalize(const Ctx& c, const uint32_t* keyU, const uint32_t* keyL, int Q, float* upper,
+                           float* lower, float* g);
+// NEXT-4(iii): bounds under monotonicity on parts of the domain (region.cu, reading R26).
+// mon / a_host / b_host / weights: HOST arrays of length d, already validated by the caller.
+int launch_bounds_region(const Ctx& c, const float* X, const float* y, int64_t N, int32_t d, const float* Xq,
+                         int64_t Q, float M, const int32_t* mon, const float* a_host, const float* b_host,
+                         int norm, const float* weights, float* upper, float* lower, float* g);
 // NEXT-2: weighted sums of the k best upper / lower bound values; wk_host: host float[k]
 RecLayout bounds_topk_layout(const Xform& xf);
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
@@ -51,6 +59,13 @@ int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* X
 int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
                          const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
                          unsigned long long* stats_dev);
+
+// LIPFIT_BOUNDS_AUTO (include/lipfit.h): the exactly pruned pass when the box tests can pay for themselves --
+// few enough coordinates for the boxes to separate (d <= 8: measured 9.7x / 5.3x / 2.0x on the config 2 / 5 /
+// 3 workloads, d = 4 / 5 / 8) and enough pairs (>= 2^32, N >= 8192, Q >= 4096) to amortise two radix sorts.
+inline bool bounds_prefers_pruned(const Xform& xf, int64_t N, int64_t Q) {
+    return xf.d <= 8 && N >= 8192 && Q >= 4096 && N * Q >= (1LL << 32);
+}
 
 // Eq.(7) objective / gradient with the same exact pruning (prune.cu).  F_dev: device double (required,
 // zeroed here); grad: device float in the original order or NULL; eps may be NULL.

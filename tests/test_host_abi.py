@@ -148,3 +148,15 @@ def _gloo_worker(rank, world, q):
     t = bench.max_over_ranks(float(rank + 1), device="cpu")
     q.put((rank, lo, hi, t))
     dist.destroy_process_group()
+
+
+def test_bench_gpus_n_starts_n_ranks_by_itself():
+    """`python bench.py --gpus N` not started by torchrun re-launches itself under torchrun with N ranks on
+    127.0.0.1 (the driver's own launch line), passing its arguments through."""
+    import bench
+    cmd = bench.torchrun_command(8, ["--gpus", "8", "--steps", "3"], 29555)
+    assert cmd[1:3] == ["-m", "torch.distributed.run"]
+    assert "--nproc-per-node=8" in cmd and "--nnodes=1" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29555"
+    assert cmd[-4:] == ["--gpus", "8", "--steps", "3"] and cmd[-5].endswith("bench.py")
+    assert 1024 <= bench.free_port() <= 65535
