@@ -506,9 +506,10 @@ def run_other_config(B, c):
             us = e0.elapsed_time(e1) * 1e3 / 200
             out["back_to_back"] = {"us_per_step": us, "value": r["pairs"] / (us * 1e-6) / 1e9, "unit": UNIT,
                                    "note": "200 consecutive lipfit_bounds calls, no L2 flush"}
-            out["regime"] = ("latency-bound: 1e7 pairs are ~3 us of arithmetic at peak; the 60 % target does not "
-                             "apply (SURVEY.md §8(d)); bytes moved per step = %d" % (wl.X.nbytes + wl.y.nbytes
-                                                                                       + wl.Xq.nbytes + 3 * 4 * wl.Q))
+            moved = wl.X.nbytes + wl.y.nbytes + wl.Xq.nbytes + 3 * 4 * wl.Q
+            out["regime"] = ("latency-bound: 1e7 pairs are ~3 us of arithmetic at peak; the 60 percent target does "
+                             f"not apply (SURVEY.md §8(d)); bytes moved per step = {moved}")
+            out["hbm_gbs_at_step_time"] = moved / (out["ms_per_step"] * 1e-3) / 1e9
         if cpu:
             base, sel, ref = oracle_sample_rate(wl, 4.0)
             out["cpu_baseline"] = base
