@@ -884,10 +884,23 @@ def main():
                          "the config 2 / 3 / 5 workloads, 12 = exactly pruned smoothing objective (NEXT-4(ii)), "
                          "13 = region monotonicity (NEXT-4(iii)), 14 = an off-table shape on the generic kernel")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity legs")
+    ap.add_argument("--pipes", action="store_true",
+                    help="print the measured issue rates of the fp32 instruction classes (lipfit_pipe_throughput) "
+                         "behind DESIGN.md's 'alu' peak, then exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.pipes:
+        import paper_2606_04670_b200 as L
+        rows = []
+        for which in range(16):
+            name, lanes, instr = L.pipe_throughput(which)
+            rows.append({"instruction": name, "lane_results_per_clk_per_sm": round(lanes, 2),
+                         "warp_instr_per_clk_per_sm": round(instr, 3)})
+        print(json.dumps({"pipes": rows, "how": "32 warps / SM, 8 independent chains each, clock64 span of the "
+                                                "slowest CTA (csrc/pipes.cu)"}))
+        return 0
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not started by torchrun: start the N ranks ourselves (one process per GPU, NCCL for the timing scalar)
         env = dict(os.environ)

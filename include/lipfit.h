@@ -331,6 +331,16 @@ int lipfit_release_workspace(void);
  * (default).  lipfit_get_timing returns the accumulated device milliseconds and the number of launches. */
 void lipfit_set_timing(int32_t on);
 int lipfit_get_timing(int32_t which, double* total_ms, int64_t* launches);
+/* DIAGNOSTIC behind the "alu" roofline peak (bench.py --pipes): measured issue rate on the
+ * current device of one fp32 instruction class, which = 0 FFMA, 1 FADD, 2 FADD2 (packed f32x2), 3 FFMA2,
+ * 4 FMNMX, 5 FMNMX3 (3-input), 6 MUFU.SQRT, 7 FFMA and FMNMX interleaved, 8 FADD2 and FMNMX3 interleaved,
+ * 9 FADD with the |.| source modifier, 10-15 further FMA-pipe / ALU-pipe mixes (lipfit_pipe_name says which).  32 warps per SM run 8 independent chains each; the two HOST outputs
+ * (either may be NULL) are lane-results per clock per SM (a packed instruction retires 2 per lane, FMNMX3 folds
+ * 2 comparisons) and warp instructions per clock per SM.  Synchronises the stream; LIPFIT_E_PARAM for an
+ * unknown `which` (lipfit_pipe_name returns "" then). */
+int lipfit_pipe_throughput(int32_t which, double* lane_results_per_clk_sm /* host */,
+                           double* warp_instr_per_clk_sm /* host */, void* cuda_stream);
+const char* lipfit_pipe_name(int32_t which);
 /* Name of the selection kernel lipfit_knn_ex would use for (d, side, norm, flags). */
 int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, int32_t flags, char* out, int32_t cap);
 /* Name of the kernel variant lipfit_bounds would dispatch to for (d, mask, norm), e.g.

@@ -6,4 +6,4 @@ is its thin ctypes binding with the same entry-point names.
 from . import binding  # noqa: F401
 from .binding import *  # noqa: F401,F403
 from .binding import (LipfitError, bounds_variant, get_timing, knn_variant, launch_count, load,  # noqa: F401
-                      release_workspace, set_timing, status_string, version)
+                      pipe_throughput, release_workspace, set_timing, status_string, version)

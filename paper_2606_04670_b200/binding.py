@@ -25,7 +25,7 @@ EXPORTS = [
     "lipfit_lipschitz_constant", "lipfit_lipschitz_constant_host", "lipfit_knn_variant",
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
     "lipfit_bounds_pruned", "lipfit_smooth_objective_pruned",
-    "lipfit_bounds_ex", "lipfit_bounds_host_ex", "lipfit_bounds_region",
+    "lipfit_bounds_ex", "lipfit_bounds_host_ex", "lipfit_bounds_region", "lipfit_pipe_throughput", "lipfit_pipe_name",
 ]
 LIPFIT_BOUNDS_AUTO, LIPFIT_BOUNDS_BRUTE, LIPFIT_BOUNDS_PRUNED = 0, 1, 2
 LIPFIT_MAX_TOPK = 8
@@ -35,7 +35,8 @@ LIPFIT_KNN_NO_TENSOR_CORES = 1
 
 __all__ = [n for n in EXPORTS if n not in ("lipfit_status_string", "lipfit_version", "lipfit_launch_count",
                                            "lipfit_bounds_variant", "lipfit_set_timing", "lipfit_get_timing",
-                                           "lipfit_knn_variant", "lipfit_release_workspace")] + [
+                                           "lipfit_knn_variant", "lipfit_release_workspace", "lipfit_pipe_name",
+                                           "lipfit_pipe_throughput")] + [
     "LIPFIT_L1", "LIPFIT_L2", "LIPFIT_LINF", "LIPFIT_MAX_DIM", "LIPFIT_MAX_K", "LIPFIT_MAX_TOPK",
     "LIPFIT_LOCAL_KNOTS", "LIPFIT_KNN_NO_TENSOR_CORES", "LIPFIT_BOUNDS_AUTO", "LIPFIT_BOUNDS_BRUTE",
     "LIPFIT_BOUNDS_PRUNED"]
@@ -109,6 +110,9 @@ def load():
     lib.lipfit_set_timing.restype = None
     lib.lipfit_knn_variant.argtypes = [i32, i32, i32, i32, C.c_char_p, i32]
     lib.lipfit_release_workspace.argtypes = []
+    lib.lipfit_pipe_throughput.argtypes = [i32, P, P, P]
+    lib.lipfit_pipe_name.argtypes = [i32]
+    lib.lipfit_pipe_name.restype = C.c_char_p
     lib.lipfit_set_timing.argtypes = [i32]
     lib.lipfit_get_timing.argtypes = [i32, P, P]
     _lib = lib
@@ -125,6 +129,14 @@ def version() -> str:
 
 def launch_count() -> int:
     return int(load().lipfit_launch_count())
+
+
+def pipe_throughput(which: int):
+    """(name, lane-results / clk / SM, warp instructions / clk / SM) of instruction class `which` (diagnostic)."""
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    _check(load().lipfit_pipe_throughput(int(which), C.cast(C.byref(a), C.c_void_p), C.cast(C.byref(b), C.c_void_p),
+                                         _stream(None)), "lipfit_pipe_throughput")
+    return load().lipfit_pipe_name(int(which)).decode(), float(a.value), float(b.value)
 
 
 def release_workspace() -> None:

@@ -19,7 +19,7 @@ LIB = os.path.join(HERE, "liblipfit.so")
 STAMP = LIB + ".srchash"
 OBJDIR = os.path.join(HERE, "build")
 
-UNITS = ["prepack.cu", "bounds.cu", "knn.cu", "knn_tc.cu", "smooth.cu", "local.cu", "prune.cu", "region.cu", "api.cu", "api_smooth.cu", "lbfgs.cpp"]
+UNITS = ["prepack.cu", "bounds.cu", "knn.cu", "knn_tc.cu", "smooth.cu", "local.cu", "prune.cu", "region.cu", "pipes.cu", "api.cu", "api_smooth.cu", "lbfgs.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
@@ -50,7 +50,8 @@ def is_fresh() -> bool:
 
 def _compile(unit: str) -> str:
     obj = os.path.join(OBJDIR, unit.rsplit(".", 1)[0] + ".o")
-    cmd = ["nvcc", *NVCC_FLAGS, "-c", os.path.join(CSRC, unit), "-o", obj]
+    extra = ["-Xcompiler", "-fopenmp"] if unit.endswith(".cpp") else []    # host LBFGS vector kernels
+    cmd = ["nvcc", *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, unit), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed for {unit}:\n{r.stdout}\n{r.stderr}")
@@ -64,7 +65,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with cf.ThreadPoolExecutor(max_workers=min(8, len(UNITS))) as ex:
         objs = list(ex.map(_compile, UNITS))
     cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp",
-           *objs, "-cudart", "static", "-ldl"]
+           *objs, "-cudart", "static", "-ldl", "-lgomp"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")

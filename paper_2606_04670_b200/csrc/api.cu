@@ -72,6 +72,22 @@ int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, cha
 
 int lipfit_release_workspace(void) { return workspace_release(); }
 
+int lipfit_pipe_throughput(int32_t which, double* lane_results_per_clk_sm, double* warp_instr_per_clk_sm,
+                           void* cuda_stream) {
+    Ctx c;
+    int rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    return pipe_throughput(c, which, lane_results_per_clk_sm, warp_instr_per_clk_sm);
+}
+const char* lipfit_pipe_name(int32_t which) {
+    static const char* const names[] = {"FFMA", "FADD", "FADD2 (add.f32x2)", "FFMA2 (fma.f32x2)", "FMNMX", "FMNMX3 (3-input min)",
+                                        "MUFU.SQRT", "FFMA + FMNMX interleaved", "FADD2 + FMNMX3 interleaved",
+                                        "FADD with |.| source modifier", "FADD2 + FMNMX interleaved",
+                                        "FFMA + FMNMX3 interleaved", "2 FADD2 + 1 FMNMX3", "1 FADD2 + 2 FMNMX3",
+                                        "FADD2 + FADD interleaved", "2 FFMA + 1 FMNMX3"};
+    return (which >= 0 && which < 16) ? names[which] : "";
+}
+
 int lipfit_knn_variant(int32_t d, int32_t side, int32_t norm, int32_t flags, char* out, int32_t cap) {
     if (!out || cap < 1) return LIPFIT_E_NULL;
     if (check_norm(norm) || side < -1 || side > 1 || (flags & ~LIPFIT_KNN_NO_TENSOR_CORES)) return LIPFIT_E_PARAM;
@@ -206,13 +222,16 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
-    RecLayout lay = bounds_topk_layout(xf);
+    RecLayout lay = bounds_topk_layout(xf, norm);
+    if (lay.rf == 0) return LIPFIT_E_PARAM;
+    const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // as lipfit_bounds_ex
+    const float* centre = lay.mscale ? X : nullptr;
     Workspace rec;
     rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);
     if (rc) return rc;
-    rc = launch_prepack(c, X, y, nullptr, N, xf, lay, rec.as<float>());
+    rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>(), centre);
     if (rc) return rc;
-    return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xf, norm, M, k, wk, upper, lower, g);
+    return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, k, wk, upper, lower, g, centre);
 }
 
 int lipfit_bounds_host_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,

@@ -535,6 +535,8 @@ int launch_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
 }
 
 // throughput flavour of the packed f32x2 kernels: duplicated records (the layout says so)
+// (Measured alternatives on config 2, profiles/r2_profiles.md: 2 or 3 query pairs per thread at 3-4 CTAs per
+// SM, 256-thread CTAs, separate running extrema for even / odd records (2-input FMNMX only): all >= this one.)
 template <class P2, int RP>
 int launch_packed(const Ctx& c, BoundsArgs& a) {
     constexpr int THREADS = 128, R = 2 * RP;
@@ -704,9 +706,12 @@ int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, in
 // ---------------------------------------------------------------------------------------------
 // NEXT-2: approximation with k > 1 neighbours:
 //   upper = sum_j wk[j] * (j-th smallest of y^k + M D^u),  lower = sum_j wk[j] * (j-th largest of y^k - M D^l).
-// The same fused pass; every query keeps its kTopK best upper and lower candidates sorted in registers.
-// The hot loop is the pair arithmetic plus one compare per side against the worst kept value; the
-// rare candidates that pass (rate ~ k ln(N)/N) are inserted by an unrolled compare-exchange chain.
+// The same fused pass with the SAME pair arithmetic as lipfit_bounds (the specialised / folded cores of the
+// variant table, the generic core elsewhere); every query keeps its K best upper and lower candidates sorted
+// in registers (K = 4 for k <= 4, else 8).  The hot loop is the pair arithmetic plus one compare per side
+// against the worst kept value and ONE branch; the rare candidates that pass (rate ~ K ln(N) / N) are inserted
+// by an unrolled compare-exchange chain.  Small Q: the data are cut into chunks (as in bounds_kernel), every
+// (query block, chunk) tile writes its two K-lists to a workspace and a merge kernel forms the weighted sums.
 // ---------------------------------------------------------------------------------------------
 constexpr int kTopK = LIPFIT_MAX_TOPK;
 
@@ -714,11 +719,32 @@ struct TopkWeights {
     float w[kTopK];
 };
 
-template <int NORM, int DP, int R>
+template <int K>
+__device__ __forceinline__ void topk_insert_min(float (&U)[K], float v) {  // U ascending, U[K-1] = worst kept
+    U[K - 1] = v;
+#pragma unroll
+    for (int i = K - 1; i > 0; --i) {
+        const float lo_ = fminf(U[i - 1], U[i]), hi_ = fmaxf(U[i - 1], U[i]);
+        U[i - 1] = lo_;
+        U[i] = hi_;
+    }
+}
+template <int K>
+__device__ __forceinline__ void topk_insert_max(float (&L)[K], float v) {  // L descending
+    L[K - 1] = v;
+#pragma unroll
+    for (int i = K - 1; i > 0; --i) {
+        const float hi_ = fmaxf(L[i - 1], L[i]), lo_ = fminf(L[i - 1], L[i]);
+        L[i - 1] = hi_;
+        L[i] = lo_;
+    }
+}
+
+template <class Core, int R, int K>
 __global__ void __launch_bounds__(128, 2)
-bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk) {
-    using Core = GenCore<NORM, DP>;
+bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk, float* __restrict__ part) {
     constexpr int THREADS = 128;
+    constexpr int D = Core::D;
     constexpr int RF = Core::RF;
     constexpr int TILE = tile_records<RF>();
     __shared__ __align__(128) float sbuf[2 * TILE * RF];
@@ -731,23 +757,35 @@ bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk)
     __syncthreads();
     uint32_t phase = 0;
     const float inf = __int_as_float(0x7f800000);
-    for (int qb = blockIdx.x; qb < a.nqb; qb += gridDim.x) {
-        float q[R][DP];
-        float U[R][kTopK], L[R][kTopK];  // U ascending (U[K-1] = worst kept), L descending
+    const int ntiles = a.nqb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int qb = tile / a.nch;
+        const int ch = tile - qb * a.nch;
+        float q[R][D];
+        float U[R][K], L[R][K];  // U ascending (U[K-1] = worst kept), L descending
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
             qi = qi < a.Q ? qi : a.Q - 1;
             const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
 #pragma unroll
-            for (int j = 0; j < DP; ++j) q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+            for (int j = 0; j < D; ++j) {
+                if (Core::kGeneric) {
+                    q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+                } else {
+                    const int o = a.xf.perm[j];
+                    q[r][j] = a.xf.sw[j] * (a.centre ? __ldg(src + o) - __ldg(a.centre + o) : __ldg(src + o));
+                }
+            }
 #pragma unroll
-            for (int j = 0; j < kTopK; ++j) {
+            for (int j = 0; j < K; ++j) {
                 U[r][j] = inf;
                 L[r][j] = -inf;
             }
         }
-        RecordStream<TILE> rs(a.rec, RF, 0, a.N, sbuf, bars, &phase);
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
         for (int t = 0; t < rs.ntiles; ++t) {
             const float* s = rs.acquire(t);
             const int n = rs.count(t);
@@ -758,23 +796,10 @@ bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk)
                 for (int r = 0; r < R; ++r) {
                     float hi, lo;
                     Core::pair(q[r], x, ff, a.M, hi, lo);
-                    if (hi < U[r][kTopK - 1]) {  // rare: insert into the sorted list
-                        U[r][kTopK - 1] = hi;
-#pragma unroll
-                        for (int i = kTopK - 1; i > 0; --i) {
-                            const float lo_ = fminf(U[r][i - 1], U[r][i]), hi_ = fmaxf(U[r][i - 1], U[r][i]);
-                            U[r][i - 1] = lo_;
-                            U[r][i] = hi_;
-                        }
-                    }
-                    if (lo > L[r][kTopK - 1]) {
-                        L[r][kTopK - 1] = lo;
-#pragma unroll
-                        for (int i = kTopK - 1; i > 0; --i) {
-                            const float hi_ = fmaxf(L[r][i - 1], L[r][i]), lo_ = fminf(L[r][i - 1], L[r][i]);
-                            L[r][i - 1] = hi_;
-                            L[r][i] = lo_;
-                        }
+                    const bool pu = hi < U[r][K - 1], pl = lo > L[r][K - 1];
+                    if (pu | pl) {  // rare: insert into the sorted lists
+                        if (pu) topk_insert_min<K>(U[r], hi);
+                        if (pl) topk_insert_max<K>(L[r], lo);
                     }
                 }
             }
@@ -783,10 +808,16 @@ bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
-            if (qi < a.Q) {
+            if (qi >= a.Q) continue;
+            if (Core::kFold) {  // the per-query constant of the folded lower values (finite entries only)
+                const float sq = Core::query_term(q[r]);
+#pragma unroll
+                for (int j = 0; j < K; ++j) L[r][j] += sq;
+            }
+            if (a.nch == 1) {
                 float su = 0.f, sl = 0.f;
 #pragma unroll
-                for (int j = 0; j < kTopK; ++j) {  // slots past k have weight 0 (and may hold +-inf: skip them)
+                for (int j = 0; j < K; ++j) {  // slots past k have weight 0 (and may hold +-inf: skip them)
                     if (wk.w[j] != 0.f) {
                         su = fmaf(wk.w[j], U[r][j], su);
                         sl = fmaf(wk.w[j], L[r][j], sl);
@@ -795,67 +826,172 @@ bounds_topk_kernel(const BoundsArgs a, const FreeFlags ff, const TopkWeights wk)
                 if (a.upper) a.upper[qi] = su;
                 if (a.lower) a.lower[qi] = sl;
                 if (a.g) a.g[qi] = 0.5f * (su + sl);
+            } else {
+                float* dst = part + (static_cast<size_t>(ch) * a.Q + qi) * (2 * K);
+#pragma unroll
+                for (int j = 0; j < K; ++j) {
+                    dst[j] = U[r][j];
+                    dst[K + j] = L[r][j];
+                }
             }
         }
     }
 }
 
+// merges the K-lists of the data chunks of one query and forms the weighted sums
+template <int K>
+__global__ void __launch_bounds__(128)
+bounds_topk_merge_kernel(const float* __restrict__ part, int Q, int nch, const TopkWeights wk,
+                         float* __restrict__ upper, float* __restrict__ lower, float* __restrict__ g) {
+    const int qi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (qi >= Q) return;
+    float U[K], L[K];
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+        U[j] = __int_as_float(0x7f800000);
+        L[j] = __int_as_float(0xff800000);
+    }
+    for (int ch = 0; ch < nch; ++ch) {
+        const float* src = part + (static_cast<size_t>(ch) * Q + qi) * (2 * K);
+#pragma unroll
+        for (int j = 0; j < K; ++j) {
+            const float u = src[j], l = src[K + j];
+            if (u < U[K - 1]) topk_insert_min<K>(U, u);
+            if (l > L[K - 1]) topk_insert_max<K>(L, l);
+        }
+    }
+    float su = 0.f, sl = 0.f;
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+        if (wk.w[j] != 0.f) {
+            su = fmaf(wk.w[j], U[j], su);
+            sl = fmaf(wk.w[j], L[j], sl);
+        }
+    }
+    if (upper) upper[qi] = su;
+    if (lower) lower[qi] = sl;
+    if (g) g[qi] = 0.5f * (su + sl);
+}
+
 namespace {
 
-template <int NORM, int DP>
-int launch_topk(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk) {
-    constexpr int R = DP <= 8 ? 2 : 1;
-    auto kern = bounds_topk_kernel<NORM, DP, R>;
+template <class Core, int R, int K>
+int launch_topk_t(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk) {
+    constexpr int THREADS = 128;
+    auto kern = bounds_topk_kernel<Core, R, K>;
     int occ = 0;
-    LIPFIT_CUDA(occupancy_of(&occ, kern, 128, 0));
+    LIPFIT_CUDA(occupancy_of(&occ, kern, THREADS, 0));
     if (occ < 1) occ = 1;
-    a.nqb = (a.Q + 128 * R - 1) / (128 * R);
     const int slots = c.num_sms * occ;
+    constexpr int TILE = tile_records<Core::RF>();
+    a.nqb = (a.Q + THREADS * R - 1) / (THREADS * R);
+    // enough (query block, chunk) tiles to fill the chip twice; a chunk at least 8 smem tiles long and at
+    // most 64 chunks (the merge reads nch lists per query)
+    int want = (2 * slots + a.nqb - 1) / a.nqb;
+    int max_ch = (a.N + 8 * TILE - 1) / (8 * TILE);
+    if (max_ch > 64) max_ch = 64;
+    int nch = want < 1 ? 1 : want;
+    if (nch > max_ch) nch = max_ch;
+    if (nch < 1) nch = 1;
+    int chunk = (a.N + nch - 1) / nch;
+    chunk = ((chunk + TILE - 1) / TILE) * TILE;
+    nch = (a.N + chunk - 1) / chunk;
+    a.nch = nch;
+    a.chunk = chunk;
+    Workspace part;
+    if (nch > 1) {
+        int rc = part.alloc(sizeof(float) * 2 * K * static_cast<size_t>(nch) * a.Q, c.stream);
+        if (rc) return rc;
+    }
+    const long long ntiles = static_cast<long long>(a.nqb) * nch;
     KernelTimer kt(TK_BOUNDS_TOPK, c.stream);
-    kern<<<a.nqb < slots ? a.nqb : slots, 128, 0, c.stream>>>(a, ff, wk);
+    kern<<<static_cast<int>(ntiles < slots ? ntiles : slots), THREADS, 0, c.stream>>>(a, ff, wk, part.as<float>());
     kt.stop();
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
+    if (nch > 1) {
+        bounds_topk_merge_kernel<K><<<(a.Q + 127) / 128, 128, 0, c.stream>>>(part.as<float>(), a.Q, nch, wk, a.upper,
+                                                                              a.lower, a.g);
+        ++g_launches;
+        LIPFIT_CUDA(cudaGetLastError());
+    }
     return LIPFIT_OK;
 }
 
-int topk_dp(int d) { return d <= 4 ? 4 : (d <= 8 ? 8 : (d <= 16 ? 16 : 32)); }
+template <class Core, int RBIG>
+int launch_topk_core(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+    // small Q: one query per thread (more tiles to spread); k <= 4: lists of 4
+    const bool small = (static_cast<long long>(a.Q) + RBIG - 1) / RBIG < 2LL * c.num_sms * 128;
+    if (k <= 4) {
+        if (small || RBIG == 1) return launch_topk_t<Core, 1, 4>(c, a, ff, wk);
+        return launch_topk_t<Core, RBIG, 4>(c, a, ff, wk);
+    }
+    if (small || RBIG == 1) return launch_topk_t<Core, 1, 8>(c, a, ff, wk);
+    return launch_topk_t<Core, RBIG, 8>(c, a, ff, wk);
+}
+
+template <int NORM, int DU, int DC>
+int topk_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+    return launch_topk_core<SpecCore<NORM, DU, DC>, 4>(c, a, ff, wk, k);
+}
+template <int DU, int DC>
+int topk_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+    return launch_topk_core<FoldL1Core<DU, DC>, 4>(c, a, ff, wk, k);
+}
+template <int NORM, int DU, int DC>
+int topk_mfold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+    a.M = 1.f;  // M rides in the coordinates (layouts with mscale)
+    return launch_topk_core<SpecCore<NORM, DU, DC>, 4>(c, a, ff, wk, k);
+}
+template <int NORM, int DP>
+int topk_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+    return launch_topk_core<GenCore<NORM, DP>, (DP <= 8 ? 2 : 1)>(c, a, ff, wk, k);
+}
+
+using TopkLaunch = int (*)(const Ctx&, BoundsArgs&, const FreeFlags&, const TopkWeights&, int);
+
+// same order as kVariants
+const TopkLaunch kTopkLaunch[] = {
+    &topk_spec<2, 2, 0>, &topk_fold<2, 2>, &topk_mfold<3, 7, 1>, &topk_mfold<2, 0, 5>, &topk_spec<2, 3, 0>,
+    &topk_spec<2, 0, 3>, &topk_spec<1, 4, 0>, &topk_spec<2, 4, 0>, &topk_spec<3, 8, 0>, &topk_spec<2, 5, 0>,
+    &topk_gen<1, 4>, &topk_gen<2, 4>, &topk_gen<3, 4>, &topk_gen<1, 8>, &topk_gen<2, 8>, &topk_gen<3, 8>,
+    &topk_gen<1, 16>, &topk_gen<2, 16>, &topk_gen<3, 16>, &topk_gen<1, 32>, &topk_gen<2, 32>, &topk_gen<3, 32>,
+};
+static_assert(sizeof(kTopkLaunch) / sizeof(kTopkLaunch[0]) == sizeof(kVariants) / sizeof(kVariants[0]),
+              "one top-k launcher per bounds variant");
 
 }  // namespace
 
-RecLayout bounds_topk_layout(const Xform& xf) {
-    const int dp = topk_dp(xf.d);
-    return RecLayout{dp + 4, dp};
+// records of the top-k pass: the variant's plain (not duplicated) layout
+RecLayout bounds_topk_layout(const Xform& xf, int norm) {
+    const Variant* v = pick(xf, norm);
+    return v ? v->lay : RecLayout{0, 0};
 }
 
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
-                       int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g) {
+                       int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g,
+                       const float* centre) {
+    const Variant* v = pick(xf, norm);
+    if (!v) return LIPFIT_E_PARAM;
+    if (centre && v->dC < 0) return LIPFIT_E_PARAM;
     BoundsArgs a{};
     a.rec = rec;
     a.Xq = Xq;
+    a.centre = centre;
     a.upper = upper;
     a.lower = lower;
     a.g = g;
     a.N = static_cast<int>(N);
     a.Q = static_cast<int>(Q);
     a.d = xf.d;
+    a.rf = v->lay.rf;
+    a.vslot = v->lay.vslot;
     a.M = M;
     a.xf = xf;
     TopkWeights wk;
     for (int j = 0; j < kTopK; ++j) wk.w[j] = j < k ? wk_host[j] : 0.f;
     FreeFlags ff = make_free_flags(xf);
-    const int dp = topk_dp(xf.d);
-#define TOPK_GO(NORM)                                              \
-    do {                                                           \
-        if (dp == 4) return launch_topk<NORM, 4>(c, a, ff, wk);    \
-        if (dp == 8) return launch_topk<NORM, 8>(c, a, ff, wk);    \
-        if (dp == 16) return launch_topk<NORM, 16>(c, a, ff, wk);  \
-        return launch_topk<NORM, 32>(c, a, ff, wk);                \
-    } while (0)
-    if (norm == 1) TOPK_GO(1);
-    if (norm == 2) TOPK_GO(2);
-    TOPK_GO(3);
-#undef TOPK_GO
+    return kTopkLaunch[v - kVariants](c, a, ff, wk, k);
 }
 
 }  // namespace lipfit

@@ -5,14 +5,82 @@
 #include <algorithm>
 #include <cmath>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace lipfit {
 namespace {
 
-double dot(const std::vector<double>& a, const std::vector<double>& b) {
+// Vector kernels of the recursion.  Long vectors (config 5: n = 2e5, 40 history vectors) are cut into a FIXED
+// number of chunks that OpenMP threads share; every chunk is summed sequentially and the partial sums are added
+// in chunk order, so the results do not depend on the number of threads (same bits on any host).
+constexpr int kChunks = 64;
+constexpr size_t kParallelFrom = 1 << 15;
+
+inline int host_threads(size_t n) {
+#ifdef _OPENMP
+    if (n < kParallelFrom) return 1;
+    const int t = omp_get_max_threads();
+    return t < 1 ? 1 : (t > 16 ? 16 : t);
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
+template <class F>  // F(begin, end) -> partial sum of the chunk
+double chunked_sum(size_t n, const F& f) {
+    if (n < kParallelFrom) return f(static_cast<size_t>(0), n);
+    double part[kChunks];
+    const size_t step = (n + kChunks - 1) / kChunks;
+    const int nt = host_threads(n);
+    (void)nt;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int c = 0; c < kChunks; ++c) {
+        const size_t b = std::min(n, static_cast<size_t>(c) * step), e = std::min(n, b + step);
+        part[c] = f(b, e);
+    }
     double s = 0.0;
-    for (size_t i = 0; i < a.size(); ++i) s += a[i] * b[i];
+    for (int c = 0; c < kChunks; ++c) s += part[c];
     return s;
+}
+
+double dot(const std::vector<double>& a, const std::vector<double>& b) {
+    const double* pa = a.data();
+    const double* pb = b.data();
+    return chunked_sum(a.size(), [=](size_t i0, size_t i1) {
+        double s = 0.0;
+        for (size_t i = i0; i < i1; ++i) s += pa[i] * pb[i];
+        return s;
+    });
+}
+// d += a * v, then returns dot(w, d) (w may be null: returns 0): one pass instead of two
+double axpy_dot(std::vector<double>& d, double a, const std::vector<double>& v, const std::vector<double>* w) {
+    double* pd = d.data();
+    const double* pv = v.data();
+    const double* pw = w ? w->data() : nullptr;
+    return chunked_sum(d.size(), [=](size_t i0, size_t i1) {
+        double s = 0.0;
+        for (size_t i = i0; i < i1; ++i) {
+            pd[i] += a * pv[i];
+            if (pw) s += pw[i] * pd[i];
+        }
+        return s;
+    });
+}
+// d *= a, then returns dot(w, d)
+double scale_dot(std::vector<double>& d, double a, const std::vector<double>* w) {
+    double* pd = d.data();
+    const double* pw = w ? w->data() : nullptr;
+    return chunked_sum(d.size(), [=](size_t i0, size_t i1) {
+        double s = 0.0;
+        for (size_t i = i0; i < i1; ++i) {
+            pd[i] *= a;
+            if (pw) s += pw[i] * pd[i];
+        }
+        return s;
+    });
 }
 double norm_inf(const std::vector<double>& a) {
     double m = 0.0;
@@ -87,19 +155,22 @@ int lbfgs_minimize(int n, double* x_io, const LbfgsEval& eval, int max_iter, dou
         d = g;
         const int m = static_cast<int>(S.size());
         std::vector<double> alpha(m);
-        for (int j = m - 1; j >= 0; --j) {
-            alpha[j] = rho[j] * dot(S[j], d);
-            for (int i = 0; i < n; ++i) d[i] -= alpha[j] * Y[j][i];
-        }
         if (m > 0) {
-            double gamma = dot(S[m - 1], Y[m - 1]) / dot(Y[m - 1], Y[m - 1]);
-            for (double& v : d) v *= gamma;
+            // first loop: alpha_j = rho_j s_j.d, d -= alpha_j y_j; the update of d and the next dot product
+            // share one pass over the vectors
+            double sd = dot(S[m - 1], d);
+            for (int j = m - 1; j >= 0; --j) {
+                alpha[j] = rho[j] * sd;
+                sd = axpy_dot(d, -alpha[j], Y[j], j > 0 ? &S[j - 1] : nullptr);
+            }
+            const double gamma = dot(S[m - 1], Y[m - 1]) / dot(Y[m - 1], Y[m - 1]);
+            double yd = scale_dot(d, gamma, &Y[0]);
+            for (int j = 0; j < m; ++j) {
+                const double beta = rho[j] * yd;
+                yd = axpy_dot(d, alpha[j] - beta, S[j], j + 1 < m ? &Y[j + 1] : nullptr);
+            }
         }
-        for (int j = 0; j < m; ++j) {
-            double beta = rho[j] * dot(Y[j], d);
-            for (int i = 0; i < n; ++i) d[i] += (alpha[j] - beta) * S[j][i];
-        }
-        for (double& v : d) v = -v;
+        (void)scale_dot(d, -1.0, nullptr);
         double dg0 = dot(g, d);
         if (!(dg0 < 0.0)) {  // not a descent direction: restart from steepest descent
             S.clear();

@@ -110,7 +110,9 @@ __host__ __device__ constexpr int local_table_tile() {
     return RF <= 8 ? 128 : local_tile_records<RF>() / 2;
 }
 
-template <int NORM, int DP, int R>
+// DP: padded coordinates of a record (layout); DA <= DP: the coordinates that exist (d), the only ones the
+// distance arithmetic visits (for d <= 8 a compile-time constant: no work on padding)
+template <int NORM, int DP, int DA, int R>
 __global__ void __launch_bounds__(kLocThreads, 2)
 local_table_kernel(const TableArgs a, const Knots kn) {
     constexpr int RF = DP + 4;
@@ -133,7 +135,7 @@ local_table_kernel(const TableArgs a, const Knots kn) {
     const int ntiles = a.nrb * a.nch;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int rb = tile / a.nch, ch = tile - rb * a.nch;
-        float xi[R][DP], yi[R], dmin[R], dmin2[R], rnn[R];
+        float xi[R][DA], yi[R], dmin[R], dmin2[R], rnn[R];
         float* myM = sM + threadIdx.x;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -141,7 +143,7 @@ local_table_kernel(const TableArgs a, const Knots kn) {
             i = i < a.N ? i : a.N - 1;
             const float* src = a.rec + static_cast<size_t>(i) * RF;
 #pragma unroll
-            for (int j = 0; j < DP; ++j) xi[r][j] = __ldg(src + j);
+            for (int j = 0; j < DA; ++j) xi[r][j] = __ldg(src + j);
             yi[r] = __ldg(src + DP);
 #pragma unroll
             for (int j = 0; j < kJ; ++j) myM[(r * kJ + j) * kLocThreads] = 0.f;
@@ -165,7 +167,7 @@ local_table_kernel(const TableArgs a, const Knots kn) {
                     // can raise their bin (ratio > M  <=>  dy > M D, tested with the 2-ulp MUFU root and a
                     // 2^-20 margin so that no raise is missed) or that are a nearest neighbour so far: a few
                     // hundred of the N pairs of a row.
-                    const float acc = PairAccU<NORM, DP, 0>::run(xi[r], x);
+                    const float acc = PairAccU<NORM, DA, 0>::run(xi[r], x);
                     const float dy = fabsf(yi[r] - x[DP]);
                     float* pb = myM + (r * kJ + local_knot_index(acc, kn, sk4)) * kLocThreads;
                     const float Mb = *pb;
@@ -243,7 +245,7 @@ struct EvalArgs {
     Xform xf;
 };
 
-template <int NORM, int DP, int R>
+template <int NORM, int DP, int DA, int R>
 __global__ void __launch_bounds__(kLocThreads, 2)
 local_eval_kernel(const EvalArgs a, const Knots kn) {
     constexpr int RF = DP + 4 + kJ;
@@ -262,14 +264,14 @@ local_eval_kernel(const EvalArgs a, const Knots kn) {
     const int ntiles = a.nqb * a.nch;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int qb = tile / a.nch, ch = tile - qb * a.nch;
-        float q[R][DP], U[R], L[R];
+        float q[R][DA], U[R], L[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             int qi = (qb * R + r) * kLocThreads + static_cast<int>(threadIdx.x);
             qi = qi < a.Q ? qi : a.Q - 1;
             const float* src = a.Xq + static_cast<size_t>(qi) * a.d;
 #pragma unroll
-            for (int j = 0; j < DP; ++j) q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
+            for (int j = 0; j < DA; ++j) q[r][j] = (j < a.d) ? a.xf.sw[j] * __ldg(src + a.xf.perm[j]) : 0.f;
             U[r] = __int_as_float(0x7f800000);
             L[r] = __int_as_float(0xff800000);
         }
@@ -288,7 +290,7 @@ local_eval_kernel(const EvalArgs a, const Knots kn) {
                 for (int r = 0; r < R; ++r) {
                     // L2: the knots of this kernel are squared (launch_values_local), so the bin is decided on
                     // the squared distance and the square root (one MUFU, <= 2 ulp) only scales M_k
-                    const float acc = PairAccU<NORM, DP, 0>::run(q[r], x);
+                    const float acc = PairAccU<NORM, DA, 0>::run(q[r], x);
                     const float Mk = mk[local_knot_index(acc, kn, sk4)];
                     const float D = NORM == 2 ? fast_sqrt(acc) : acc;
                     const float MD = D > 0.f ? Mk * D : 0.f;  // M_k may be +inf at a duplicate: inf * 0 := 0
@@ -339,10 +341,10 @@ void local_schedule(int units, int per_block, int N, int tile, int slots, int* n
     *chunk = ck;
 }
 
-template <int NORM, int DP>
+template <int NORM, int DP, int DA>
 int launch_table(const Ctx& c, TableArgs& a, const Knots& kn) {
     constexpr int R = local_r(DP);
-    auto kern = local_table_kernel<NORM, DP, R>;
+    auto kern = local_table_kernel<NORM, DP, DA, R>;
     int occ = 0;
     LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
     if (occ < 1) occ = 1;
@@ -357,10 +359,10 @@ int launch_table(const Ctx& c, TableArgs& a, const Knots& kn) {
     return LIPFIT_OK;
 }
 
-template <int NORM, int DP>
+template <int NORM, int DP, int DA>
 int launch_eval(const Ctx& c, EvalArgs& a, const Knots& kn) {
     constexpr int R = local_r(DP);
-    auto kern = local_eval_kernel<NORM, DP, R>;
+    auto kern = local_eval_kernel<NORM, DP, DA, R>;
     int occ = 0;
     LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
     if (occ < 1) occ = 1;
@@ -375,30 +377,37 @@ int launch_eval(const Ctx& c, EvalArgs& a, const Knots& kn) {
     return LIPFIT_OK;
 }
 
-#define LOCAL_DISPATCH(FN, ARGS)                                          \
-    do {                                                                  \
-        if (norm == 1) {                                                  \
-            if (dp == 4) return FN<1, 4> ARGS;                            \
-            if (dp == 8) return FN<1, 8> ARGS;                            \
-            if (dp == 16) return FN<1, 16> ARGS;                          \
-            return FN<1, 32> ARGS;                                        \
-        } else if (norm == 2) {                                           \
-            if (dp == 4) return FN<2, 4> ARGS;                            \
-            if (dp == 8) return FN<2, 8> ARGS;                            \
-            if (dp == 16) return FN<2, 16> ARGS;                          \
-            return FN<2, 32> ARGS;                                        \
-        } else {                                                          \
-            if (dp == 4) return FN<3, 4> ARGS;                            \
-            if (dp == 8) return FN<3, 8> ARGS;                            \
-            if (dp == 16) return FN<3, 16> ARGS;                          \
-            return FN<3, 32> ARGS;                                        \
-        }                                                                 \
+// d <= 8: the number of coordinates is a template parameter (DA = d inside records padded to DP = 4 / 8);
+// d > 8: padded arithmetic (DA = DP = 16 / 32)
+#define LOCAL_DISPATCH_N(FN, ARGS, NORM)                 \
+    switch (d) {                                         \
+        case 1: return FN<NORM, 4, 1> ARGS;              \
+        case 2: return FN<NORM, 4, 2> ARGS;              \
+        case 3: return FN<NORM, 4, 3> ARGS;              \
+        case 4: return FN<NORM, 4, 4> ARGS;              \
+        case 5: return FN<NORM, 8, 5> ARGS;              \
+        case 6: return FN<NORM, 8, 6> ARGS;              \
+        case 7: return FN<NORM, 8, 7> ARGS;              \
+        case 8: return FN<NORM, 8, 8> ARGS;              \
+        default: break;                                  \
+    }                                                    \
+    if (d <= 16) return FN<NORM, 16, 16> ARGS;           \
+    return FN<NORM, 32, 32> ARGS;
+#define LOCAL_DISPATCH(FN, ARGS)                         \
+    do {                                                 \
+        if (norm == 1) {                                 \
+            LOCAL_DISPATCH_N(FN, ARGS, 1)                \
+        } else if (norm == 2) {                          \
+            LOCAL_DISPATCH_N(FN, ARGS, 2)                \
+        } else {                                         \
+            LOCAL_DISPATCH_N(FN, ARGS, 3)                \
+        }                                                \
     } while (0)
 
-int dispatch_table(const Ctx& c, TableArgs& a, const Knots& kn, int norm, int dp) {
+int dispatch_table(const Ctx& c, TableArgs& a, const Knots& kn, int norm, int d) {
     LOCAL_DISPATCH(launch_table, (c, a, kn));
 }
-int dispatch_eval(const Ctx& c, EvalArgs& a, const Knots& kn, int norm, int dp) {
+int dispatch_eval(const Ctx& c, EvalArgs& a, const Knots& kn, int norm, int d) {
     LOCAL_DISPATCH(launch_eval, (c, a, kn));
 }
 
@@ -448,7 +457,7 @@ int launch_local_lipschitz(const Ctx& c, const float* X, const float* y, int64_t
     a.tab = wtab.as<uint32_t>();
     a.nn = wnn.as<unsigned long long>();
     a.N = N;
-    if ((rc = dispatch_table(c, a, kn, norm, dp))) return rc;
+    if ((rc = dispatch_table(c, a, kn, norm, xf.d))) return rc;
     const int ne = N * kJ;
     local_table_final_kernel<<<(ne + 255) / 256, 256, 0, c.stream>>>(a.tab, a.nn, N, table);
     ++g_launches;
@@ -483,7 +492,7 @@ int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N6
     a.xf = xf;
     LIPFIT_CUDA(cudaMemsetAsync(a.keyU, 0xFF, sizeof(uint32_t) * Q, c.stream));
     LIPFIT_CUDA(cudaMemsetAsync(a.keyL, 0x00, sizeof(uint32_t) * Q, c.stream));
-    if ((rc = dispatch_eval(c, a, kn, norm, dp))) return rc;
+    if ((rc = dispatch_eval(c, a, kn, norm, xf.d))) return rc;
     local_eval_final_kernel<<<(Q + 255) / 256, 256, 0, c.stream>>>(a.keyU, a.keyL, Q, upper, lower, g);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
