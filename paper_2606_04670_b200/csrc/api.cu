@@ -222,7 +222,7 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
     Ctx c;
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
-    RecLayout lay = bounds_topk_layout(xf, norm);
+    RecLayout lay = bounds_topk_layout(c, xf, norm, Q);
     if (lay.rf == 0) return LIPFIT_E_PARAM;
     const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // as lipfit_bounds_ex
     const float* centre = lay.mscale ? X : nullptr;
@@ -231,7 +231,7 @@ int lipfit_bounds_topk(const float* X, const float* y, int64_t N, int32_t d, con
     if (rc) return rc;
     rc = launch_prepack(c, X, y, nullptr, N, xfp, lay, rec.as<float>(), centre);
     if (rc) return rc;
-    return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, k, wk, upper, lower, g, centre);
+    return launch_bounds_topk(c, rec.as<float>(), N, Xq, Q, xfp, norm, M, k, wk, upper, lower, g, centre, lay.dup);
 }
 
 int lipfit_bounds_host_ex(const float* X, const float* y, int64_t N, int32_t d, const float* Xq,

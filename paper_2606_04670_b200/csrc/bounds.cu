@@ -873,17 +873,132 @@ bounds_topk_merge_kernel(const float* __restrict__ part, int Q, int nch, const T
     if (g) g[qi] = 0.5f * (su + sl);
 }
 
+// Packed-f32x2 flavour of the same pass for the variants that have a packed pair policy (throughput flavour,
+// duplicated records): RP pairs of queries per thread, pair2() as in bounds_packed_kernel, four sorted lists
+// per query pair.  One branch per (record, query pair).
+template <class P2, int RP, int K>
+__global__ void __launch_bounds__(128, 2)
+bounds_topk_packed_kernel(const BoundsArgs a, const TopkWeights wk, float* __restrict__ part) {
+    constexpr int THREADS = 128;
+    constexpr int D = P2::D;
+    constexpr int RFL = P2::RFL;
+    constexpr int RF = 2 * RFL;
+    constexpr int TILE = tile_records<RF>();
+    constexpr int R = 2 * RP;
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+    const float inf = __int_as_float(0x7f800000);
+    const int ntiles = a.nqb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int qb = tile / a.nch;
+        const int ch = tile - qb * a.nch;
+        float2 q[RP][D];
+        float U[R][K], L[R][K];
+#pragma unroll
+        for (int rp = 0; rp < RP; ++rp) {
+            int q0 = (qb * R + 2 * rp) * THREADS + static_cast<int>(threadIdx.x);
+            int q1 = q0 + THREADS;
+            q0 = q0 < a.Q ? q0 : a.Q - 1;
+            q1 = q1 < a.Q ? q1 : a.Q - 1;
+            const float* s0 = a.Xq + static_cast<size_t>(q0) * a.d;
+            const float* s1 = a.Xq + static_cast<size_t>(q1) * a.d;
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const int o = a.xf.perm[j];
+                const float cj = a.centre ? __ldg(a.centre + o) : 0.f;
+                q[rp][j] = make_float2(a.xf.sw[j] * (__ldg(s0 + o) - cj), a.xf.sw[j] * (__ldg(s1 + o) - cj));
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                U[r][j] = inf;
+                L[r][j] = -inf;
+            }
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            for (int j = 0; j < n; ++j) {
+                float2 x[RFL];
+#pragma unroll
+                for (int c = 0; c < RF / 4; ++c) {
+                    const float4 v = reinterpret_cast<const float4*>(s + j * RF)[c];
+                    x[2 * c] = make_float2(v.x, v.y);
+                    x[2 * c + 1] = make_float2(v.z, v.w);
+                }
+#pragma unroll
+                for (int rp = 0; rp < RP; ++rp) {
+                    float2 hi, lo;
+                    P2::pair2(q[rp], x, hi, lo);
+                    const bool p0 = hi.x < U[2 * rp][K - 1], p1 = hi.y < U[2 * rp + 1][K - 1];
+                    const bool p2 = lo.x > L[2 * rp][K - 1], p3 = lo.y > L[2 * rp + 1][K - 1];
+                    if (p0 | p1 | p2 | p3) {  // rare
+                        if (p0) topk_insert_min<K>(U[2 * rp], hi.x);
+                        if (p1) topk_insert_min<K>(U[2 * rp + 1], hi.y);
+                        if (p2) topk_insert_max<K>(L[2 * rp], lo.x);
+                        if (p3) topk_insert_max<K>(L[2 * rp + 1], lo.y);
+                    }
+                }
+            }
+            rs.release(t);
+        }
+#pragma unroll
+        for (int rp = 0; rp < RP; ++rp) {
+            const float2 sq2 = P2::query_term2(q[rp]);  // per-query constant of the folded lower values
+            const float sqv[2] = {sq2.x, sq2.y};
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int r = 2 * rp + e;
+                const int qi = (qb * R + r) * THREADS + static_cast<int>(threadIdx.x);
+                if (qi >= a.Q) continue;
+#pragma unroll
+                for (int j = 0; j < K; ++j) L[r][j] += sqv[e];
+                if (a.nch == 1) {
+                    float su = 0.f, sl = 0.f;
+#pragma unroll
+                    for (int j = 0; j < K; ++j) {
+                        if (wk.w[j] != 0.f) {
+                            su = fmaf(wk.w[j], U[r][j], su);
+                            sl = fmaf(wk.w[j], L[r][j], sl);
+                        }
+                    }
+                    if (a.upper) a.upper[qi] = su;
+                    if (a.lower) a.lower[qi] = sl;
+                    if (a.g) a.g[qi] = 0.5f * (su + sl);
+                } else {
+                    float* dst = part + (static_cast<size_t>(ch) * a.Q + qi) * (2 * K);
+#pragma unroll
+                    for (int j = 0; j < K; ++j) {
+                        dst[j] = U[r][j];
+                        dst[K + j] = L[r][j];
+                    }
+                }
+            }
+        }
+    }
+}
+
 namespace {
 
-template <class Core, int R, int K>
-int launch_topk_t(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk) {
+// schedule + launch shared by the two flavours: KERN(args, part) over (query block, chunk) tiles
+template <int K, int TILE, class Launch>
+int launch_topk_sched(const Ctx& c, BoundsArgs& a, const TopkWeights& wk, const void* kern, int R, const Launch& go) {
     constexpr int THREADS = 128;
-    auto kern = bounds_topk_kernel<Core, R, K>;
     int occ = 0;
-    LIPFIT_CUDA(occupancy_of(&occ, kern, THREADS, 0));
+    LIPFIT_CUDA(occupancy_cached(kern, THREADS, 0, &occ));
     if (occ < 1) occ = 1;
     const int slots = c.num_sms * occ;
-    constexpr int TILE = tile_records<Core::RF>();
     a.nqb = (a.Q + THREADS * R - 1) / (THREADS * R);
     // enough (query block, chunk) tiles to fill the chip twice; a chunk at least 8 smem tiles long and at
     // most 64 chunks (the merge reads nch lists per query)
@@ -905,7 +1020,7 @@ int launch_topk_t(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWe
     }
     const long long ntiles = static_cast<long long>(a.nqb) * nch;
     KernelTimer kt(TK_BOUNDS_TOPK, c.stream);
-    kern<<<static_cast<int>(ntiles < slots ? ntiles : slots), THREADS, 0, c.stream>>>(a, ff, wk, part.as<float>());
+    go(static_cast<int>(ntiles < slots ? ntiles : slots), part.as<float>());
     kt.stop();
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
@@ -916,6 +1031,23 @@ int launch_topk_t(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWe
         LIPFIT_CUDA(cudaGetLastError());
     }
     return LIPFIT_OK;
+}
+
+template <class Core, int R, int K>
+int launch_topk_t(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk) {
+    auto kern = bounds_topk_kernel<Core, R, K>;
+    return launch_topk_sched<K, tile_records<Core::RF>()>(
+        c, a, wk, reinterpret_cast<const void*>(kern), R,
+        [&](int grid, float* part) { kern<<<grid, 128, 0, c.stream>>>(a, ff, wk, part); });
+}
+
+template <class P2, int K>
+int launch_topk_packed_t(const Ctx& c, BoundsArgs& a, const TopkWeights& wk) {
+    constexpr int RP = 2;
+    auto kern = bounds_topk_packed_kernel<P2, RP, K>;
+    return launch_topk_sched<K, tile_records<2 * P2::RFL>()>(
+        c, a, wk, reinterpret_cast<const void*>(kern), 2 * RP,
+        [&](int grid, float* part) { kern<<<grid, 128, 0, c.stream>>>(a, wk, part); });
 }
 
 template <class Core, int RBIG>
@@ -930,25 +1062,36 @@ int launch_topk_core(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const Top
     return launch_topk_t<Core, RBIG, 8>(c, a, ff, wk);
 }
 
+// dup: the records are in the duplicated layout of the packed-f32x2 kernels (bounds_layout chose the
+// throughput flavour of a packed variant)
 template <int NORM, int DU, int DC>
-int topk_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+int topk_spec(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k, bool) {
     return launch_topk_core<SpecCore<NORM, DU, DC>, 4>(c, a, ff, wk, k);
 }
+template <class P2>
+int topk_packed(const Ctx& c, BoundsArgs& a, const TopkWeights& wk, int k) {
+    return k <= 4 ? launch_topk_packed_t<P2, 4>(c, a, wk) : launch_topk_packed_t<P2, 8>(c, a, wk);
+}
 template <int DU, int DC>
-int topk_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+int topk_fold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k, bool dup) {
+    if (dup) return topk_packed<PackedFoldL1<DU, DC>>(c, a, wk, k);
     return launch_topk_core<FoldL1Core<DU, DC>, 4>(c, a, ff, wk, k);
 }
 template <int NORM, int DU, int DC>
-int topk_mfold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+int topk_mfold(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k, bool dup) {
+    if (dup) {
+        if (NORM == 2) return topk_packed<PackedL2<DU, DC>>(c, a, wk, k);
+        return topk_packed<PackedLinf<DU, DC>>(c, a, wk, k);
+    }
     a.M = 1.f;  // M rides in the coordinates (layouts with mscale)
     return launch_topk_core<SpecCore<NORM, DU, DC>, 4>(c, a, ff, wk, k);
 }
 template <int NORM, int DP>
-int topk_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k) {
+int topk_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, const TopkWeights& wk, int k, bool) {
     return launch_topk_core<GenCore<NORM, DP>, (DP <= 8 ? 2 : 1)>(c, a, ff, wk, k);
 }
 
-using TopkLaunch = int (*)(const Ctx&, BoundsArgs&, const FreeFlags&, const TopkWeights&, int);
+using TopkLaunch = int (*)(const Ctx&, BoundsArgs&, const FreeFlags&, const TopkWeights&, int, bool);
 
 // same order as kVariants
 const TopkLaunch kTopkLaunch[] = {
@@ -962,15 +1105,14 @@ static_assert(sizeof(kTopkLaunch) / sizeof(kTopkLaunch[0]) == sizeof(kVariants) 
 
 }  // namespace
 
-// records of the top-k pass: the variant's plain (not duplicated) layout
-RecLayout bounds_topk_layout(const Xform& xf, int norm) {
-    const Variant* v = pick(xf, norm);
-    return v ? v->lay : RecLayout{0, 0};
+// records of the top-k pass: the same layout lipfit_bounds would use (duplicated for the packed flavour)
+RecLayout bounds_topk_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q) {
+    return bounds_layout(c, xf, norm, Q);
 }
 
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                        int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g,
-                       const float* centre) {
+                       const float* centre, bool dup) {
     const Variant* v = pick(xf, norm);
     if (!v) return LIPFIT_E_PARAM;
     if (centre && v->dC < 0) return LIPFIT_E_PARAM;
@@ -991,7 +1133,7 @@ int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* X
     TopkWeights wk;
     for (int j = 0; j < kTopK; ++j) wk.w[j] = j < k ? wk_host[j] : 0.f;
     FreeFlags ff = make_free_flags(xf);
-    return kTopkLaunch[v - kVariants](c, a, ff, wk, k);
+    return kTopkLaunch[v - kVariants](c, a, ff, wk, k, dup);
 }
 
 }  // namespace lipfit

@@ -49,11 +49,11 @@ int launch_bounds_region(const Ctx& c, const float* X, const float* y, int64_t N
                          int64_t Q, float M, const int32_t* mon, const float* a_host, const float* b_host,
                          int norm, const float* weights, float* upper, float* lower, float* g);
 // NEXT-2: weighted sums of the k best upper / lower bound values; wk_host: host float[k]
-// rec: records in bounds_topk_layout (the variant's plain layout; mscale / centre as for lipfit_bounds)
-RecLayout bounds_topk_layout(const Xform& xf, int norm);
+// rec: records in bounds_topk_layout (= bounds_layout; mscale / centre / dup as for lipfit_bounds)
+RecLayout bounds_topk_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                        int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g,
-                       const float* centre = nullptr);
+                       const float* centre, bool dup);
 
 // NEXT-4(ii): bounds with exact spatial pruning (prune.cu); X, Xq: ORIGINAL row-major arrays.
 // stats_dev: device uint64[3] (zeroed by the caller) or NULL: [0] += tiles of 32 x 32 pairs evaluated,

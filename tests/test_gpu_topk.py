@@ -53,6 +53,18 @@ def test_k1_equals_lipfit_bounds_and_configs():
         _check(wl.X, wl.y, wl.Xq, wl.M, [0.5, 0.3, 0.2], wl.mask, wl.norm, wl.weights, stated=True)
 
 
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+@pytest.mark.parametrize("k", [3, 8])
+def test_packed_throughput_flavour_and_chunked_small_q(cfg, k):
+    """Q >= 303104 runs the packed-f32x2 top-k kernel of the config's variant (duplicated records); a small Q
+    against many data runs the one-query-per-thread kernel over data chunks + the merge kernel."""
+    wk = np.full(k, 1.0 / k, np.float32)
+    wl = make_workload(cfg, N=700, Q=310000)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wk, wl.mask, wl.norm, wl.weights, stated=True)
+    wl = make_workload(cfg, N=60000, Q=257)
+    _check(wl.X, wl.y, wl.Xq, wl.M, wk, wl.mask, wl.norm, wl.weights, stated=True)
+
+
 def test_edges_and_errors():
     import torch
     import paper_2606_04670_b200 as L
