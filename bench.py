@@ -617,9 +617,9 @@ def run_other_config(B, c):
         out.update({"workload": "config 2 data and queries, k = 4 best bounds with weights [0.4, 0.3, 0.2, 0.1]",
                     "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
                     "unit": UNIT, "kernel": "bounds_topk",
-                    # the k = 1 work (18 lane-ops per pair in the plain form) + one compare per side against the
-                    # worst kept value
-                    "roofline": B.roofline(pairs, SURVEY_OPS[2] + 2, SURVEY_OPS[2] + 2, kms, "bounds_topk")})
+                    # the k = 1 work (18 lane-ops per pair in the plain form, 13 in the folded form the kernel
+                    # executes) + one compare per side against the worst kept value
+                    "roofline": B.roofline(pairs, SURVEY_OPS[2] + 2, EXECUTED_OPS[2] + 2, kms, "bounds_topk")})
         if cpu:
             base, sel, ref = oracle_sample_rate(
                 wl, 3.0, lambda xs: oracle.bounds_topk(wl.X, wl.y, xs, wl.M, wk, wl.mask, wl.norm, wl.weights))

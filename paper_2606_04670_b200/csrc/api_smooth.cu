@@ -93,7 +93,7 @@ int lipfit_smooth_objective_pruned(const float* X, const float* y, int64_t N, in
     Workspace fdev;
     rc = fdev.alloc(sizeof(double) + 2 * sizeof(unsigned long long), c.stream);
     if (rc) return rc;
-    LIPFIT_CUDA(cudaMemsetAsync(fdev.p, 0, sizeof(double) + 2 * sizeof(unsigned long long), c.stream));
+    LIPFIT_CUDA(cudaMemsetAsync(fdev.p, 0, sizeof(double) + 2 * sizeof(unsigned long long), c.stream));  // stats
     unsigned long long* stats = reinterpret_cast<unsigned long long*>(fdev.as<double>() + 1);
     rc = launch_smooth_objective_pruned(c, X, y, eps, N, xf, norm, M, p, fdev.as<double>(), grad,
                                         pairs_evaluated ? stats : nullptr);
@@ -131,10 +131,15 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
     if ((rc = eps_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = grad_h.alloc(sizeof(float) * n))) return rc;
     if ((rc = fv_h.alloc(sizeof(double) * 2))) return rc;
-    rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>(), X /* centre */);
-    if (rc) return rc;
-
     const bool use_pruned = smooth_prefers_pruned(xf, N);
+    Workspace order;  // pruned pass: the Morton order of the data, computed once (X does not change)
+    if (use_pruned) {
+        if ((rc = smooth_pruned_order(c, X, N, xf, order))) return rc;
+    } else {
+        rc = launch_prepack(c, X, nullptr, nullptr, N, scale_xform(xf, M), lay, rec.as<float>(), X /* centre */);
+        if (rc) return rc;
+    }
+
     std::vector<double> viol;  // max violation seen by each evaluation
     auto eval = [&](const double* x, double* f, double* g) -> int {
         float* eh = eps_h.as<float>();
@@ -143,7 +148,7 @@ int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
         int r = use_pruned
                     ? launch_smooth_objective_pruned(c, X, y_inout, eps_d.as<float>(), N, xf, norm, M, p,
                                                      fv_d.as<double>(), grad_d.as<float>(), nullptr,
-                                                     fv_d.as<double>() + 1)
+                                                     fv_d.as<double>() + 1, order.as<int32_t>())
                     : launch_smooth_objective(c, rec.as<float>(), y_inout, eps_d.as<float>(), N, xf, norm, p,
                                               fv_d.as<double>(), grad_d.as<float>(), fv_d.as<double>() + 1);
         if (r) return r;

@@ -71,9 +71,12 @@ inline bool bounds_prefers_pruned(const Xform& xf, int64_t N, int64_t Q) {
 
 // Eq.(7) objective / gradient with the same exact pruning (prune.cu).  F_dev: device double (required,
 // zeroed here); grad: device float in the original order or NULL; eps may be NULL.
+// order_dev: the Morton order of the data from smooth_pruned_order (depends on X only; NULL: computed here).
 int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N,
                                    const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
-                                   unsigned long long* stats_dev, double* maxviol_dev = nullptr);
+                                   unsigned long long* stats_dev, double* maxviol_dev = nullptr,
+                                   const int32_t* order_dev = nullptr);
+int smooth_pruned_order(const Ctx& c, const float* X, int64_t N, const Xform& xf, Workspace& dorder);
 // lipfit_smooth evaluates Eq.(7) with the pruned pass when it wins: no constrained coordinate (the
 // dominated orthant of a monotone mask defeats the box test) and enough data to fill the chip
 inline bool smooth_prefers_pruned(const Xform& xf, int64_t N) { return xf.dC == 0 && N >= 8192; }

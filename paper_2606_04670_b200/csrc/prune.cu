@@ -481,8 +481,8 @@ struct SmoothPruneArgs {
     int N, ntiles;
     float M, p;
     FreeFlags ff;
-    double* F;         // device, zeroed
-    double* maxviol;   // device, zeroed, may be NULL: max over pairs of V_ik
+    double* fpart;     // [ntiles] per-tile share of F (reduced in tile order by smooth_pruned_final_kernel)
+    float* vpart;      // [ntiles] per-tile max over pairs of V_ik
     float* grad;       // original order, may be NULL
     unsigned long long* stats;
 };
@@ -613,12 +613,35 @@ smooth_pruned_kernel(const SmoothPruneArgs a) {
     for (int o = 16; o > 0; o >>= 1) Fi += __shfl_xor_sync(0xffffffffu, Fi, o);
     vmax = warp_max(vmax);
     if (lane == 0) {
-        atomicAdd(a.F, Fi);
-        // non-negative doubles order like their bit patterns
-        if (a.maxviol)
-            atomicMax(reinterpret_cast<unsigned long long*>(a.maxviol),
-                      static_cast<unsigned long long>(__double_as_longlong(static_cast<double>(vmax))));
+        a.fpart[A] = Fi;  // fixed summation order inside the warp (xor tree) and over the tiles: reproducible
+        a.vpart[A] = vmax;
         if (a.stats) atomicAdd(&a.stats[0], n_eval);
+    }
+}
+
+// Single block, fixed order: F = sum of the per-tile shares, maxviol = their maximum.
+__global__ void __launch_bounds__(256)
+smooth_pruned_final_kernel(const double* __restrict__ fpart, const float* __restrict__ vpart, int ntiles,
+                           double* __restrict__ F, double* __restrict__ maxviol) {
+    __shared__ double rf_[256], rv_[256];
+    double f = 0.0, v = 0.0;
+    for (int t = threadIdx.x; t < ntiles; t += 256) {
+        f += fpart[t];
+        v = fmax(v, static_cast<double>(vpart[t]));
+    }
+    rf_[threadIdx.x] = f;
+    rv_[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            rf_[threadIdx.x] += rf_[threadIdx.x + o];
+            rv_[threadIdx.x] = fmax(rv_[threadIdx.x], rv_[threadIdx.x + o]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        *F = rf_[0];
+        if (maxviol) *maxviol = rv_[0];
     }
 }
 
@@ -736,15 +759,13 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
     }
 }
 
-int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N64,
-                                   const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
-                                   unsigned long long* stats_dev, double* maxviol_dev) {
+// Morton order of the data (coordinate ranges, keys, radix sort): depends on X only, so lipfit_smooth computes
+// it once and reuses it for every evaluation of the LBFGS loop.
+int smooth_pruned_order(const Ctx& c, const float* X, int64_t N64, const Xform& xf, Workspace& dorder) {
     const int N = static_cast<int>(N64);
-    const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
     int bits = 32 / xf.d;
     if (bits > 16) bits = 16;
-    const int ntiles = (N + kTile - 1) / kTile;
-    Workspace range, dkeys, dorder, rec, box;
+    Workspace range, dkeys;
     int rc = range.alloc(sizeof(uint32_t) * 2 * kMaxDim, c.stream);
     if (rc) return rc;
     prune_range_init_kernel<<<1, 32, 0, c.stream>>>(range.as<uint32_t>());
@@ -753,32 +774,51 @@ int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y,
     prune_range_kernel<<<rgrid, 256, 0, c.stream>>>(X, N, xf, range.as<uint32_t>());
     g_launches += 2;
     LIPFIT_CUDA(cudaGetLastError());
-    if ((rc = sorted_keys(c, X, N, xf, range.as<uint32_t>(), bits, dkeys, dorder))) return rc;
+    return sorted_keys(c, X, N, xf, range.as<uint32_t>(), bits, dkeys, dorder);
+}
+
+int launch_smooth_objective_pruned(const Ctx& c, const float* X, const float* y, const float* eps, int64_t N64,
+                                   const Xform& xf, int norm, float M, float p, double* F_dev, float* grad,
+                                   unsigned long long* stats_dev, double* maxviol_dev, const int32_t* order_dev) {
+    const int N = static_cast<int>(N64);
+    const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
+    const int ntiles = (N + kTile - 1) / kTile;
+    Workspace dorder, rec, box, fpart, vpart;
+    int rc;
+    if (!order_dev) {
+        if ((rc = smooth_pruned_order(c, X, N64, xf, dorder))) return rc;
+        order_dev = dorder.as<int32_t>();
+    }
     if ((rc = rec.alloc(sizeof(float) * static_cast<size_t>(ntiles) * kTile * (dp + 4), c.stream))) return rc;
     if ((rc = box.alloc(sizeof(float) * static_cast<size_t>(ntiles) * (2 * dp + 4), c.stream))) return rc;
-    LIPFIT_CUDA(cudaMemsetAsync(F_dev, 0, sizeof(double), c.stream));
-    if (maxviol_dev) LIPFIT_CUDA(cudaMemsetAsync(maxviol_dev, 0, sizeof(double), c.stream));
+    if ((rc = fpart.alloc(sizeof(double) * static_cast<size_t>(ntiles), c.stream))) return rc;
+    if ((rc = vpart.alloc(sizeof(float) * static_cast<size_t>(ntiles), c.stream))) return rc;
     const Xform xfp = padded_xform(xf, dp);
     SmoothPruneArgs a;
     a.rec = rec.as<float>();
     a.box = box.as<float>();
-    a.order = dorder.as<int32_t>();
+    a.order = order_dev;
     a.eps = eps;
     a.N = N;
     a.ntiles = ntiles;
     a.M = M;
     a.p = p;
     a.ff = make_free_flags(xfp);
-    a.F = F_dev;
-    a.maxviol = maxviol_dev;
+    a.fpart = fpart.as<double>();
+    a.vpart = vpart.as<float>();
     a.grad = grad;
     a.stats = stats_dev;
-    PruneLaunch pl{X, y, dorder.as<int32_t>(), rec.as<float>(), box.as<float>()};
+    PruneLaunch pl{X, y, order_dev, rec.as<float>(), box.as<float>()};
     switch (norm) {
-        case LIPFIT_L1: return launch_smooth_pruned_n<1>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
-        case LIPFIT_L2: return launch_smooth_pruned_n<2>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
-        default: return launch_smooth_pruned_n<3>(dp, xf.dC, c, pl, xfp, xf.d, eps, a);
+        case LIPFIT_L1: rc = launch_smooth_pruned_n<1>(dp, xf.dC, c, pl, xfp, xf.d, eps, a); break;
+        case LIPFIT_L2: rc = launch_smooth_pruned_n<2>(dp, xf.dC, c, pl, xfp, xf.d, eps, a); break;
+        default: rc = launch_smooth_pruned_n<3>(dp, xf.dC, c, pl, xfp, xf.d, eps, a); break;
     }
+    if (rc) return rc;
+    smooth_pruned_final_kernel<<<1, 256, 0, c.stream>>>(a.fpart, a.vpart, ntiles, F_dev, maxviol_dev);
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
 }
 
 

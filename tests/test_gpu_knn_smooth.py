@@ -218,6 +218,18 @@ def test_objective_shapes(norm, d, mask):
     check_objective(X, y, 0.7, mask, norm, w, 0.5, sigma=0.2, seed=d)
 
 
+@pytest.mark.parametrize("scale", [1.0e4, 1.0e7, 1.0e-6])
+@pytest.mark.parametrize("mask", [[1] * 5, None])
+def test_gradient_fixed_point_scale(scale, mask):
+    """The gradient sums are 64-bit fixed point with a scale chosen per evaluation from N (z_max - z_min)
+    (csrc/smooth.cu): data with |y| of order 1e4 or 1e7 (row sums far beyond 2^23, where a fixed 2^-40 scale
+    wrapped silently) and of order 1e-6 (where a coarse scale would lose everything) must still match the oracle.
+    Both passes: the all-pairs kernel (mask) and, for N >= 8192 without a mask, what lipfit_smooth would use."""
+    wl = make_workload(5, N=6007)
+    y = (wl.y.astype(np.float64) * scale).astype(np.float32)
+    check_objective(wl.X, y, wl.M * scale, mask, wl.norm, None, wl.p, sigma=0.05 * scale, seed=3)
+
+
 def test_objective_consistent_data_is_zero():
     wl = make_workload(1, N=900)
     F, g = _gpu_obj(wl.X, wl.y, wl.M, None, wl.mask, wl.norm, None, 1.0)
