@@ -15,7 +15,7 @@ fraction of the pairs) is printed BESIDE it under "effective", never mixed into 
 With no --configs flag (N = 1) the line also carries, under "configs", the other BASELINE.json configs
 (1, 3, 4, 5: smoothing + bounds after) and the NEXT rows (6 local Lipschitz, 7 top-k bounds, 8 Lipschitz
 constant, 9/10/11 exactly pruned bounds on the config 2/3/5 workloads, 12 exactly pruned smoothing pass,
-13 region monotonicity, 14 an off-table shape on the generic kernel), each with ms_per_step, value,
+13 region monotonicity, 14 off-table shapes: even-rounded and generic kernels), each with ms_per_step, value,
 roofline (kernel time from CUDA events), cpu_baseline (cores, sample, compiler flags) and a pass/fail parity
 on exactly the oracle's sample.  Config 3 is the LARGEST workload (1e12 pairs); config 2 stays the top-level
 line because it is the full-size BASELINE config the metric is quoted on.
@@ -706,30 +706,37 @@ def run_other_config(B, c):
             out["cpu_baseline"] = base
             out["parity"] = B.parity_bounds(wl, fn(), sel, ref)
     elif c == 14:
-        # an OFF-TABLE shape on the generic kernel: d = 6, mask [+1,0,0,-1,0,0], L2 -> bounds_generic<L2,DP8>,
-        # unstructured normal data (inputs.random_problem), N = 1e5, Q = 1e6: 1e11 pairs
-        mask = [1, 0, 0, -1, 0, 0]
-        Xn, yn, Xqn = random_problem(14, 100_000, 1_000_000, 6)
-        X, y, Xq = B.t(Xn), B.t(yn), B.t(Xqn)
-        fn = lambda: L.lipfit_bounds_ex(X, y, Xq, 1.5, mask, 2, None, policy=L.LIPFIT_BOUNDS_BRUTE)
-        ms = B.time_steps(fn, few, 3)
-        kms, _ = B.kernel_ms(0, fn, 1)
-        pairs = Xn.shape[0] * Xqn.shape[0]
-        kernel = L.bounds_variant(6, mask, 2)
-        # plain form: 4 free x 2 + 2 constrained x 5 + epilogue 4 + 2 sqrt = 24; executed by the flag arithmetic
-        # over DP = 8 padded coordinates: 8 x (sub, mul, 2 max, 2 fma) + 2 sqrt + 2 fma + min + max = 54
-        out.update({"workload": "off-table shape: d=6 mask [+1,0,0,-1,0,0] L2 M=1.5, N=1e5 Q=1e6 normal data",
-                    "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
-                    "unit": UNIT, "kernel": kernel, "roofline": B.roofline(pairs, 24, 54, kms, kernel)})
+        # OFF-TABLE shapes (no tuned kernel), unstructured normal data (inputs.random_problem), N = 1e5, Q = 1e6:
+        #   d = 6, mask [+1,0,0,-1,0,0], L2 -> even-rounded compile-time arithmetic "bounds<L2,U4,C2,padded>"
+        #   d = 12, mask [+1,0,-1,0,...], L2 -> the generic kernel "bounds_generic<L2,DP16>" (flag arithmetic)
+        def leg(d, mask, ops_plain, ops_exec):
+            Xn, yn, Xqn = random_problem(14 + d, 100_000, 1_000_000, d)
+            X, y, Xq = B.t(Xn), B.t(yn), B.t(Xqn)
+            fn = lambda: L.lipfit_bounds_ex(X, y, Xq, 1.5, mask, 2, None, policy=L.LIPFIT_BOUNDS_BRUTE)
+            ms = B.time_steps(fn, few, 3)
+            kms, _ = B.kernel_ms(0, fn, 1)
+            pairs = Xn.shape[0] * Xqn.shape[0]
+            kernel = L.bounds_variant(d, mask, 2)
+            res = {"workload": f"off-table shape: d={d} mask {mask} L2 M=1.5, N=1e5 Q=1e6 normal data",
+                   "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
+                   "unit": UNIT, "kernel": kernel, "roofline": B.roofline(pairs, ops_plain, ops_exec, kms, kernel)}
+            if cpu:
+                sel = oracle_subset(Xqn.shape[0], 600)
+                ref = oracle.bounds(Xn, yn, Xqn[sel], 1.5, mask, 2, None)
+                worst = max(float(np.abs(o.cpu().numpy()[sel].astype(np.float64) - r).max()) for o, r in zip(fn(), ref))
+                mag = max(float(np.abs(r).max()) for r in ref[:2])
+                tol = 1e-5 * float(yn.max() - yn.min()) + (d + 4) * 2.0 ** -24 * mag
+                res["parity"] = {"max_abs_err": worst, "tol": tol, "ok": bool(worst <= tol), "queries": int(len(sel)),
+                                 "note": "unstructured inputs: the stated bar + the fp32 rounding of the candidate "
+                                         "(DESIGN.md §6)"}
+            return res
+        # plain form: 2 per free + 5 per constrained coordinate + epilogue 4 + 2 sqrt: d=6 (4+2): 24; executed the same
+        out.update(leg(6, [1, 0, 0, -1, 0, 0], 24, 24))
+        # d=12 (8 free + 4 constrained): plain 16 + 20 + 6 = 42; executed by the flag arithmetic over DP = 16 padded
+        # coordinates: 16 x (sub, mul, 2 max, 2 fma) + 2 sqrt + 2 fma + min + max = 102
+        out["generic_kernel"] = leg(12, [1, 0, -1, 0] * 3, 42, 102)
         if cpu:
-            sel = oracle_subset(Xqn.shape[0], 600)
-            ref = oracle.bounds(Xn, yn, Xqn[sel], 1.5, mask, 2, None)
-            worst = max(float(np.abs(o.cpu().numpy()[sel].astype(np.float64) - r).max()) for o, r in zip(fn(), ref))
-            mag = max(float(np.abs(r).max()) for r in ref[:2])
-            tol = 1e-5 * float(yn.max() - yn.min()) + (6 + 4) * 2.0 ** -24 * mag
-            out["parity"] = {"max_abs_err": worst, "tol": tol, "ok": bool(worst <= tol), "queries": int(len(sel)),
-                             "note": "unstructured inputs: the stated bar + the fp32 rounding of the candidate "
-                                     "(DESIGN.md §6)"}
+            out["parity"]["ok"] = bool(out["parity"]["ok"] and out["generic_kernel"]["parity"]["ok"])
     return out
 
 
@@ -882,7 +889,7 @@ def main():
                          "comma list: 1, 3, 4, 5 = BASELINE.json configs; 6 = local Lipschitz (NEXT-1), 7 = top-k "
                          "bounds (NEXT-2), 8 = Lipschitz constant (NEXT-3), 9 / 10 / 11 = exactly pruned bounds on "
                          "the config 2 / 3 / 5 workloads, 12 = exactly pruned smoothing objective (NEXT-4(ii)), "
-                         "13 = region monotonicity (NEXT-4(iii)), 14 = an off-table shape on the generic kernel")
+                         "13 = region monotonicity (NEXT-4(iii)), 14 = off-table shapes (even-rounded / generic kernels)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline / parity legs")
     ap.add_argument("--pipes", action="store_true",
                     help="print the measured issue rates of the fp32 instruction classes (lipfit_pipe_throughput) "

@@ -65,7 +65,7 @@ int lipfit_bounds_variant(int32_t d, const int32_t* mono_mask, int32_t norm, cha
     Xform xf;
     int rc = make_xform(d, mono_mask, nullptr, false, false, &xf);
     if (rc) return rc;
-    std::strncpy(out, bounds_variant_name(xf, norm), static_cast<size_t>(cap) - 1);
+    std::strncpy(out, bounds_variant_name(bounds_xform(xf, norm), norm), static_cast<size_t>(cap) - 1);
     out[cap - 1] = '\0';
     return LIPFIT_OK;
 }
@@ -125,9 +125,10 @@ int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const
     if (rc) return rc;
     const bool pruned = policy == LIPFIT_BOUNDS_PRUNED || (policy == LIPFIT_BOUNDS_AUTO && bounds_prefers_pruned(xf, N, Q));
     if (!pruned) {
-        RecLayout lay = bounds_layout(c, xf, norm, Q);
+        const Xform xfb = bounds_xform(xf, norm);  // off-table shapes with d <= 8: even-rounded coordinate counts
+        RecLayout lay = bounds_layout(c, xfb, norm, Q);
         if (lay.rf == 0) return LIPFIT_E_PARAM;
-        const Xform xfp = lay.mscale ? scale_xform(xf, M) : xf;  // some kernel families fold M into the coordinates
+        const Xform xfp = lay.mscale ? scale_xform(xfb, M) : xfb;  // some kernel families fold M into the coordinates
         const float* centre = lay.mscale ? X : nullptr;          // ... and those are translated to the first datum
         Workspace rec;
         rc = rec.alloc(sizeof(float) * static_cast<size_t>(N) * lay.rf, c.stream);

@@ -476,6 +476,7 @@ struct Variant {
     RecLayout lay;
     // launches with the given R flavour (0 = big-R throughput kernel, 1 = small-R latency kernel)
     int (*launch)(const Ctx&, BoundsArgs&, const FreeFlags&, int flavour);
+    bool padded_list = false;  // reached through bounds_xform() only (see kVariants)
 };
 
 template <class Core, int R, int THREADS, int MINB>
@@ -624,6 +625,16 @@ int launch_gen(const Ctx& c, BoundsArgs& a, const FreeFlags& ff, int flavour) {
     { 2, DU, DC, NAME, {record_floats(DU + DC), DU + DC, -1, true, false, true}, &launch_l2p<DU, DC> }
 #define GEN(NORM, DP, NAME) \
     { NORM, DP, -1, NAME, {DP + 4, DP}, &launch_gen<NORM, DP> }
+// Off-table shapes with d <= 8: the counts of unconstrained / constrained coordinates are rounded up to even
+// numbers with zero-weight padding coordinates (bounds_xform), which contribute |0 - 0| = relu(0 - 0) = 0 to every
+// norm, so any (d, mask) with roundup2(dU) + roundup2(dC) <= 8 runs compile-time pair arithmetic (2 lane-ops per
+// unconstrained and 5 (Linf: 3) per constrained coordinate) instead of the generic kernel's flag arithmetic
+// (6 per padded coordinate of DP = 4 / 8).
+#define PAD(NORM, DU, DC, NAME) \
+    { NORM, DU, DC, NAME, {record_floats(DU + DC), DU + DC}, &launch_spec<NORM, DU, DC>, true }
+#define PAD3(DU, DC, TAG) \
+    PAD(1, DU, DC, "bounds<L1," TAG ",padded>"), PAD(2, DU, DC, "bounds<L2," TAG ",padded>"), \
+        PAD(3, DU, DC, "bounds<Linf," TAG ",padded>")
 
 const Variant kVariants[] = {
     // shapes of BASELINE.json configs 1, 2, 3, 5 (+ the symmetric versions of the same dims)
@@ -637,6 +648,12 @@ const Variant kVariants[] = {
     SPEC(2, 4, 0, "bounds<L2,U4,C0>"),
     SPEC(3, 8, 0, "bounds<Linf,U8,C0>"),
     SPEC(2, 5, 0, "bounds<L2,U5,C0>"),
+    // even-rounded shapes for everything else with d <= 8 (bounds_xform pads the transform to one of these)
+    PAD3(2, 0, "U2,C0"), PAD3(4, 0, "U4,C0"), PAD3(6, 0, "U6,C0"), PAD3(8, 0, "U8,C0"),
+    PAD3(0, 2, "U0,C2"), PAD3(2, 2, "U2,C2"), PAD3(4, 2, "U4,C2"), PAD3(6, 2, "U6,C2"),
+    PAD3(0, 4, "U0,C4"), PAD3(2, 4, "U2,C4"), PAD3(4, 4, "U4,C4"),
+    PAD3(0, 6, "U0,C6"), PAD3(2, 6, "U2,C6"),
+    PAD3(0, 8, "U0,C8"),
     // generic fall-back (any mask / d up to 32): still a GPU kernel, never a CPU path
     GEN(1, 4, "bounds_generic<L1,DP4>"), GEN(2, 4, "bounds_generic<L2,DP4>"),
     GEN(3, 4, "bounds_generic<Linf,DP4>"),
@@ -648,9 +665,12 @@ const Variant kVariants[] = {
     GEN(3, 32, "bounds_generic<Linf,DP32>"),
 };
 
-const Variant* pick(const Xform& xf, int norm) {
+// exact table shapes first (in table order: the tuned config kernels come before the even-rounded list), then
+// the generic kernels.  with_padded_list = false (top-k pass: it has no kernels for that list) skips the list.
+const Variant* pick(const Xform& xf, int norm, bool with_padded_list = true) {
     for (const Variant& v : kVariants)
-        if (v.dC >= 0 && v.norm == norm && v.dU == xf.dU && v.dC == xf.dC) return &v;
+        if (v.dC >= 0 && v.norm == norm && v.dU == xf.dU && v.dC == xf.dC && (with_padded_list || !v.padded_list))
+            return &v;
     for (const Variant& v : kVariants)
         if (v.dC < 0 && v.norm == norm && v.dU >= xf.d) return &v;
     return nullptr;
@@ -662,6 +682,32 @@ namespace {
 // Small problems (cannot fill the chip with 8-query threads): one query per thread.
 int bounds_flavour(const Ctx& c, int64_t Q) { return ((Q + 7) / 8 < 2LL * c.num_sms * 128) ? 1 : 0; }
 }  // namespace
+
+// The transform lipfit_bounds_ex really uses: shapes without a tuned kernel and with d <= 8 get zero-weight
+// padding coordinates so that both counts are even (see PAD above); everything else is returned unchanged.
+Xform bounds_xform(const Xform& xf, int norm) {
+    for (const Variant& v : kVariants)
+        if (v.dC >= 0 && !v.padded_list && v.norm == norm && v.dU == xf.dU && v.dC == xf.dC) return xf;
+    const int du = (xf.dU + 1) & ~1, dc = (xf.dC + 1) & ~1;
+    if (xf.d > 8 || du + dc > 8 || (du == xf.dU && dc == xf.dC)) return xf;
+    Xform o = xf;
+    o.dU = du;
+    o.dC = dc;
+    o.d = du + dc;
+    for (int j = 0; j < kMaxDim; ++j) {
+        o.perm[j] = 0;
+        o.sw[j] = 0.f;
+    }
+    for (int j = 0; j < xf.dU; ++j) {
+        o.perm[j] = xf.perm[j];
+        o.sw[j] = xf.sw[j];
+    }
+    for (int j = 0; j < xf.dC; ++j) {
+        o.perm[du + j] = xf.perm[xf.dU + j];
+        o.sw[du + j] = xf.sw[xf.dU + j];
+    }
+    return o;
+}
 
 RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q) {
     const Variant* v = pick(xf, norm);
@@ -694,7 +740,7 @@ int launch_bounds(const Ctx& c, const float* rec, int64_t N, const float* Xq, in
     a.g = g;
     a.N = static_cast<int>(N);
     a.Q = static_cast<int>(Q);
-    a.d = xf.d;
+    a.d = xf.dsrc;
     a.rf = v->lay.rf;
     a.vslot = v->lay.vslot;
     a.M = M;
@@ -1097,6 +1143,11 @@ using TopkLaunch = int (*)(const Ctx&, BoundsArgs&, const FreeFlags&, const Topk
 const TopkLaunch kTopkLaunch[] = {
     &topk_spec<2, 2, 0>, &topk_fold<2, 2>, &topk_mfold<3, 7, 1>, &topk_mfold<2, 0, 5>, &topk_spec<2, 3, 0>,
     &topk_spec<2, 0, 3>, &topk_spec<1, 4, 0>, &topk_spec<2, 4, 0>, &topk_spec<3, 8, 0>, &topk_spec<2, 5, 0>,
+    // the even-rounded list of kVariants has no top-k kernels: pick(..., false) never returns those entries
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
     &topk_gen<1, 4>, &topk_gen<2, 4>, &topk_gen<3, 4>, &topk_gen<1, 8>, &topk_gen<2, 8>, &topk_gen<3, 8>,
     &topk_gen<1, 16>, &topk_gen<2, 16>, &topk_gen<3, 16>, &topk_gen<1, 32>, &topk_gen<2, 32>, &topk_gen<3, 32>,
 };
@@ -1107,13 +1158,20 @@ static_assert(sizeof(kTopkLaunch) / sizeof(kTopkLaunch[0]) == sizeof(kVariants) 
 
 // records of the top-k pass: the same layout lipfit_bounds would use (duplicated for the packed flavour)
 RecLayout bounds_topk_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q) {
-    return bounds_layout(c, xf, norm, Q);
+    const Variant* v = pick(xf, norm, false);
+    if (!v) return RecLayout{0, 0};
+    RecLayout lay = v->lay;
+    if (lay.packed && bounds_flavour(c, Q) == 0) {  // throughput flavour of a packed variant: duplicated records
+        lay.rf *= 2;
+        lay.dup = true;
+    }
+    return lay;
 }
 
 int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* Xq, int64_t Q, const Xform& xf,
                        int norm, float M, int k, const float* wk_host, float* upper, float* lower, float* g,
                        const float* centre, bool dup) {
-    const Variant* v = pick(xf, norm);
+    const Variant* v = pick(xf, norm, false);
     if (!v) return LIPFIT_E_PARAM;
     if (centre && v->dC < 0) return LIPFIT_E_PARAM;
     BoundsArgs a{};
@@ -1125,7 +1183,7 @@ int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* X
     a.g = g;
     a.N = static_cast<int>(N);
     a.Q = static_cast<int>(Q);
-    a.d = xf.d;
+    a.d = xf.dsrc;
     a.rf = v->lay.rf;
     a.vslot = v->lay.vslot;
     a.M = M;

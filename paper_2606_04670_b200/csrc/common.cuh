@@ -24,7 +24,8 @@ constexpr int kMaxDim = LIPFIT_MAX_DIM;
 struct Xform {
     int32_t perm[kMaxDim];
     float sw[kMaxDim];
-    int32_t d, dU, dC;
+    int32_t d, dU, dC;  // packed coordinates: d = dU + dC (zero-weight padding coordinates included)
+    int32_t dsrc;       // floats per row of the caller's X / Xq (= d unless the transform was padded)
 };
 
 // Floats per packed record [x'_0 .. x'_{d-1}, y, pad]: a multiple of 4 so that a record is a

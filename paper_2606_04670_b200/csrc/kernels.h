@@ -23,6 +23,9 @@ struct RecLayout {
     bool packed = false;  // the variant has a packed-f32x2 throughput kernel (bounds_layout sets dup when it is used)
 };
 RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
+// the transform the all-pairs bounds pass really uses for (xf, norm): xf itself, or xf with zero-weight padding
+// coordinates for off-table shapes with d <= 8 (bounds.cu); apply it before bounds_layout / prepack / launch_bounds
+Xform bounds_xform(const Xform& xf, int norm);
 RecLayout smooth_layout(const Xform& xf, int norm);
 
 // a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].

@@ -176,6 +176,7 @@ int make_xform(int32_t d, const int32_t* mono_mask, const float* weights, bool s
         }
     xf->dC = n - xf->dU;
     xf->d = d;
+    xf->dsrc = d;
     for (int i = d; i < kMaxDim; ++i) {
         xf->perm[i] = 0;
         xf->sw[i] = 0.f;
@@ -202,7 +203,7 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
                const float* __restrict__ centre, float* __restrict__ rec) {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    const float* src = X + static_cast<size_t>(k) * xf.d;
+    const float* src = X + static_cast<size_t>(k) * xf.dsrc;
     float* dst = rec + static_cast<size_t>(k) * rf;
     float v = y ? y[k] : 0.f;
     if (eps) v += eps[k];
@@ -235,7 +236,7 @@ prepack_dup_kernel(const float* __restrict__ X, const float* __restrict__ y, int
                    int cslot, const float* __restrict__ centre, float* __restrict__ rec) {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
-    const float* src = X + static_cast<size_t>(k) * xf.d;
+    const float* src = X + static_cast<size_t>(k) * xf.dsrc;
     float* dst = rec + static_cast<size_t>(k) * rf;
     const float v = y ? y[k] : 0.f;
     auto coord = [&](int j) {
