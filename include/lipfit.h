@@ -68,7 +68,8 @@ enum lipfit_status {
     LIPFIT_E_SIZE = -3,  /* N < 1, Q < 0, k < 1, k > N, k > LIPFIT_MAX_K, N or Q > 2^31-1 */
     LIPFIT_E_PARAM = -4, /* M < 0 or non-finite, mask not in {-1,0,1}, w < 0 or non-finite, bad norm/side, p <= 0 */
     LIPFIT_E_CUDA = -5,  /* a CUDA runtime call failed (no device, launch error, ...) */
-    LIPFIT_E_NOMEM = -6  /* workspace allocation failed */
+    LIPFIT_E_NOMEM = -6, /* workspace allocation failed */
+    LIPFIT_E_LIMIT = -7  /* sizes beyond the fixed scratch of a no-allocation entry point (lipfit_bounds_noalloc) */
 };
 
 /* ---- Eq.(2),(3) PAPER.md:103-116 with the distance of Eq.(4) PAPER.md:142 ------------------
@@ -92,6 +93,27 @@ int lipfit_bounds_host(const float* X, const float* y, int64_t N, int32_t d,
                        const float* Xq, int64_t Q, float M,
                        const int32_t* mono_mask, int32_t norm, const float* weights,
                        float* upper, float* lower, float* g, void* cuda_stream);
+
+/* ---- Eq.(2),(3) without ANY device allocation ------------------------------------------------------
+ * For callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid allocation.  Same upper / lower / g as lipfit_bounds_ex(..., LIPFIT_BOUNDS_BRUTE, ...) (every pair is
+ * visited; the generic pair arithmetic for any d <= 32, mask, norm, weights), same arguments, layout, ownership
+ * and asynchrony on `cuda_stream` -- but the scratch (packed records, chunk-merge keys) is a FIXED file-scope
+ * device array of 8 MiB inside the library (every GPU that loads the library holds it until the process exits)
+ * and the call issues kernel launches only: no cudaMalloc / cudaFree / cudaMallocAsync, no allocating routine.
+ * Limits (LIPFIT_E_LIMIT beyond them, nothing launched):
+ *     N * (DP + 4) <= LIPFIT_NOALLOC_MAX_RECORD_FLOATS,  DP = d rounded up to 4 / 8 / 16 / 32
+ *         (N <= 131072 for d <= 4, 87381 for d <= 8, 52428 for d <= 16, 29127 for d <= 32),
+ *     Q <= LIPFIT_NOALLOC_MAX_Q = 524288 per call (split larger query sets into several calls).
+ * The scratch is SHARED by all calls and keeps the last call's contents; each call rewrites / re-initialises
+ * what it reads, so consecutive calls on one stream are independent -- but calls that OVERLAP on the GPU (two
+ * streams, two host threads) race on it: serialise them.  The first call on a device looks the array's
+ * address up (cudaGetSymbolAddress, with that device current); do that first call outside a graph capture. */
+#define LIPFIT_NOALLOC_MAX_RECORD_FLOATS (1 << 20)
+#define LIPFIT_NOALLOC_MAX_Q (1 << 19)
+int lipfit_bounds_noalloc(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q, float M,
+                          const int32_t* mono_mask, int32_t norm, const float* weights,
+                          float* upper, float* lower, float* g, void* cuda_stream);
 
 /* ---- Evaluation policy of Eq.(2),(3) -------------------------------------------------------------
  * The result of lipfit_bounds is always the minimum / maximum over ALL N data (within the fp32 tolerance

@@ -26,7 +26,9 @@ EXPORTS = [
     "lipfit_distance_quantiles", "lipfit_local_lipschitz", "lipfit_values_local", "lipfit_bounds_topk",
     "lipfit_bounds_pruned", "lipfit_smooth_objective_pruned",
     "lipfit_bounds_ex", "lipfit_bounds_host_ex", "lipfit_bounds_region", "lipfit_pipe_throughput", "lipfit_pipe_name",
+    "lipfit_bounds_noalloc",
 ]
+LIPFIT_NOALLOC_MAX_RECORD_FLOATS, LIPFIT_NOALLOC_MAX_Q = 1 << 20, 1 << 19
 LIPFIT_BOUNDS_AUTO, LIPFIT_BOUNDS_BRUTE, LIPFIT_BOUNDS_PRUNED = 0, 1, 2
 LIPFIT_MAX_TOPK = 8
 LIPFIT_LOCAL_KNOTS = 16
@@ -39,7 +41,7 @@ __all__ = [n for n in EXPORTS if n not in ("lipfit_status_string", "lipfit_versi
                                            "lipfit_pipe_throughput")] + [
     "LIPFIT_L1", "LIPFIT_L2", "LIPFIT_LINF", "LIPFIT_MAX_DIM", "LIPFIT_MAX_K", "LIPFIT_MAX_TOPK",
     "LIPFIT_LOCAL_KNOTS", "LIPFIT_KNN_NO_TENSOR_CORES", "LIPFIT_BOUNDS_AUTO", "LIPFIT_BOUNDS_BRUTE",
-    "LIPFIT_BOUNDS_PRUNED"]
+    "LIPFIT_BOUNDS_PRUNED", "LIPFIT_NOALLOC_MAX_RECORD_FLOATS", "LIPFIT_NOALLOC_MAX_Q"]
 
 
 class LipfitError(RuntimeError):
@@ -84,6 +86,7 @@ def load():
     lib.lipfit_bounds_host.argtypes = lib.lipfit_bounds.argtypes
     lib.lipfit_bounds_ex.argtypes = [P, P, i64, i32, P, i64, f32, P, i32, P, P, P, P, i32, P, P]
     lib.lipfit_bounds_host_ex.argtypes = lib.lipfit_bounds_ex.argtypes
+    lib.lipfit_bounds_noalloc.argtypes = lib.lipfit_bounds.argtypes
     lib.lipfit_bounds_region.argtypes = [P, P, i64, i32, P, i64, f32, P, P, P, i32, P, P, P, P, P]
     lib.lipfit_knn.argtypes = [P, i64, i32, P, i64, P, i32, i32, P, i32, P, P, P]
     lib.lipfit_knn_host.argtypes = lib.lipfit_knn.argtypes
@@ -227,6 +230,29 @@ def lipfit_bounds_ex(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, 
                                  outs[2].data_ptr(), int(policy), n if count_pairs else None, _stream(stream))
     _check(rc, "lipfit_bounds_ex")
     return (*outs, [int(v) for v in n]) if count_pairs else tuple(outs)
+
+
+def lipfit_bounds_noalloc(X, y, Xq, M: float, mono_mask=None, norm: int = LIPFIT_L2, weights=None, out=None,
+                          stream=None):
+    """(upper, lower, g) through lipfit_bounds_noalloc: no device allocation inside the library (fixed 8 MiB
+    scratch; LipfitError -7 beyond N (DP + 4) <= 2^20 floats or Q <= 2^19).  `out`: three preallocated float32
+    CUDA tensors of length Q (so that this binding allocates nothing either)."""
+    torch = _torch()
+    X, y, Xq = _dev_f32(X, 2, "X"), _dev_f32(y, 1, "y"), _dev_f32(Xq, 2, "Xq")
+    N, d = X.shape
+    Q = Xq.shape[0]
+    if Xq.shape[1] != d or y.shape[0] != N:
+        raise ValueError("shape mismatch")
+    m, w = _host_params(d, mono_mask, weights)
+    outs = list(out) if out is not None else [torch.empty(Q, dtype=torch.float32, device=X.device) for _ in range(3)]
+    for o in outs:
+        if _dev_f32(o, 1, "out").shape[0] != Q:
+            raise ValueError("shape mismatch")
+    rc = load().lipfit_bounds_noalloc(X.data_ptr(), y.data_ptr(), N, d, Xq.data_ptr(), Q, float(M), _np_ptr(m),
+                                      int(norm), _np_ptr(w), outs[0].data_ptr(), outs[1].data_ptr(),
+                                      outs[2].data_ptr(), _stream(stream))
+    _check(rc, "lipfit_bounds_noalloc")
+    return tuple(outs)
 
 
 def lipfit_bounds_region(X, y, Xq, M: float, mon, a, b, norm: int = LIPFIT_L2, weights=None, stream=None):

@@ -42,6 +42,7 @@ const char* lipfit_status_string(int code) {
         case LIPFIT_E_PARAM: return "bad parameter";
         case LIPFIT_E_CUDA: return "CUDA error (no device or launch failure)";
         case LIPFIT_E_NOMEM: return "out of device memory";
+        case LIPFIT_E_LIMIT: return "sizes beyond the fixed scratch of a no-allocation entry point";
         default: return "unknown status";
     }
 }
@@ -176,6 +177,25 @@ int lipfit_bounds_pruned(const float* X, const float* y, int64_t N, int32_t d, c
                          float* lower, float* g, int64_t* pairs_evaluated, void* cuda_stream) {
     return lipfit_bounds_ex(X, y, N, d, Xq, Q, M, mono_mask, norm, weights, upper, lower, g, LIPFIT_BOUNDS_PRUNED,
                             pairs_evaluated, cuda_stream);
+}
+
+int lipfit_bounds_noalloc(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,
+                          float M, const int32_t* mono_mask, int32_t norm, const float* weights, float* upper,
+                          float* lower, float* g, void* cuda_stream) {
+    NvtxRange nvtx_range("lipfit_bounds_noalloc");
+    int rc = check_sizes(N, d, Q);
+    if (rc) return rc;
+    if (check_norm(norm) || check_M(M)) return LIPFIT_E_PARAM;
+    Xform xf;
+    rc = make_xform(d, mono_mask, weights, false, false, &xf);
+    if (rc) return rc;
+    if (!X || !y) return LIPFIT_E_NULL;
+    if (Q == 0) return LIPFIT_OK;
+    if (!Xq || (!upper && !lower && !g)) return LIPFIT_E_NULL;
+    Ctx c;
+    rc = make_ctx(cuda_stream, &c);
+    if (rc) return rc;
+    return launch_bounds_noalloc(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g);
 }
 
 int lipfit_bounds_region(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,

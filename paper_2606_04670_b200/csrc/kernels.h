@@ -120,6 +120,11 @@ int launch_axpy(const Ctx& c, float* y, const float* eps, int64_t N);
 // cudaMemPoolTrimTo(private pool of the current device, 0)
 int workspace_release();
 
+// noalloc.cu: all-pairs bounds whose scratch is a fixed file-scope device array (no allocation of any kind);
+// LIPFIT_E_LIMIT when N (DP + 4) or Q exceed it.  X, Xq: ORIGINAL row-major arrays.
+int launch_bounds_noalloc(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
+                          const Xform& xf, int norm, float M, float* upper, float* lower, float* g);
+
 // diagnostic (pipes.cu): measured issue rate of one fp32 instruction class on the current device
 int pipe_throughput(const Ctx& c, int which, double* lane_results_per_clk_sm, double* warp_instr_per_clk_sm);
 
