@@ -636,10 +636,11 @@ def run_other_config(B, c):
         out.update({"workload": "config 5 data (d=5, N=200000, L2), symmetric distance",
                     "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
                     "unit": "G ordered pairs/s (each unordered pair is visited once)",
-                    "L": float(fn().cpu().numpy()[0]), "kernel": "smooth_pairs<L2,DP8,lipconst>",
+                    "L": float(fn().cpu().numpy()[0]), "kernel": "smooth_pairs<L2,U5,C0,lipconst>",
                     # plain form per ORDERED pair: 5 sub + 5 fma + sqrt + |dy| + divide + max = 14; executed per
-                    # VISITED unordered pair: 5 sub + 5 fma + dy + 2 mul + compare + loop share ~ 16 (8 per ordered)
-                    "roofline": B.roofline(pairs, 14, 8, kms, "smooth_pairs<L2,DP8,lipconst>",
+                    # VISITED unordered pair (exact-d symmetric kernel): 5 sub + 5 fma + dy + 2 mul + compare = 14
+                    # (7 per ordered pair); survivors of the filter take the fp64 ratio
+                    "roofline": B.roofline(pairs, 14, 7, kms, "smooth_pairs<L2,U5,C0,lipconst>",
                                            unit_name="ordered_pair")})
         if cpu:
             n = 20000      # the oracle is O(N^2) on the host: the first 20000 data (4e8 ordered pairs)

@@ -272,7 +272,9 @@ typedef struct lipfit_smooth_info {
 
 /* Minimises F from eps = 0 by LBFGS on the host, each evaluation one
  * device pass; then y_inout <- y + eps on the device.  eps_out [N] device or
- * NULL; info host or NULL.  Synchronises the stream. */
+ * NULL; info host or NULL.  Synchronises the stream.  Stops at gnorm_inf <= tol_grad (status 0), at
+ * max_iter (status 1), or (status 2) when no decrease can be found / the quasi-Newton model predicts a
+ * decrease below 1e-9 |F|, the resolution of the fp32-evaluated objective. */
 int lipfit_smooth(const float* X, float* y_inout, int64_t N, int32_t d, float M,
                   const int32_t* mono_mask, int32_t norm, const float* weights, float p,
                   int32_t max_iter, double tol_grad, float* eps_out, lipfit_smooth_info* info,

@@ -27,6 +27,7 @@ RecLayout bounds_layout(const Ctx& c, const Xform& xf, int norm, int64_t Q);
 // coordinates for off-table shapes with d <= 8 (bounds.cu); apply it before bounds_layout / prepack / launch_bounds
 Xform bounds_xform(const Xform& xf, int norm);
 RecLayout smooth_layout(const Xform& xf, int norm);
+RecLayout lipconst_layout(const Xform& xf, int norm);  // records of launch_lipschitz_constant
 
 // a1: build the records; y may be NULL (value 0), eps may be NULL; value = y[k] + eps[k].
 // centre: device float[d] in the ORIGINAL coordinate order or NULL.  When given, the packed coordinates are

@@ -113,7 +113,7 @@ struct Trial {
 }  // namespace
 
 int lbfgs_minimize(int n, double* x_io, const LbfgsEval& eval, int max_iter, double tol_grad,
-                   int history, LbfgsResult* out, const LbfgsAccept& on_accept) {
+                   int history, LbfgsResult* out, const LbfgsAccept& on_accept, double ftol_rel) {
     const double c1 = 1e-4, c2 = 0.9;
     const int max_ls = 40;
     std::vector<double> x(x_io, x_io + n), g(n), d(n), xt(n), gt(n), xb(n), gb(n);
@@ -178,6 +178,10 @@ int lbfgs_minimize(int n, double* x_io, const LbfgsEval& eval, int max_iter, dou
             rho.clear();
             for (int i = 0; i < n; ++i) d[i] = -g[i];
             dg0 = -dot(g, g);
+        }
+        if (ftol_rel > 0.0 && !S.empty() && -dg0 <= ftol_rel * std::fabs(f)) {
+            res.status = 2;  // predicted decrease below the resolution of the objective
+            break;
         }
         // ---- strong-Wolfe line search (Nocedal & Wright Alg. 3.5 / 3.6) ----
         double a = (S.empty()) ? std::min(1.0, 1.0 / std::max(norm1(g), 1e-300)) : 1.0;

@@ -21,7 +21,11 @@ using LbfgsEval = std::function<int(const double* x, double* f, double* g)>;
 // called with the index of the evaluation that produced the accepted iterate
 using LbfgsAccept = std::function<void(int eval_index)>;
 
+// ftol_rel > 0: also stop (status 2) when the decrease the quasi-Newton model predicts for the unit step,
+// -g'd, is <= ftol_rel * |f|: the iterate sits at the resolution of an objective that is evaluated with
+// rounding noise (lipfit_smooth: fp32 pair arithmetic), where a line search can only burn evaluations.
 int lbfgs_minimize(int n, double* x, const LbfgsEval& eval, int max_iter, double tol_grad,
-                   int history, LbfgsResult* out, const LbfgsAccept& on_accept = nullptr);
+                   int history, LbfgsResult* out, const LbfgsAccept& on_accept = nullptr,
+                   double ftol_rel = 0.0);
 
 }  // namespace lipfit

@@ -653,7 +653,31 @@ int dispatch_pairs(const Ctx& c, SmoothArgs& a, const FreeFlags& ff, const Xform
     return rc;
 }
 
+// NEXT-3 with the symmetric distance (no constrained coordinate: the paper's lipschitz_constant())
+// and d <= 8: compile-time pair arithmetic over exactly the d coordinates (2 lane-ops per coordinate) instead of
+// the flag arithmetic over DP padded ones (4 per padded coordinate).
+bool lipconst_spec(const Xform& xf) { return xf.dC == 0 && xf.d <= 8; }
+
+template <int NORM>
+int dispatch_lipconst_spec(const Ctx& c, SmoothArgs& a, const FreeFlags& ff, int d) {
+    switch (d) {
+        case 1: return launch_pairs<SpecAcc<NORM, 1, 0>, 8, kModeLipConst>(c, a, ff);
+        case 2: return launch_pairs<SpecAcc<NORM, 2, 0>, 8, kModeLipConst>(c, a, ff);
+        case 3: return launch_pairs<SpecAcc<NORM, 3, 0>, 8, kModeLipConst>(c, a, ff);
+        case 4: return launch_pairs<SpecAcc<NORM, 4, 0>, 8, kModeLipConst>(c, a, ff);
+        case 5: return launch_pairs<SpecAcc<NORM, 5, 0>, 8, kModeLipConst>(c, a, ff);
+        case 6: return launch_pairs<SpecAcc<NORM, 6, 0>, 4, kModeLipConst>(c, a, ff);
+        case 7: return launch_pairs<SpecAcc<NORM, 7, 0>, 4, kModeLipConst>(c, a, ff);
+        default: return launch_pairs<SpecAcc<NORM, 8, 0>, 4, kModeLipConst>(c, a, ff);
+    }
+}
+
 }  // namespace
+
+RecLayout lipconst_layout(const Xform& xf, int norm) {
+    if (lipconst_spec(xf)) return RecLayout{record_floats(xf.d), xf.d};
+    return smooth_layout(xf, norm);
+}
 
 RecLayout smooth_layout(const Xform& xf, int norm) {
     if (is_spec(xf, norm)) return RecLayout{record_floats(xf.d), xf.d};
@@ -756,8 +780,9 @@ int launch_smooth_objective(const Ctx& c, const float* base, const float* y, con
 int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, const float* y, int64_t N64,
                               const Xform& xf, int norm, float* L_dev) {
     const int N = static_cast<int>(N64);
-    const RecLayout lay = smooth_layout(xf, norm);
-    const int R = smooth_rows(xf, norm);
+    const bool spec = lipconst_spec(xf);
+    const RecLayout lay = lipconst_layout(xf, norm);
+    const int R = spec ? (xf.d <= 5 ? 8 : 4) : smooth_rows(xf, norm);
     SmoothArgs a{};
     a.N = N;
     a.nrb = (N + kSmThreads * R - 1) / (kSmThreads * R);
@@ -810,7 +835,11 @@ int launch_lipschitz_constant(const Ctx& c, const float* X, const float* base, c
     a.norm = norm;
     a.xf = xf;
     FreeFlags ff = make_free_flags(xf);
-    rc = dispatch_pairs<kModeLipConst>(c, a, ff, xf, norm);
+    if (spec)
+        rc = norm == 1 ? dispatch_lipconst_spec<1>(c, a, ff, xf.d)
+                       : (norm == 2 ? dispatch_lipconst_spec<2>(c, a, ff, xf.d) : dispatch_lipconst_spec<3>(c, a, ff, xf.d));
+    else
+        rc = dispatch_pairs<kModeLipConst>(c, a, ff, xf, norm);
     if (rc) return rc;
     lipconst_final_kernel<<<1, 1, 0, c.stream>>>(a.lmax, L_dev);
     ++g_launches;
