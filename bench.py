@@ -733,9 +733,10 @@ def run_other_config(B, c):
             return res
         # plain form: 2 per free + 5 per constrained coordinate + epilogue 4 + 2 sqrt: d=6 (4+2): 24; executed the same
         out.update(leg(6, [1, 0, 0, -1, 0, 0], 24, 24))
-        # d=12 (8 free + 4 constrained): plain 16 + 20 + 6 = 42; executed by the flag arithmetic over DP = 16 padded
-        # coordinates: 16 x (sub, mul, 2 max, 2 fma) + 2 sqrt + 2 fma + min + max = 102
-        out["generic_kernel"] = leg(12, [1, 0, -1, 0] * 3, 42, 102)
+        # d=12 (6 free + 6 constrained): plain 12 + 30 + 6 = 48; executed by the chunked generic arithmetic over
+        # DP = 16 padded coordinates: one chunk of 4 free coordinates (8) + two chunks of flag arithmetic
+        # (8 x (sub, mul, 2 max, 2 fma) = 48), the padding chunk skipped, + 2 sqrt + 2 fma + min + max = 62
+        out["generic_kernel"] = leg(12, [1, 0, -1, 0] * 3, 48, 62)
         if cpu:
             out["parity"]["ok"] = bool(out["parity"]["ok"] and out["generic_kernel"]["parity"]["ok"])
     return out

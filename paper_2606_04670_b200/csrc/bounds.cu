@@ -107,7 +107,8 @@ struct GenCore {
     static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags& ff,
                                                 float M, float& hi, float& lo) {
         float au, al;
-        PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
+        if (DP >= 16) PairAccChunked<NORM, DP>::run(q, x, ff, au, al);  // d > 8: chunks under uniform conditions
+        else PairAccGeneric<NORM, DP>::run(q, x, ff, au, al);
         float y = x[VSLOT];
         hi = fmaf(M, PairAccGeneric<NORM, DP>::finish(au), y);
         lo = fmaf(-M, PairAccGeneric<NORM, DP>::finish(al), y);

@@ -87,6 +87,9 @@ struct PairAccU {
 // without a branch.  Padding coordinates have x = q = 0, hence contribute 0 to every norm.
 struct FreeFlags {
     float fr[kMaxDim];
+    // chunks of 4 packed coordinates (make_free_flags): the first nfree4 chunks hold unconstrained coordinates
+    // only, chunks [nfree4, nall4) hold the rest of the d coordinates, chunks >= nall4 are pure padding
+    int32_t nfree4, nall4;
 };
 
 template <int NORM, int DP>
@@ -132,6 +135,58 @@ struct PairAccGeneric {
         return pu;
     }
     static __device__ __forceinline__ float finish(float a) { return NORM == 2 ? fast_sqrt(a) : a; }
+};
+
+// Chunked form of the generic arithmetic for the bounds kernels of d > 8 (bounds.cu GenCore): the DP padded
+// coordinates are visited in chunks of 4 under UNIFORM (kernel-parameter) conditions -- chunks of unconstrained
+// coordinates take the plain 2 operations per coordinate, the (at most dC/4 + 2) remaining chunks the flag
+// arithmetic (6 per coordinate), padding chunks are skipped.  Same values as PairAccGeneric::run (adding the
+// zeros of a padding coordinate changes no sum, square sum or maximum).
+template <int NORM, int DP>
+struct PairAccChunked {
+    static __device__ __forceinline__ void run(const float* __restrict__ q, const float* __restrict__ x,
+                                               const FreeFlags& ff, float& au, float& al) {
+        float s = 0.f, pu = 0.f, pl = 0.f;
+#pragma unroll
+        for (int c = 0; c < DP / 4; ++c) {
+            if (c < ff.nfree4) {
+#pragma unroll
+                for (int j = 4 * c; j < 4 * c + 4; ++j) {
+                    const float dlt = q[j] - x[j];
+                    if (NORM == 1) s += fabsf(dlt);
+                    if (NORM == 2) s = fmaf(dlt, dlt, s);
+                    if (NORM == 3) s = fmaxf(s, fabsf(dlt));
+                }
+            } else if (c < ff.nall4) {
+#pragma unroll
+                for (int j = 4 * c; j < 4 * c + 4; ++j) {
+                    const float dlt = q[j] - x[j];
+                    const float t = ff.fr[j] * dlt;
+                    const float u = fmaxf(dlt, -t);
+                    const float l = fmaxf(-dlt, t);
+                    if (NORM == 1) {
+                        pu += u;
+                        pl += l;
+                    }
+                    if (NORM == 2) {
+                        pu = fmaf(u, u, pu);
+                        pl = fmaf(l, l, pl);
+                    }
+                    if (NORM == 3) {
+                        pu = fmaxf(pu, u);
+                        pl = fmaxf(pl, l);
+                    }
+                }
+            }
+        }
+        if (NORM == 3) {
+            au = fmaxf(s, pu);
+            al = fmaxf(s, pl);
+        } else {
+            au = s + pu;
+            al = s + pl;
+        }
+    }
 };
 
 // Uniform policy wrappers (used by the smoothing kernel): D coordinates per point, RF floats per

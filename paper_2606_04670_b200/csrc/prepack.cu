@@ -193,6 +193,8 @@ Xform scale_xform(const Xform& xf, float s) {
 FreeFlags make_free_flags(const Xform& xf) {
     FreeFlags ff;
     for (int j = 0; j < kMaxDim; ++j) ff.fr[j] = (j < xf.dU) ? 1.f : 0.f;
+    ff.nfree4 = xf.dU / 4;
+    ff.nall4 = (xf.d + 3) / 4;
     return ff;
 }
 
