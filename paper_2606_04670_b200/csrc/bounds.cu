@@ -62,14 +62,19 @@ struct SpecCore {
     }
 };
 
-// Weighted L1 with constrained coordinates, folded (the coordinates arrive PRE-MULTIPLIED BY M):
-//   P  = sum_free |delta_j| + sum_constr (delta_j)_+                    ( = M D^u )
-//   M D^l = P - sum_constr delta_j = P - (sq - sx),  sq / sx = sum of the constrained coordinates of q / x
-//   hi = y + P,      lo = y - M D^l = (2 y - sx) - hi + sq = c' - hi + sq
-// c' = 2y - sx rides in the record, sq is constant per query and is added AFTER the running maximum, and y
-// starts the accumulation chain: 9 FMA-pipe + 2 ALU-pipe operations per pair instead of 14 + 2.
-// (Valid for L1 only: no square root stands between the sums.  Rounding: the terms of lo are of magnitude
-// M |x|, so its error is a few 2^-24 M |x| -- inside the budget of DESIGN.md §6, measured in the tests.)
+// Weighted L1 with constrained coordinates, folded (the coordinates arrive PRE-MULTIPLIED BY M).  With
+// delta = q - x per coordinate, sq / sx = sum of the constrained coordinates of the query / the datum:
+//   (delta)_+ = max(q, x) - x   and   (-delta)_+ = max(q, x) - q        (exact identities)
+//   T     = sum_free |delta_j| + sum_constr max(q_j, x_j)
+//   M D^u = T - sx,   M D^l = T - sq
+//   hi = y + M D^u = (y - sx) + T,      lo = y - M D^l = (2 y - sx) - hi + sq = c' - hi + sq
+// The record carries y - sx in its value slot (it starts the accumulation chain) and c' = 2 y - sx; sq is constant
+// per query and is added AFTER the running maximum.  Per pair: unconstrained coordinate = sub + add(|.|) on the
+// FMA pipe, constrained coordinate = ONE max on the ALU pipe + one add (instead of sub + relu + add), + one sub
+// for lo: 7 FMA-pipe + 2 ALU-pipe operations for config 2's shape, plus the min / max of the running extrema
+// (the plain form of SURVEY.md: 12 + 6).  (Valid for L1 only: no square root stands between the sums.  Rounding:
+// max(q, x) - x and c' - hi cancel terms of magnitude M |x|, so both bounds carry a few 2^-24 M |x| -- inside the
+// budget of DESIGN.md §6, measured in the tests; api.cu translates the data to the first datum to keep |x| small.)
 template <int DU, int DC>
 struct FoldL1Core {
     static constexpr int D = DU + DC;
@@ -80,11 +85,11 @@ struct FoldL1Core {
     static constexpr bool kFold = true;
     static __device__ __forceinline__ void pair(const float* q, const float* x, const FreeFlags&, float,
                                                 float& hi, float& lo) {
-        float a = x[VSLOT];
+        float a = x[VSLOT];  // y - sx
 #pragma unroll
         for (int j = 0; j < DU; ++j) a += fabsf(q[j] - x[j]);
 #pragma unroll
-        for (int j = DU; j < D; ++j) a += fmaxf(q[j] - x[j], 0.f);
+        for (int j = DU; j < D; ++j) a += fmaxf(q[j], x[j]);
         hi = a;
         lo = x[CSLOT] - a;
     }
@@ -231,9 +236,9 @@ bounds_kernel(const BoundsArgs a, const FreeFlags ff) {
 // ---------------------------------------------------------------------------------------------
 // Packed-f32x2 version of the folded L1 bounds (sm_100 FADD2): a thread keeps RP PAIRS of queries as
 // (q_r, q_r+1) register pairs; records arrive duplicated (x, x) so that one FADD2 forms the difference of
-// both queries, one FADD2 accumulates both positive parts, one FADD2 forms both lower candidates.
-// |.| has no packed form: the free coordinates are accumulated with two scalar FADD (|.| modifier).
-// Per pair of the same arithmetic: 8.5 issue slots instead of 12.6.
+// both queries (free coordinates), one FADD2 accumulates both max(q, x) (constrained coordinates), one FADD2
+// forms both lower candidates.  |.| has no packed form: the free coordinates are accumulated with two scalar
+// FADD (|.| modifier).
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ float2 sub2(float2 a, float2 b) {  // a - b, one FADD2
     return __fadd2_rn(a, make_float2(-b.x, -b.y));
@@ -246,7 +251,7 @@ struct PackedFoldL1 {
     static constexpr int D = DU + DC;
     static constexpr int RFL = record_floats(D + 1);
     static __device__ __forceinline__ void pair2(const float2* qq, const float2* x, float2& hi, float2& lo) {
-        float2 acc = x[D];  // (y, y)
+        float2 acc = x[D];  // (y - sx, y - sx), see FoldL1Core
 #pragma unroll
         for (int j = 0; j < DU; ++j) {
             const float2 dlt = sub2(qq[j], x[j]);
@@ -254,10 +259,8 @@ struct PackedFoldL1 {
             acc.y += fabsf(dlt.y);
         }
 #pragma unroll
-        for (int j = DU; j < D; ++j) {
-            const float2 dlt = sub2(qq[j], x[j]);
-            acc = __fadd2_rn(acc, make_float2(fmaxf(dlt.x, 0.f), fmaxf(dlt.y, 0.f)));
-        }
+        for (int j = DU; j < D; ++j)  // (delta)_+ = max(q, x) - x: the subtraction rides in the record
+            acc = __fadd2_rn(acc, make_float2(fmaxf(qq[j].x, x[j].x), fmaxf(qq[j].y, x[j].y)));
         hi = acc;
         lo = sub2(x[D + 1], acc);  // c' - hi
     }

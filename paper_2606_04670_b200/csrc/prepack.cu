@@ -215,10 +215,11 @@ prepack_kernel(const float* __restrict__ X, const float* __restrict__ y,
         return xf.sw[j] * (centre ? src[o] - __ldg(centre + o) : src[o]);
     };
     float cval = 0.f;
-    if (cslot >= 0) {  // c' = 2 y - sum of the constrained (packed) coordinates, see bounds.cu FoldL1Core
-        float sc = 0.f;
+    if (cslot >= 0) {  // folded L1 records (bounds.cu FoldL1Core): with sx = sum of the constrained (packed)
+        float sc = 0.f;  // coordinates, the value slot holds y - sx and the c' slot 2 y - sx
         for (int j = xf.dU; j < xf.d; ++j) sc += coord(j);
         cval = 2.f * v - sc;
+        v -= sc;
     }
     for (int j0 = 0; j0 < rf; j0 += 4) {
         float t[4];
@@ -240,16 +241,17 @@ prepack_dup_kernel(const float* __restrict__ X, const float* __restrict__ y, int
     if (k >= N) return;
     const float* src = X + static_cast<size_t>(k) * xf.dsrc;
     float* dst = rec + static_cast<size_t>(k) * rf;
-    const float v = y ? y[k] : 0.f;
+    float v = y ? y[k] : 0.f;
     auto coord = [&](int j) {
         const int o = xf.perm[j];
         return xf.sw[j] * (centre ? src[o] - __ldg(centre + o) : src[o]);
     };
     float cval = 0.f;
-    if (cslot >= 0) {
+    if (cslot >= 0) {  // as prepack_kernel: value slot y - sx, c' slot 2 y - sx
         float sc = 0.f;
         for (int j = xf.dU; j < xf.d; ++j) sc += coord(j);
         cval = 2.f * v - sc;
+        v -= sc;
     }
     for (int j0 = 0; j0 < rf / 2; j0 += 2) {
         float t[2];
