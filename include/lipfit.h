@@ -121,7 +121,10 @@ int lipfit_bounds_noalloc(const float* X, const float* y, int64_t N, int32_t d, 
  *   LIPFIT_BOUNDS_BRUTE   every (query, datum) pair, the fused all-pairs kernels (step a2): N Q pair
  *                         evaluations "proportional to N" per query as in PAPER.md:130.
  *   LIPFIT_BOUNDS_PRUNED  exact spatial pruning (NEXT-4(ii), see lipfit_bounds_pruned below).
- *   LIPFIT_BOUNDS_AUTO    what lipfit_bounds / lipfit_bounds_host do: PRUNED when d <= 8, N >= 8192,
+ *   LIPFIT_BOUNDS_AUTO    what lipfit_bounds / lipfit_bounds_host do: a single-launch kernel that keeps all N data
+ *                         in shared memory when the call is latency-bound (N (DP + 4) floats <= 46 KB and
+ *                         N Q <= 2^25 pairs: BASELINE configs[0] takes 14 us instead of 25 us), else
+ *                         PRUNED when d <= 8, N >= 8192,
  *                         Q >= 4096 and N Q >= 2^32 (few enough coordinates for bounding boxes to separate,
  *                         enough pairs to pay for two radix sorts: 9.7x / 5.3x / 2.0x on the config 2 / 5 / 3
  *                         workloads), BRUTE otherwise.  Pruning cannot help when M D is small against the

@@ -19,7 +19,7 @@ LIB = os.path.join(HERE, "liblipfit.so")
 STAMP = LIB + ".srchash"
 OBJDIR = os.path.join(HERE, "build")
 
-UNITS = ["prepack.cu", "bounds.cu", "knn.cu", "knn_tc.cu", "smooth.cu", "local.cu", "prune.cu", "region.cu", "pipes.cu", "noalloc.cu", "api.cu", "api_smooth.cu", "lbfgs.cpp"]
+UNITS = ["prepack.cu", "bounds.cu", "knn.cu", "knn_tc.cu", "smooth.cu", "local.cu", "prune.cu", "region.cu", "pipes.cu", "noalloc.cu", "small.cu", "api.cu", "api_smooth.cu", "lbfgs.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 

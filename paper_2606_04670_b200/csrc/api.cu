@@ -125,6 +125,16 @@ int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const
     rc = make_ctx(cuda_stream, &c);
     if (rc) return rc;
     const bool pruned = policy == LIPFIT_BOUNDS_PRUNED || (policy == LIPFIT_BOUNDS_AUTO && bounds_prefers_pruned(xf, N, Q));
+    if (policy == LIPFIT_BOUNDS_AUTO && bounds_small_applies(xf, N, Q)) {  // latency-bound call: one launch (small.cu)
+        rc = launch_bounds_small(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g);
+        if (rc) return rc;
+        if (pairs_evaluated) {
+            LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+            pairs_evaluated[0] = N * Q;
+            pairs_evaluated[1] = pairs_evaluated[2] = 0;
+        }
+        return LIPFIT_OK;
+    }
     if (!pruned) {
         const Xform xfb = bounds_xform(xf, norm);  // off-table shapes with d <= 8: even-rounded coordinate counts
         RecLayout lay = bounds_layout(c, xfb, norm, Q);

@@ -121,6 +121,12 @@ int launch_axpy(const Ctx& c, float* y, const float* eps, int64_t N);
 // cudaMemPoolTrimTo(private pool of the current device, 0)
 int workspace_release();
 
+// small.cu: step a2 for latency-bound calls (all N data fit a CTA's shared memory, <= 2^25 pairs): one kernel
+// launch, a1 inside the kernel, no workspace.  X, Xq: ORIGINAL row-major arrays.
+bool bounds_small_applies(const Xform& xf, int64_t N, int64_t Q);
+int launch_bounds_small(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
+                        const Xform& xf, int norm, float M, float* upper, float* lower, float* g);
+
 // noalloc.cu: all-pairs bounds whose scratch is a fixed file-scope device array (no allocation of any kind);
 // LIPFIT_E_LIMIT when N (DP + 4) or Q exceed it.  X, Xq: ORIGINAL row-major arrays.
 int launch_bounds_noalloc(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,

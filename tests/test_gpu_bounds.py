@@ -40,6 +40,15 @@ def _check(X, y, Xq, M, mask, norm, w=None, stated=False):
     assert np.abs(up - U).max(initial=0) <= tol, (np.abs(up - U).max(), tol)
     assert np.abs(lo - L_).max(initial=0) <= tol, (np.abs(lo - L_).max(), tol)
     assert np.abs(gg - g).max(initial=0) <= tol
+    # lipfit_bounds = LIPFIT_BOUNDS_AUTO may have taken the single-launch small-problem kernel or the pruned pass:
+    # the all-pairs kernels of step a2 (LIPFIT_BOUNDS_BRUTE) must meet the same bar on the same inputs
+    import torch
+    import paper_2606_04670_b200 as L
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to("cuda:0")
+    if len(Xq):
+        bu, bl, bg = L.lipfit_bounds_ex(t(X), t(y), t(Xq), M, mask, norm, w, policy=L.LIPFIT_BOUNDS_BRUTE)
+        assert np.abs(bu.cpu().numpy() - U).max() <= tol and np.abs(bl.cpu().numpy() - L_).max() <= tol
+        assert np.abs(bg.cpu().numpy() - g).max() <= tol
     return up, lo, gg
 
 
