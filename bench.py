@@ -704,9 +704,9 @@ def run_other_config(B, c):
         out.update({"workload": "config 2 data and queries; case III on x1 (a=.3, b=.6), case I on x2 (a=b=.4)",
                     "ms_per_step": float(np.mean(ms)), "kernel_ms": kms, "value": pairs / (np.mean(ms) * 1e-3) / 1e9,
                     "unit": UNIT, "kernel": "bounds_region<L1,DP4>",
-                    # per coordinate 2 sub + max + min + 2 accumulate = 6 (every coordinate carries two
-                    # transformed values), epilogue 4: 28 lane-ops per pair at d = 4
-                    "roofline": B.roofline(pairs, 28, 28, kms, "bounds_region<L1,DP4>")})
+                    # restricted coordinate: 2 sub + max + min + 2 accumulate = 6 (two transformed values), free
+                    # coordinate: sub + add = 2, epilogue 4 + 2: 2 x 6 + 2 x 2 + 6 = 22 lane-ops per pair here
+                    "roofline": B.roofline(pairs, 22, 22, kms, "bounds_region<L1,DP4>")})
         if cpu:
             base, sel, ref = oracle_sample_rate(
                 wl, 3.0, lambda xs: oracle.bounds_region(wl.X, wl.y, xs, wl.M, mon, a, b, wl.norm, wl.weights))

@@ -29,6 +29,7 @@ namespace {
 
 // host-built description of the per-coordinate transforms (padding coordinates: w = 0)
 struct RegionXform {
+    int32_t perm[kMaxDim];              // packed coordinate j = original coordinate perm[j]: restricted ones first
     float w[kMaxDim];
     float alo[kMaxDim], bhi[kMaxDim];   // clamp bounds of mid (may be -inf / +inf)
     float a0[kMaxDim], b0[kMaxDim];     // finite reference points of A(t), B(t) and of mid
@@ -55,8 +56,8 @@ region_pack_kernel(const float* __restrict__ X, const float* __restrict__ y, int
     float4* dst = reinterpret_cast<float4*>(out + static_cast<size_t>(k) * rf);
     for (int j = 0; j < dp; j += 2) {
         float P0 = 0.f, N0 = 0.f, P1 = 0.f, N1 = 0.f;
-        if (j < rx.d) region_transform(rx, j, src[j], P0, N0);
-        if (j + 1 < rx.d) region_transform(rx, j + 1, src[j + 1], P1, N1);
+        if (j < rx.d) region_transform(rx, j, src[rx.perm[j]], P0, N0);
+        if (j + 1 < rx.d) region_transform(rx, j + 1, src[rx.perm[j + 1]], P1, N1);
         dst[j >> 1] = make_float4(P0, N0, P1, N1);
     }
     if (y) dst[dp >> 1] = make_float4(y[k], 0.f, 0.f, 0.f);
@@ -68,6 +69,7 @@ struct RegionArgs {
     float *upper, *lower, *g;
     uint32_t *keyU, *keyL;
     int N, Q, nqb, nch, chunk;
+    int nr2;  // the first nr2 PAIRS of packed coordinates hold the restricted ones (mon != 0), the rest are free
     float M;
 };
 
@@ -76,41 +78,62 @@ __host__ __device__ constexpr int region_tile_records() {
     return DP <= 4 ? 256 : (DP <= 8 ? 128 : (DP <= 16 ? 64 : 32));
 }
 
-template <int NORM, int DP>
-__device__ __forceinline__ void region_pair(const float* q, const float* x, float M, float& hi, float& lo) {
+// Pairs of packed coordinates under a UNIFORM condition: restricted pairs take the two-transform arithmetic
+// (6 operations per coordinate), pairs of unrestricted coordinates (P = N = w t, so dP = -dN = delta and
+// u = l = |delta|) the plain 2 per coordinate.
+// NR2: number of leading coordinate pairs that take the restricted arithmetic (compile time).
+template <int NORM, int DP, int NR2>
+__device__ __forceinline__ void region_pair(const float* q, const float* x, float M, int nr2_rt, float& hi,
+                                            float& lo) {
+    (void)nr2_rt;
+    constexpr int nr2 = NR2;
     float su = 0.f, sl = 0.f;  // L1 / L2: sums; Linf: su = max u, sl = min over (dP, dN) (= -max l)
+    float sf = 0.f;            // unrestricted coordinates: shared by both bounds
 #pragma unroll
-    for (int j = 0; j < DP; ++j) {
-        const float dP = q[2 * j] - x[2 * j];
-        const float dN = x[2 * j + 1] - q[2 * j + 1];
-        if (NORM == 3) {
-            su = fmaxf(fmaxf(su, dP), dN);  // FMNMX3
-            sl = fminf(fminf(sl, dP), dN);
+    for (int c = 0; c < DP / 2; ++c) {
+        if (c < nr2) {
+#pragma unroll
+            for (int j = 2 * c; j < 2 * c + 2; ++j) {
+                const float dP = q[2 * j] - x[2 * j];
+                const float dN = x[2 * j + 1] - q[2 * j + 1];
+                if (NORM == 3) {
+                    su = fmaxf(fmaxf(su, dP), dN);  // FMNMX3
+                    sl = fminf(fminf(sl, dP), dN);
+                } else {
+                    const float u = fmaxf(dP, dN), m = fminf(dP, dN);  // u >= 0 >= m
+                    if (NORM == 1) {
+                        su += u;
+                        sl -= m;
+                    } else {
+                        su = fmaf(u, u, su);
+                        sl = fmaf(m, m, sl);
+                    }
+                }
+            }
         } else {
-            const float u = fmaxf(dP, dN), m = fminf(dP, dN);  // u >= 0 >= m
-            if (NORM == 1) {
-                su += u;
-                sl -= m;
-            } else {
-                su = fmaf(u, u, su);
-                sl = fmaf(m, m, sl);
+#pragma unroll
+            for (int j = 2 * c; j < 2 * c + 2; ++j) {
+                const float dlt = q[2 * j] - x[2 * j];
+                if (NORM == 1) sf += fabsf(dlt);
+                if (NORM == 2) sf = fmaf(dlt, dlt, sf);
+                if (NORM == 3) sf = fmaxf(sf, fabsf(dlt));
             }
         }
     }
     const float y = x[2 * DP];
     if (NORM == 2) {
-        hi = fmaf(M, fast_sqrt(su), y);
-        lo = fmaf(-M, fast_sqrt(sl), y);
+        hi = fmaf(M, fast_sqrt(su + sf), y);
+        lo = fmaf(-M, fast_sqrt(sl + sf), y);
     } else if (NORM == 1) {
-        hi = fmaf(M, su, y);
-        lo = fmaf(-M, sl, y);
+        hi = fmaf(M, su + sf, y);
+        lo = fmaf(-M, sl + sf, y);
     } else {
-        hi = fmaf(M, su, y);
-        lo = fmaf(M, sl, y);  // sl = -max l
+        hi = fmaf(M, fmaxf(su, sf), y);
+        lo = fmaf(-M, fmaxf(-sl, sf), y);
     }
 }
 
-template <int NORM, int DP, int R>
+template <int NORM, int DP, int R, int NR2>
 __global__ void __launch_bounds__(128, 2)
 bounds_region_kernel(const RegionArgs a) {
     constexpr int THREADS = 128;
@@ -165,7 +188,7 @@ bounds_region_kernel(const RegionArgs a) {
 #pragma unroll
                 for (int r = 0; r < R; ++r) {
                     float hi, lo;
-                    region_pair<NORM, DP>(q[r], x, a.M, hi, lo);
+                    region_pair<NORM, DP, NR2>(q[r], x, a.M, a.nr2, hi, lo);
                     U[r] = fminf(U[r], hi);
                     L[r] = fmaxf(L[r], lo);
                 }
@@ -189,10 +212,10 @@ bounds_region_kernel(const RegionArgs a) {
     }
 }
 
-template <int NORM, int DP, int R>
+template <int NORM, int DP, int R, int NR2>
 int launch_region_t(const Ctx& c, RegionArgs& a) {
     constexpr int THREADS = 128;
-    auto kern = bounds_region_kernel<NORM, DP, R>;
+    auto kern = bounds_region_kernel<NORM, DP, R, NR2>;
     int occ = 0;
     LIPFIT_CUDA(occupancy_of(&occ, kern, THREADS, 0));
     if (occ < 1) occ = 1;
@@ -229,14 +252,24 @@ int launch_region_t(const Ctx& c, RegionArgs& a) {
     return LIPFIT_OK;
 }
 
+template <int NORM, int DP, int R, int NR2>
+int launch_region_r(const Ctx& c, RegionArgs& a) {
+    if (a.nr2 == NR2) return launch_region_t<NORM, DP, R, NR2>(c, a);
+    if constexpr (NR2 > 0) return launch_region_r<NORM, DP, R, NR2 - 1>(c, a);
+    return LIPFIT_E_PARAM;
+}
+
 template <int NORM>
 int launch_region_n(const Ctx& c, RegionArgs& a, int dp, bool small) {
-    // throughput flavour: R queries per thread; small Q: one query per thread so that the chip fills
+    // throughput flavour: R queries per thread; small Q: one query per thread so that the chip fills.
+    // DP <= 8: one kernel per number of restricted coordinate pairs (0 .. DP / 2); DP >= 16: every pair takes the
+    // restricted arithmetic (valid for any coordinate; a runtime-uniform count was measured and is SLOWER: ptxas
+    // predicates both bodies).
     switch (dp) {
-        case 4: return small ? launch_region_t<NORM, 4, 1>(c, a) : launch_region_t<NORM, 4, 4>(c, a);
-        case 8: return small ? launch_region_t<NORM, 8, 1>(c, a) : launch_region_t<NORM, 8, 4>(c, a);
-        case 16: return small ? launch_region_t<NORM, 16, 1>(c, a) : launch_region_t<NORM, 16, 2>(c, a);
-        default: return launch_region_t<NORM, 32, 1>(c, a);
+        case 4: return small ? launch_region_r<NORM, 4, 1, 2>(c, a) : launch_region_r<NORM, 4, 4, 2>(c, a);
+        case 8: return small ? launch_region_r<NORM, 8, 1, 4>(c, a) : launch_region_r<NORM, 8, 4, 4>(c, a);
+        case 16: return small ? launch_region_t<NORM, 16, 1, 8>(c, a) : launch_region_t<NORM, 16, 2, 8>(c, a);
+        default: return launch_region_t<NORM, 32, 1, 16>(c, a);
     }
 }
 
@@ -247,14 +280,24 @@ int launch_bounds_region(const Ctx& c, const float* X, const float* y, int64_t N
                          int norm, const float* weights, float* upper, float* lower, float* g) {
     RegionXform rx{};
     rx.d = d;
+    int order[kMaxDim], nres = 0, nord = 0;
+    for (int i = 0; i < d; ++i)
+        if (mon && mon[i] != 0) order[nord++] = i;  // restricted coordinates first
+    nres = nord;
+    for (int i = 0; i < d; ++i)
+        if (!(mon && mon[i] != 0)) order[nord++] = i;
+    // (an odd number of restricted coordinates: the pair that holds the last one also holds the first free
+    // coordinate or padding; it takes the restricted arithmetic, which is valid for any coordinate)
     for (int j = 0; j < kMaxDim; ++j) {
-        const int m = (j < d && mon) ? mon[j] : 0;
-        const float w = j < d ? (weights ? weights[j] : 1.f) : 0.f;
+        const int i = j < d ? order[j] : 0;
+        rx.perm[j] = i;
+        const int m = (j < d && mon) ? mon[i] : 0;
+        const float w = j < d ? (weights ? weights[i] : 1.f) : 0.f;
         rx.w[j] = w;
         float a = -INFINITY, b = INFINITY;
         if (m != 0) {
-            a = a_host[j];
-            b = b_host[j];
+            a = a_host[i];
+            b = b_host[i];
         }
         const bool incA = (m == 1 || m == 4), incB = (m == 1 || m == 3);
         const bool hasA = m != 0 && std::isfinite(a), hasB = m != 0 && std::isfinite(b);
@@ -290,6 +333,7 @@ int launch_bounds_region(const Ctx& c, const float* X, const float* y, int64_t N
     a.N = n;
     a.Q = q;
     a.M = M;
+    a.nr2 = (nres + 1) / 2;
     const bool small = (Q + 3) / 4 < 2LL * c.num_sms * 128;
     if (norm == 1) return launch_region_n<1>(c, a, dp, small);
     if (norm == 2) return launch_region_n<2>(c, a, dp, small);
