@@ -495,7 +495,8 @@ def run_other_config(B, c):
                                       "roofline")})
         out["workload"] = f"BASELINE.json configs[{c - 1}]"
         if c == 1:
-            out["kernel"] = "bounds_small<L2,D2> (one launch: a1 inside the kernel, all data in shared memory)"
+            out["kernel"] = "bounds_small<L2,D2>"   # one launch: a1 inside the kernel, all data in shared memory
+            out["roofline"] = B.roofline(r["pairs"], SURVEY_OPS[1], EXECUTED_OPS[1], r["kernel_ms"], out["kernel"])
             out["policy"] = "LIPFIT_BOUNDS_AUTO (every pair evaluated)"
             # latency-bound config: an isolated, L2-flushed step exposes the host launch latency; also report the
             # steady state of back-to-back calls (inputs stay in L2; 200 calls between two events)
