@@ -85,3 +85,34 @@ def test_knn_routes_match_the_oracle(seed):
         assert info["key_error_ratio"] <= 1.0, info
         np.testing.assert_array_equal(idx.cpu().numpy(), oi, err_msg=str((d, norm, side, N, Q, k, tc)))
         np.testing.assert_array_equal(dist.cpu().numpy(), od.astype(np.float32))
+
+
+@pytest.mark.parametrize("seed", range(48))
+def test_lipschitz_constant_and_smoothing_objective_shapes(seed):
+    """lipfit_lipschitz_constant (exact-d symmetric kernels for d <= 8, generic otherwise) and the Eq.(7)
+    objective / gradient through both passes (all pairs, exactly pruned) on random shapes against the oracle."""
+    import paper_2606_04670_b200 as L
+    rng = np.random.default_rng(50_000 + seed)
+    d = int(rng.choice([1, 2, 3, 4, 5, 6, 7, 8, 11, 16, 20]))
+    norm = int(rng.integers(1, 4))
+    symmetric = seed % 3 != 0
+    mask = None if symmetric else rng.choice([-1, 0, 1], size=d).astype(np.int32)
+    N = int(rng.choice([2, 33, 500, 1300, 2600]))
+    w = None if rng.random() < 0.5 else rng.choice([0.5, 1.0, 2.0], size=d).astype(np.float32)
+    X, _, _ = random_problem(60_000 + seed, N, 1, d, spread=0.5)
+    # a smooth monotone-compatible signal plus noise: finite Lipschitz constant when symmetric
+    s = np.zeros(d) if mask is None else mask.astype(np.float64)
+    y = ((X.astype(np.float64) * (s + 0.3)).sum(axis=1) + 0.2 * rng.standard_normal(N)).astype(np.float32)
+    Xd, yd = _dev(X), _dev(y)
+    ref = oracle.lipschitz_constant(X, y, mask, norm, w)
+    got = float(L.lipfit_lipschitz_constant(Xd, yd, mask, norm, w).cpu()[0])
+    assert (np.isinf(ref) and np.isinf(got)) or got == float(np.float32(ref)), (d, norm, symmetric, N, got, ref)
+    M, p = 0.6, 0.7
+    eps = (0.1 * rng.standard_normal(N)).astype(np.float32)
+    F, grad = oracle.smooth_objective(X, y, M, eps.astype(np.float64), mask, norm, w, p)
+    gscale = max(np.abs(grad).max(), 1e-30)
+    Fa, ga = L.lipfit_smooth_objective(Xd, yd, M, _dev(eps), mask, norm, w, p)
+    Fp, gp = L.lipfit_smooth_objective_pruned(Xd, yd, M, _dev(eps), mask, norm, w, p)
+    for name, Fg, gg in (("all pairs", Fa, ga), ("pruned", Fp, gp)):
+        assert abs(Fg - F) <= 1e-5 * max(abs(F), 1e-30), (name, d, norm, N, Fg, F)
+        assert np.abs(gg.cpu().numpy() - grad).max() <= 1e-5 * gscale, (name, d, norm, N)
