@@ -283,21 +283,41 @@ struct PackedLinf {
     static constexpr int D = DU + DC;
     static constexpr int RFL = record_floats(D);
     static __device__ __forceinline__ void pair2(const float2* qq, const float2* x, float2& hi, float2& lo) {
-        float2 sm = make_float2(0.f, 0.f);
+        // s = max_free |delta_j| as a chain of 3-input maxima that STARTS from |delta_0| (not from 0): n values
+        // cost (n - 1) / 2 FMNMX3 -- 3 for config 3's 7 free coordinates instead of 4; an odd one out is folded
+        // into the first constrained coordinate's pair of maxima (or a last 2-input maximum).
+        float2 dl[D];
 #pragma unroll
-        for (int j = 0; j < DU; ++j) {
-            const float2 dlt = sub2(qq[j], x[j]);
-            sm.x = fmaxf(sm.x, fabsf(dlt.x));
-            sm.y = fmaxf(sm.y, fabsf(dlt.y));
+        for (int j = 0; j < D; ++j) dl[j] = sub2(qq[j], x[j]);
+        float2 sm = make_float2(0.f, 0.f);  // (DU == 0: the constrained maxima start from 0, which is their relu)
+        constexpr int NCH = DU >= 1 ? (DU - 1) / 2 : 0;     // full (a, b) pairs after the first value
+        constexpr bool LEFT = DU >= 1 && ((DU - 1) % 2 == 1);  // one free value left over
+        if (DU >= 1) sm = make_float2(fabsf(dl[0].x), fabsf(dl[0].y));
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const float2 a = dl[1 + 2 * c], b = dl[2 + 2 * c];
+            sm.x = fmaxf(fmaxf(sm.x, fabsf(a.x)), fabsf(b.x));  // FMNMX3
+            sm.y = fmaxf(fmaxf(sm.y, fabsf(a.y)), fabsf(b.y));
         }
         float2 pu = sm, pl = sm;
+        if (LEFT) {
+            const float2 e = dl[DU - 1];
+            if (DC >= 1) {  // s >= 0 already: max(s, relu(d)) == max(s, d)
+                pu.x = fmaxf(fmaxf(pu.x, fabsf(e.x)), dl[DU].x);
+                pu.y = fmaxf(fmaxf(pu.y, fabsf(e.y)), dl[DU].y);
+                pl.x = fmaxf(fmaxf(pl.x, fabsf(e.x)), -dl[DU].x);
+                pl.y = fmaxf(fmaxf(pl.y, fabsf(e.y)), -dl[DU].y);
+            } else {
+                pu.x = pl.x = fmaxf(pu.x, fabsf(e.x));
+                pu.y = pl.y = fmaxf(pu.y, fabsf(e.y));
+            }
+        }
 #pragma unroll
-        for (int j = DU; j < D; ++j) {
-            const float2 dlt = sub2(qq[j], x[j]);
-            pu.x = fmaxf(pu.x, dlt.x);  // s >= 0 already: max(s, relu(d)) == max(s, d)
-            pu.y = fmaxf(pu.y, dlt.y);
-            pl.x = fmaxf(pl.x, -dlt.x);
-            pl.y = fmaxf(pl.y, -dlt.y);
+        for (int j = DU + ((LEFT && DC >= 1) ? 1 : 0); j < D; ++j) {
+            pu.x = fmaxf(pu.x, dl[j].x);
+            pu.y = fmaxf(pu.y, dl[j].y);
+            pl.x = fmaxf(pl.x, -dl[j].x);
+            pl.y = fmaxf(pl.y, -dl[j].y);
         }
         hi = __fadd2_rn(x[D], pu);
         lo = sub2(x[D], pl);

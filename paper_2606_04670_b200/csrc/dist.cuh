@@ -24,7 +24,8 @@ struct PairAcc {
             float dlt = q[j] - x[j];
             if (NORM == 1) s += fabsf(dlt);
             if (NORM == 2) s = fmaf(dlt, dlt, s);
-            if (NORM == 3) s = fmaxf(s, fabsf(dlt));
+            // the chain of maxima starts from |delta_0|, not from 0: n values then fold into (n - 1) / 2 FMNMX3
+            if (NORM == 3) s = (j == 0) ? fabsf(dlt) : fmaxf(s, fabsf(dlt));
         }
         float pu = s, pl = s;
 #pragma unroll
@@ -64,7 +65,7 @@ struct PairAccU {
             float dlt = q[j] - x[j];
             if (NORM == 1) s += fabsf(dlt);
             if (NORM == 2) s = fmaf(dlt, dlt, s);
-            if (NORM == 3) s = fmaxf(s, fabsf(dlt));
+            if (NORM == 3) s = (j == 0) ? fabsf(dlt) : fmaxf(s, fabsf(dlt));
         }
 #pragma unroll
         for (int j = DU; j < DU + DC; ++j) {
