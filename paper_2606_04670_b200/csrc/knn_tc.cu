@@ -29,8 +29,8 @@
 //                           queries, append the hits of the row messages (lane = column) / compact the
 //                           pools exactly as in knn.cu, and publish lowered thresholds back through shared
 //                           memory.
-// Every work item starts with a seeding phase (kTcTilesA tiles) that gives each query a finite threshold
-// before the sweep (see kTcGroupA).
+// Every work item starts with a seeding phase (tc_tiles_a() tiles) that gives each query a finite threshold
+// before the sweep.
 #include <cuda_bf16.h>
 
 #include "knn_common.cuh"
@@ -57,18 +57,21 @@ constexpr int kTcMinimaA = 96;      // seeding minima per query (phase A); they 
 constexpr int kTcRingFloats = kTcRing * kTcRowFloats;
 static_assert(32 * (kTcMinimaA + 1) <= kTcRingFloats, "phase A minima overlay the ring");
 constexpr int kTcStages = 4;
-// Threshold seeding (phase A of a work item): the first kTcTilesA B tiles are multiplied once more up
-// front; the detectors only take the minimum key of every group of kTcGroupA tiles per query, kTcMinimaA
+// Threshold seeding (phase A of a work item): the first tc_tiles_a() B tiles are multiplied once more up
+// front; the detectors only take the minimum key of every group of 4 or 8 tiles per query, kTcMinimaA
 // minima in all, and the appender sets the query's starting threshold to the ksel-th smallest of them
 // (each minimum is the key of a different datum, so at least ksel data lie at or below it).  Without it
 // the first ~1 % of the tiles of an item carry half of its appends and compactions (the thresholds
-// start at +inf), a burst the appenders cannot absorb.
-constexpr int kTcGroupA = 4;  // tiles per seeding minimum
-constexpr int kTcTilesA = kTcMinimaA * kTcGroupA;
-constexpr int kTcMinTilesA = 2 * kTcTilesA;  // shorter items are not worth the extra tiles
-constexpr int kTcMaxKselA = 64;              // of 96 minima
+// start at +inf), a burst the appenders cannot absorb.  Groups of 8 tiles (a threshold of rank ~50 among
+// the first 98 304 data instead of 49 152) pay for their extra tiles on long items only: measured on
+// config 4 (7813 tiles per item) 76.0 ms with groups of 4, 74.5 with 8, 80.2 with 16.
+constexpr int kTcGroupShort = 4, kTcGroupLong = 8;  // tiles per seeding minimum
+constexpr int kTcLongItem = 4096;                   // tiles: items at least this long use kTcGroupLong
+constexpr int kTcMaxKselA = 88;                     // of 96 minima (k <= 80)
 __host__ __device__ __forceinline__ int tc_tiles_a(int tb, int te, int ksel) {
-    return (te - tb >= kTcMinTilesA && ksel <= kTcMaxKselA) ? kTcTilesA : 0;
+    if (ksel > kTcMaxKselA) return 0;
+    if (te - tb >= kTcLongItem) return kTcMinimaA * kTcGroupLong;
+    return te - tb >= 2 * kTcMinimaA * kTcGroupShort ? kTcMinimaA * kTcGroupShort : 0;  // shorter: not worth it
 }
 constexpr int kTcK = 64;                          // bf16 per operand row (= one 128-byte swizzle row)
 constexpr int kTcTileBytes = kTcBN * kTcK * 2;    // 16 KB: 128 rows x 128 B
@@ -472,7 +475,8 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                 while (ld_acquire_s(&tail_s[warp]) != head) __nanosleep(LIPFIT_TC_POLL_NS);
                 tail_seen = head;
                 float gm = __int_as_float(0x7f800000);
-                for (int vt = 0; vt < nA; ++vt, ++gB) {
+                const int grp = nA / kTcMinimaA;
+                for (int vt = 0, ing = 0, ng = 0; vt < nA; ++vt, ++gB) {
                     const uint32_t b = gB & 1u, ua = gB >> 1;
                     mbar_wait_sleep(&acc_full[h][b], ua & 1u);
                     tc_fence_after();
@@ -487,9 +491,10 @@ knn_tc_select_kernel(const KnnTcArgs g) {
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&acc_empty[h][b]);
-                    if ((vt + 1) % kTcGroupA == 0) {
-                        ring[lane * (kTcMinimaA + 1) + vt / kTcGroupA] = gm;
+                    if (++ing == grp) {
+                        ring[lane * (kTcMinimaA + 1) + ng++] = gm;
                         gm = __int_as_float(0x7f800000);
+                        ing = 0;
                     }
                 }
                 __syncwarp();

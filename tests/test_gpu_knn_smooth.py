@@ -147,11 +147,13 @@ def test_tensor_core_and_cuda_core_selection_agree(d):
     np.testing.assert_array_equal(a[1], b[1])
 
 
-@pytest.mark.parametrize("k", [32, 56])
+@pytest.mark.parametrize("k", [32, 56, 80, 100])
 def test_tensor_core_threshold_seeding(k):
     """Work items that sweep >= 768 B tiles seed their thresholds from group minima of the first tiles
-    (knn_tc.cu, phase A).  Full one-chunk items (seeded) and a chunked tail block (not seeded) in one
-    call; a sample of the queries against the oracle, all of them against the CUDA-core selection."""
+    (knn_tc.cu, phase A; k + margin <= 88 of the 96 minima, so k = 100 runs unseeded; items of >= 4096 tiles,
+    groups of 8 tiles, are covered by the full-size config 4 test).  Full one-chunk items (seeded) and a
+    chunked tail block (not seeded) in one call; a sample of the queries against the oracle, all of them
+    against the CUDA-core selection."""
     N, Q, d = 100003, 148 * 256 + 100, 16
     X, _, Xq = random_problem(77 + k, N, Q, d)
     gi, gd = _gpu_knn(X, Xq, k)
