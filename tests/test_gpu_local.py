@@ -145,3 +145,28 @@ def test_local_pipeline_interpolates_the_data():
         L.lipfit_local_lipschitz(Xd, yd, knots[:8], wl.norm)                     # J must be LIPFIT_LOCAL_KNOTS
     with pytest.raises(L.LipfitError):
         L.lipfit_local_lipschitz(Xd, yd, knots[::-1].copy(), wl.norm)            # knots must be non-decreasing
+
+
+@pytest.mark.parametrize("norm", NORMS)
+@pytest.mark.parametrize("case", ["quantiles", "wide", "repeated", "zero_first", "one_ulp_apart"])
+def test_knot_lookup_paths(norm, case):
+    """The kernels look a distance up among the knots either through a cell table on the float bits (when no
+    cell of the 1024-cell table holds two knots) or by a two-level search (local.cu: local_lut_params).  Knot
+    sets that take the table (quantiles; 12 octaves wide, coarse cells) and sets that cannot (a repeated knot,
+    a zero knot, two knots one ulp apart) against the oracle, tables and evaluation."""
+    d, N, Q = 5, 2500, 1500
+    X, y, Xq = _problem(90, N, Q, d)
+    pi, pk = sample_pairs(14, N, 20000)
+    knots = oracle.distance_quantiles(X, pi, pk, J, norm, None).astype(np.float32)
+    if case == "wide":
+        knots = (knots[7] * 2.0 ** np.linspace(-6, 6, J)).astype(np.float32)
+    elif case == "repeated":
+        knots[5] = knots[4]
+    elif case == "zero_first":
+        knots[0] = 0.0
+    elif case == "one_ulp_apart":
+        knots[9] = np.nextafter(knots[8], np.float32(np.inf))
+    assert np.all(np.diff(knots) >= 0)
+    got, _ = _check_table(X, y, knots, norm, None, min_same=0.99)
+    table = oracle.local_lipschitz(X, y, knots.astype(np.float64), norm, None).astype(np.float32)
+    _check_values(X, y, Xq, knots, table, norm, None)
