@@ -349,6 +349,119 @@ local_eval_kernel(const EvalArgs a, const Knots kn) {
     }
 }
 
+// ---- packed f32x2 evaluation (L2, d <= 8) ----------------------------------------------------
+// A thread keeps its 8 queries as 4 register pairs (q_r, q_r+1); the records carry every coordinate twice,
+//     [x'_0, x'_0, x'_1, x'_1, .. (2 * DE floats, DE = d rounded up to even), y, 0, 0, 0, M_k[0..15]],
+// so that an LDS.128 yields two operands of FADD2 / FFMA2: the 2 d distance instructions of a pair become d,
+// and y +- M_k D one FADD2 each per two pairs.  Same operations in the same order as local_eval_kernel:
+// bit-identical outputs.
+__global__ void __launch_bounds__(256)
+local_eval_pack2_kernel(const float* __restrict__ X, const float* __restrict__ y, const float* __restrict__ table,
+                        int N, Xform xf, int de, float* __restrict__ rec) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int rf = 2 * de + 4 + kJ;
+    float* dst = rec + static_cast<size_t>(k) * rf;
+    const float* src = X + static_cast<size_t>(k) * xf.d;
+    for (int j = 0; j < de; ++j) {
+        const float v = j < xf.d ? xf.sw[j] * src[xf.perm[j]] : 0.f;
+        dst[2 * j] = v;
+        dst[2 * j + 1] = v;
+    }
+    dst[2 * de] = y[k];
+    dst[2 * de + 1] = dst[2 * de + 2] = dst[2 * de + 3] = 0.f;
+    for (int j = 0; j < kJ; ++j) dst[2 * de + 4 + j] = table[static_cast<size_t>(k) * kJ + j];
+}
+
+constexpr int kLocPairs = 4;  // query pairs per thread (measured on config 6: 2 / 3 / 4 pairs 191 / 184 / 181 ms)
+__device__ __forceinline__ float2 local_sub2(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+
+template <int DA, bool LUT>
+__global__ void __launch_bounds__(kLocThreads, 2)
+local_eval_packed_kernel(const EvalArgs a, const Knots kn) {
+    constexpr int DE = (DA + 1) & ~1;
+    constexpr int RF = 2 * DE + 4 + kJ;
+    constexpr int TILE = local_tile_records<RF>();
+    constexpr int RP = kLocPairs;
+    __shared__ __align__(128) float sbuf[2 * TILE * RF];
+    __shared__ __align__(8) uint64_t bars[2];
+    __shared__ float4 sk4[4];
+    __shared__ float2 slut[LUT ? kLutCells : 1];
+    local_knot_groups(kn, sk4);
+    if (LUT) local_knot_lut_build(kn, slut);
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    uint32_t phase = 0;
+    const int ntiles = a.nqb * a.nch;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int qb = tile / a.nch, ch = tile - qb * a.nch;
+        float2 q[RP][DA], U[RP], L[RP];
+#pragma unroll
+        for (int rp = 0; rp < RP; ++rp) {
+            int q0 = (qb * 2 * RP + 2 * rp) * kLocThreads + static_cast<int>(threadIdx.x);
+            int q1 = q0 + kLocThreads;
+            q0 = q0 < a.Q ? q0 : a.Q - 1;
+            q1 = q1 < a.Q ? q1 : a.Q - 1;
+            const float* s0 = a.Xq + static_cast<size_t>(q0) * a.d;
+            const float* s1 = a.Xq + static_cast<size_t>(q1) * a.d;
+#pragma unroll
+            for (int j = 0; j < DA; ++j)
+                q[rp][j] = make_float2(a.xf.sw[j] * __ldg(s0 + a.xf.perm[j]), a.xf.sw[j] * __ldg(s1 + a.xf.perm[j]));
+            U[rp] = make_float2(__int_as_float(0x7f800000), __int_as_float(0x7f800000));
+            L[rp] = make_float2(__int_as_float(0xff800000), __int_as_float(0xff800000));
+        }
+        const int begin = ch * a.chunk;
+        const int end = min(a.N, begin + a.chunk);
+        RecordStream<TILE> rs(a.rec, RF, begin, end, sbuf, bars, &phase);
+        for (int t = 0; t < rs.ntiles; ++t) {
+            const float* s = rs.acquire(t);
+            const int n = rs.count(t);
+            for (int jrec = 0; jrec < n; ++jrec) {
+                float xr[2 * DE];
+                local_load_record<2 * DE>(s + jrec * RF, xr);
+                const float yk = s[jrec * RF + 2 * DE];
+                const float2 y2 = make_float2(yk, yk);
+                const float* mk = s + jrec * RF + 2 * DE + 4;  // the datum's step table stays in shared memory
+#pragma unroll
+                for (int rp = 0; rp < RP; ++rp) {
+                    float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int j = 0; j < DA; ++j) {
+                        const float2 dl = local_sub2(q[rp][j], make_float2(xr[2 * j], xr[2 * j + 1]));
+                        acc = __ffma2_rn(dl, dl, acc);
+                    }
+                    const float M0 = mk[LUT ? local_knot_lut(acc.x, kn, slut) : local_knot_index(acc.x, kn, sk4)];
+                    const float M1 = mk[LUT ? local_knot_lut(acc.y, kn, slut) : local_knot_index(acc.y, kn, sk4)];
+                    const float D0 = fast_sqrt(acc.x), D1 = fast_sqrt(acc.y);
+                    // M_k may be +inf at a duplicate: inf * 0 := 0
+                    const float2 MD = make_float2(D0 > 0.f ? M0 * D0 : 0.f, D1 > 0.f ? M1 * D1 : 0.f);
+                    const float2 hi = __fadd2_rn(y2, MD), lo = local_sub2(y2, MD);
+                    U[rp] = make_float2(fminf(U[rp].x, hi.x), fminf(U[rp].y, hi.y));
+                    L[rp] = make_float2(fmaxf(L[rp].x, lo.x), fmaxf(L[rp].y, lo.y));
+                }
+            }
+            rs.release(t);
+        }
+#pragma unroll
+        for (int rp = 0; rp < RP; ++rp) {
+            const int q0 = (qb * 2 * RP + 2 * rp) * kLocThreads + static_cast<int>(threadIdx.x);
+            const int q1 = q0 + kLocThreads;
+            if (q0 < a.Q) {
+                atomicMin(a.keyU + q0, f2key(U[rp].x));
+                atomicMax(a.keyL + q0, f2key(L[rp].x));
+            }
+            if (q1 < a.Q) {
+                atomicMin(a.keyU + q1, f2key(U[rp].y));
+                atomicMax(a.keyL + q1, f2key(L[rp].y));
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256)
 local_eval_final_kernel(const uint32_t* __restrict__ keyU, const uint32_t* __restrict__ keyL, int Q,
                         float* __restrict__ upper, float* __restrict__ lower, float* __restrict__ g) {
@@ -423,6 +536,40 @@ int launch_eval_l(const Ctx& c, EvalArgs& a, const Knots& kn) {
 template <int NORM, int DP, int DA>
 int launch_eval(const Ctx& c, EvalArgs& a, const Knots& kn) {
     return kn.lut_shift >= 0 ? launch_eval_l<NORM, DP, DA, true>(c, a, kn) : launch_eval_l<NORM, DP, DA, false>(c, a, kn);
+}
+
+template <int DA, bool LUT>
+int launch_eval_packed_l(const Ctx& c, EvalArgs& a, const Knots& kn) {
+    constexpr int RF = 2 * ((DA + 1) & ~1) + 4 + kJ;
+    auto kern = local_eval_packed_kernel<DA, LUT>;
+    int occ = 0;
+    LIPFIT_CUDA(occupancy_of(&occ, kern, kLocThreads, 0));
+    if (occ < 1) occ = 1;
+    const int slots = c.num_sms * occ;
+    local_schedule(a.Q, kLocThreads * 2 * kLocPairs, a.N, local_tile_records<RF>(), slots, &a.nqb, &a.nch, &a.chunk);
+    const long long nt = static_cast<long long>(a.nqb) * a.nch;
+    KernelTimer kt(TK_LOCAL_EVAL, c.stream);
+    kern<<<static_cast<int>(nt < slots ? nt : slots), kLocThreads, 0, c.stream>>>(a, kn);
+    kt.stop();
+    ++g_launches;
+    LIPFIT_CUDA(cudaGetLastError());
+    return LIPFIT_OK;
+}
+template <int DA>
+int launch_eval_packed(const Ctx& c, EvalArgs& a, const Knots& kn) {
+    return kn.lut_shift >= 0 ? launch_eval_packed_l<DA, true>(c, a, kn) : launch_eval_packed_l<DA, false>(c, a, kn);
+}
+int dispatch_eval_packed(const Ctx& c, EvalArgs& a, const Knots& kn, int d) {
+    switch (d) {
+        case 1: return launch_eval_packed<1>(c, a, kn);
+        case 2: return launch_eval_packed<2>(c, a, kn);
+        case 3: return launch_eval_packed<3>(c, a, kn);
+        case 4: return launch_eval_packed<4>(c, a, kn);
+        case 5: return launch_eval_packed<5>(c, a, kn);
+        case 6: return launch_eval_packed<6>(c, a, kn);
+        case 7: return launch_eval_packed<7>(c, a, kn);
+        default: return launch_eval_packed<8>(c, a, kn);
+    }
 }
 
 // Kernel knots (squared for L2) -> cell table parameters; lut_shift = -1 when the knot set does not allow a
@@ -541,12 +688,17 @@ int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N6
                         float* lower, float* g) {
     const int N = static_cast<int>(N64), Q = static_cast<int>(Q64);
     const int dp = local_dp(xf.d);
-    const int rf = dp + 4 + kJ;
+    const bool packed = norm == 2 && xf.d <= 8;  // packed f32x2 kernel: duplicated coordinates
+    const int de = (xf.d + 1) & ~1;
+    const int rf = packed ? 2 * de + 4 + kJ : dp + 4 + kJ;
     Workspace wrec, wkeys;
     int rc;
     if ((rc = wrec.alloc(sizeof(float) * static_cast<size_t>(N) * rf, c.stream))) return rc;
     if ((rc = wkeys.alloc(sizeof(uint32_t) * 2 * static_cast<size_t>(Q), c.stream))) return rc;
-    local_eval_pack_kernel<<<(N + 255) / 256, 256, 0, c.stream>>>(X, y, table, N, xf, dp, wrec.as<float>());
+    if (packed)
+        local_eval_pack2_kernel<<<(N + 255) / 256, 256, 0, c.stream>>>(X, y, table, N, xf, de, wrec.as<float>());
+    else
+        local_eval_pack_kernel<<<(N + 255) / 256, 256, 0, c.stream>>>(X, y, table, N, xf, dp, wrec.as<float>());
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
     Knots kn;  // L2: squared knots, correctly rounded (the kernel compares squared distances with them)
@@ -564,7 +716,7 @@ int launch_values_local(const Ctx& c, const float* X, const float* y, int64_t N6
     a.xf = xf;
     LIPFIT_CUDA(cudaMemsetAsync(a.keyU, 0xFF, sizeof(uint32_t) * Q, c.stream));
     LIPFIT_CUDA(cudaMemsetAsync(a.keyL, 0x00, sizeof(uint32_t) * Q, c.stream));
-    if ((rc = dispatch_eval(c, a, kn, norm, xf.d))) return rc;
+    if ((rc = packed ? dispatch_eval_packed(c, a, kn, xf.d) : dispatch_eval(c, a, kn, norm, xf.d))) return rc;
     local_eval_final_kernel<<<(Q + 255) / 256, 256, 0, c.stream>>>(a.keyU, a.keyL, Q, upper, lower, g);
     ++g_launches;
     LIPFIT_CUDA(cudaGetLastError());
