@@ -127,9 +127,16 @@ int lipfit_bounds_noalloc(const float* X, const float* y, int64_t N, int32_t d, 
  *                         PRUNED when d <= 8, N >= 8192,
  *                         Q >= 4096 and N Q >= 2^32 (few enough coordinates for bounding boxes to separate,
  *                         enough pairs to pay for two radix sorts: 9.7x / 5.3x / 2.0x on the config 2 / 5 / 3
- *                         workloads), BRUTE otherwise.  Pruning cannot help when M D is small against the
- *                         spread of y everywhere (M = 0 in the limit): PRUNED then visits every pair at about
- *                         half the all-pairs rate; callers who know that pass LIPFIT_BOUNDS_BRUTE.
+ *                         workloads), BRUTE otherwise.  Pruning cannot help when the candidates y + M D of far
+ *                         data compete with those of near data everywhere (M D comparable to the spread of y
+ *                         across the whole domain): the pruned pass then visits most pairs at about half the
+ *                         all-pairs rate.  AUTO guards against that: the pruned kernel keeps the running fraction
+ *                         of pairs its finished groups of 32 queries evaluated and, above 40 %, stops handing out
+ *                         groups; the call then runs BRUTE instead (ONE stream synchronisation inside the call,
+ *                         after the pruned kernel, to read that decision back; only for Q >= 4608 x the number
+ *                         of SMs, i.e. when the groups come in enough waves for stopping to save work).  The
+ *                         result is the same exact minimum / maximum whichever pass runs.  Callers who must not
+ *                         synchronise pass LIPFIT_BOUNDS_BRUTE or LIPFIT_BOUNDS_PRUNED.
  * pairs_evaluated: HOST int64[3] or NULL, as in lipfit_bounds_pruned ([0] = N Q under BRUTE); non-NULL
  * synchronises the stream.  Unknown policy: LIPFIT_E_PARAM. */
 enum lipfit_bounds_policy { LIPFIT_BOUNDS_AUTO = 0, LIPFIT_BOUNDS_BRUTE = 1, LIPFIT_BOUNDS_PRUNED = 2 };

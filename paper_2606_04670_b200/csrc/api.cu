@@ -135,7 +135,31 @@ int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const
         }
         return LIPFIT_OK;
     }
-    if (!pruned) {
+    if (pruned) {
+        Workspace stats;
+        if (pairs_evaluated) {
+            rc = stats.alloc(4 * sizeof(unsigned long long), c.stream);
+            if (rc) return rc;
+            LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 4 * sizeof(unsigned long long), c.stream));
+        }
+        bool declined = false;  // AUTO: the finished query groups evaluated too many of their pairs for pruning to pay
+        rc = launch_bounds_pruned(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g,
+                                  pairs_evaluated ? stats.as<unsigned long long>() : nullptr,
+                                  policy == LIPFIT_BOUNDS_AUTO ? kPrunedGuardLimit : 0.f, &declined);
+        if (rc) return rc;
+        if (!declined) {
+            if (pairs_evaluated) {
+                unsigned long long h[4] = {0, 0, 0, 0};
+                LIPFIT_CUDA(cudaMemcpyAsync(h, stats.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+                LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+                pairs_evaluated[0] = static_cast<int64_t>(h[0]) * 1024;
+                pairs_evaluated[1] = static_cast<int64_t>(h[1]);
+                pairs_evaluated[2] = static_cast<int64_t>(h[2]);
+            }
+            return LIPFIT_OK;
+        }
+    }
+    {
         const Xform xfb = bounds_xform(xf, norm);  // off-table shapes with d <= 8: even-rounded coordinate counts
         RecLayout lay = bounds_layout(c, xfb, norm, Q);
         if (lay.rf == 0) return LIPFIT_E_PARAM;
@@ -155,24 +179,6 @@ int lipfit_bounds_ex(const float* X, const float* y, int64_t N, int32_t d, const
         }
         return LIPFIT_OK;
     }
-    Workspace stats;
-    if (pairs_evaluated) {
-        rc = stats.alloc(4 * sizeof(unsigned long long), c.stream);
-        if (rc) return rc;
-        LIPFIT_CUDA(cudaMemsetAsync(stats.p, 0, 4 * sizeof(unsigned long long), c.stream));
-    }
-    rc = launch_bounds_pruned(c, X, y, N, Xq, Q, xf, norm, M, upper, lower, g,
-                              pairs_evaluated ? stats.as<unsigned long long>() : nullptr);
-    if (rc) return rc;
-    if (pairs_evaluated) {
-        unsigned long long h[4] = {0, 0, 0, 0};
-        LIPFIT_CUDA(cudaMemcpyAsync(h, stats.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
-        LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
-        pairs_evaluated[0] = static_cast<int64_t>(h[0]) * 1024;
-        pairs_evaluated[1] = static_cast<int64_t>(h[1]);
-        pairs_evaluated[2] = static_cast<int64_t>(h[2]);
-    }
-    return LIPFIT_OK;
 }
 
 int lipfit_bounds(const float* X, const float* y, int64_t N, int32_t d, const float* Xq, int64_t Q,

@@ -62,9 +62,13 @@ int launch_bounds_topk(const Ctx& c, const float* rec, int64_t N, const float* X
 // NEXT-4(ii): bounds with exact spatial pruning (prune.cu); X, Xq: ORIGINAL row-major arrays.
 // stats_dev: device uint64[3] (zeroed by the caller) or NULL: [0] += tiles of 32 x 32 pairs evaluated,
 // [1] += tiles that passed the warp-box test, [2] += lanes whose own test asked for an evaluated tile.
+// guard_limit > 0 (LIPFIT_BOUNDS_AUTO): the kernel keeps the running fraction of pairs its finished query groups
+// evaluated; above guard_limit (from max(64, groups / 64) finished groups on, while fewer than half are done) the
+// groups not yet started return at once.  One read-back + stream synchronisation after the kernel sets *declined:
+// the outputs are then incomplete and the caller runs the all-pairs kernels instead.
 int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N, const float* Xq, int64_t Q,
                          const Xform& xf, int norm, float M, float* upper, float* lower, float* g,
-                         unsigned long long* stats_dev);
+                         unsigned long long* stats_dev, float guard_limit = 0.f, bool* declined = nullptr);
 
 // LIPFIT_BOUNDS_AUTO (include/lipfit.h): the exactly pruned pass when the box tests can pay for themselves --
 // few enough coordinates for the boxes to separate (d <= 8: measured 9.7x / 5.3x / 2.0x on the config 2 / 5 /
@@ -72,6 +76,10 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
 inline bool bounds_prefers_pruned(const Xform& xf, int64_t N, int64_t Q) {
     return xf.d <= 8 && N >= 8192 && Q >= 4096 && N * Q >= (1LL << 32);
 }
+// ... and only while the finished query groups evaluate at most this fraction of their pairs: the pruned kernel evaluates
+// a pair at 0.35-0.55 of the all-pairs kernels' rate (configs 2 / 5 / 3: 1.23 vs 3.1, 0.68 vs 1.19, 1.05 vs 1.84
+// Tpairs/s), so beyond ~40 % the all-pairs pass is the faster exact answer.
+constexpr float kPrunedGuardLimit = 0.40f;
 
 // Eq.(7) objective / gradient with the same exact pruning (prune.cu).  F_dev: device double (required,
 // zeroed here); grad: device float in the original order or NULL; eps may be NULL.

@@ -201,6 +201,13 @@ struct PruneArgs {
     FreeFlags ff;
     float *upper, *lower, *g;
     unsigned long long* stats;  // [0] tiles evaluated (x 1024 pairs), [1] stage-1 survivors, [2] lanes that needed them
+    // Guard of LIPFIT_BOUNDS_AUTO (NULL: none).  guard[0] += tiles evaluated by FINISHED query groups,
+    // guard[1] += finished groups, guard[2] = 1 once the finished groups have evaluated more than guard_limit
+    // of their pairs (checked from guard_min finished groups on, while fewer than half of all groups are done):
+    // groups that have not started yet then return at once, and the caller runs the all-pairs kernels.
+    unsigned long long* guard;
+    float guard_limit;
+    int guard_min;
 };
 
 template <int NORM, int DP, int DC>
@@ -275,6 +282,8 @@ bounds_pruned_kernel(const PruneArgs a) {
     unsigned long long n_eval = 0, n_surv = 0, n_mine = 0;
     for (int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w < nwarps;
          w += gridDim.x * (blockDim.x >> 5)) {
+        if (a.guard && *reinterpret_cast<volatile unsigned long long*>(a.guard + 2) != 0ull) break;  // warp-uniform
+        const unsigned long long n_eval_before = n_eval;
         const int pos = min(w * 32 + lane, a.Q - 1);
         const bool live = (w * 32 + lane) < a.Q;
         const int qi = a.qorder[pos];
@@ -379,6 +388,15 @@ bounds_pruned_kernel(const PruneArgs a) {
             if (a.upper) a.upper[qi] = U;
             if (a.lower) a.lower[qi] = L;
             if (a.g) a.g[qi] = 0.5f * (U + L);
+        }
+        if (a.guard && lane == 0) {
+            const unsigned long long tiles = atomicAdd(a.guard, n_eval - n_eval_before) + (n_eval - n_eval_before);
+            const unsigned long long done = atomicAdd(a.guard + 1, 1ull) + 1ull;
+            // fraction of their pairs the finished groups evaluated = tiles * 32 / (done * N)
+            if (done >= static_cast<unsigned long long>(a.guard_min) && 2ull * done < static_cast<unsigned long long>(nwarps) &&
+                static_cast<float>(tiles) * static_cast<float>(kTile) >
+                    a.guard_limit * static_cast<float>(done) * static_cast<float>(a.N))
+                atomicExch(a.guard + 2, 1ull);
         }
     }
     if (a.stats && lane == 0) {
@@ -710,9 +728,10 @@ Xform padded_xform(const Xform& xf, int dp) {
 
 int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N64, const float* Xq,
                          int64_t Q64, const Xform& xf, int norm, float M, float* upper, float* lower,
-                         float* g, unsigned long long* stats_dev) {
+                         float* g, unsigned long long* stats_dev, float guard_limit, bool* declined) {
     const int N = static_cast<int>(N64), Q = static_cast<int>(Q64);
     const int dp = xf.d <= 4 ? 4 : xf.d <= 8 ? 8 : xf.d <= 16 ? 16 : 32;
+    if (declined) *declined = false;
     int bits = 32 / xf.d;  // <= 32 key bits in all: four radix passes; 2^32 cells >> any N
     if (bits > 16) bits = 16;
     const int ntiles = (N + kTile - 1) / kTile;
@@ -751,12 +770,38 @@ int launch_bounds_pruned(const Ctx& c, const float* X, const float* y, int64_t N
     a.lower = lower;
     a.g = g;
     a.stats = stats_dev;
+    a.guard = nullptr;
+    a.guard_limit = 0.f;
+    a.guard_min = 0;
     PruneLaunch pl{X, y, dorder.as<int32_t>(), rec.as<float>(), box.as<float>()};
-    switch (norm) {
-        case LIPFIT_L1: return launch_pruned_n<1>(dp, xf.dC, c, pl, a);
-        case LIPFIT_L2: return launch_pruned_n<2>(dp, xf.dC, c, pl, a);
-        default: return launch_pruned_n<3>(dp, xf.dC, c, pl, a);
-    }
+    auto launch = [&]() {
+        switch (norm) {
+            case LIPFIT_L1: return launch_pruned_n<1>(dp, xf.dC, c, pl, a);
+            case LIPFIT_L2: return launch_pruned_n<2>(dp, xf.dC, c, pl, a);
+            default: return launch_pruned_n<3>(dp, xf.dC, c, pl, a);
+        }
+    };
+    // LIPFIT_BOUNDS_AUTO: the kernel watches the fraction of pairs its finished query groups evaluated and stops
+    // handing out groups once that exceeds guard_limit; ONE read-back + stream synchronisation after the kernel
+    // tells the caller whether the outputs are complete.  The first finishers report when every resident warp
+    // (~24 per SM) is about to finish its first group, so stopping only saves work when there are many waves of
+    // groups: below 6 waves the guard stays off (measured on an adversarial config 2 shaped workload, nothing
+    // prunable: Q = 1e6, 8.8 waves: guarded 46 ms, pruned pass alone 65 ms, all-pairs 32 ms; Q = 2.6e5, 2.3 waves:
+    // 4.6 / 3.1 / 2.1 ms -- the guard would only add the all-pairs pass on top of a finished pruned one).
+    if (!(guard_limit > 0.f && declined) || (Q + 31) / 32 < 6 * 24 * c.num_sms) return launch();
+    Workspace guard;
+    if ((rc = guard.alloc(4 * sizeof(unsigned long long), c.stream))) return rc;
+    LIPFIT_CUDA(cudaMemsetAsync(guard.p, 0, 4 * sizeof(unsigned long long), c.stream));
+    const int nwarps = (Q + 31) / 32;
+    a.guard = guard.as<unsigned long long>();
+    a.guard_limit = guard_limit;
+    a.guard_min = nwarps / 64 > 64 ? nwarps / 64 : 64;
+    if ((rc = launch())) return rc;
+    unsigned long long h[4] = {0, 0, 0, 0};
+    LIPFIT_CUDA(cudaMemcpyAsync(h, guard.p, sizeof(h), cudaMemcpyDeviceToHost, c.stream));
+    LIPFIT_CUDA(cudaStreamSynchronize(c.stream));
+    *declined = h[2] != 0ull;
+    return LIPFIT_OK;
 }
 
 // Morton order of the data (coordinate ranges, keys, radix sort): depends on X only, so lipfit_smooth computes

@@ -183,3 +183,38 @@ def test_lipfit_smooth_uses_the_pruned_pass_without_a_mask():
     assert np.abs(go).max() <= 1e-3 * max(1.0, info["gnorm_inf"] * 1e3)  # stationary for the oracle's gradient too
     Fu, gu = L.lipfit_smooth_objective(X, _dev(wl.y), wl.M, eps, None, wl.norm, None, wl.p)
     assert abs(Fu - info["F"]) <= 1e-5 * Fu                              # SURVEY.md §8(c) rule (S), both passes
+
+
+def test_auto_policy_guard_declines_when_pruning_cannot_help():
+    """Under LIPFIT_BOUNDS_AUTO the pruned kernel watches the fraction of pairs its finished query groups
+    evaluated and, above 40 %, stops handing out groups; the call then runs the all-pairs kernels
+    (include/lipfit.h).  Adversarial case: the data lie on a cone y = -M |x - x0| and the queries sit around x0,
+    so for every query all N candidates y_k + M D tie up to rounding and no box can be excluded; control: a
+    config 2 shaped workload, where AUTO keeps the pruned pass.  Either way the outputs are the exact minimum /
+    maximum (oracle on a query sample)."""
+    import torch
+    import paper_2606_04670_b200 as L
+    N, Q, d, M = 16384, 1000000, 4, 2.0                                  # Q >= 4608 x SMs: the guard is on
+    rng = np.random.default_rng(77)
+    X = rng.random((N, d), dtype=np.float32)
+    x0 = np.full(d, 0.5, np.float32)
+    y = (-M * np.sqrt(((X.astype(np.float64) - x0) ** 2).sum(axis=1))).astype(np.float32)
+    Xq = (x0 + 1e-3 * rng.standard_normal((Q, d))).astype(np.float32)
+    Xd, yd, Qd = _dev(X), _dev(y), _dev(Xq)
+    up, lo, g, pairs = L.lipfit_bounds_ex(Xd, yd, Qd, M, None, L2, None, policy=L.LIPFIT_BOUNDS_AUTO, count_pairs=True)
+    assert pairs[0] == N * Q and pairs[1] == 0                           # declined: every pair, all-pairs kernels
+    upp, lop, gp, pp = L.lipfit_bounds_ex(Xd, yd, Qd, M, None, L2, None, policy=L.LIPFIT_BOUNDS_PRUNED,
+                                          count_pairs=True)
+    assert pp[0] > 0.4 * N * Q                                           # the forced pruned pass: no pruning here
+    torch.cuda.synchronize()
+    rows = oracle_subset(Q, 300)
+    U, Lo, _ = oracle.bounds(X, y, Xq[rows], M, None, L2, None)
+    tol = 1e-5 * float(y.max() - y.min()) + (d + 4) * 2.0 ** -24 * max(np.abs(U).max(), np.abs(Lo).max())
+    for a, b in ((up, upp), (lo, lop)):
+        assert float((a - b).abs().max()) <= tol
+    assert np.abs(up.cpu().numpy()[rows] - U).max() <= tol and np.abs(lo.cpu().numpy()[rows] - Lo).max() <= tol
+    # control: config 2's shape at N Q = 2^32 keeps the pruned pass
+    wl = make_workload(2, N=16384, Q=1000000)
+    *_, pc = L.lipfit_bounds_ex(_dev(wl.X), _dev(wl.y), _dev(wl.Xq), wl.M, wl.mask, wl.norm, wl.weights,
+                                policy=L.LIPFIT_BOUNDS_AUTO, count_pairs=True)
+    assert 0 < pc[0] < 0.4 * wl.N * wl.Q
