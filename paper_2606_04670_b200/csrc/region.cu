@@ -87,27 +87,25 @@ __device__ __forceinline__ void region_pair(const float* q, const float* x, floa
                                             float& lo) {
     (void)nr2_rt;
     constexpr int nr2 = NR2;
-    float su = 0.f, sl = 0.f;  // L1 / L2: sums; Linf: su = max u, sl = min over (dP, dN) (= -max l)
+    float su = 0.f, sl = 0.f;  // Linf: su = max u, sl = min over (dP, dN) (= -max l)
+    float2 acc = make_float2(0.f, 0.f);  // L1: (sum u, sum m), m <= 0;  L2: (sum u^2, sum m^2)
     float sf = 0.f;            // unrestricted coordinates: shared by both bounds
 #pragma unroll
     for (int c = 0; c < DP / 2; ++c) {
         if (c < nr2) {
 #pragma unroll
             for (int j = 2 * c; j < 2 * c + 2; ++j) {
-                const float dP = q[2 * j] - x[2 * j];
-                const float dN = x[2 * j + 1] - q[2 * j + 1];
+                // (dP, -dN) = (qP - xP, qN - xN): the two transformed values of a coordinate sit side by side in
+                // the query and in the record, so both differences are ONE FADD2; the sign of the second rides
+                // in the operand modifiers of the min / max, and (u, m) accumulate with one FADD2 / FFMA2
+                const float2 d2 = __fadd2_rn(make_float2(q[2 * j], q[2 * j + 1]), make_float2(-x[2 * j], -x[2 * j + 1]));
+                const float dP = d2.x, dN = -d2.y;
                 if (NORM == 3) {
                     su = fmaxf(fmaxf(su, dP), dN);  // FMNMX3
                     sl = fminf(fminf(sl, dP), dN);
                 } else {
-                    const float u = fmaxf(dP, dN), m = fminf(dP, dN);  // u >= 0 >= m
-                    if (NORM == 1) {
-                        su += u;
-                        sl -= m;
-                    } else {
-                        su = fmaf(u, u, su);
-                        sl = fmaf(m, m, sl);
-                    }
+                    const float2 um = make_float2(fmaxf(dP, dN), fminf(dP, dN));  // u >= 0 >= m
+                    acc = NORM == 1 ? __fadd2_rn(acc, um) : __ffma2_rn(um, um, acc);
                 }
             }
         } else {
@@ -119,6 +117,13 @@ __device__ __forceinline__ void region_pair(const float* q, const float* x, floa
                 if (NORM == 3) sf = fmaxf(sf, fabsf(dlt));
             }
         }
+    }
+    if (NORM == 1) {
+        su = acc.x;
+        sl = -acc.y;
+    } else if (NORM == 2) {
+        su = acc.x;
+        sl = acc.y;
     }
     const float y = x[2 * DP];
     if (NORM == 2) {
