@@ -11,6 +11,29 @@
 
 namespace lipfit {
 
+// delta_j = q_j - x_j for D coordinates.  Neighbouring coordinates of the query (registers of the thread) and of
+// the record (one LDS.128) are register pairs already, so two differences are ONE packed FADD2 (add.rn.f32x2,
+// same rounding as the scalar subtraction: bit-identical results): the unpacked kernels are issue-bound, and
+// this halves the issue slots of their subtractions without any change of layout.
+#ifndef LIPFIT_PACK_DELTAS
+#define LIPFIT_PACK_DELTAS 1
+#endif
+template <int D>
+__device__ __forceinline__ void pair_deltas(const float* __restrict__ q, const float* __restrict__ x, float* dl) {
+#if LIPFIT_PACK_DELTAS
+#pragma unroll
+    for (int j = 0; j + 1 < D; j += 2) {
+        const float2 t = __fadd2_rn(make_float2(q[j], q[j + 1]), make_float2(-x[j], -x[j + 1]));
+        dl[j] = t.x;
+        dl[j + 1] = t.y;
+    }
+    if (D & 1) dl[D - 1] = q[D - 1] - x[D - 1];
+#else
+#pragma unroll
+    for (int j = 0; j < D; ++j) dl[j] = q[j] - x[j];
+#endif
+}
+
 // Accumulated "pre-norm" quantities: L1 -> sums, L2 -> sums of squares, Linf -> maxima.
 // S is the part shared by both sides (unconstrained coordinates); PU / PL the one-sided parts.
 template <int NORM, int DU, int DC>
@@ -18,10 +41,12 @@ struct PairAcc {
     // q, x: D = DU + DC packed coordinates in registers.
     static __device__ __forceinline__ void run(const float* __restrict__ q,
                                                const float* __restrict__ x, float& au, float& al) {
+        float dl[DU + DC > 0 ? DU + DC : 1];
+        pair_deltas<DU + DC>(q, x, dl);
         float s = 0.f;
 #pragma unroll
         for (int j = 0; j < DU; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             if (NORM == 1) s += fabsf(dlt);
             if (NORM == 2) s = fmaf(dlt, dlt, s);
             // the chain of maxima starts from |delta_0|, not from 0: n values then fold into (n - 1) / 2 FMNMX3
@@ -30,7 +55,7 @@ struct PairAcc {
         float pu = s, pl = s;
 #pragma unroll
         for (int j = DU; j < DU + DC; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             if (NORM == 1) {
                 float r = fmaxf(dlt, 0.f);
                 pu += r;
@@ -59,17 +84,19 @@ template <int NORM, int DU, int DC>
 struct PairAccU {
     static __device__ __forceinline__ float run(const float* __restrict__ q,
                                                 const float* __restrict__ x) {
+        float dl[DU + DC > 0 ? DU + DC : 1];
+        pair_deltas<DU + DC>(q, x, dl);
         float s = 0.f;
 #pragma unroll
         for (int j = 0; j < DU; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             if (NORM == 1) s += fabsf(dlt);
             if (NORM == 2) s = fmaf(dlt, dlt, s);
             if (NORM == 3) s = (j == 0) ? fabsf(dlt) : fmaxf(s, fabsf(dlt));
         }
 #pragma unroll
         for (int j = DU; j < DU + DC; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             if (NORM == 1) s += fmaxf(dlt, 0.f);
             if (NORM == 2) {
                 float r = fmaxf(dlt, 0.f);
@@ -98,10 +125,12 @@ struct PairAccGeneric {
     static __device__ __forceinline__ void run(const float* __restrict__ q,
                                                const float* __restrict__ x, const FreeFlags& ff,
                                                float& au, float& al) {
+        float dl[DP];
+        pair_deltas<DP>(q, x, dl);
         float pu = 0.f, pl = 0.f;
 #pragma unroll
         for (int j = 0; j < DP; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             float t = ff.fr[j] * dlt;
             float u = fmaxf(dlt, -t);
             float l = fmaxf(-dlt, t);
@@ -124,10 +153,12 @@ struct PairAccGeneric {
     static __device__ __forceinline__ float run_u(const float* __restrict__ q,
                                                   const float* __restrict__ x,
                                                   const FreeFlags& ff) {
+        float dl[DP];
+        pair_deltas<DP>(q, x, dl);
         float pu = 0.f;
 #pragma unroll
         for (int j = 0; j < DP; ++j) {
-            float dlt = q[j] - x[j];
+            float dlt = dl[j];
             float u = fmaxf(dlt, -(ff.fr[j] * dlt));
             if (NORM == 1) pu += u;
             if (NORM == 2) pu = fmaf(u, u, pu);
@@ -150,10 +181,12 @@ struct PairAccChunked {
         float s = 0.f, pu = 0.f, pl = 0.f;
 #pragma unroll
         for (int c = 0; c < DP / 4; ++c) {
+            float dl[4];
+            if (c < ff.nall4) pair_deltas<4>(q + 4 * c, x + 4 * c, dl);
             if (c < ff.nfree4) {
 #pragma unroll
                 for (int j = 4 * c; j < 4 * c + 4; ++j) {
-                    const float dlt = q[j] - x[j];
+                    const float dlt = dl[j - 4 * c];
                     if (NORM == 1) s += fabsf(dlt);
                     if (NORM == 2) s = fmaf(dlt, dlt, s);
                     if (NORM == 3) s = fmaxf(s, fabsf(dlt));
@@ -161,7 +194,7 @@ struct PairAccChunked {
             } else if (c < ff.nall4) {
 #pragma unroll
                 for (int j = 4 * c; j < 4 * c + 4; ++j) {
-                    const float dlt = q[j] - x[j];
+                    const float dlt = dl[j - 4 * c];
                     const float t = ff.fr[j] * dlt;
                     const float u = fmaxf(dlt, -t);
                     const float l = fmaxf(-dlt, t);
